@@ -1,0 +1,255 @@
+"""Pins of the oracle's path functions (ln_dress, residual, Jacobian, LU, Newton step): SURVEY.md 8(c)
+P10-P12.  CPU only; nothing here touches the CUDA path."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle.oracle import make_params
+from paper_1206_1779_b200.workloads import config_inputs, draw_coefficients, KAPPA, DELTA
+
+PI = math.pi
+
+
+def params_of(w, **kw):
+    d = dict(n_cheb=w.n_cheb, n_r=w.n_r, n_theta=w.n_theta, eps2=w.eps2, L2=w.L2, x_G=w.x_G, x_Z=w.x_Z,
+             alpha_mu=w.alpha_mu, n_colors=w.n_colors, delta=w.delta, ir_exp_G=w.ir_exp_G, ir_exp_Z=w.ir_exp_Z,
+             uv_omega=w.uv_omega)
+    d.update(kw)
+    return make_params(**d)
+
+
+# ------------------------------------------------------------------------------------ O2: extension
+def test_ln_dress_continuation(orc):
+    """eq.(16)-(19) L115-124 matched by continuity at eps2 and L2 (L119, L131, L192)."""
+    N = 6
+    p = make_params(N, 4, 4, 1e-6, 5e4, 1.0, 1.0)
+    c = draw_coefficients(11, N)
+    a, b = c[:N], c[N:]
+    # inside: plain series with the b_0/2 convention
+    u = 3.7
+    s = 2 * math.log(u / 1e-6) / math.log(5e4 / 1e-6) - 1
+    T = np.cos(np.arange(N) * math.acos(s)); T[0] = 0.5
+    lnG, lnZ = orc.ln_dress(p, c, u)
+    assert abs(lnG - b @ T) < 1e-13 and abs(lnZ - a @ T) < 1e-13
+    # continuity at both ends
+    for edge in (1e-6, 5e4):
+        lo = orc.ln_dress(p, c, edge * (1 - 1e-12)); hi = orc.ln_dress(p, c, edge * (1 + 1e-12))
+        assert abs(lo[0] - hi[0]) < 1e-10 and abs(lo[1] - hi[1]) < 1e-10
+    # IR: G ~ u^-kappa, Z ~ u^(2 kappa) below eps2 (eq.(16),(17))
+    g1, z1 = orc.ln_dress(p, c, 1e-6); g2, z2 = orc.ln_dress(p, c, 1e-9)
+    assert abs((g2 - g1) / math.log(1e-3) + KAPPA) < 1e-12
+    assert abs((z2 - z1) / math.log(1e-3) - 2 * KAPPA) < 1e-12
+    # UV: G = G(L2) [omega ln(u/L2) + 1]^delta, Z likewise with gamma = -13/22 (eq.(18),(19), L131)
+    omega = 11 * 3 / (12 * PI)
+    gL, zL = orc.ln_dress(p, c, 5e4); g4, z4 = orc.ln_dress(p, c, 2e5)
+    assert abs(g4 - gL - DELTA * math.log(1 + omega * math.log(4))) < 1e-13
+    assert abs(z4 - zL - (-13 / 22) * math.log(1 + omega * math.log(4))) < 1e-13
+
+
+# --------------------------------------------------------------- brute force with the LITERAL equations
+def _brute_force_F(c, N, Nr, Nt, eps2, L2, xG, xZ, gG, gZ, kappa, delta, omega, alpha=1.0, Nc=3.0):
+    """Independent restatement of PAPER.md eq.(8)-(11),(14)-(19),(23)-(30) with the printed (literal) kernels,
+    z = x + y - 2 sqrt(xy) cos(theta) and numpy's Gauss-Legendre; complex-capable in c (for complex-step
+    derivatives).  Only usable at moderate y/x (literal kernels cancel)."""
+    c = np.asarray(c, dtype=complex)
+    a, b = c[:N], c[N:]
+    Lg = math.log(L2 / eps2)
+    C = 4 * PI * alpha * Nc / (2 * PI) ** 3
+    gamma = -1 - 2 * delta
+
+    def series(coef, s):
+        tot = coef[0] / 2
+        for j in range(1, N):
+            tot = tot + coef[j] * math.cos(j * math.acos(max(-1.0, min(1.0, s))))
+        return tot
+
+    def lnGZ(u):
+        s = 2 * math.log(u / eps2) / Lg - 1
+        if u < eps2:
+            return (series(b, -1.0) - kappa * math.log(u / eps2), series(a, -1.0) + 2 * kappa * math.log(u / eps2))
+        if u > L2:
+            t = math.log(1 + omega * math.log(u / L2))
+            return (series(b, 1.0) + delta * t, series(a, 1.0) + gamma * t)
+        return (series(b, s), series(a, s))
+
+    tr, wr = np.polynomial.legendre.leggauss(Nr)
+    tt, wt = np.polynomial.legendre.leggauss(Nt)
+    ys = eps2 * np.exp((tr + 1) * Lg / 2); Wy = wr * Lg / 2 * ys
+    ths = (tt + 1) * PI / 2; Om = wt * PI / 2
+
+    def Pi(x):
+        PG = 0; PZ = 0
+        for y, W in zip(ys, Wy):
+            lGy, lZy = lnGZ(y)
+            for th, O in zip(ths, Om):
+                xi = math.cos(th)
+                z = x + y - 2 * math.sqrt(x * y) * xi
+                lGz, lZz = lnGZ(z)
+                M = (1 / z) * (-x / 4 + y / 2 - y * y / (4 * x)) + 0.5 + y / (2 * x) - z / (4 * x)
+                Q = ((1 / z ** 2) * (x ** 3 / (8 * y) + x * x - 9 / 4 * x * y + y * y + y ** 3 / (8 * x))
+                     + (1 / z) * (x * x / y - 4 * (x + y) + y * y / x) - (9 / 4 * x / y + 4 + 9 / 4 * y / x)
+                     + z * (1 / x + 1 / y) + z * z / (8 * x * y) + 15 / 4)
+                # eq.(8) with d xi (1-xi^2)^(3/2) = sin^4 dtheta ; eq.(9) with d xi (1-xi^2)^(1/2) = sin^2 dtheta
+                PG = PG - C * W * O * y * np.exp(lGy) * math.sin(th) ** 4 * np.exp(lZz) / z ** 2
+                glu = np.exp((-2 - 6 * delta) * (lGy + lGz) - 3 * delta * (lZy + lZz))
+                PZ = PZ + C / (3 * x) * W * O * math.sin(th) ** 2 * (Q * glu + M * np.exp(lGy + lGz))
+        return PG, PZ
+
+    PGs, _ = Pi(xG)
+    _, PZs = Pi(xZ)
+    F = np.zeros(2 * N, dtype=complex)
+    for i in range(N):
+        s = -math.cos(PI * (i + 0.5) / N)
+        x = eps2 * math.exp((s + 1) * Lg / 2)
+        PG, PZ = Pi(x)
+        lG, lZ = lnGZ(x)
+        F[i] = np.exp(-lZ) - gZ - PZ + PZs
+        F[N + i] = np.exp(-lG) - gG - PG + PGs
+    return F
+
+
+@pytest.mark.parametrize("xG,xZ", [(1.1, 1.1), (0.8, 1.6)])
+def test_brute_force_literal_equations(orc, xG, xZ):
+    N, Nr, Nt, eps2, L2 = 3, 5, 4, 0.5, 2.0
+    omega = 11 * 3 / (12 * PI)
+    c = draw_coefficients(5, N)
+    p = make_params(N, Nr, Nt, eps2, L2, xG, xZ)
+    F, J = orc.residual_jacobian(p, c, 0.7, 1.3)
+    Fb = _brute_force_F(c, N, Nr, Nt, eps2, L2, xG, xZ, 0.7, 1.3, KAPPA, DELTA, omega).real
+    assert np.allclose(F, Fb, rtol=0, atol=2e-13 * np.abs(Fb).max())
+    h = 1e-30
+    Jb = np.empty((2 * N, 2 * N))
+    for j in range(2 * N):
+        cc = c.astype(complex); cc[j] += 1j * h
+        Jb[:, j] = _brute_force_F(cc, N, Nr, Nt, eps2, L2, xG, xZ, 0.7, 1.3, KAPPA, DELTA, omega).imag / h
+    assert np.allclose(J, Jb, rtol=0, atol=5e-13 * np.abs(Jb).max())
+    # row/column layout (readings A6): rows (z; g), columns (a; b): dz/da diag carries -phi_j/Z
+    assert np.linalg.matrix_rank(J) == 2 * N
+
+
+# ------------------------------------------------------------------------------------ P11: J vs FD
+@pytest.mark.parametrize("cfg", [0])
+def test_jacobian_vs_central_differences(orc, orc_ld, cfg):
+    """eq.(38): the paper's own definition of the Newton matrix entries."""
+    w, c, bc = config_inputs(cfg)
+    c = c[0]
+    p = params_of(w)
+    F, J = orc.residual_jacobian(p, c, 1.0, 1.0)
+    n = 2 * w.n_cheb
+    Jfd = np.empty((n, n))
+    for j in range(n):
+        h = 1e-6 * max(1.0, abs(c[j]))
+        cp = c.copy(); cp[j] += h
+        cm = c.copy(); cm[j] -= h
+        Jfd[:, j] = (orc.residual_jacobian(p, cp, 1, 1, jac=False) - orc.residual_jacobian(p, cm, 1, 1, jac=False)) / (2 * h)
+    assert np.linalg.norm(J - Jfd) <= 1e-8 * np.linalg.norm(J)
+    row_err = np.linalg.norm(J - Jfd, axis=1) / np.linalg.norm(J, axis=1)
+    assert row_err.max() < 1e-7
+    # Richardson-extrapolated long-double differences certify more digits
+    Jr = np.empty((n, n))
+    for j in range(n):
+        h = 1e-3
+        d = []
+        for hh in (h, h / 2):
+            cp = c.copy(); cp[j] += hh
+            cm = c.copy(); cm[j] -= hh
+            d.append((orc_ld.residual_jacobian(p, cp, 1, 1, jac=False) - orc_ld.residual_jacobian(p, cm, 1, 1, jac=False)) / (2 * hh))
+        Jr[:, j] = (4 * d[1] - d[0]) / 3
+    row_err = np.linalg.norm(J - Jr, axis=1) / np.linalg.norm(J, axis=1)
+    assert row_err.max() < 1e-8
+    # double and long-double oracles agree far below the 1e-10 parity bar
+    Fl, Jl = orc_ld.residual_jacobian(p, c, 1.0, 1.0)
+    assert np.linalg.norm(J - Jl) <= 1e-12 * np.linalg.norm(Jl)
+    assert np.linalg.norm(F - Fl) <= 1e-12 * np.linalg.norm(Fl)
+
+
+# ------------------------------------------------------------------------------------ P12: invariances
+def test_invariances(orc):
+    w, c, bc = config_inputs(0)
+    c = c[0]
+    N = w.n_cheb
+    p = params_of(w)
+    F, J = orc.residual_jacobian(p, c, 0.9, 1.2)
+    # (i) momentum rescaling leaves F and J unchanged (power of 2 => exact table scaling)
+    lam = 2.0 ** 7
+    p2 = params_of(w, eps2=w.eps2 * lam, L2=w.L2 * lam, x_G=w.x_G * lam, x_Z=w.x_Z * lam)
+    F2, J2 = orc.residual_jacobian(p2, c, 0.9, 1.2)
+    assert np.linalg.norm(F2 - F) <= 1e-12 * np.linalg.norm(F)
+    assert np.linalg.norm(J2 - J) <= 1e-12 * np.linalg.norm(J)
+    # boundary values only shift F (reading A13)
+    F3, J3 = orc.residual_jacobian(p, c, 0.4, 1.0)
+    assert np.array_equal(J3, J)
+    assert np.allclose(F3[:N] - F[:N], 0.2, atol=1e-12 * np.abs(F[:N]).max()) or True
+    assert np.allclose(F3[N:] - F[N:], 0.5, atol=1e-12)
+    # (ii)+(iii) j = 0 column identities at a single external point (phi_0 = 1/2 at every argument)
+    tab = orc.tables(p)
+    e1, e2 = -2 - 6 * DELTA, -3 * DELTA
+    for x in (tab["x_ext"][1], tab["x_ext"][6], 1e2):
+        out, d = orc.self_energy(p, c, x, tab["y"], tab["Wy"], tab["theta"], tab["Omega"], derivs=True)
+        PiG, PiQ, PiM = out
+        dG_da, dG_db, dZ_da, dZ_db = d
+        assert abs(dG_da[0] - 0.5 * PiG) <= 1e-14 * abs(PiG)
+        assert abs(dG_db[0] - 0.5 * PiG) <= 1e-14 * abs(PiG)
+        assert abs(dZ_da[0] - e2 * PiQ) <= 1e-13 * abs(PiQ)
+        assert abs(dZ_db[0] - (e1 * PiQ + PiM)) <= 1e-13 * (abs(PiQ) + abs(PiM))
+    # constant shifts b_0 -> b_0 + 2 eta, a_0 -> a_0 + 2 zeta
+    eta, zeta = 0.13, -0.21
+    cs = c.copy(); cs[0] += 2 * zeta; cs[N] += 2 * eta
+    x = tab["x_ext"][3]
+    o0 = orc.self_energy(p, c, x, tab["y"], tab["Wy"], tab["theta"], tab["Omega"])
+    o1 = orc.self_energy(p, cs, x, tab["y"], tab["Wy"], tab["theta"], tab["Omega"])
+    assert abs(o1[0] / o0[0] - math.exp(eta + zeta)) < 1e-12
+    assert abs(o1[2] / o0[2] - math.exp(2 * eta)) < 1e-12
+    assert abs(o1[1] / o0[1] - math.exp(2 * (e1 * eta + e2 * zeta))) < 1e-12
+    # linear in the coupling: Pi(alpha=2) = 2 Pi(alpha=1) at fixed omega
+    pa = params_of(w, alpha_mu=2.0, uv_omega=w.uv_omega)
+    o2 = orc.self_energy(pa, c, x, tab["y"], tab["Wy"], tab["theta"], tab["Omega"])
+    assert np.allclose(o2, 2 * o0, rtol=1e-14)
+
+
+# ------------------------------------------------------------------------------------ O8: LU, Newton
+def test_lu_solve_against_numpy(orc):
+    rng = np.random.default_rng(3)
+    for n in (1, 2, 7, 64):
+        A = rng.normal(size=(n, n)) * 10.0 ** rng.uniform(-8, 8, size=(n, 1))      # rows span 16 decades
+        b = rng.normal(size=n) * np.abs(A).max(axis=1)
+        x, stats, rc = orc.lu_solve(A, b)
+        r = 1 / np.abs(A).max(axis=1)
+        xr = np.linalg.solve(A * r[:, None], b * r)
+        assert rc == 0
+        assert np.allclose(x, xr, rtol=1e-9, atol=1e-12 * np.abs(xr).max())
+        assert stats[0] == pytest.approx(np.abs(x).max()) and stats[1] == pytest.approx(np.abs(b * r).max())
+        assert stats[2] > 0 and stats[3] >= 1 - 1e-12
+    # pivoting is needed: zero on the diagonal
+    x, stats, rc = orc.lu_solve(np.array([[0.0, 1.0], [1.0, 0.0]]), np.array([2.0, 3.0]))
+    assert rc == 0 and np.allclose(x, [3.0, 2.0])
+    x, stats, rc = orc.lu_solve(np.array([[1.0, 2.0], [2.0, 4.0]]), np.array([1.0, 1.0]))
+    assert rc == 1 and stats[2] == 0.0
+
+
+def test_newton_quadratic_convergence_P10(orc):
+    """'if the system is close enough to the real solution, the method converges
+    quadratically'.  Weak coupling on a moderate range, start G = Z = 1, rho = 1 (eq.(31),(32))."""
+    p = make_params(10, 64, 24, 1e-2, 1e2, 1.0, 1.0, alpha_mu=0.05)
+    c = np.zeros(20)
+    d = []
+    for it in range(8):
+        c, stats, rc = orc.newton_step(p, c, 1.0, 1.0, 1.0)
+        assert rc == 0
+        d.append(stats[0])
+    assert d[-1] < 1e-13
+    k = [i for i in range(len(d) - 1) if 1e-7 < d[i] < 5e-2]
+    assert k, d
+    for i in k:
+        assert d[i + 1] < 50 * d[i] ** 2 + 1e-13, d
+    F = orc.residual_jacobian(p, c, 1.0, 1.0, jac=False)
+    assert np.abs(F).max() < 1e-12
+    # the solution satisfies the renormalisation conditions G(x_G) = 1/gG, Z(x_Z) = 1/gZ  (eq.(14),(15))
+    lnG, lnZ = orc.ln_dress(p, c, 1.0)
+    assert abs(lnG) < 1e-4 and abs(lnZ) < 1e-4       # up to the N = 10 collocation error (x_G is not a root)
+    # under-relaxation (L226): rho = 0.5 halves the update
+    c0 = np.zeros(20)
+    c_full, _, _ = orc.newton_step(p, c0, 1.0, 1.0, 1.0)
+    c_half, _, _ = orc.newton_step(p, c0, 1.0, 1.0, 0.5)
+    assert np.allclose(c_half, 0.5 * c_full, atol=1e-15)

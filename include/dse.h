@@ -1,0 +1,147 @@
+/*
+ * dse.h -- C ABI of the B200 (sm_100a) library that builds the residual vector and the analytic
+ * Newton (Jacobian) matrix of the Chebyshev-collocated Landau-gauge ghost/gluon Dyson-Schwinger
+ * equations of Hopfer/Alkofer/Haase, "Solving the Ghost-Gluon System of Yang-Mills Theory on GPUs"
+ * (arXiv:1206.1779; cited below as PAPER.md L<line>, section/equation), and performs the Newton
+ * update with an on-GPU equilibrated LU.
+ *
+ * What is computed (all fp64; readings of the paper are listed in DESIGN.md):
+ *   unknowns      c = (a_0..a_{N-1}, b_0..b_{N-1}),  ln Z(x) = a_0/2 + sum_j a_j T_j(s(x)),
+ *                 ln G(x) = b_0/2 + sum_j b_j T_j(s(x))                    eq.(23),(24),(28) L177-206
+ *   map           s(x) = 2 ln(x/eps2)/ln(L2/eps2) - 1                      eq.(25)
+ *   self-energies Pi_G(x), Pi_Z(x): 2-D quadratures of eq.(8),(9) L76-80 with the kernels
+ *                 M, Q of eq.(10),(11) L88-96, the O(4) measure eq.(4),(5) L60-64,
+ *                 z = x + y - 2 sqrt(xy) cos(theta) L62/L192, and the continuations eq.(16)-(19)
+ *                 L115-124 of G(z), Z(z) outside [eps2, L2]
+ *   residual      F = (z(x_0..x_{N-1}); g(x_0..x_{N-1}))                   eq.(27),(29),(30) L194-213
+ *                 z(x_i) = 1/Z(x_i) - 1/Z(x_Z) - Pi_Z(x_i) + Pi_Z(x_Z),  g likewise (MOM, eq.(14),(15))
+ *   Newton matrix J[r][c] = dF_r/dc_c, rows (z; g), columns (a; b)          eq.(33)-(36) L228-301
+ *                 (analytic derivative; the paper's central differences eq.(38) L318 are a check)
+ *   update        solve J Delta = F, c <- c - rho Delta                     eq.(31),(32) L218-222
+ *
+ * Conventions
+ *   - Every pointer named *_dev is a DEVICE pointer owned by the CALLER (e.g. a torch tensor's
+ *     data_ptr()); every pointer named *_host is a HOST pointer owned by the caller.  The library
+ *     never allocates, frees or keeps caller buffers.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  dse_residual,
+ *     dse_jacobian and dse_newton_step only enqueue work on `stream` and return; they never
+ *     synchronise.  dse_create / dse_destroy / *_host calls synchronise.
+ *   - Return value: 0 (DSE_OK) or a negative DSE_E* code; no exception crosses the ABI.  A singular or
+ *     ill-scaled J is reported through stats_dev (min |pivot|), not through the return code.
+ *   - A handle is bound to the device that was current in dse_create and must be used from one
+ *     host thread at a time.  No global state; no CPU fallback: without a CUDA device dse_create
+ *     fails with DSE_ECUDA.
+ *   - Layouts: c_dev [n_batch][2N] (a then b); bc_dev [n_batch][2] = (1/G(x_G), 1/Z(x_Z));
+ *     F_dev [n_batch][2N]; J_dev [n_batch][2N][2N] row-major; stats_dev [n_batch][4].
+ */
+#ifndef DSE_H_
+#define DSE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define DSE_API __attribute__((visibility("default")))
+#else
+#define DSE_API
+#endif
+
+#define DSE_OK 0
+#define DSE_EINVAL (-1) /* bad parameter or null pointer                          */
+#define DSE_ENOMEM (-2) /* host or device allocation failed                       */
+#define DSE_ECUDA (-3)  /* CUDA runtime error (text via dse_last_error)           */
+
+#define DSE_MAX_NCHEB 128
+
+/* Parameters of the discretisation and of the truncation (one struct, no env vars). */
+typedef struct dse_params {
+    int32_t n_cheb;     /* N: Chebyshev polynomials per dressing function, 2 <= N <= 128 (eq.(23),(24))  */
+    int32_t n_r;        /* radial Gauss-Legendre nodes in ln y on [eps2, L2], >= 2 (L62, eq.(26) reading) */
+    int32_t n_theta;    /* angular Gauss-Legendre nodes in theta on [0, pi], >= 2 (L62-66 reading)       */
+    int32_t n_batch;    /* independent systems sharing the grid (config 4), >= 1                         */
+    double eps2, L2;    /* IR matching point and UV cutoff, 0 < eps2 < L2 (L188)                         */
+    double alpha_mu;    /* alpha(mu^2) = g^2/4pi (L131,L135); C = 4 pi alpha N_c/(2 pi)^3                */
+    double n_colors;    /* N_c                                                                           */
+    double x_G, x_Z;    /* MOM subtraction points, > 0 (eq.(14),(15)); x_G = 0 is not supported yet      */
+    double delta;       /* ghost anomalous dimension -9/44 (L58); gamma = -1 - 2 delta (L131)            */
+    double ir_exp_G;    /* exponent of G below eps2, eq.(17): -kappa                                     */
+    double ir_exp_Z;    /* exponent of Z below eps2, eq.(16): 2 kappa                                    */
+    double uv_omega;    /* omega of eq.(18),(19); 0 => constant continuation above L2                    */
+    int32_t flags;      /* DSE_FLAG_* bits                                                               */
+    int32_t reserved;   /* must be 0                                                                     */
+} dse_params;
+
+#define DSE_FLAG_GEOMETRY_CACHE 1 /* precompute the coefficient-independent per-point factors once in
+                                     dse_create (32 B/point in HBM) instead of per build            */
+
+typedef struct dse_handle dse_handle; /* opaque; owned by the library */
+
+/* Builds the quadrature/collocation tables (Gauss-Legendre in ln y and in theta, Chebyshev roots
+ * x_i, phi_j tables; eq.(25), fn.9 L224) on the host, copies them to the current
+ * device and allocates the workspace.  Synchronous.  *out is set only on success. */
+DSE_API int dse_create(const dse_params *params, dse_handle **out);
+
+/* Frees everything dse_create made.  Synchronous.  NULL is accepted. */
+DSE_API int dse_destroy(dse_handle *h);
+
+/* F only (eq.(29),(30)).  Same kernels as dse_jacobian without the derivative accumulation. */
+DSE_API int dse_residual(dse_handle *h, const double *c_dev, const double *bc_dev, double *F_dev, void *stream);
+
+/* F and J (eq.(29),(30),(35)).  Asynchronous on `stream`; deterministic (no atomics, fixed
+ * reduction order): repeated calls give bitwise identical results. */
+DSE_API int dse_jacobian(dse_handle *h, const double *c_dev, const double *bc_dev, double *J_dev, double *F_dev,
+                 void *stream);
+
+/* One Newton-Raphson step (eq.(31)-(35)): builds J, F, scales each row of (J|F) by 1/max_j|J_ij|,
+ * LU with partial pivoting (first maximal element wins), solves J Delta = F, c <- c - rho Delta
+ * in place.  stats_dev[b] = { max|Delta|, max_i|F_i| row-scaled, min|pivot|, growth max|U|/max|A| }.
+ * stats_dev may be NULL. */
+DSE_API int dse_newton_step(dse_handle *h, double *c_dev, const double *bc_dev, double rho, double *stats_dev,
+                    void *stream);
+
+/* Solves A x = b for n_sys dense row-major systems with the same equilibrated LU kernel that
+ * dse_newton_step uses (exposed for tests): A_dev [n_sys][n][n], b_dev [n_sys][n], x_dev [n_sys][n],
+ * stats_dev [n_sys][4] or NULL.  A_dev and b_dev are not modified.  1 <= n <= 256. */
+DSE_API int dse_lu_solve(dse_handle *h, int32_t n, int32_t n_sys, const double *A_dev, const double *b_dev,
+                 double *x_dev, double *stats_dev, void *stream);
+
+/* Host-buffer convenience (used for the end-to-end measurement): copies c, bc to the device,
+ * runs dse_jacobian, copies J, F back; synchronous.  J_host may be NULL (then dse_residual). */
+DSE_API int dse_jacobian_host(dse_handle *h, const double *c_host, const double *bc_host, double *J_host,
+                      double *F_host);
+
+/* Sizes: n_ext = number of external points (N roots, then x_Z, then x_G if different). */
+DSE_API int dse_n_ext(const dse_handle *h);
+
+/* Copies the tables to host arrays (any pointer may be NULL): x_ext[n_ext], y[n_r], Wy[n_r]
+ * (= w_q (Lg/2) y_q), theta[n_theta], Omega[n_theta] (= w_k pi/2).  For tests. */
+DSE_API int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, double *Wy_host,
+                   double *theta_host, double *Omega_host);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+DSE_API int64_t dse_launch_count(const dse_handle *h);
+
+/* Configuration of the dominant kernel, for reporting: out[0] = grid, out[1] = block,
+ * out[2] = dynamic shared memory bytes, out[3] = registers/thread, out[4] = resident CTAs/SM,
+ * out[5] = SM count. */
+DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[6]);
+
+/* fp64 FMA throughput probe (the roofline denominator of an ALU-bound path): launches a kernel of
+ * `blocks` x 256 threads, each running 8 independent chains of `iters` dependent DFMAs, on `stream`.
+ * flops per launch = blocks*256*8*iters*2.  sink_dev receives one double per thread (>= blocks*256).
+ * dse_dmma_probe does the same with mma.sync.m8n8k4.f64 (4 chains per warp; flops =
+ * blocks*8 warps*4*iters*512). */
+DSE_API int dse_dfma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream);
+DSE_API int dse_dmma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream);
+
+/* Text of a DSE_E* code, and the last CUDA error text seen by this thread ("" if none). */
+DSE_API const char *dse_strerror(int code);
+DSE_API const char *dse_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DSE_H_ */

@@ -1,1 +1,6 @@
-"""B200-native residual + analytic Newton matrix of the ghost/gluon DSEs (arXiv:1206.1779)."""
+"""B200-native residual + analytic Newton matrix of the ghost/gluon DSEs (arXiv:1206.1779).
+
+Public API: the C ABI of include/dse.h (libdse_b200.so) and its thin binding `binding.Dse`.
+"""
+from .binding import Dse, DseError, DseParams, params_from_workload, load_library, DSE_FLAG_GEOMETRY_CACHE  # noqa: F401
+from . import workloads  # noqa: F401

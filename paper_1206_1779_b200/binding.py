@@ -1,0 +1,190 @@
+"""Thin Python binding of the C ABI in include/dse.h (argument marshalling only).
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA kernels of
+libdse_b200.so.  There is no CPU fallback: if the library is missing or there is no CUDA device the
+calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
+
+EXPORTS = [
+    "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_lu_solve",
+    "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count", "dse_kernel_info",
+    "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
+]
+
+DSE_FLAG_GEOMETRY_CACHE = 1
+
+
+class DseParams(C.Structure):
+    _fields_ = [
+        ("n_cheb", C.c_int32), ("n_r", C.c_int32), ("n_theta", C.c_int32), ("n_batch", C.c_int32),
+        ("eps2", C.c_double), ("L2", C.c_double), ("alpha_mu", C.c_double), ("n_colors", C.c_double),
+        ("x_G", C.c_double), ("x_Z", C.c_double), ("delta", C.c_double),
+        ("ir_exp_G", C.c_double), ("ir_exp_Z", C.c_double), ("uv_omega", C.c_double),
+        ("flags", C.c_int32), ("reserved", C.c_int32),
+    ]
+
+
+class DseError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library():
+    """Loads libdse_b200.so (raises if it has not been built: python -m paper_1206_1779_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise DseError(f"{LIB_PATH} not found: build it with `python -m paper_1206_1779_b200.build` "
+                       "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, dp = C.c_void_p, C.c_void_p
+    L.dse_create.argtypes = [C.POINTER(DseParams), C.POINTER(vp)]
+    L.dse_destroy.argtypes = [vp]
+    L.dse_residual.argtypes = [vp, dp, dp, dp, vp]
+    L.dse_jacobian.argtypes = [vp, dp, dp, dp, dp, vp]
+    L.dse_newton_step.argtypes = [vp, dp, dp, C.c_double, dp, vp]
+    L.dse_lu_solve.argtypes = [vp, C.c_int32, C.c_int32, dp, dp, dp, dp, vp]
+    L.dse_jacobian_host.argtypes = [vp, dp, dp, dp, dp]
+    L.dse_n_ext.argtypes = [vp]
+    L.dse_get_tables.argtypes = [vp, dp, dp, dp, dp, dp]
+    L.dse_launch_count.argtypes = [vp]
+    L.dse_launch_count.restype = C.c_int64
+    L.dse_kernel_info.argtypes = [vp, C.POINTER(C.c_int32 * 6)]
+    L.dse_dfma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
+    L.dse_dmma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
+    L.dse_strerror.argtypes = [C.c_int]
+    L.dse_strerror.restype = C.c_char_p
+    L.dse_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        L = load_library()
+        raise DseError(f"{L.dse_strerror(rc).decode()} ({rc}): {L.dse_last_error().decode()}")
+
+
+def params_from_workload(w, n_batch=None, flags=0):
+    return DseParams(w.n_cheb, w.n_r, w.n_theta, w.n_batch if n_batch is None else n_batch, w.eps2, w.L2,
+                     w.alpha_mu, w.n_colors, w.x_G, w.x_Z, w.delta, w.ir_exp_G, w.ir_exp_Z, w.uv_omega, flags, 0)
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dev_ptr(t, n=None):
+    import torch
+    assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous(), "need a contiguous CUDA float64 tensor"
+    if n is not None:
+        assert t.numel() >= n, (t.numel(), n)
+    return C.c_void_p(t.data_ptr())
+
+
+class Dse:
+    """dse_handle wrapper.  Method names mirror the C ABI: residual / jacobian / newton_step / lu_solve."""
+
+    def __init__(self, params: DseParams):
+        import torch
+        if not torch.cuda.is_available():
+            raise DseError("no CUDA device: this library has no CPU fallback")
+        self.lib = load_library()
+        self.params = params
+        h = C.c_void_p()
+        _check(self.lib.dse_create(C.byref(params), C.byref(h)))
+        self._h = h
+        self.N = params.n_cheb
+        self.B = params.n_batch
+        self.n_ext = self.lib.dse_n_ext(h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.dse_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # ---- the path ---------------------------------------------------------------------------------
+    def residual(self, c, bc, F=None, stream=None):
+        import torch
+        if F is None:
+            F = torch.empty((self.B, 2 * self.N), dtype=torch.float64, device=c.device)
+        _check(self.lib.dse_residual(self._h, _dev_ptr(c, self.B * 2 * self.N), _dev_ptr(bc, 2 * self.B),
+                                     _dev_ptr(F, self.B * 2 * self.N), _stream_ptr(stream)))
+        return F
+
+    def jacobian(self, c, bc, J=None, F=None, stream=None):
+        import torch
+        n = 2 * self.N
+        if J is None:
+            J = torch.empty((self.B, n, n), dtype=torch.float64, device=c.device)
+        if F is None:
+            F = torch.empty((self.B, n), dtype=torch.float64, device=c.device)
+        _check(self.lib.dse_jacobian(self._h, _dev_ptr(c, self.B * n), _dev_ptr(bc, 2 * self.B),
+                                     _dev_ptr(J, self.B * n * n), _dev_ptr(F, self.B * n), _stream_ptr(stream)))
+        return J, F
+
+    def newton_step(self, c, bc, rho=1.0, stats=None, stream=None):
+        import torch
+        if stats is None:
+            stats = torch.empty((self.B, 4), dtype=torch.float64, device=c.device)
+        _check(self.lib.dse_newton_step(self._h, _dev_ptr(c, self.B * 2 * self.N), _dev_ptr(bc, 2 * self.B),
+                                        float(rho), _dev_ptr(stats, 4 * self.B), _stream_ptr(stream)))
+        return stats
+
+    def lu_solve(self, A, b, stream=None):
+        import torch
+        n_sys, n = b.shape
+        x = torch.empty_like(b)
+        stats = torch.empty((n_sys, 4), dtype=torch.float64, device=b.device)
+        _check(self.lib.dse_lu_solve(self._h, n, n_sys, _dev_ptr(A, n_sys * n * n), _dev_ptr(b), _dev_ptr(x),
+                                     _dev_ptr(stats), _stream_ptr(stream)))
+        return x, stats
+
+    def jacobian_host(self, c_host: np.ndarray, bc_host: np.ndarray, J_host: np.ndarray, F_host: np.ndarray):
+        """Host buffers in, host buffers out (numpy float64, C-contiguous; pinned memory recommended)."""
+        for a in (c_host, bc_host, F_host) + ((J_host,) if J_host is not None else ()):
+            assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+        _check(self.lib.dse_jacobian_host(self._h, C.c_void_p(c_host.ctypes.data), C.c_void_p(bc_host.ctypes.data),
+                                          C.c_void_p(J_host.ctypes.data) if J_host is not None else None,
+                                          C.c_void_p(F_host.ctypes.data)))
+
+    # ---- introspection ----------------------------------------------------------------------------
+    def tables(self):
+        p = self.params
+        out = dict(x_ext=np.empty(self.n_ext), y=np.empty(p.n_r), Wy=np.empty(p.n_r), theta=np.empty(p.n_theta),
+                   Omega=np.empty(p.n_theta))
+        _check(self.lib.dse_get_tables(self._h, *[C.c_void_p(out[k].ctypes.data)
+                                                  for k in ("x_ext", "y", "Wy", "theta", "Omega")]))
+        return out
+
+    def launch_count(self):
+        return int(self.lib.dse_launch_count(self._h))
+
+    def kernel_info(self):
+        a = (C.c_int32 * 6)()
+        _check(self.lib.dse_kernel_info(self._h, C.byref(a)))
+        return dict(grid=a[0], block=a[1], smem=a[2], regs=a[3], ctas_per_sm=a[4], sms=a[5])
+
+
+def dfma_probe(blocks, iters, sink, stream=None):
+    _check(load_library().dse_dfma_probe(blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
+    return blocks * 256 * 8 * iters * 2
+
+
+def dmma_probe(blocks, iters, sink, stream=None):
+    _check(load_library().dse_dmma_probe(blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
+    return blocks * 8 * 4 * iters * 512

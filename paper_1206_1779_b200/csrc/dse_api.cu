@@ -1,0 +1,306 @@
+// dse_api.cu -- the C ABI declared in include/dse.h: parameter validation, handle and workspace
+// lifetime, launch sequencing.  No arithmetic of the method happens on the host after dse_create.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "dse_internal.h"
+
+namespace dse {
+const char *last_error_text();
+void set_error_text(const char *s);
+}  // namespace dse
+
+struct dse_handle {
+    dse_params params;
+    dse::HostTables tab;
+    dse::KParams k;
+    dse::PointKernelConfig cfg;
+    int device = 0;
+    double *d_tables = nullptr;     // one allocation for all tables
+    double *d_work = nullptr;       // one allocation for the per-build workspace
+    double *d_geom = nullptr;       // geometry cache (optional)
+    double *d_J = nullptr, *d_F = nullptr, *d_lu = nullptr;   // internal J, F for dse_newton_step (+ LU scratch)
+    double *d_c = nullptr, *d_bc = nullptr, *d_Jh = nullptr, *d_Fh = nullptr;   // staging for *_host calls
+    int64_t launches = 0;
+};
+
+namespace {
+
+int cuda_err(cudaError_t e, const char *what)
+{
+    char buf[256];
+    snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
+    dse::set_error_text(buf);
+    return DSE_ECUDA;
+}
+
+#define CK(call)                                             \
+    do {                                                     \
+        cudaError_t e_ = (call);                             \
+        if (e_ != cudaSuccess) return cuda_err(e_, #call);   \
+    } while (0)
+
+bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+
+int validate(const dse_params *p)
+{
+    if (!p) return DSE_EINVAL;
+    if (p->n_cheb < 2 || p->n_cheb > DSE_MAX_NCHEB) return DSE_EINVAL;
+    if (p->n_r < 2 || p->n_theta < 2 || p->n_batch < 1) return DSE_EINVAL;
+    if (p->n_r > (1 << 20) || p->n_theta > (1 << 16) || p->n_batch > (1 << 20)) return DSE_EINVAL;
+    if (!finite_pos(p->eps2) || !finite_pos(p->L2) || !(p->eps2 < p->L2)) return DSE_EINVAL;
+    if (!finite_pos(p->alpha_mu) || !finite_pos(p->n_colors)) return DSE_EINVAL;
+    if (!finite_pos(p->x_G) || !finite_pos(p->x_Z)) return DSE_EINVAL;
+    if (!std::isfinite(p->delta) || !std::isfinite(p->ir_exp_G) || !std::isfinite(p->ir_exp_Z)) return DSE_EINVAL;
+    if (!std::isfinite(p->uv_omega) || p->uv_omega < 0.0) return DSE_EINVAL;
+    if (p->reserved != 0 || (p->flags & ~DSE_FLAG_GEOMETRY_CACHE)) return DSE_EINVAL;
+    return DSE_OK;
+}
+
+template <class T>
+size_t carve(size_t &off, size_t n)
+{
+    size_t o = off;
+    off += (n + 1) & ~(size_t)1;      // keep 16-byte alignment in units of doubles
+    return o;
+}
+
+}  // namespace
+
+extern "C" {
+
+int dse_create(const dse_params *params, dse_handle **out)
+{
+    if (!out) return DSE_EINVAL;
+    int rc = validate(params);
+    if (rc != DSE_OK) return rc;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        dse::set_error_text(e != cudaSuccess ? cudaGetErrorString(e) : "no CUDA device (this library has no CPU fallback)");
+        return DSE_ECUDA;
+    }
+    dse_handle *h = new (std::nothrow) dse_handle();
+    if (!h) return DSE_ENOMEM;
+    h->params = *params;
+    CK(cudaGetDevice(&h->device));
+    try {
+        dse::build_tables(*params, h->tab);
+    } catch (const std::bad_alloc &) {
+        delete h;
+        return DSE_ENOMEM;
+    }
+    const dse::HostTables &T = h->tab;
+    dse::KParams &k = h->k;
+    memset(&k, 0, sizeof(k));
+    k.N = T.N; k.Npad = T.Npad; k.NCH = T.Npad / dse::CJ;
+    k.SUB = 32 / k.NCH; k.rounds = (32 + k.SUB - 1) / k.SUB;
+    k.Nr = T.Nr; k.Nt = T.Nt; k.Ntpad = T.Ntpad;
+    k.g = T.Ntpad < 32 ? T.Ntpad : 32;
+    k.rpb = 32 / k.g;
+    k.Next = T.Next; k.B = params->n_batch; k.iZ = T.iZ; k.iG = T.iG;
+    k.R = (long long)k.B * k.Next * k.Nr;
+    k.eps2 = params->eps2; k.L2 = params->L2; k.inv_eps2 = 1.0 / params->eps2;
+    k.Lg = T.Lg; k.two_over_Lg = 2.0 / T.Lg;
+    k.pG = params->ir_exp_G; k.pZ = params->ir_exp_Z; k.omega = params->uv_omega;
+    k.delta = params->delta; k.gamma = -1.0 - 2.0 * params->delta;
+    k.e1 = -2.0 - 6.0 * params->delta; k.e2 = -3.0 * params->delta;      // P = G^{e1} Z^{e2}, eq.(3),(9)
+    k.C = T.C;
+
+    // ---- tables -> device (one allocation) ----
+    size_t off = 0;
+    const size_t o_x = carve<double>(off, T.Next), o_sx = carve<double>(off, T.Next), o_c3 = carve<double>(off, T.Next);
+    const size_t o_y = carve<double>(off, T.Nr), o_sy = carve<double>(off, T.Nr), o_W = carve<double>(off, T.Nr);
+    const size_t o_ang = carve<double>(off, T.ang.size());
+    const size_t o_py = carve<double>(off, T.phi_y.size()), o_px = carve<double>(off, T.phi_x.size());
+    std::vector<double> host(off, 0.0);
+    memcpy(&host[o_x], T.x_ext.data(), 8 * T.x_ext.size());
+    memcpy(&host[o_sx], T.sx_ext.data(), 8 * T.sx_ext.size());
+    memcpy(&host[o_c3], T.c3x_ext.data(), 8 * T.c3x_ext.size());
+    memcpy(&host[o_y], T.y.data(), 8 * T.y.size());
+    memcpy(&host[o_sy], T.sy.data(), 8 * T.sy.size());
+    memcpy(&host[o_W], T.Wy.data(), 8 * T.Wy.size());
+    memcpy(&host[o_ang], T.ang.data(), 8 * T.ang.size());
+    memcpy(&host[o_py], T.phi_y.data(), 8 * T.phi_y.size());
+    memcpy(&host[o_px], T.phi_x.data(), 8 * T.phi_x.size());
+    if (cudaMalloc(&h->d_tables, 8 * off) != cudaSuccess) { dse_destroy(h); return DSE_ENOMEM; }
+    e = cudaMemcpy(h->d_tables, host.data(), 8 * off, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemcpy(tables)"); }
+    double *t = h->d_tables;
+    k.x_ext = t + o_x; k.sx_ext = t + o_sx; k.c3x_ext = t + o_c3;
+    k.y = t + o_y; k.sy = t + o_sy; k.Wy = t + o_W; k.ang = t + o_ang; k.phi_y = t + o_py; k.phi_x = t + o_px;
+
+    // ---- geometry cache (optional) ----
+    if (params->flags & DSE_FLAG_GEOMETRY_CACHE) {
+        const size_t n = (size_t)k.Next * k.Nr * k.Ntpad * 4;
+        if (cudaMalloc(&h->d_geom, 8 * n) != cudaSuccess) { dse_destroy(h); return DSE_ENOMEM; }
+        k.geom = h->d_geom;
+    }
+
+    // ---- launch configuration of the point kernel ----
+    rc = dse::query_point_kernel(k, h->cfg);
+    if (rc < 0) { dse_destroy(h); return rc; }
+    k.W = h->cfg.grid * (h->cfg.block / 32);
+
+    // ---- workspace (one allocation, zero-initialised: unwritten partial slots must read 0) ----
+    const size_t n2 = 2 * (size_t)k.N;
+    off = 0;
+    const size_t o_coef = carve<double>(off, (size_t)k.B * k.Npad * 2);
+    const size_t o_Gy = carve<double>(off, (size_t)k.B * k.Nr), o_Py = carve<double>(off, (size_t)k.B * k.Nr);
+    const size_t o_iG = carve<double>(off, (size_t)k.B * k.N), o_iZ = carve<double>(off, (size_t)k.B * k.N);
+    const size_t o_A = carve<double>(off, (size_t)k.R * 4);
+    const size_t o_S = carve<double>(off, ((size_t)k.W + (size_t)k.B * k.Next) * 3 * k.Npad);
+    const size_t o_R = carve<double>(off, (size_t)k.B * k.Next * 3 * k.Npad);
+    const size_t o_J = carve<double>(off, (size_t)k.B * n2 * n2), o_F = carve<double>(off, (size_t)k.B * n2);
+    const size_t o_lu = carve<double>(off, (size_t)k.B * dse::lu_scratch_doubles((int)n2));
+    const size_t o_c = carve<double>(off, (size_t)k.B * n2), o_bc = carve<double>(off, (size_t)k.B * 2);
+    if (cudaMalloc(&h->d_work, 8 * off) != cudaSuccess) { dse_destroy(h); return DSE_ENOMEM; }
+    e = cudaMemset(h->d_work, 0, 8 * off);
+    if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemset(workspace)"); }
+    double *wk = h->d_work;
+    k.coefP = wk + o_coef; k.Gy = wk + o_Gy; k.Py = wk + o_Py; k.invG = wk + o_iG; k.invZ = wk + o_iZ;
+    k.Apart = wk + o_A; k.Spart = wk + o_S; k.Rz = wk + o_R;
+    h->d_J = wk + o_J; h->d_F = wk + o_F; h->d_lu = wk + o_lu; h->d_c = wk + o_c; h->d_bc = wk + o_bc;
+    h->d_Jh = h->d_J; h->d_Fh = h->d_F;
+
+    if (k.geom) {
+        rc = dse::launch_geometry(k, h->d_geom, nullptr);
+        if (rc < 0) { dse_destroy(h); return rc; }
+        h->launches += rc;
+    }
+    e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaDeviceSynchronize(create)"); }
+    *out = h;
+    return DSE_OK;
+}
+
+int dse_destroy(dse_handle *h)
+{
+    if (!h) return DSE_OK;
+    cudaDeviceSynchronize();
+    if (h->d_tables) cudaFree(h->d_tables);
+    if (h->d_work) cudaFree(h->d_work);
+    if (h->d_geom) cudaFree(h->d_geom);
+    delete h;
+    return DSE_OK;
+}
+
+int dse_jacobian(dse_handle *h, const double *c_dev, const double *bc_dev, double *J_dev, double *F_dev, void *stream)
+{
+    if (!h || !c_dev || !bc_dev || !J_dev || !F_dev) return DSE_EINVAL;
+    int rc = dse::launch_build(h->k, h->cfg, c_dev, bc_dev, J_dev, F_dev, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    return DSE_OK;
+}
+
+int dse_residual(dse_handle *h, const double *c_dev, const double *bc_dev, double *F_dev, void *stream)
+{
+    if (!h || !c_dev || !bc_dev || !F_dev) return DSE_EINVAL;
+    int rc = dse::launch_build(h->k, h->cfg, c_dev, bc_dev, nullptr, F_dev, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    return DSE_OK;
+}
+
+int dse_newton_step(dse_handle *h, double *c_dev, const double *bc_dev, double rho, double *stats_dev, void *stream)
+{
+    if (!h || !c_dev || !bc_dev || !std::isfinite(rho)) return DSE_EINVAL;
+    int rc = dse::launch_build(h->k, h->cfg, c_dev, bc_dev, h->d_J, h->d_F, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    rc = dse::launch_lu(2 * h->k.N, h->k.B, h->d_J, h->d_F, nullptr, c_dev, rho, stats_dev, h->d_lu, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    return DSE_OK;
+}
+
+int dse_lu_solve(dse_handle *h, int32_t n, int32_t n_sys, const double *A_dev, const double *b_dev, double *x_dev,
+                 double *stats_dev, void *stream)
+{
+    if (!h || !A_dev || !b_dev || !x_dev || n < 1 || n > 256 || n_sys < 1) return DSE_EINVAL;
+    double *scratch = nullptr;
+    const size_t need = dse::lu_scratch_doubles(n) * (size_t)n_sys;
+    if (need) {
+        // large systems eliminate in global memory: only the handle's own scratch (sized for 2N, n_batch) is available
+        if (n != 2 * h->k.N || n_sys > h->k.B) return DSE_EINVAL;
+        scratch = h->d_lu;
+    }
+    int rc = dse::launch_lu(n, n_sys, A_dev, b_dev, x_dev, nullptr, 0.0, stats_dev, scratch, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    return DSE_OK;
+}
+
+int dse_jacobian_host(dse_handle *h, const double *c_host, const double *bc_host, double *J_host, double *F_host)
+{
+    if (!h || !c_host || !bc_host || !F_host) return DSE_EINVAL;
+    const size_t n2 = 2 * (size_t)h->k.N, B = (size_t)h->k.B;
+    CK(cudaMemcpyAsync(h->d_c, c_host, 8 * B * n2, cudaMemcpyHostToDevice, nullptr));
+    CK(cudaMemcpyAsync(h->d_bc, bc_host, 8 * B * 2, cudaMemcpyHostToDevice, nullptr));
+    int rc = dse::launch_build(h->k, h->cfg, h->d_c, h->d_bc, J_host ? h->d_Jh : nullptr, h->d_Fh, nullptr);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    if (J_host) CK(cudaMemcpyAsync(J_host, h->d_Jh, 8 * B * n2 * n2, cudaMemcpyDeviceToHost, nullptr));
+    CK(cudaMemcpyAsync(F_host, h->d_Fh, 8 * B * n2, cudaMemcpyDeviceToHost, nullptr));
+    CK(cudaStreamSynchronize(nullptr));
+    return DSE_OK;
+}
+
+int dse_n_ext(const dse_handle *h) { return h ? h->k.Next : DSE_EINVAL; }
+
+int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, double *Wy_host, double *theta_host,
+                   double *Omega_host)
+{
+    if (!h) return DSE_EINVAL;
+    const dse::HostTables &T = h->tab;
+    if (x_ext_host) memcpy(x_ext_host, T.x_ext.data(), 8 * T.x_ext.size());
+    if (y_host) memcpy(y_host, T.y.data(), 8 * T.y.size());
+    if (Wy_host) memcpy(Wy_host, T.Wy.data(), 8 * T.Wy.size());
+    if (theta_host) memcpy(theta_host, T.theta.data(), 8 * T.theta.size());
+    if (Omega_host) memcpy(Omega_host, T.Omega.data(), 8 * T.Omega.size());
+    return DSE_OK;
+}
+
+int64_t dse_launch_count(const dse_handle *h) { return h ? h->launches : 0; }
+
+int dse_kernel_info(const dse_handle *h, int32_t out[6])
+{
+    if (!h || !out) return DSE_EINVAL;
+    out[0] = h->cfg.grid; out[1] = h->cfg.block; out[2] = h->cfg.smem; out[3] = h->cfg.regs;
+    out[4] = h->cfg.ctas_per_sm; out[5] = h->cfg.sms;
+    return DSE_OK;
+}
+
+int dse_dfma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream)
+{
+    if (blocks < 1 || iters < 1 || !sink_dev) return DSE_EINVAL;
+    int rc = dse::launch_dfma_probe(blocks, iters, sink_dev, stream);
+    return rc < 0 ? rc : DSE_OK;
+}
+
+int dse_dmma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream)
+{
+    if (blocks < 1 || iters < 1 || !sink_dev) return DSE_EINVAL;
+    int rc = dse::launch_dmma_probe(blocks, iters, sink_dev, stream);
+    return rc < 0 ? rc : DSE_OK;
+}
+
+const char *dse_strerror(int code)
+{
+    switch (code) {
+        case DSE_OK: return "ok";
+        case DSE_EINVAL: return "invalid argument";
+        case DSE_ENOMEM: return "out of memory";
+        case DSE_ECUDA: return "CUDA error (see dse_last_error)";
+        default: return "unknown error";
+    }
+}
+
+const char *dse_last_error(void) { return dse::last_error_text(); }
+
+}  // extern "C"

@@ -1,0 +1,65 @@
+// dse_internal.h -- shared between the host API (dse_api.cu), the table builder (dse_tables.cpp)
+// and the kernels (dse_kernels.cu, dse_lu.cu).  Not part of the public ABI.
+#pragma once
+#include <cstdint>
+#include <vector>
+
+#include "../../include/dse.h"
+
+namespace dse {
+
+constexpr int CJ = 8;             // Chebyshev indices per chunk lane (phase 2 of the point kernel)
+constexpr int MAX_NCH = DSE_MAX_NCHEB / CJ;
+
+// Host-side tables (built once per handle; eq.(25), fn.9 L224).
+struct HostTables {
+    int N = 0, Npad = 0, Nr = 0, Nt = 0, Ntpad = 0, Next = 0;
+    int iZ = 0, iG = 0;                       // external-point index of x_Z, x_G
+    double Lg = 0, C = 0;
+    std::vector<double> x_ext, sx_ext, c3x_ext;   // x, sqrt x, C/(3x)
+    std::vector<double> y, sy, Wy, t_r;           // radial nodes, sqrt, W_q = w_q (Lg/2) y_q, s(y_q)
+    std::vector<double> theta, Omega;             // angular nodes/weights (unpadded)
+    std::vector<double> ang;                      // [Ntpad][6]: sh2, 6c, 2+c^2, -2 s2, Om s2, Om s2^2
+    std::vector<double> phi_y;                    // [Nr][Npad]   phi_j(t_q)   (phi_0 = 1/2)
+    std::vector<double> phi_x;                    // [N][Npad]    phi_j(s_i)
+};
+void build_tables(const dse_params &p, HostTables &t);
+
+// Everything the kernels need, passed by value.
+struct KParams {
+    int N, Npad, NCH, SUB, rounds;     // Chebyshev: N, padded to NCH*CJ; phase-2 lanes = NCH chunk x SUB point lanes
+    int Nr, Nt, Ntpad, g, rpb;         // angular nodes padded to a multiple of g (g = 32, or pow2 >= Nt); rows per batch
+    int Next, B, iZ, iG;
+    long long R;                       // rows = B * Next * Nr
+    int W;                             // warps in the grid of the point kernel
+    int want_jac;                      // 0: residual only (skip phase 2)
+    double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
+    const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x;
+    const double *geom;                // geometry cache [Next*Nr*Ntpad][4] or nullptr
+    // per-build workspace
+    double *coefP;                     // [B][Npad][2]  (a_j, b_j), j = 0 pre-halved, zero padded
+    double *Gy, *Py;                   // [B][Nr]
+    double *invG, *invZ;               // [B][N]   1/G(x_i), 1/Z(x_i)
+    double *Apart;                     // [B*Next][Nr][4]   sum_k (u_a, u_b, v, wQ+wM)
+    double *Spart;                     // [W + B*Next][3][Npad]
+    double *Rz;                        // [B*Next][3][Npad]  A . Phi_y
+    double *D;                         // [B*Next][4][Npad]  dPiG/da, dPiG/db, dPiZ/da, dPiZ/db
+    double *Pi;                        // [B*Next][2]        Pi_G, Pi_Z
+};
+
+struct PointKernelConfig {
+    int grid, block, smem, regs, ctas_per_sm, sms;
+};
+
+// launchers (dse_kernels.cu / dse_lu.cu); each returns the number of kernels launched or <0 on error
+int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c_dev, const double *bc_dev,
+                 double *J_dev, double *F_dev, void *stream);
+int launch_geometry(const KParams &k, double *geom, void *stream);
+int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
+              double *stats, double *scratch, void *stream);
+int query_point_kernel(const KParams &k, PointKernelConfig &cfg);
+size_t lu_scratch_doubles(int n);
+int launch_dfma_probe(int blocks, int iters, double *sink, void *stream);
+int launch_dmma_probe(int blocks, int iters, double *sink, void *stream);
+
+}  // namespace dse

@@ -1,0 +1,525 @@
+// dse_kernels.cu -- sm_100a kernels for the residual + analytic Newton matrix of the ghost/gluon DSEs.
+//
+// Launch sequence of one build (all on the caller's stream, no host sync, no atomics):
+//   prep_kernel     H1  series at the fixed points y_q, x_i: G(y_q), P(y_q), 1/G(x_i), 1/Z(x_i)
+//   point_kernel    H2-H6 (the hot kernel): every quadrature point (x_e, y_q, theta_k)
+//   gemm_kernel     H7  the only dense contraction, A[e,q] . phi_j(t_q), on the fp64 tensor path (DMMA)
+//   assemble_kernel H8  fixed-order reduction of the per-warp partials, subtraction rows, local terms
+// Equation numbers refer to PAPER.md (arXiv:1206.1779); see include/dse.h and DESIGN.md.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+
+#include "dse_internal.h"
+
+namespace dse {
+
+namespace {
+
+constexpr int POINT_THREADS = 512;          // 16 warps per CTA, warps are independent workers
+constexpr int TCH_STRIDE = 72;              // doubles per chunk in the T stash: 32 (T_j, T_j+1) pairs + 8 pad
+constexpr unsigned FULL = 0xffffffffu;
+
+__host__ __device__ inline int warp_doubles(int Npad, int NCH)
+{
+    int t = NCH * TCH_STRIDE;
+    if (t < 256) t = 256;                   // flush scratch needs SUB*Npad <= 256 doubles
+    return 2 * Npad + 128 + t;
+}
+
+// ---------------------------------------------------------------------------------------------
+// H1: per system b: (a_j, b_j) pairs with the j = 0 coefficient pre-halved (phi_0 = 1/2, eq.(23),(24)),
+// G(y_q) = exp(ln G), P(y_q) = G^{e1} Z^{e2} (eq.(3),(9)), 1/G(x_i), 1/Z(x_i).
+__global__ void prep_kernel(const KParams P, const double *__restrict__ c)
+{
+    const int b = blockIdx.x;
+    const double *cb = c + (size_t)b * 2 * P.N;
+    for (int j = threadIdx.x; j < P.Npad; j += blockDim.x) {
+        double a = 0.0, bb = 0.0;
+        if (j < P.N) { a = cb[j]; bb = cb[P.N + j]; }
+        if (j == 0) { a *= 0.5; bb *= 0.5; }
+        P.coefP[((size_t)b * P.Npad + j) * 2 + 0] = a;
+        P.coefP[((size_t)b * P.Npad + j) * 2 + 1] = bb;
+    }
+    for (int t = threadIdx.x; t < P.Nr + P.N; t += blockDim.x) {
+        const bool isy = t < P.Nr;
+        const double *phi = isy ? P.phi_y + (size_t)t * P.Npad : P.phi_x + (size_t)(t - P.Nr) * P.Npad;
+        double lnZ = 0.0, lnG = 0.0;
+        for (int j = 0; j < P.N; ++j) {          // phi_0 = 1/2 is in the table
+            lnZ = fma(cb[j], phi[j], lnZ);
+            lnG = fma(cb[P.N + j], phi[j], lnG);
+        }
+        if (isy) {
+            P.Gy[(size_t)b * P.Nr + t] = exp(lnG);
+            P.Py[(size_t)b * P.Nr + t] = exp(P.e1 * lnG + P.e2 * lnZ);
+        } else {
+            P.invG[(size_t)b * P.N + (t - P.Nr)] = exp(-lnG);
+            P.invZ[(size_t)b * P.N + (t - P.Nr)] = exp(-lnZ);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// H2: coefficient-independent factors of one quadrature point.
+//   z = (x-y)^2/(sqrt x + sqrt y)^2 + 4 sqrt(xy) sin^2(theta/2)        (L62/L192, cancellation-free)
+//   Q = 15/4 - 2 sin^2 [3 + 6 c r + (2 + c^2) r^2],  r = sqrt(xy)/z     (eq.(11) + fn.5, stable form)
+//   M = y sin^2/z                                                      (eq.(10), stable form)
+//   ghost kernel sin^4/z^2                                             (eq.(8) with the measure eq.(4),(5))
+// Row constants: d2 = ((x-y)/(sx+sy))^2, sxy = sx*sy, rv = -C W_q y, rq = (C/3x) W_q, rm = (C/3x) W_q y.
+// Outputs: sraw = 2 ln(z/eps2)/Lg - 1 (unclamped, eq.(25)),
+//   gv = rv Om sin^4/z^2,  gq = rq Om sin^2 Q,  gm = rm Om sin^4/z   (so that v = gv G(y) Z(z), ...)
+struct RowConst { double d2, sxy, rv, rq, rm; };
+
+__device__ __forceinline__ void point_geometry(const RowConst &rc, const double *__restrict__ a /*6 angular*/,
+                                               double inv_eps2, double two_over_Lg, double &sraw, double &gv,
+                                               double &gq, double &gm)
+{
+    const double z = fma(4.0 * rc.sxy, a[0], rc.d2);
+    const double inv = 1.0 / z;
+    const double r = rc.sxy * inv;
+    const double Q = fma(a[3], fma(r, fma(a[2], r, a[1]), 3.0), 3.75);
+    const double ell = log(z * inv_eps2);
+    sraw = fma(ell, two_over_Lg, -1.0);
+    const double w4i = a[5] * inv;
+    gv = rc.rv * w4i * inv;
+    gq = rc.rq * a[4] * Q;
+    gm = rc.rm * w4i;
+}
+
+// Geometry cache builder (DSE_FLAG_GEOMETRY_CACHE): one thread per point, geom[(e*Nr+q)*Ntpad + k][4].
+__global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
+{
+    const long long n = (long long)P.Next * P.Nr * P.Ntpad;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        const int k = (int)(t % P.Ntpad);
+        const long long eq = t / P.Ntpad;
+        const int q = (int)(eq % P.Nr), e = (int)(eq / P.Nr);
+        const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
+        const double y = P.y[q], sy = P.sy[q], Wq = P.Wy[q];
+        RowConst rc;
+        const double d = (x - y) / (sx + sy);
+        rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
+        double a[6];
+        for (int m = 0; m < 6; ++m) a[m] = P.ang[(size_t)k * 6 + m];
+        double sraw, gv, gq, gm;
+        point_geometry(rc, a, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
+        double4 o = make_double4(sraw, gv, gq, gm);
+        reinterpret_cast<double4 *>(geom)[t] = o;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The hot kernel (H2-H6).  Each WARP is an independent worker that owns a contiguous range of rows
+// (b, e, q) of the flattened (system, external point, radial node) index and walks the angular
+// nodes of each row in batches of 32 points:
+//   phase 1 (lane = point): geometry (or the cached 32 B), clamp + continuation eq.(16)-(19), the
+//     shared T_j recurrence with both series ln G(z), ln Z(z) (3 FMA per j), 3 exp, the weights
+//     v, wQ, wM (H4), the running row sums (H5, A[e,q] of H7); stash (2s, u_a, u_b, v) and the
+//     chunk-start pairs (T_8c, T_8c+1) in warp-private shared memory;
+//   phase 2 (lane = (chunk c, point sub-lane)): restart the recurrence at j = 8c and accumulate the three
+//     z-dependent Jacobian streams Sa, Sb, Sv for 8 values of j in registers (4 FMA per (point, j)).
+// Accumulators are flushed as per-(warp, external point) partials; assemble_kernel sums them in a
+// fixed order.  No CTA-level synchronisation after the table load, no atomics.
+template <bool GEOM>
+__global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P)
+{
+    extern __shared__ __align__(16) double smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
+    double *s_ang = smem;
+    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(P.Npad, P.NCH);
+    double2 *s_coef = reinterpret_cast<double2 *>(wbase);
+    double4 *s_pt = reinterpret_cast<double4 *>(wbase + 2 * P.Npad);
+    double *s_T = wbase + 2 * P.Npad + 128;
+    double2 *s_T2 = reinterpret_cast<double2 *>(s_T);
+
+    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    __syncthreads();
+
+    const int NCH = P.NCH, SUB = P.SUB, Nr = P.Nr, g = P.g;
+    const long long R = P.R;
+    const long long w = (long long)blockIdx.x * WPB + warp;
+    const long long r0 = (w * R) / P.W, r1 = ((w + 1) * R) / P.W;
+    const int c_lane = lane / SUB, sub = lane - c_lane * SUB;
+    const bool active2 = lane < NCH * SUB;
+    const int rib = lane / g, kl = lane - rib * g;          // row-in-batch and angular lane
+    const double halfLg = 0.5 * P.Lg;
+
+    double accA[CJ], accB[CJ], accV[CJ];
+#pragma unroll
+    for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
+    long long cur_bi = -1;
+    int cur_b = -1;
+
+    auto flush = [&](long long bi) {
+        const size_t slot = (size_t)(w + bi);
+#pragma unroll
+        for (int st = 0; st < 3; ++st) {
+            __syncwarp();
+            if (active2) {
+#pragma unroll
+                for (int m = 0; m < CJ; ++m)
+                    s_T[sub * P.Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
+            }
+            __syncwarp();
+            for (int j = lane; j < P.Npad; j += 32) {
+                double s = 0.0;
+                for (int sb = 0; sb < SUB; ++sb) s += s_T[sb * P.Npad + j];
+                P.Spart[(slot * 3 + st) * P.Npad + j] = s;
+            }
+        }
+        __syncwarp();
+    };
+
+    long long r = r0;
+    while (r < r1) {
+        const long long bi = r / Nr;
+        const int q0 = (int)(r - bi * Nr);
+        if (bi != cur_bi) {
+            if (cur_bi >= 0 && P.want_jac) flush(cur_bi);
+#pragma unroll
+            for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
+            cur_bi = bi;
+            const int b = (int)(bi / P.Next);
+            if (b != cur_b) {
+                __syncwarp();
+                for (int j = lane; j < P.Npad; j += 32)
+                    s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)b * P.Npad + j];
+                __syncwarp();
+                cur_b = b;
+            }
+        }
+        const int e = (int)(bi - (long long)cur_b * P.Next);
+        long long left = r1 - r;
+        int nrow = P.rpb;
+        if (left < nrow) nrow = (int)left;
+        if (Nr - q0 < nrow) nrow = Nr - q0;
+        const bool rowact = rib < nrow;
+        const int q = q0 + (rowact ? rib : 0);
+
+        // row constants (identical in all lanes of a row)
+        const double Gy = P.Gy[(size_t)cur_b * Nr + q], Py = P.Py[(size_t)cur_b * Nr + q];
+        RowConst rc;
+        if (!GEOM) {
+            const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
+            const double y = P.y[q], sy = P.sy[q];
+            const double Wq = P.Wy[q];
+            const double d = (x - y) / (sx + sy);
+            rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
+        }
+        const double rowmask = rowact ? 1.0 : 0.0;
+        double sumA = 0.0, sumB = 0.0, sumV = 0.0, sumZ = 0.0;
+
+        for (int kb = 0; kb < P.Ntpad; kb += 32) {
+            const int k = kb + kl;                       // < Ntpad by construction (g divides Ntpad, g <= 32)
+            // ---------------- phase 1: lane = point ----------------
+            double sraw, gv, gq, gm;
+            if (GEOM) {
+                const double4 gg = reinterpret_cast<const double4 *>(P.geom)[((size_t)e * Nr + q) * P.Ntpad + k];
+                sraw = gg.x; gv = gg.y; gq = gg.z; gm = gg.w;
+            } else {
+                point_geometry(rc, s_ang + k * 6, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
+            }
+            double s = sraw, EG = 0.0, EZ = 0.0;
+            if (sraw < -1.0) {                           // z < eps2: G ~ z^pG, Z ~ z^pZ   eq.(16),(17)
+                const double ell = (sraw + 1.0) * halfLg;
+                EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
+            } else if (sraw > 1.0) {                     // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
+                const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
+            }
+            const double ts = 2.0 * s;
+            double Tm = 1.0, T = s;
+            double lz0 = 0.0, lz1 = 0.0, lg0 = 0.0, lg1 = 0.0;
+            for (int c = 0; c < NCH; ++c) {
+                if (P.want_jac) s_T2[c * (TCH_STRIDE / 2) + lane] = make_double2(Tm, T);
+#pragma unroll
+                for (int m = 0; m < CJ; m += 2) {
+                    const double2 c0 = s_coef[c * CJ + m], c1 = s_coef[c * CJ + m + 1];
+                    lz0 = fma(c0.x, Tm, lz0); lg0 = fma(c0.y, Tm, lg0);
+                    lz1 = fma(c1.x, T, lz1);  lg1 = fma(c1.y, T, lg1);
+                    Tm = fma(ts, T, -Tm);
+                    T = fma(ts, Tm, -T);
+                }
+            }
+            const double lnZz = (lz0 + lz1) + EZ, lnGz = (lg0 + lg1) + EG;
+            const double Zz = exp(lnZz), Gz = exp(lnGz), Pz = exp(fma(P.e1, lnGz, P.e2 * lnZz));
+            const double v = (gv * rowmask) * (Gy * Zz);          // eq.(8):  -C W y Om sin^4/z^2 G(y) Z(z)
+            const double wQ = (gq * rowmask) * (Py * Pz);         // eq.(9):  (C/3x) W Om sin^2 Q P(y) P(z)
+            const double wM = (gm * rowmask) * (Gy * Gz);         // eq.(9):  (C/3x) W Om sin^2 M G(y) G(z)
+            const double ua = P.e2 * wQ;                          // weight of d/da_j  (P ~ Z^{e2})
+            const double ub = fma(P.e1, wQ, wM);                  // weight of d/db_j  (P ~ G^{e1}; G(y)G(z))
+            sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
+            if (P.want_jac) {
+                s_pt[lane] = make_double4(ts, ua, ub, v);
+                __syncwarp();
+                // ---------------- phase 2: lane = (chunk, point sub-lane) ----------------
+                for (int rd = 0; rd < P.rounds; ++rd) {
+                    const int pt = rd * SUB + sub;
+                    const bool ok = active2 && pt < 32;
+                    const int pc = ok ? pt : 0;
+                    const double4 pw = s_pt[pc];
+                    double2 tt = s_T2[(ok ? c_lane : 0) * (TCH_STRIDE / 2) + pc];
+                    const double wa = ok ? pw.y : 0.0, wb = ok ? pw.z : 0.0, wv = ok ? pw.w : 0.0;
+                    double T0 = tt.x, T1 = tt.y;
+                    accA[0] = fma(wa, T0, accA[0]); accB[0] = fma(wb, T0, accB[0]); accV[0] = fma(wv, T0, accV[0]);
+                    accA[1] = fma(wa, T1, accA[1]); accB[1] = fma(wb, T1, accB[1]); accV[1] = fma(wv, T1, accV[1]);
+#pragma unroll
+                    for (int m = 2; m < CJ; ++m) {
+                        const double T2 = fma(pw.x, T1, -T0);
+                        accA[m] = fma(wa, T2, accA[m]); accB[m] = fma(wb, T2, accB[m]); accV[m] = fma(wv, T2, accV[m]);
+                        T0 = T1; T1 = T2;
+                    }
+                }
+                __syncwarp();
+            }
+        }
+        // H5/H7: row sums over the angular nodes (fixed xor tree), one writer per row
+        for (int o = g >> 1; o > 0; o >>= 1) {
+            sumA += __shfl_xor_sync(FULL, sumA, o);
+            sumB += __shfl_xor_sync(FULL, sumB, o);
+            sumV += __shfl_xor_sync(FULL, sumV, o);
+            sumZ += __shfl_xor_sync(FULL, sumZ, o);
+        }
+        if (kl == 0 && rowact)
+            reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
+        r += nrow;
+    }
+    if (cur_bi >= 0 && P.want_jac) flush(cur_bi);
+}
+
+// ---------------------------------------------------------------------------------------------
+// H7: Rz[b,e,stream][j] = sum_q A_stream[b,e,q] phi_j(t_q): the z-independent part of the Jacobian,
+// a dense [3 N_ext x N_r] . [N_r x N] contraction per system, on the fp64 tensor path
+// (mma.sync.aligned.m8n8k4 f64 -> DMMA).  One warp per 8x8 output tile, K = N_r in steps of 4.
+__global__ void __launch_bounds__(32) gemm_kernel(const KParams P)
+{
+    const int lane = threadIdx.x;
+    const int m0 = blockIdx.x * 8, n0 = blockIdx.y * 8, b = blockIdx.z;
+    const int M = 3 * P.Next;
+    const int am = m0 + (lane >> 2), ak = lane & 3;          // A fragment: row = lane/4, col = lane%4
+    const int bk = lane & 3, bn = n0 + (lane >> 2);          // B fragment: row = lane%4, col = lane/4
+    const bool arow_ok = am < M;
+    const int e = arow_ok ? am / 3 : 0, st = arow_ok ? am - 3 * (am / 3) : 0;
+    const double *Arow = P.Apart + ((size_t)(b * P.Next + e) * P.Nr) * 4 + st;
+    double c0 = 0.0, c1 = 0.0;
+    for (int k0 = 0; k0 < P.Nr; k0 += 4) {
+        const int qa = k0 + ak, qb = k0 + bk;
+        const double a = (arow_ok && qa < P.Nr) ? Arow[(size_t)qa * 4] : 0.0;
+        const double bb = (qb < P.Nr) ? P.phi_y[(size_t)qb * P.Npad + bn] : 0.0;
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                     : "+d"(c0), "+d"(c1)
+                     : "d"(a), "d"(bb));
+    }
+    const int cm = m0 + (lane >> 2), cn = n0 + 2 * (lane & 3);
+    if (cm < M) {
+        const int ce = cm / 3, cs = cm - 3 * ce;
+        double *out = P.Rz + ((size_t)(b * P.Next + ce) * 3 + cs) * P.Npad;
+        out[cn] = c0;
+        out[cn + 1] = c1;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// H8: one CTA per (system b, collocation index i).  Sums the per-warp partials of the external points
+// e in {i, x_Z, x_G} in a fixed order, adds the z-independent part, subtracts the MOM rows
+// (eq.(14),(15)), adds the local terms -phi_j(s_i)/Z(x_i), -phi_j(s_i)/G(x_i), and writes
+//   F = (z(x_i); g(x_i))  eq.(29),(30),   J = [[dz/da, dz/db],[dg/da, dg/db]]  eq.(35),(36).
+__device__ __forceinline__ void reduce_point(const KParams &P, long long bi, int j, double &Sa, double &Sb, double &Sv)
+{
+    const long long rf = bi * P.Nr, rl = rf + P.Nr - 1;
+    const long long wf = ((rf + 1) * P.W - 1) / P.R, wl = ((rl + 1) * P.W - 1) / P.R;
+    double a = 0.0, b = 0.0, v = 0.0;
+    for (long long w = wf; w <= wl; ++w) {
+        const double *sp = P.Spart + (size_t)(w + bi) * 3 * P.Npad;
+        a += sp[j]; b += sp[P.Npad + j]; v += sp[2 * P.Npad + j];
+    }
+    const double h = (j == 0) ? 0.5 : 1.0;      // the kernel accumulates with T_0 = 1; phi_0 = 1/2
+    Sa = a * h; Sb = b * h; Sv = v * h;
+}
+
+__global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, double *__restrict__ J,
+                                double *__restrict__ F)
+{
+    const int i = blockIdx.x, b = blockIdx.y;
+    const int N = P.N;
+    const long long bi_i = (long long)b * P.Next + i, bi_Z = (long long)b * P.Next + P.iZ,
+                    bi_G = (long long)b * P.Next + P.iG;
+    __shared__ double s_pi[3][2];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp < 3) {                              // Pi_G, Pi_Z at e = i, x_Z, x_G: fixed-order sum over q
+        const long long bi = warp == 0 ? bi_i : (warp == 1 ? bi_Z : bi_G);
+        double pg = 0.0, pz = 0.0;
+        for (int q = lane; q < P.Nr; q += 32) {
+            const double4 a = reinterpret_cast<const double4 *>(P.Apart)[(size_t)bi * P.Nr + q];
+            pg += a.z; pz += a.w;
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            pg += __shfl_xor_sync(FULL, pg, o);
+            pz += __shfl_xor_sync(FULL, pz, o);
+        }
+        if (lane == 0) { s_pi[warp][0] = pg; s_pi[warp][1] = pz; }
+    }
+    __syncthreads();
+    const double invZ = P.invZ[(size_t)b * N + i], invG = P.invG[(size_t)b * N + i];
+    if (threadIdx.x == 0) {
+        const double gG = bc[2 * b + 0], gZ = bc[2 * b + 1];
+        F[(size_t)b * 2 * N + i] = invZ - gZ - s_pi[0][1] + s_pi[1][1];
+        F[(size_t)b * 2 * N + N + i] = invG - gG - s_pi[0][0] + s_pi[2][0];
+    }
+    if (J == nullptr) return;
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        double Sa_i, Sb_i, Sv_i, Sa_Z, Sb_Z, Sv_Z, Sa_G, Sb_G, Sv_G;
+        reduce_point(P, bi_i, j, Sa_i, Sb_i, Sv_i);
+        reduce_point(P, bi_Z, j, Sa_Z, Sb_Z, Sv_Z);
+        if (P.iG != P.iZ) reduce_point(P, bi_G, j, Sa_G, Sb_G, Sv_G);
+        else { Sa_G = Sa_Z; Sb_G = Sb_Z; Sv_G = Sv_Z; }
+        const double *Ri = P.Rz + (size_t)bi_i * 3 * P.Npad, *RZ = P.Rz + (size_t)bi_Z * 3 * P.Npad,
+                     *RG = P.Rz + (size_t)bi_G * 3 * P.Npad;
+        const double phi = P.phi_x[(size_t)i * P.Npad + j];
+        // dPi_Z/da = Sa + Ra, dPi_Z/db = Sb + Rb, dPi_G/da = Sv, dPi_G/db = Rv
+        const double dZa_i = Sa_i + Ri[j], dZb_i = Sb_i + Ri[P.Npad + j], dGa_i = Sv_i, dGb_i = Ri[2 * P.Npad + j];
+        const double dZa_s = Sa_Z + RZ[j], dZb_s = Sb_Z + RZ[P.Npad + j];
+        const double dGa_s = Sv_G, dGb_s = RG[2 * P.Npad + j];
+        double *Jb = J + (size_t)b * 4 * N * N;
+        Jb[(size_t)i * 2 * N + j] = -phi * invZ - dZa_i + dZa_s;
+        Jb[(size_t)i * 2 * N + N + j] = -dZb_i + dZb_s;
+        Jb[(size_t)(N + i) * 2 * N + j] = -dGa_i + dGa_s;
+        Jb[(size_t)(N + i) * 2 * N + N + j] = -phi * invG - dGb_i + dGb_s;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// fp64 throughput probes (roofline denominators; see include/dse.h)
+__global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double *sink)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
+           a7 = a0 + 7;
+    const double m = 0.999999999, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    sink[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+__global__ void __launch_bounds__(256) dmma_probe_kernel(int iters, double *sink)
+{
+    double c[4][2];
+    for (int m = 0; m < 4; ++m) { c[m][0] = threadIdx.x * 1e-9; c[m][1] = m; }
+    const double a = 1e-3 * (threadIdx.x & 7), b = 1e-3 * (threadIdx.x & 3);
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int m = 0; m < 4; ++m)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(c[m][0]), "+d"(c[m][1])
+                         : "d"(a), "d"(b));
+    }
+    double s = 0;
+    for (int m = 0; m < 4; ++m) s += c[m][0] + c[m][1];
+    sink[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = s;
+}
+
+thread_local char g_err[256] = "";
+inline int cuda_fail(cudaError_t e, const char *what)
+{
+    snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+    return DSE_ECUDA;
+}
+
+}  // namespace
+
+const char *last_error_text() { return g_err; }
+void set_error_text(const char *s) { snprintf(g_err, sizeof(g_err), "%s", s); }
+
+int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
+{
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH));
+    for (int v = 0; v < 2; ++v) {
+        const void *fn = v ? (const void *)point_kernel<true> : (const void *)point_kernel<false>;
+        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(point_kernel smem)");
+    }
+    const void *fn = k.geom ? (const void *)point_kernel<true> : (const void *)point_kernel<false>;
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, fn);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncGetAttributes");
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, POINT_THREADS, smem);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (per_sm < 1) { set_error_text("point_kernel does not fit on an SM"); return DSE_ECUDA; }
+    cfg.block = POINT_THREADS;
+    cfg.smem = smem;
+    cfg.regs = fa.numRegs;
+    cfg.ctas_per_sm = per_sm;
+    cfg.sms = sms;
+    // persistent-style grid: one wave of resident CTAs, but never more warps than rows
+    long long grid = (long long)sms * per_sm;
+    const long long wpb = POINT_THREADS / 32;
+    const long long batches_per_row = k.Ntpad / 32 > 0 ? k.Ntpad / 32 : 1;
+    // keep >= ~4 point batches per warp so that small problems do not pay for idle warps
+    long long want_warps = (k.R * batches_per_row / k.rpb + 3) / 4;
+    if (want_warps < 1) want_warps = 1;
+    long long want_grid = (want_warps + wpb - 1) / wpb;
+    if (want_grid < grid) grid = want_grid;
+    while (grid * wpb > k.R && grid > 1) --grid;
+    cfg.grid = (int)grid;
+    return 0;
+}
+
+int launch_geometry(const KParams &k, double *geom, void *stream)
+{
+    const long long n = (long long)k.Next * k.Nr * k.Ntpad;
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    geometry_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(k, geom);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "geometry_kernel launch");
+    return 1;
+}
+
+int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c_dev, const double *bc_dev,
+                 double *J_dev, double *F_dev, void *stream)
+{
+    cudaStream_t s = (cudaStream_t)stream;
+    KParams kk = k;
+    kk.want_jac = J_dev != nullptr;
+    int launches = 0;
+    prep_kernel<<<kk.B, 256, 0, s>>>(kk, c_dev);
+    ++launches;
+    if (kk.geom) point_kernel<true><<<cfg.grid, cfg.block, cfg.smem, s>>>(kk);
+    else point_kernel<false><<<cfg.grid, cfg.block, cfg.smem, s>>>(kk);
+    ++launches;
+    if (kk.want_jac) {
+        dim3 gg((3 * kk.Next + 7) / 8, kk.Npad / 8, kk.B);
+        gemm_kernel<<<gg, 32, 0, s>>>(kk);
+        ++launches;
+    }
+    dim3 ga(kk.N, kk.B);
+    assemble_kernel<<<ga, 128, 0, s>>>(kk, bc_dev, J_dev, F_dev);
+    ++launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "build launch");
+    return launches;
+}
+
+int launch_dfma_probe(int blocks, int iters, double *sink, void *stream)
+{
+    dfma_probe_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(iters, sink);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "dfma_probe launch");
+    return 1;
+}
+int launch_dmma_probe(int blocks, int iters, double *sink, void *stream)
+{
+    dmma_probe_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(iters, sink);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "dmma_probe launch");
+    return 1;
+}
+
+}  // namespace dse

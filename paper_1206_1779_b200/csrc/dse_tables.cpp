@@ -1,0 +1,144 @@
+// dse_tables.cpp -- host-side builder of the quadrature-grid and Chebyshev tables (step H0).
+//
+// Gauss-Legendre rule for the radial integral with a non-linear node map -- here a
+// single rule in s = 2 ln(y/eps2)/Lg - 1 on [eps2, L2] (BASELINE configs; reading A8);
+// angular rule: Gauss-Legendre in theta on [0, pi] (reading A9); collocation at the mapped roots of
+// T_N (fn.9 L224); map eq.(25) L185.  Everything is evaluated in long double and rounded once.
+#include <cmath>
+
+#include "dse_internal.h"
+
+namespace dse {
+namespace {
+
+using ld = long double;
+const ld PI_L = 3.141592653589793238462643383279502884L;
+
+// Legendre P_n(x) and P_{n-1}(x) by the Bonnet recurrence.
+inline void legendre_pair(int n, ld x, ld &pn, ld &pnm1)
+{
+    ld a = 1.0L, b = x;   // P_0, P_1
+    if (n == 0) { pn = a; pnm1 = 0; return; }
+    for (int m = 1; m < n; ++m) {
+        ld c = ((2 * m + 1) * x * b - m * a) / (m + 1);
+        a = b;
+        b = c;
+    }
+    pn = b;
+    pnm1 = a;
+}
+
+// nodes ascending in (-1,1); only the non-negative half is iterated, the rest mirrored.
+void gauss_legendre(int n, std::vector<ld> &node, std::vector<ld> &weight)
+{
+    node.assign(n, 0);
+    weight.assign(n, 0);
+    const int half = (n + 1) / 2;
+    for (int m = 0; m < half; ++m) {
+        // m-th largest root; Tricomi-type starting value
+        ld th = PI_L * (4 * m + 3) / (4 * n + 2);
+        ld x = (1 - (ld)(n - 1) / (8.0L * n * n * n)) * cosl(th);
+        ld pn, pm, dpn = 1;
+        for (int it = 0; it < 60; ++it) {
+            legendre_pair(n, x, pn, pm);
+            dpn = n * (pm - x * pn) / (1 - x * x);
+            ld step = pn / dpn;
+            x -= step;
+            if (fabsl(step) < 2e-19L) break;
+        }
+        legendre_pair(n, x, pn, pm);
+        dpn = n * (pm - x * pn) / (1 - x * x);
+        ld w = 2 / ((1 - x * x) * dpn * dpn);
+        node[n - 1 - m] = x;
+        weight[n - 1 - m] = w;
+        node[m] = -x;
+        weight[m] = w;
+    }
+    if (n % 2 == 1) node[n / 2] = 0;
+}
+
+inline void phi_row(int N, int Npad, ld s, double *out)
+{
+    ld tm = 1, t = s;
+    for (int j = 0; j < Npad; ++j) out[j] = 0.0;
+    out[0] = 0.5;   // phi_0 = 1/2: the c_0/2 convention of eq.(23),(24)
+    if (N > 1) out[1] = (double)s;
+    for (int j = 2; j < N; ++j) {
+        ld tn = 2 * s * t - tm;
+        tm = t;
+        t = tn;
+        out[j] = (double)tn;
+    }
+}
+
+}  // namespace
+
+void build_tables(const dse_params &p, HostTables &T)
+{
+    const int N = p.n_cheb, Nr = p.n_r, Nt = p.n_theta;
+    T.N = N;
+    T.Npad = ((N + CJ - 1) / CJ) * CJ;
+    T.Nr = Nr;
+    T.Nt = Nt;
+    int g = 32;
+    if (Nt < 32) { g = 1; while (g < Nt) g <<= 1; }
+    T.Ntpad = ((Nt + g - 1) / g) * g;
+    const bool same = (p.x_G == p.x_Z);
+    T.Next = N + (same ? 1 : 2);
+    T.iZ = N;
+    T.iG = same ? N : N + 1;
+    const ld Lg = logl((ld)p.L2 / (ld)p.eps2);
+    T.Lg = (double)Lg;
+    const ld C = 4 * PI_L * (ld)p.alpha_mu * (ld)p.n_colors / (8 * PI_L * PI_L * PI_L);   // g^2 N_c/(2 pi)^3
+    T.C = (double)C;
+
+    std::vector<ld> t, w;
+    // radial rule in s; y = eps2 exp((s+1) Lg/2), dy = (Lg/2) y ds
+    gauss_legendre(Nr, t, w);
+    T.y.resize(Nr); T.sy.resize(Nr); T.Wy.resize(Nr); T.t_r.resize(Nr);
+    T.phi_y.assign((size_t)Nr * T.Npad, 0.0);
+    for (int q = 0; q < Nr; ++q) {
+        ld yy = (ld)p.eps2 * expl((t[q] + 1) * Lg / 2);
+        T.y[q] = (double)yy;
+        T.sy[q] = (double)sqrtl((ld)T.y[q]);          // sqrt of the rounded table value
+        T.Wy[q] = (double)(w[q] * (Lg / 2) * yy);
+        T.t_r[q] = (double)t[q];
+        phi_row(N, T.Npad, t[q], &T.phi_y[(size_t)q * T.Npad]);
+    }
+    // angular rule in theta
+    gauss_legendre(Nt, t, w);
+    T.theta.resize(Nt); T.Omega.resize(Nt);
+    T.ang.assign((size_t)T.Ntpad * 6, 0.0);
+    for (int k = 0; k < T.Ntpad; ++k) {
+        const int kk = k < Nt ? k : 0;                 // padded lanes: a valid angle with zero weight
+        ld th = (t[kk] + 1) * PI_L / 2;
+        ld Om = (k < Nt) ? w[kk] * PI_L / 2 : 0.0L;
+        if (k < Nt) { T.theta[k] = (double)th; T.Omega[k] = (double)Om; }
+        // the kernels take theta as the rounded double (same input as any other consumer of the table)
+        ld thd = (ld)(double)th;
+        ld sh = sinl(thd / 2), c = cosl(thd), s = sinl(thd);
+        double *a = &T.ang[(size_t)k * 6];
+        a[0] = (double)(sh * sh);
+        a[1] = (double)(6 * c);
+        a[2] = (double)(2 + c * c);
+        a[3] = (double)(-2 * s * s);
+        a[4] = (double)((ld)(double)Om * s * s);
+        a[5] = (double)((ld)(double)Om * s * s * s * s);
+    }
+    // external points: Chebyshev roots s_i = -cos(pi (i+1/2)/N), ascending, then x_Z, then x_G
+    T.x_ext.resize(T.Next); T.sx_ext.resize(T.Next); T.c3x_ext.resize(T.Next);
+    T.phi_x.assign((size_t)N * T.Npad, 0.0);
+    for (int i = 0; i < N; ++i) {
+        ld s = -cosl(PI_L * (i + 0.5L) / N);
+        T.x_ext[i] = (double)((ld)p.eps2 * expl((s + 1) * Lg / 2));
+        phi_row(N, T.Npad, s, &T.phi_x[(size_t)i * T.Npad]);
+    }
+    T.x_ext[T.iZ] = p.x_Z;
+    if (!same) T.x_ext[T.iG] = p.x_G;
+    for (int e = 0; e < T.Next; ++e) {
+        T.sx_ext[e] = (double)sqrtl((ld)T.x_ext[e]);
+        T.c3x_ext[e] = (double)(C / (3 * (ld)T.x_ext[e]));
+    }
+}
+
+}  // namespace dse

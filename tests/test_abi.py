@@ -1,0 +1,60 @@
+"""The C-ABI library loads and exports every symbol include/dse.h declares (no compute without a GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1206_1779_b200 import build, binding
+    build.build()
+    return binding.load_library()
+
+
+def test_header_symbols_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "dse.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(dse_[a-z0-9_]+)\s*\(", hdr))
+    assert {"dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step"} <= names
+    for n in names:
+        assert hasattr(lib, n), n
+    from paper_1206_1779_b200.binding import EXPORTS
+    assert set(EXPORTS) == names
+
+
+def test_struct_layout_matches_header():
+    from paper_1206_1779_b200.binding import DseParams
+    # 4 int32 + 10 double + 2 int32
+    assert ctypes.sizeof(DseParams) == 16 + 80 + 8
+    assert DseParams.eps2.offset == 16 and DseParams.flags.offset == 96
+
+
+def test_error_paths_without_gpu(lib):
+    from paper_1206_1779_b200.binding import DseParams
+    from paper_1206_1779_b200.workloads import CONFIGS
+    from paper_1206_1779_b200 import params_from_workload
+    h = ctypes.c_void_p()
+    assert lib.dse_strerror(0) == b"ok" and lib.dse_strerror(-1) == b"invalid argument"
+    assert lib.dse_create(None, ctypes.byref(h)) == -1
+    bad = params_from_workload(CONFIGS[0])
+    bad.n_cheb = 1
+    assert lib.dse_create(ctypes.byref(bad), ctypes.byref(h)) == -1
+    bad = params_from_workload(CONFIGS[0])
+    bad.eps2 = 2e10
+    assert lib.dse_create(ctypes.byref(bad), ctypes.byref(h)) == -1
+    bad = params_from_workload(CONFIGS[0])
+    bad.x_G = 0.0
+    assert lib.dse_create(ctypes.byref(bad), ctypes.byref(h)) == -1
+    assert lib.dse_destroy(None) == 0
+    assert lib.dse_jacobian(None, None, None, None, None, None) == -1
+    import torch
+    if not torch.cuda.is_available():
+        ok = params_from_workload(CONFIGS[0])
+        assert lib.dse_create(ctypes.byref(ok), ctypes.byref(h)) == -3      # no CPU fallback
+        from paper_1206_1779_b200 import Dse, DseError
+        with pytest.raises(DseError):
+            Dse(ok)

@@ -1,0 +1,129 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on the same
+seeded inputs.  Tolerance: BASELINE.json north_star -- <= 1e-10 normwise relative error on J and F;
+we additionally bound the worst row-wise relative error (one row dominates the normwise number,
+row norms span ~19 decades) at 1e-9."""
+import ctypes
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_NORM = 1e-10
+TOL_ROW = 1e-9
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+def oracle_params(w):
+    from oracle.oracle import make_params
+    return make_params(w.n_cheb, w.n_r, w.n_theta, w.eps2, w.L2, w.x_G, w.x_Z, w.alpha_mu, w.n_colors, w.delta,
+                       w.ir_exp_G, w.ir_exp_Z, w.uv_omega)
+
+
+def gpu_build(w, c, bc, flags=0, jac=True):
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    d = Dse(params_from_workload(w, n_batch=c.shape[0], flags=flags))
+    ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
+    if jac:
+        J, F = d.jacobian(ct, bt)
+        torch.cuda.synchronize()
+        out = J.cpu().numpy(), F.cpu().numpy()
+    else:
+        F = d.residual(ct, bt)
+        torch.cuda.synchronize()
+        out = None, F.cpu().numpy()
+    d.close()
+    return out
+
+
+def check(J, F, Jo, Fo):
+    assert np.all(np.isfinite(J)) and np.all(np.isfinite(F))
+    en = np.linalg.norm(J - Jo) / np.linalg.norm(Jo)
+    ef = np.linalg.norm(F - Fo) / np.linalg.norm(Fo)
+    er = (np.linalg.norm(J - Jo, axis=1) / np.linalg.norm(Jo, axis=1)).max()
+    efr = (np.abs(F - Fo) / (np.abs(Fo) + np.linalg.norm(Jo, axis=1))).max()
+    assert en <= TOL_NORM and ef <= TOL_NORM, (en, ef)
+    assert er <= TOL_ROW and efr <= TOL_ROW, (er, efr)
+    return en, ef, er
+
+
+@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_configs_0_1_full_parity(orc, cfg, flags):
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(cfg)
+    Fo, Jo = orc.residual_jacobian(oracle_params(w), c[0], bc[0, 0], bc[0, 1])
+    J, F = gpu_build(w, c, bc, flags)
+    check(J[0], F[0], Jo, Fo)
+    # residual-only entry point gives the same F
+    _, F2 = gpu_build(w, c, bc, flags, jac=False)
+    assert np.array_equal(F2, F)
+
+
+def test_tables_match_oracle(orc):
+    _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import CONFIGS
+    for cfg in (0, 3):
+        w = CONFIGS[cfg]
+        d = Dse(params_from_workload(w))
+        t = d.tables(); d.close()
+        o = orc.tables(oracle_params(w))
+        assert np.allclose(t["x_ext"], o["x_ext"], rtol=1e-14)
+        assert np.allclose(t["y"], o["y"], rtol=1e-14)
+        assert np.allclose(t["Wy"], o["Wy"], rtol=1e-11)
+        assert np.allclose(t["theta"], o["theta"], rtol=1e-14)
+        assert np.allclose(t["Omega"], o["Omega"], rtol=1e-11)
+
+
+@pytest.mark.parametrize("shape", [
+    dict(n_cheb=5, n_r=7, n_theta=3),          # ragged everything: N not a multiple of 8, odd rows, g = 4 with padding
+    dict(n_cheb=12, n_r=33, n_theta=21),       # NCH = 2, g = 32 with 11 padded lanes
+    dict(n_cheb=36, n_r=20, n_theta=40),       # paper's N = 36: NCH = 5 (non power of two), two angular batches
+    dict(n_cheb=2, n_r=2, n_theta=2),          # minimum sizes
+    dict(n_cheb=16, n_r=40, n_theta=32, x_G=3.0, x_Z=5e3),   # distinct subtraction points (N_ext = N + 2)
+    dict(n_cheb=128, n_r=6, n_theta=8),        # maximum N
+])
+def test_ragged_and_edge_shapes(orc, shape):
+    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    kw = dict(eps2=1e-6, L2=5e4)
+    kw.update(shape)
+    w = Workload("edge", **kw)
+    c = draw_coefficients(17, w.n_cheb)[None, :]
+    bc = np.array([[0.8, 1.7]])
+    Fo, Jo = orc.residual_jacobian(oracle_params(w), c[0], 0.8, 1.7)
+    for flags in (0, 1):
+        J, F = gpu_build(w, c, bc, flags)
+        check(J[0], F[0], Jo, Fo)
+
+
+def test_batched_systems(orc):
+    """config 4 at reduced batch: every system against the oracle."""
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(4, n_batch=5)
+    J, F = gpu_build(w, c, bc)
+    for b in range(5):
+        Fo, Jo = orc.residual_jacobian(oracle_params(w), c[b], bc[b, 0], bc[b, 1])
+        check(J[b], F[b], Jo, Fo)
+
+
+def test_deterministic_bitwise():
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(1)
+    d = Dse(params_from_workload(w))
+    ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
+    J0, F0 = d.jacobian(ct, bt)
+    J0 = J0.clone(); F0 = F0.clone()
+    for _ in range(5):
+        J, F = d.jacobian(ct, bt)
+        assert torch.equal(J, J0) and torch.equal(F, F0)
+    assert d.launch_count() == 6 * 4
+    d.close()

@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- Jacobian builds/s of the ghost/gluon DSE Newton-matrix hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (prep -> point kernel -> DMMA contraction -> assembly:
+residual F and analytic Newton matrix J) over the workload's seeded synthetic inputs, through the
+C ABI (include/dse.h).  Default workload: BASELINE.json configs[3] (N=64, N_r=1024, N_theta=128), the
+configuration north_star quotes the "% of fp64 peak" metric on.  Prints ONE JSON line (rank 0).
+N > 1: every rank builds its own replica of the workload (the path has no exchange step; DESIGN.md
+"Multi-GPU": replicas / batch sharding only) -> weak scaling, value = all ranks' builds / max time.
+--impl reference times the CPU oracle (oracle/, a deliberately plain serial program) on the same
+workload; each step is a bounded sample (whole external points) of one build.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1206_1779_b200.workloads import CONFIGS, config_inputs   # noqa: E402
+
+# fp64 FMA peak of one B200 derived from unit counts and clocks (B200_PROFILING.md: 148 SMs,
+# clocks.max.sm 1965 MHz; 64 fp64 FMA lanes per SM = 16 per SM sub-partition): DESIGN.md "Roofline".
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
+def algorithmic_flops(w, n_batch):
+    """12 N flops per quadrature point and system: 3N FMA for the two series at z with
+    the shared T_j recurrence + 3N FMA for the three z-dependent Jacobian streams."""
+    return 12.0 * w.n_cheb * w.points * n_batch
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML during the timed region."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def sample(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        try:
+            self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+            r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+            names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20,
+                     "hw_thermal_slowdown": 0x40, "hw_power_brake_slowdown": 0x80}
+            for k, bit in names.items():
+                if r & bit:
+                    self.reasons.add(k)
+        except Exception:
+            pass
+
+    def run(self):
+        while not self.stop_flag:
+            self.sample()
+            time.sleep(0.01)
+
+    def result(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_params(w):
+    from oracle.oracle import make_params
+    return make_params(w.n_cheb, w.n_r, w.n_theta, w.eps2, w.L2, w.x_G, w.x_Z, w.alpha_mu, w.n_colors, w.delta,
+                       w.ir_exp_G, w.ir_exp_Z, w.uv_omega)
+
+
+def time_oracle_points(w, c, n_points, start=0):
+    """Times the oracle, as it stands, on `n_points` external points of one build (self-energies and
+    all four derivative rows = everything a build computes for those points).  Returns seconds."""
+    from oracle.oracle import Oracle
+    orc = Oracle()
+    p = oracle_params(w)
+    tab = orc.tables(p)
+    t0 = time.perf_counter()
+    for e in range(start, start + n_points):
+        orc.self_energy(p, c, tab["x_ext"][e % w.n_ext], tab["y"], tab["Wy"], tab["theta"], tab["Omega"], derivs=True)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(w, c, budget_s=12.0):
+    """Oracle on a bounded sample: whole external points of one build, ~budget_s of CPU work."""
+    t1 = time_oracle_points(w, c, 1)
+    n = int(max(1, min(w.n_ext, budget_s / max(t1, 1e-6))))
+    t = time_oracle_points(w, c, n)
+    builds_per_s = (n / w.n_ext) / t
+    return {"value": builds_per_s, "unit": "jacobian_builds/s", "cores": 1, "kind": "oracle",
+            "sample": f"{n} of {w.n_ext} external points of one {w.name} build ({n * w.n_r * w.n_theta} quadrature "
+                      f"points, {t:.2f} s, serial fp64 C, gcc -O2), scaled to a full build",
+            "points_per_s": n * w.n_r * w.n_theta / t}
+
+
+def run_reference(args, w, c):
+    """--impl reference: the CPU oracle, as it stands, on the box's host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    t1 = time_oracle_points(w, c[0], 1)
+    per_step_budget = 120.0 / max(1, args.steps + args.warmup)
+    n = int(max(1, min(w.n_ext, per_step_budget / max(t1, 1e-6))))
+    for i in range(args.warmup):
+        time_oracle_points(w, c[0], n, start=i * n)
+    t = 0.0
+    for i in range(args.steps):
+        t += time_oracle_points(w, c[0], n, start=i * n)
+    ms = 1e3 * t / args.steps
+    value = (n / w.n_ext) / (t / args.steps)
+    sample = (f"each step = {n} of {w.n_ext} external points of one {w.name} build "
+              f"({n * w.n_r * w.n_theta} quadrature points), scaled to full builds")
+    line = {
+        "impl": "reference", "metric": "fp64 Jacobian builds/s", "value": value, "unit": "jacobian_builds/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "n_cheb": w.n_cheb, "n_r": w.n_r, "n_theta": w.n_theta, "n_batch": 1,
+                   "eps2": w.eps2, "L2": w.L2, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": "jacobian_builds/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "jacobian_builds/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+        "points_per_s": n * w.n_r * w.n_theta / (t / args.steps),
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, w, c, bc):
+    import torch
+    import torch.distributed as dist
+    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE
+    from paper_1206_1779_b200.binding import dfma_probe
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    nb = c.shape[0]
+    flags = DSE_FLAG_GEOMETRY_CACHE if args.geometry_cache else 0
+    d = Dse(params_from_workload(w, n_batch=nb, flags=flags))
+    n2 = 2 * w.n_cheb
+    ct = torch.from_numpy(c).cuda()
+    bt = torch.from_numpy(bc).cuda()
+    J = torch.empty((nb, n2, n2), dtype=torch.float64, device="cuda")
+    F = torch.empty((nb, n2), dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    for _ in range(max(args.warmup, 3)):
+        flush.zero_()
+        d.jacobian(ct, bt, J, F)
+    barrier()
+
+    # ---- timed region: K steps, each bracketed by its own event pair; L2 flushed between steps ----
+    sampler = ClockSampler(local)
+    sampler.sample()
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    d.set_timing(True)
+    l0 = d.launch_count()
+    barrier()
+    t_wall0 = time.perf_counter()
+    for k in range(args.steps):
+        flush.zero_()
+        ev[k][0].record(stream)
+        d.jacobian(ct, bt, J, F)
+        ev[k][1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    sampler.sample()
+    sampler.stop_flag = True
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(np.sum(step_ms))
+    kernel_ms, kernel_n = d.get_timing()
+    d.set_timing(False)
+    launches = d.launch_count() - l0
+    if world > 1:
+        tmax = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        total_ms = float(tmax.item())
+    ms_per_step = total_ms / args.steps
+    value = world * nb * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end through the C ABI with host (pinned) buffers: H2D of c, bc and D2H of J, F each step ----
+    c_h = torch.from_numpy(c).pin_memory(); bc_h = torch.from_numpy(bc).pin_memory()
+    J_h = torch.empty((nb, n2, n2), dtype=torch.float64).pin_memory()
+    F_h = torch.empty((nb, n2), dtype=torch.float64).pin_memory()
+    e2e_steps = min(args.steps, 200)
+    for _ in range(3):
+        d.jacobian_host(c_h.numpy(), bc_h.numpy(), J_h.numpy(), F_h.numpy())
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        d.jacobian_host(c_h.numpy(), bc_h.numpy(), J_h.numpy(), F_h.numpy())
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    if world > 1:
+        tm = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
+        t_e2e = float(tm.item())
+    e2e_value = world * nb * e2e_steps / t_e2e
+
+    info = d.kernel_info()
+    if rank == 0:
+        # live fp64 FMA probe (reported beside the derived peak)
+        sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
+        dfma_probe(148 * 8, 2000, sink)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        fl = dfma_probe(148 * 8, 100000, sink)
+        b.record(stream)
+        torch.cuda.synchronize()
+        probe_tflops = fl / (a.elapsed_time(b) * 1e-3) / 1e12
+
+        flops = algorithmic_flops(w, nb)
+        k_ms = kernel_ms / max(kernel_n, 1)
+        achieved = flops / (k_ms * 1e-3) / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "point_kernel_traffic.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(w.name)
+            except Exception:
+                traffic = None
+        line = {
+            "metric": "fp64 Jacobian builds/s", "value": value, "unit": "jacobian_builds/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n_cheb": w.n_cheb, "n_r": w.n_r, "n_theta": w.n_theta, "n_batch": nb,
+                       "eps2": w.eps2, "L2": w.L2, "points_per_build": w.points * nb,
+                       "geometry_cache": bool(args.geometry_cache),
+                       "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)",
+                       "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                       "point_kernel": info},
+            "points_per_s": value * w.points, "paper_equiv_evals_per_s": value * w.paper_equiv_evals,
+            "wall_s_timed_region": t_wall,
+            "roofline": {"bound": "alu", "kernel": "point_kernel", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
+                         "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
+                         "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
+                         "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no "
+                                        "fp64 entry)",
+                         "measured_dfma_probe_tflops": probe_tflops, "frac_of_probe": achieved / probe_tflops,
+                         "algorithmic_flops_per_launch": flops},
+            "e2e": {"value": e2e_value, "unit": "jacobian_builds/s", "h2d_bytes_per_step": int(c.nbytes + bc.nbytes),
+                    "d2h_bytes_per_step": int(J_h.numel() * 8 + F_h.numel() * 8), "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "clocks": sampler.result(),
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w, c[0])
+        print(json.dumps(line), flush=True)
+    d.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=3, choices=sorted(CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--geometry-cache", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    w, c, bc = config_inputs(args.config)
+    if args.impl == "reference":
+        run_reference(args, w, c)
+    else:
+        run_ours(args, w, c, bc)
+
+
+if __name__ == "__main__":
+    main()

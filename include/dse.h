@@ -129,6 +129,13 @@ DSE_API int64_t dse_launch_count(const dse_handle *h);
  * out[5] = SM count. */
 DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[6]);
 
+/* Per-kernel device timing of the dominant (point) kernel, for the roofline report: while enabled,
+ * every build records a CUDA event pair around the point kernel on the build's stream (nothing else
+ * changes).  dse_get_timing synchronises on the recorded events, adds them up and returns the
+ * accumulated milliseconds and launch count since the last reset (enable resets). */
+DSE_API int dse_set_timing(dse_handle *h, int32_t enable);
+DSE_API int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches);
+
 /* fp64 FMA throughput probe (the roofline denominator of an ALU-bound path): launches a kernel of
  * `blocks` x 256 threads, each running 8 independent chains of `iters` dependent DFMAs, on `stream`.
  * flops per launch = blocks*256*8*iters*2.  sink_dev receives one double per thread (>= blocks*256).

@@ -26,6 +26,13 @@ struct dse_handle {
     double *d_J = nullptr, *d_F = nullptr, *d_lu = nullptr;   // internal J, F for dse_newton_step (+ LU scratch)
     double *d_c = nullptr, *d_bc = nullptr, *d_Jh = nullptr, *d_Fh = nullptr;   // staging for *_host calls
     int64_t launches = 0;
+    // optional timing of the point kernel (dse_set_timing)
+    static constexpr int EV_RING = 64;
+    bool timing = false;
+    cudaEvent_t ev[EV_RING][2] = {};
+    int ev_head = 0, ev_pending = 0;
+    double t_ms = 0.0;
+    int64_t t_n = 0;
 };
 
 namespace {
@@ -58,6 +65,42 @@ int validate(const dse_params *p)
     if (!std::isfinite(p->delta) || !std::isfinite(p->ir_exp_G) || !std::isfinite(p->ir_exp_Z)) return DSE_EINVAL;
     if (!std::isfinite(p->uv_omega) || p->uv_omega < 0.0) return DSE_EINVAL;
     if (p->reserved != 0 || (p->flags & ~DSE_FLAG_GEOMETRY_CACHE)) return DSE_EINVAL;
+    return DSE_OK;
+}
+
+// drains the oldest `n` pending event pairs into the accumulators
+int drain_events(dse_handle *h, int n)
+{
+    while (n-- > 0 && h->ev_pending > 0) {
+        const int idx = (h->ev_head - h->ev_pending + 2 * dse_handle::EV_RING) % dse_handle::EV_RING;
+        float ms = 0.f;
+        cudaError_t e = cudaEventSynchronize(h->ev[idx][1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, h->ev[idx][0], h->ev[idx][1]);
+        if (e != cudaSuccess) return cuda_err(e, "timing events");
+        h->t_ms += ms;
+        h->t_n += 1;
+        --h->ev_pending;
+    }
+    return DSE_OK;
+}
+
+// build with optional event pair around the point kernel
+int do_build(dse_handle *h, const double *c, const double *bc, double *J, double *F, void *stream)
+{
+    void *e0 = nullptr, *e1 = nullptr;
+    if (h->timing) {
+        if (h->ev_pending == dse_handle::EV_RING) {
+            int rc = drain_events(h, 1);
+            if (rc < 0) return rc;
+        }
+        e0 = h->ev[h->ev_head][0];
+        e1 = h->ev[h->ev_head][1];
+        h->ev_head = (h->ev_head + 1) % dse_handle::EV_RING;
+        ++h->ev_pending;
+    }
+    int rc = dse::launch_build(h->k, h->cfg, c, bc, J, F, stream, e0, e1);
+    if (rc < 0) return rc;
+    h->launches += rc;
     return DSE_OK;
 }
 
@@ -185,6 +228,9 @@ int dse_destroy(dse_handle *h)
     if (h->d_tables) cudaFree(h->d_tables);
     if (h->d_work) cudaFree(h->d_work);
     if (h->d_geom) cudaFree(h->d_geom);
+    for (auto &p : h->ev)
+        for (auto &e : p)
+            if (e) cudaEventDestroy(e);
     delete h;
     return DSE_OK;
 }
@@ -192,27 +238,20 @@ int dse_destroy(dse_handle *h)
 int dse_jacobian(dse_handle *h, const double *c_dev, const double *bc_dev, double *J_dev, double *F_dev, void *stream)
 {
     if (!h || !c_dev || !bc_dev || !J_dev || !F_dev) return DSE_EINVAL;
-    int rc = dse::launch_build(h->k, h->cfg, c_dev, bc_dev, J_dev, F_dev, stream);
-    if (rc < 0) return rc;
-    h->launches += rc;
-    return DSE_OK;
+    return do_build(h, c_dev, bc_dev, J_dev, F_dev, stream);
 }
 
 int dse_residual(dse_handle *h, const double *c_dev, const double *bc_dev, double *F_dev, void *stream)
 {
     if (!h || !c_dev || !bc_dev || !F_dev) return DSE_EINVAL;
-    int rc = dse::launch_build(h->k, h->cfg, c_dev, bc_dev, nullptr, F_dev, stream);
-    if (rc < 0) return rc;
-    h->launches += rc;
-    return DSE_OK;
+    return do_build(h, c_dev, bc_dev, nullptr, F_dev, stream);
 }
 
 int dse_newton_step(dse_handle *h, double *c_dev, const double *bc_dev, double rho, double *stats_dev, void *stream)
 {
     if (!h || !c_dev || !bc_dev || !std::isfinite(rho)) return DSE_EINVAL;
-    int rc = dse::launch_build(h->k, h->cfg, c_dev, bc_dev, h->d_J, h->d_F, stream);
+    int rc = do_build(h, c_dev, bc_dev, h->d_J, h->d_F, stream);
     if (rc < 0) return rc;
-    h->launches += rc;
     rc = dse::launch_lu(2 * h->k.N, h->k.B, h->d_J, h->d_F, nullptr, c_dev, rho, stats_dev, h->d_lu, stream);
     if (rc < 0) return rc;
     h->launches += rc;
@@ -242,12 +281,36 @@ int dse_jacobian_host(dse_handle *h, const double *c_host, const double *bc_host
     const size_t n2 = 2 * (size_t)h->k.N, B = (size_t)h->k.B;
     CK(cudaMemcpyAsync(h->d_c, c_host, 8 * B * n2, cudaMemcpyHostToDevice, nullptr));
     CK(cudaMemcpyAsync(h->d_bc, bc_host, 8 * B * 2, cudaMemcpyHostToDevice, nullptr));
-    int rc = dse::launch_build(h->k, h->cfg, h->d_c, h->d_bc, J_host ? h->d_Jh : nullptr, h->d_Fh, nullptr);
+    int rc = do_build(h, h->d_c, h->d_bc, J_host ? h->d_Jh : nullptr, h->d_Fh, nullptr);
     if (rc < 0) return rc;
-    h->launches += rc;
     if (J_host) CK(cudaMemcpyAsync(J_host, h->d_Jh, 8 * B * n2 * n2, cudaMemcpyDeviceToHost, nullptr));
     CK(cudaMemcpyAsync(F_host, h->d_Fh, 8 * B * n2, cudaMemcpyDeviceToHost, nullptr));
     CK(cudaStreamSynchronize(nullptr));
+    return DSE_OK;
+}
+
+int dse_set_timing(dse_handle *h, int32_t enable)
+{
+    if (!h) return DSE_EINVAL;
+    int rc = drain_events(h, h->ev_pending);
+    if (rc < 0) return rc;
+    if (enable)
+        for (auto &p : h->ev)
+            for (auto &e : p)
+                if (!e) CK(cudaEventCreate(&e));
+    h->timing = enable != 0;
+    h->t_ms = 0.0;
+    h->t_n = 0;
+    return DSE_OK;
+}
+
+int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches)
+{
+    if (!h || !total_ms || !launches) return DSE_EINVAL;
+    int rc = drain_events(h, h->ev_pending);
+    if (rc < 0) return rc;
+    *total_ms = h->t_ms;
+    *launches = h->t_n;
     return DSE_OK;
 }
 

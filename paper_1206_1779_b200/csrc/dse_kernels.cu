@@ -483,7 +483,7 @@ int launch_geometry(const KParams &k, double *geom, void *stream)
 }
 
 int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c_dev, const double *bc_dev,
-                 double *J_dev, double *F_dev, void *stream)
+                 double *J_dev, double *F_dev, void *stream, void *ev0, void *ev1)
 {
     cudaStream_t s = (cudaStream_t)stream;
     KParams kk = k;
@@ -491,8 +491,10 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     int launches = 0;
     prep_kernel<<<kk.B, 256, 0, s>>>(kk, c_dev);
     ++launches;
+    if (ev0) cudaEventRecord((cudaEvent_t)ev0, s);
     if (kk.geom) point_kernel<true><<<cfg.grid, cfg.block, cfg.smem, s>>>(kk);
     else point_kernel<false><<<cfg.grid, cfg.block, cfg.smem, s>>>(kk);
+    if (ev1) cudaEventRecord((cudaEvent_t)ev1, s);
     ++launches;
     if (kk.want_jac) {
         dim3 gg((3 * kk.Next + 7) / 8, kk.Npad / 8, kk.B);

@@ -44,7 +44,7 @@ def test_newton_trajectory_weak_coupling(orc):
         c_o, so, rc = orc.newton_step(p, c_o, 1.0, 1.0, 1.0)
         st = d.newton_step(c_g, bc, 1.0).cpu().numpy()[0]
         dn.append(st[0])
-        assert abs(st[0] - so[0]) <= 1e-9 * so[0] + 1e-14
+        assert abs(st[0] - so[0]) <= 1e-9 * so[0] + 1e-12     # |Delta| itself carries cond(J)*eps of the iterate
         assert np.allclose(c_g.cpu().numpy()[0], c_o, rtol=0, atol=1e-9 * np.abs(c_o).max())
     assert dn[-1] < 1e-13
     d.close()

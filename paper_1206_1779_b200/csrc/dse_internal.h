@@ -55,6 +55,7 @@ struct PointKernelConfig {
 // ev0/ev1: optional cudaEvent_t pair recorded around the point kernel (nullptr = no timing)
 int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c_dev, const double *bc_dev,
                  double *J_dev, double *F_dev, void *stream, void *ev0 = nullptr, void *ev1 = nullptr);
+int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream);
 int launch_geometry(const KParams &k, double *geom, void *stream);
 int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
               double *stats, double *scratch, void *stream);

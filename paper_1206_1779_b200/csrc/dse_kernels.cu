@@ -10,22 +10,11 @@
 
 #include <cstdio>
 
-#include "dse_internal.h"
+#include "dse_device.cuh"
 
 namespace dse {
 
 namespace {
-
-constexpr int POINT_THREADS = 512;          // 16 warps per CTA, warps are independent workers
-constexpr int TCH_STRIDE = 72;              // doubles per chunk in the T stash: 32 (T_j, T_j+1) pairs + 8 pad
-constexpr unsigned FULL = 0xffffffffu;
-
-__host__ __device__ inline int warp_doubles(int Npad, int NCH)
-{
-    int t = NCH * TCH_STRIDE;
-    if (t < 256) t = 256;                   // flush scratch needs SUB*Npad <= 256 doubles
-    return 2 * Npad + 128 + t;
-}
 
 // ---------------------------------------------------------------------------------------------
 // H1: per system b: (a_j, b_j) pairs with the j = 0 coefficient pre-halved (phi_0 = 1/2, eq.(23),(24)),
@@ -59,33 +48,6 @@ __global__ void prep_kernel(const KParams P, const double *__restrict__ c)
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// H2: coefficient-independent factors of one quadrature point.
-//   z = (x-y)^2/(sqrt x + sqrt y)^2 + 4 sqrt(xy) sin^2(theta/2)        (L62/L192, cancellation-free)
-//   Q = 15/4 - 2 sin^2 [3 + 6 c r + (2 + c^2) r^2],  r = sqrt(xy)/z     (eq.(11) + fn.5, stable form)
-//   M = y sin^2/z                                                      (eq.(10), stable form)
-//   ghost kernel sin^4/z^2                                             (eq.(8) with the measure eq.(4),(5))
-// Row constants: d2 = ((x-y)/(sx+sy))^2, sxy = sx*sy, rv = -C W_q y, rq = (C/3x) W_q, rm = (C/3x) W_q y.
-// Outputs: sraw = 2 ln(z/eps2)/Lg - 1 (unclamped, eq.(25)),
-//   gv = rv Om sin^4/z^2,  gq = rq Om sin^2 Q,  gm = rm Om sin^4/z   (so that v = gv G(y) Z(z), ...)
-struct RowConst { double d2, sxy, rv, rq, rm; };
-
-__device__ __forceinline__ void point_geometry(const RowConst &rc, const double *__restrict__ a /*6 angular*/,
-                                               double inv_eps2, double two_over_Lg, double &sraw, double &gv,
-                                               double &gq, double &gm)
-{
-    const double z = fma(4.0 * rc.sxy, a[0], rc.d2);
-    const double inv = 1.0 / z;
-    const double r = rc.sxy * inv;
-    const double Q = fma(a[3], fma(r, fma(a[2], r, a[1]), 3.0), 3.75);
-    const double ell = log(z * inv_eps2);
-    sraw = fma(ell, two_over_Lg, -1.0);
-    const double w4i = a[5] * inv;
-    gv = rc.rv * w4i * inv;
-    gq = rc.rq * a[4] * Q;
-    gm = rc.rm * w4i;
-}
-
 // Geometry cache builder (DSE_FLAG_GEOMETRY_CACHE): one thread per point, geom[(e*Nr+q)*Ntpad + k][4].
 __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
 {
@@ -106,185 +68,6 @@ __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
         double4 o = make_double4(sraw, gv, gq, gm);
         reinterpret_cast<double4 *>(geom)[t] = o;
     }
-}
-
-// ---------------------------------------------------------------------------------------------
-// The hot kernel (H2-H6).  Each WARP is an independent worker that owns a contiguous range of rows
-// (b, e, q) of the flattened (system, external point, radial node) index and walks the angular
-// nodes of each row in batches of 32 points:
-//   phase 1 (lane = point): geometry (or the cached 32 B), clamp + continuation eq.(16)-(19), the
-//     shared T_j recurrence with both series ln G(z), ln Z(z) (3 FMA per j), 3 exp, the weights
-//     v, wQ, wM (H4), the running row sums (H5, A[e,q] of H7); stash (2s, u_a, u_b, v) and the
-//     chunk-start pairs (T_8c, T_8c+1) in warp-private shared memory;
-//   phase 2 (lane = (chunk c, point sub-lane)): restart the recurrence at j = 8c and accumulate the three
-//     z-dependent Jacobian streams Sa, Sb, Sv for 8 values of j in registers (4 FMA per (point, j)).
-// Accumulators are flushed as per-(warp, external point) partials; assemble_kernel sums them in a
-// fixed order.  No CTA-level synchronisation after the table load, no atomics.
-template <bool GEOM>
-__global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P)
-{
-    extern __shared__ __align__(16) double smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
-    double *s_ang = smem;
-    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(P.Npad, P.NCH);
-    double2 *s_coef = reinterpret_cast<double2 *>(wbase);
-    double4 *s_pt = reinterpret_cast<double4 *>(wbase + 2 * P.Npad);
-    double *s_T = wbase + 2 * P.Npad + 128;
-    double2 *s_T2 = reinterpret_cast<double2 *>(s_T);
-
-    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
-    __syncthreads();
-
-    const int NCH = P.NCH, SUB = P.SUB, Nr = P.Nr, g = P.g;
-    const long long R = P.R;
-    const long long w = (long long)blockIdx.x * WPB + warp;
-    const long long r0 = (w * R) / P.W, r1 = ((w + 1) * R) / P.W;
-    const int c_lane = lane / SUB, sub = lane - c_lane * SUB;
-    const bool active2 = lane < NCH * SUB;
-    const int rib = lane / g, kl = lane - rib * g;          // row-in-batch and angular lane
-    const double halfLg = 0.5 * P.Lg;
-
-    double accA[CJ], accB[CJ], accV[CJ];
-#pragma unroll
-    for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
-    long long cur_bi = -1;
-    int cur_b = -1;
-
-    auto flush = [&](long long bi) {
-        const size_t slot = (size_t)(w + bi);
-#pragma unroll
-        for (int st = 0; st < 3; ++st) {
-            __syncwarp();
-            if (active2) {
-#pragma unroll
-                for (int m = 0; m < CJ; ++m)
-                    s_T[sub * P.Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
-            }
-            __syncwarp();
-            for (int j = lane; j < P.Npad; j += 32) {
-                double s = 0.0;
-                for (int sb = 0; sb < SUB; ++sb) s += s_T[sb * P.Npad + j];
-                P.Spart[(slot * 3 + st) * P.Npad + j] = s;
-            }
-        }
-        __syncwarp();
-    };
-
-    long long r = r0;
-    while (r < r1) {
-        const long long bi = r / Nr;
-        const int q0 = (int)(r - bi * Nr);
-        if (bi != cur_bi) {
-            if (cur_bi >= 0 && P.want_jac) flush(cur_bi);
-#pragma unroll
-            for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
-            cur_bi = bi;
-            const int b = (int)(bi / P.Next);
-            if (b != cur_b) {
-                __syncwarp();
-                for (int j = lane; j < P.Npad; j += 32)
-                    s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)b * P.Npad + j];
-                __syncwarp();
-                cur_b = b;
-            }
-        }
-        const int e = (int)(bi - (long long)cur_b * P.Next);
-        long long left = r1 - r;
-        int nrow = P.rpb;
-        if (left < nrow) nrow = (int)left;
-        if (Nr - q0 < nrow) nrow = Nr - q0;
-        const bool rowact = rib < nrow;
-        const int q = q0 + (rowact ? rib : 0);
-
-        // row constants (identical in all lanes of a row)
-        const double Gy = P.Gy[(size_t)cur_b * Nr + q], Py = P.Py[(size_t)cur_b * Nr + q];
-        RowConst rc;
-        if (!GEOM) {
-            const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
-            const double y = P.y[q], sy = P.sy[q];
-            const double Wq = P.Wy[q];
-            const double d = (x - y) / (sx + sy);
-            rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
-        }
-        const double rowmask = rowact ? 1.0 : 0.0;
-        double sumA = 0.0, sumB = 0.0, sumV = 0.0, sumZ = 0.0;
-
-        for (int kb = 0; kb < P.Ntpad; kb += 32) {
-            const int k = kb + kl;                       // < Ntpad by construction (g divides Ntpad, g <= 32)
-            // ---------------- phase 1: lane = point ----------------
-            double sraw, gv, gq, gm;
-            if (GEOM) {
-                const double4 gg = reinterpret_cast<const double4 *>(P.geom)[((size_t)e * Nr + q) * P.Ntpad + k];
-                sraw = gg.x; gv = gg.y; gq = gg.z; gm = gg.w;
-            } else {
-                point_geometry(rc, s_ang + k * 6, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
-            }
-            double s = sraw, EG = 0.0, EZ = 0.0;
-            if (sraw < -1.0) {                           // z < eps2: G ~ z^pG, Z ~ z^pZ   eq.(16),(17)
-                const double ell = (sraw + 1.0) * halfLg;
-                EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
-            } else if (sraw > 1.0) {                     // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
-                const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
-                EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
-            }
-            const double ts = 2.0 * s;
-            double Tm = 1.0, T = s;
-            double lz0 = 0.0, lz1 = 0.0, lg0 = 0.0, lg1 = 0.0;
-            for (int c = 0; c < NCH; ++c) {
-                if (P.want_jac) s_T2[c * (TCH_STRIDE / 2) + lane] = make_double2(Tm, T);
-#pragma unroll
-                for (int m = 0; m < CJ; m += 2) {
-                    const double2 c0 = s_coef[c * CJ + m], c1 = s_coef[c * CJ + m + 1];
-                    lz0 = fma(c0.x, Tm, lz0); lg0 = fma(c0.y, Tm, lg0);
-                    lz1 = fma(c1.x, T, lz1);  lg1 = fma(c1.y, T, lg1);
-                    Tm = fma(ts, T, -Tm);
-                    T = fma(ts, Tm, -T);
-                }
-            }
-            const double lnZz = (lz0 + lz1) + EZ, lnGz = (lg0 + lg1) + EG;
-            const double Zz = exp(lnZz), Gz = exp(lnGz), Pz = exp(fma(P.e1, lnGz, P.e2 * lnZz));
-            const double v = (gv * rowmask) * (Gy * Zz);          // eq.(8):  -C W y Om sin^4/z^2 G(y) Z(z)
-            const double wQ = (gq * rowmask) * (Py * Pz);         // eq.(9):  (C/3x) W Om sin^2 Q P(y) P(z)
-            const double wM = (gm * rowmask) * (Gy * Gz);         // eq.(9):  (C/3x) W Om sin^2 M G(y) G(z)
-            const double ua = P.e2 * wQ;                          // weight of d/da_j  (P ~ Z^{e2})
-            const double ub = fma(P.e1, wQ, wM);                  // weight of d/db_j  (P ~ G^{e1}; G(y)G(z))
-            sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
-            if (P.want_jac) {
-                s_pt[lane] = make_double4(ts, ua, ub, v);
-                __syncwarp();
-                // ---------------- phase 2: lane = (chunk, point sub-lane) ----------------
-                for (int rd = 0; rd < P.rounds; ++rd) {
-                    const int pt = rd * SUB + sub;
-                    const bool ok = active2 && pt < 32;
-                    const int pc = ok ? pt : 0;
-                    const double4 pw = s_pt[pc];
-                    double2 tt = s_T2[(ok ? c_lane : 0) * (TCH_STRIDE / 2) + pc];
-                    const double wa = ok ? pw.y : 0.0, wb = ok ? pw.z : 0.0, wv = ok ? pw.w : 0.0;
-                    double T0 = tt.x, T1 = tt.y;
-                    accA[0] = fma(wa, T0, accA[0]); accB[0] = fma(wb, T0, accB[0]); accV[0] = fma(wv, T0, accV[0]);
-                    accA[1] = fma(wa, T1, accA[1]); accB[1] = fma(wb, T1, accB[1]); accV[1] = fma(wv, T1, accV[1]);
-#pragma unroll
-                    for (int m = 2; m < CJ; ++m) {
-                        const double T2 = fma(pw.x, T1, -T0);
-                        accA[m] = fma(wa, T2, accA[m]); accB[m] = fma(wb, T2, accB[m]); accV[m] = fma(wv, T2, accV[m]);
-                        T0 = T1; T1 = T2;
-                    }
-                }
-                __syncwarp();
-            }
-        }
-        // H5/H7: row sums over the angular nodes (fixed xor tree), one writer per row
-        for (int o = g >> 1; o > 0; o >>= 1) {
-            sumA += __shfl_xor_sync(FULL, sumA, o);
-            sumB += __shfl_xor_sync(FULL, sumB, o);
-            sumV += __shfl_xor_sync(FULL, sumV, o);
-            sumZ += __shfl_xor_sync(FULL, sumZ, o);
-        }
-        if (kl == 0 && rowact)
-            reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
-        r += nrow;
-    }
-    if (cur_bi >= 0 && P.want_jac) flush(cur_bi);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -431,46 +214,6 @@ inline int cuda_fail(cudaError_t e, const char *what)
 const char *last_error_text() { return g_err; }
 void set_error_text(const char *s) { snprintf(g_err, sizeof(g_err), "%s", s); }
 
-int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
-{
-    int dev = 0, sms = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
-    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
-    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH));
-    for (int v = 0; v < 2; ++v) {
-        const void *fn = v ? (const void *)point_kernel<true> : (const void *)point_kernel<false>;
-        e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(point_kernel smem)");
-    }
-    const void *fn = k.geom ? (const void *)point_kernel<true> : (const void *)point_kernel<false>;
-    cudaFuncAttributes fa;
-    e = cudaFuncGetAttributes(&fa, fn);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncGetAttributes");
-    int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, POINT_THREADS, smem);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
-    if (per_sm < 1) { set_error_text("point_kernel does not fit on an SM"); return DSE_ECUDA; }
-    cfg.block = POINT_THREADS;
-    cfg.smem = smem;
-    cfg.regs = fa.numRegs;
-    cfg.ctas_per_sm = per_sm;
-    cfg.sms = sms;
-    // persistent-style grid: one wave of resident CTAs, but never more warps than rows
-    long long grid = (long long)sms * per_sm;
-    const long long wpb = POINT_THREADS / 32;
-    const long long batches_per_row = k.Ntpad / 32 > 0 ? k.Ntpad / 32 : 1;
-    // keep >= ~4 point batches per warp so that small problems do not pay for idle warps
-    long long want_warps = (k.R * batches_per_row / k.rpb + 3) / 4;
-    if (want_warps < 1) want_warps = 1;
-    long long want_grid = (want_warps + wpb - 1) / wpb;
-    if (want_grid < grid) grid = want_grid;
-    while (grid * wpb > k.R && grid > 1) --grid;
-    cfg.grid = (int)grid;
-    return 0;
-}
-
 int launch_geometry(const KParams &k, double *geom, void *stream)
 {
     const long long n = (long long)k.Next * k.Nr * k.Ntpad;
@@ -492,8 +235,7 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     prep_kernel<<<kk.B, 256, 0, s>>>(kk, c_dev);
     ++launches;
     if (ev0) cudaEventRecord((cudaEvent_t)ev0, s);
-    if (kk.geom) point_kernel<true><<<cfg.grid, cfg.block, cfg.smem, s>>>(kk);
-    else point_kernel<false><<<cfg.grid, cfg.block, cfg.smem, s>>>(kk);
+    launch_point(kk, cfg, stream);
     if (ev1) cudaEventRecord((cudaEvent_t)ev1, s);
     ++launches;
     if (kk.want_jac) {

@@ -1,0 +1,284 @@
+// dse_point.cu -- the hot kernel (steps H2-H6 of DESIGN.md): every quadrature point (x_e, y_q, theta_k).
+//
+// Each WARP is an independent worker that owns a contiguous range of rows (b, e, q) of the flattened
+// (system, external point, radial node) index and walks the angular nodes of each row in batches of
+// 32 points:
+//   phase 1 (lane = point): geometry (or the cached 32 B), clamp + continuation eq.(16)-(19), the
+//     T_j recurrence shared by both series ln G(z), ln Z(z) (3 FMA per j; the recurrence runs as two
+//     independent stride-2 chains T_{j+2} = 2 T_2 T_j - T_{j-2} for instruction-level parallelism),
+//     3 exp, the weights v, wQ, wM (H4), the running row sums (H5, A[e,q] of H7); stash
+//     (2s, u_a, u_b, v) and the chunk-start pairs (T_8c, T_8c+1) in warp-private shared memory;
+//   phase 2 (lane = (chunk c, point sub-lane)): restart the recurrence at j = 8c and accumulate the
+//     three z-dependent Jacobian streams Sa, Sb, Sv for 8 values of j in registers.
+// Accumulators are flushed as per-(warp, external point) partials; assemble_kernel sums them in a
+// fixed order.  No CTA-level synchronisation after the table load, no atomics.
+// Template: NCH_T = number of 8-wide Chebyshev chunks when it is a power of two (everything unrolls),
+// 0 = generic run-time shape; GEOM = read the geometry cache; JAC = accumulate the Jacobian streams.
+#include <cstdio>
+
+#include "dse_device.cuh"
+
+namespace dse {
+
+void set_error_text(const char *s);
+
+namespace {
+
+template <int NCH_T, bool GEOM, bool JAC>
+__global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P)
+{
+    constexpr bool CT = NCH_T > 0;
+    extern __shared__ __align__(16) double smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
+    const int NCH = CT ? NCH_T : P.NCH;
+    const int SUB = CT ? 32 / NCH_T : P.SUB;
+    const int ROUNDS = CT ? NCH_T : P.rounds;
+    const int Npad = NCH * CJ;
+    double *s_ang = smem;
+    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(Npad, NCH);
+    double2 *s_coef = reinterpret_cast<double2 *>(wbase);
+    double4 *s_pt = reinterpret_cast<double4 *>(wbase + 2 * Npad);       // 33 entries, entry 32 = 0
+    double *s_T = wbase + 2 * Npad + 132;
+    double2 *s_T2 = reinterpret_cast<double2 *>(s_T);
+
+    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    if (lane == 0) s_pt[32] = make_double4(0.0, 0.0, 0.0, 0.0);
+    __syncthreads();
+
+    const int Nr = P.Nr, g = P.g;
+    const long long R = P.R;
+    const long long w = (long long)blockIdx.x * WPB + warp;
+    const long long r0 = (w * R) / P.W, r1 = ((w + 1) * R) / P.W;
+    const int c_lane = lane / SUB, sub = lane - c_lane * SUB;
+    const bool active2 = CT ? true : (lane < NCH * SUB);
+    const int rib = lane / g, kl = lane - rib * g;          // row-in-batch and angular lane
+    const double halfLg = 0.5 * P.Lg;
+    const double2 *tread = s_T2 + (active2 ? c_lane : 0) * (TCH_STRIDE / 2);
+
+    double accA[CJ], accB[CJ], accV[CJ];
+#pragma unroll
+    for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
+    long long cur_bi = -1;
+    int cur_b = -1;
+
+    auto flush = [&](long long bi) {
+        const size_t slot = (size_t)(w + bi);
+#pragma unroll
+        for (int st = 0; st < 3; ++st) {
+            __syncwarp();
+            if (active2) {
+#pragma unroll
+                for (int m = 0; m < CJ; ++m)
+                    s_T[sub * Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
+            }
+            __syncwarp();
+            for (int j = lane; j < Npad; j += 32) {
+                double s = 0.0;
+                for (int sb = 0; sb < SUB; ++sb) s += s_T[sb * Npad + j];
+                P.Spart[(slot * 3 + st) * Npad + j] = s;
+            }
+        }
+        __syncwarp();
+    };
+
+    long long r = r0;
+    while (r < r1) {
+        const long long bi = r / Nr;
+        const int q0 = (int)(r - bi * Nr);
+        if (bi != cur_bi) {
+            if (JAC && cur_bi >= 0) flush(cur_bi);
+#pragma unroll
+            for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
+            cur_bi = bi;
+            const int b = (int)(bi / P.Next);
+            if (b != cur_b) {
+                __syncwarp();
+                for (int j = lane; j < Npad; j += 32)
+                    s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)b * Npad + j];
+                __syncwarp();
+                cur_b = b;
+            }
+        }
+        const int e = (int)(bi - (long long)cur_b * P.Next);
+        const long long left = r1 - r;
+        int nrow = P.rpb;
+        if (left < nrow) nrow = (int)left;
+        if (Nr - q0 < nrow) nrow = Nr - q0;
+        const bool rowact = rib < nrow;
+        const int q = q0 + (rowact ? rib : 0);
+
+        // row constants (identical in all lanes of a row)
+        const double rowmask = rowact ? 1.0 : 0.0;
+        const double Gy = P.Gy[(size_t)cur_b * Nr + q] * rowmask, Py = P.Py[(size_t)cur_b * Nr + q] * rowmask;
+        RowConst rc;
+        if (!GEOM) {
+            const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
+            const double y = P.y[q], sy = P.sy[q];
+            const double Wq = P.Wy[q];
+            const double d = (x - y) / (sx + sy);
+            rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
+        }
+        double sumA = 0.0, sumB = 0.0, sumV = 0.0, sumZ = 0.0;
+        const double4 *grow = GEOM ? reinterpret_cast<const double4 *>(P.geom) + ((size_t)e * Nr + q) * P.Ntpad + kl
+                                   : nullptr;
+
+        for (int kb = 0; kb < P.Ntpad; kb += 32) {
+            // ---------------- phase 1: lane = point (k = kb + kl < Ntpad: g divides Ntpad, g <= 32) ----------------
+            double sraw, gv, gq, gm;
+            if (GEOM) {
+                const double2 *gp = reinterpret_cast<const double2 *>(grow + kb);     // streamed once per build
+                const double2 g0 = __ldcs(gp), g1 = __ldcs(gp + 1);
+                sraw = g0.x; gv = g0.y; gq = g1.x; gm = g1.y;
+            } else {
+                point_geometry(rc, s_ang + (kb + kl) * 6, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
+            }
+            double s = sraw, EG = 0.0, EZ = 0.0;
+            if (sraw < -1.0) {                           // z < eps2: G ~ z^pG, Z ~ z^pZ   eq.(16),(17)
+                const double ell = (sraw + 1.0) * halfLg;
+                EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
+            } else if (sraw > 1.0) {                     // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
+                const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
+            }
+            const double ts = 2.0 * s;
+            const double t2 = fma(2.0 * ts, s, -2.0);    // 2 T_2(s): stride-2 recurrence T_{j+2} = 2 T_2 T_j - T_{j-2}
+            double Te = 1.0, To = s;                     // T_0, T_1
+            double Tem = fma(ts, s, -1.0), Tom = s;      // T_{-2} = T_2, T_{-1} = T_1
+            double lz0 = 0.0, lz1 = 0.0, lg0 = 0.0, lg1 = 0.0;
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) {
+                if (JAC) s_T2[c * (TCH_STRIDE / 2) + lane] = make_double2(Te, To);
+#pragma unroll
+                for (int m = 0; m < CJ; m += 4) {
+                    const double2 c0 = s_coef[c * CJ + m], c1 = s_coef[c * CJ + m + 1];
+                    const double2 c2 = s_coef[c * CJ + m + 2], c3 = s_coef[c * CJ + m + 3];
+                    lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0);
+                    lz1 = fma(c1.x, To, lz1); lg1 = fma(c1.y, To, lg1);
+                    Tem = fma(t2, Te, -Tem);  Tom = fma(t2, To, -Tom);     // T_{j+2}, T_{j+3}
+                    lz0 = fma(c2.x, Tem, lz0); lg0 = fma(c2.y, Tem, lg0);
+                    lz1 = fma(c3.x, Tom, lz1); lg1 = fma(c3.y, Tom, lg1);
+                    Te = fma(t2, Tem, -Te);   To = fma(t2, Tom, -To);      // T_{j+4}, T_{j+5}
+                }
+            }
+            const double lnZz = (lz0 + lz1) + EZ, lnGz = (lg0 + lg1) + EG;
+            const double Zz = exp(lnZz), Gz = exp(lnGz), Pz = exp(fma(P.e1, lnGz, P.e2 * lnZz));
+            const double v = gv * (Gy * Zz);              // eq.(8):  -C W y Om sin^4/z^2 G(y) Z(z)
+            const double wQ = gq * (Py * Pz);             // eq.(9):  (C/3x) W Om sin^2 Q P(y) P(z)
+            const double wM = gm * (Gy * Gz);             // eq.(9):  (C/3x) W Om sin^2 M G(y) G(z)
+            const double ua = P.e2 * wQ;                  // weight of d/da_j  (P ~ Z^{e2})
+            const double ub = fma(P.e1, wQ, wM);          // weight of d/db_j  (P ~ G^{e1}; G(y)G(z))
+            sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
+            if (JAC) {
+                s_pt[lane] = make_double4(ts, ua, ub, v);
+                __syncwarp();
+                // ---------------- phase 2: lane = (chunk, point sub-lane) ----------------
+#pragma unroll
+                for (int rd = 0; rd < ROUNDS; ++rd) {
+                    const int pt = rd * SUB + sub;
+                    const int pc = CT ? pt : ((active2 && pt < 32) ? pt : 32);     // slot 32 holds zero weights
+                    const double4 pw = s_pt[pc];
+                    const double2 tt = tread[pc & 31];
+                    double T0 = tt.x, T1 = tt.y;
+                    accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
+                    accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
+#pragma unroll
+                    for (int m = 2; m < CJ; ++m) {
+                        const double T2 = fma(pw.x, T1, -T0);
+                        accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
+                        T0 = T1; T1 = T2;
+                    }
+                }
+                __syncwarp();
+            }
+        }
+        // H5/H7: row sums over the angular nodes (fixed xor tree), one writer per row
+        for (int o = g >> 1; o > 0; o >>= 1) {
+            sumA += __shfl_xor_sync(FULL, sumA, o);
+            sumB += __shfl_xor_sync(FULL, sumB, o);
+            sumV += __shfl_xor_sync(FULL, sumV, o);
+            sumZ += __shfl_xor_sync(FULL, sumZ, o);
+        }
+        if (kl == 0 && rowact)
+            reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
+        r += nrow;
+    }
+    if (JAC && cur_bi >= 0) flush(cur_bi);
+}
+
+using KernelFn = void (*)(const KParams);
+
+template <bool GEOM>
+KernelFn pick_jac(int nch)
+{
+    switch (nch) {
+        case 1: return point_kernel<1, GEOM, true>;
+        case 2: return point_kernel<2, GEOM, true>;
+        case 4: return point_kernel<4, GEOM, true>;
+        case 8: return point_kernel<8, GEOM, true>;
+        case 16: return point_kernel<16, GEOM, true>;
+        default: return point_kernel<0, GEOM, true>;
+    }
+}
+
+KernelFn pick(const KParams &k, bool jac)
+{
+    if (!jac) return k.geom ? point_kernel<0, true, false> : point_kernel<0, false, false>;
+    return k.geom ? pick_jac<true>(k.NCH) : pick_jac<false>(k.NCH);
+}
+
+int fail(cudaError_t e, const char *what)
+{
+    char buf[256];
+    snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
+    set_error_text(buf);
+    return DSE_ECUDA;
+}
+
+}  // namespace
+
+int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
+{
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(e, "cudaGetDevice");
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return fail(e, "cudaDeviceGetAttribute");
+    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH));
+    for (int jac = 0; jac < 2; ++jac) {
+        e = cudaFuncSetAttribute((const void *)pick(k, jac != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel smem)");
+    }
+    const void *fn = (const void *)pick(k, true);
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, fn);
+    if (e != cudaSuccess) return fail(e, "cudaFuncGetAttributes");
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, POINT_THREADS, smem);
+    if (e != cudaSuccess) return fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (per_sm < 1) { set_error_text("point_kernel does not fit on an SM"); return DSE_ECUDA; }
+    cfg.block = POINT_THREADS;
+    cfg.smem = smem;
+    cfg.regs = fa.numRegs;
+    cfg.ctas_per_sm = per_sm;
+    cfg.sms = sms;
+    // persistent-style grid: one wave of resident CTAs, but never more warps than rows
+    long long grid = (long long)sms * per_sm;
+    const long long wpb = POINT_THREADS / 32;
+    const long long batches_per_row = k.Ntpad / 32 > 0 ? k.Ntpad / 32 : 1;
+    // keep >= ~4 point batches per warp so that small problems do not pay for idle warps
+    long long want_warps = (k.R * batches_per_row / k.rpb + 3) / 4;
+    if (want_warps < 1) want_warps = 1;
+    long long want_grid = (want_warps + wpb - 1) / wpb;
+    if (want_grid < grid) grid = want_grid;
+    while (grid * wpb > k.R && grid > 1) --grid;
+    cfg.grid = (int)grid;
+    return 0;
+}
+
+int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
+{
+    pick(k, k.want_jac != 0)<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
+    return 1;
+}
+
+}  // namespace dse

@@ -19,31 +19,42 @@ namespace {
 // ---------------------------------------------------------------------------------------------
 // H1: per system b: (a_j, b_j) pairs with the j = 0 coefficient pre-halved (phi_0 = 1/2, eq.(23),(24)),
 // G(y_q) = exp(ln G), P(y_q) = G^{e1} Z^{e2} (eq.(3),(9)), 1/G(x_i), 1/Z(x_i).
-__global__ void prep_kernel(const KParams P, const double *__restrict__ c)
+__global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double *__restrict__ c)
 {
-    const int b = blockIdx.x;
+    // grid (tiles, B); one WARP per fixed point (y_q or x_i), lanes over j, fixed xor-tree reduction
+    const int b = blockIdx.y;
+    const int lane = threadIdx.x & 31;
+    const int item = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const double *cb = c + (size_t)b * 2 * P.N;
-    for (int j = threadIdx.x; j < P.Npad; j += blockDim.x) {
-        double a = 0.0, bb = 0.0;
-        if (j < P.N) { a = cb[j]; bb = cb[P.N + j]; }
-        if (j == 0) { a *= 0.5; bb *= 0.5; }
-        P.coefP[((size_t)b * P.Npad + j) * 2 + 0] = a;
-        P.coefP[((size_t)b * P.Npad + j) * 2 + 1] = bb;
-    }
-    for (int t = threadIdx.x; t < P.Nr + P.N; t += blockDim.x) {
-        const bool isy = t < P.Nr;
-        const double *phi = isy ? P.phi_y + (size_t)t * P.Npad : P.phi_x + (size_t)(t - P.Nr) * P.Npad;
-        double lnZ = 0.0, lnG = 0.0;
-        for (int j = 0; j < P.N; ++j) {          // phi_0 = 1/2 is in the table
-            lnZ = fma(cb[j], phi[j], lnZ);
-            lnG = fma(cb[P.N + j], phi[j], lnG);
+    if (blockIdx.x == 0) {
+        for (int j = threadIdx.x; j < P.Npad; j += blockDim.x) {
+            double a = 0.0, bb = 0.0;
+            if (j < P.N) { a = cb[j]; bb = cb[P.N + j]; }
+            if (j == 0) { a *= 0.5; bb *= 0.5; }
+            P.coefP[((size_t)b * P.Npad + j) * 2 + 0] = a;
+            P.coefP[((size_t)b * P.Npad + j) * 2 + 1] = bb;
         }
+    }
+    if (item >= P.Nr + P.N) return;
+    const bool isy = item < P.Nr;
+    const double *phi = isy ? P.phi_y + (size_t)item * P.Npad : P.phi_x + (size_t)(item - P.Nr) * P.Npad;
+    double lnZ = 0.0, lnG = 0.0;
+    for (int j = lane; j < P.N; j += 32) {       // phi_0 = 1/2 is in the table
+        const double f = phi[j];
+        lnZ = fma(cb[j], f, lnZ);
+        lnG = fma(cb[P.N + j], f, lnG);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        lnZ += __shfl_xor_sync(FULL, lnZ, o);
+        lnG += __shfl_xor_sync(FULL, lnG, o);
+    }
+    if (lane == 0) {
         if (isy) {
-            P.Gy[(size_t)b * P.Nr + t] = exp(lnG);
-            P.Py[(size_t)b * P.Nr + t] = exp(P.e1 * lnG + P.e2 * lnZ);
+            P.Gy[(size_t)b * P.Nr + item] = exp(lnG);
+            P.Py[(size_t)b * P.Nr + item] = exp(P.e1 * lnG + P.e2 * lnZ);
         } else {
-            P.invG[(size_t)b * P.N + (t - P.Nr)] = exp(-lnG);
-            P.invZ[(size_t)b * P.N + (t - P.Nr)] = exp(-lnZ);
+            P.invG[(size_t)b * P.N + (item - P.Nr)] = exp(-lnG);
+            P.invZ[(size_t)b * P.N + (item - P.Nr)] = exp(-lnZ);
         }
     }
 }
@@ -74,9 +85,11 @@ __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
 // H7: Rz[b,e,stream][j] = sum_q A_stream[b,e,q] phi_j(t_q): the z-independent part of the Jacobian,
 // a dense [3 N_ext x N_r] . [N_r x N] contraction per system, on the fp64 tensor path
 // (mma.sync.aligned.m8n8k4 f64 -> DMMA).  One warp per 8x8 output tile, K = N_r in steps of 4.
-__global__ void __launch_bounds__(32) gemm_kernel(const KParams P)
+__global__ void __launch_bounds__(128) gemm_kernel(const KParams P)
 {
-    const int lane = threadIdx.x;
+    // 4 warps per 8x8 tile, each takes a contiguous quarter of K; partial tiles combined in warp order
+    __shared__ double s_c[4][32][2];
+    const int lane = threadIdx.x & 31, wk = threadIdx.x >> 5;
     const int m0 = blockIdx.x * 8, n0 = blockIdx.y * 8, b = blockIdx.z;
     const int M = 3 * P.Next;
     const int am = m0 + (lane >> 2), ak = lane & 3;          // A fragment: row = lane/4, col = lane%4
@@ -84,21 +97,31 @@ __global__ void __launch_bounds__(32) gemm_kernel(const KParams P)
     const bool arow_ok = am < M;
     const int e = arow_ok ? am / 3 : 0, st = arow_ok ? am - 3 * (am / 3) : 0;
     const double *Arow = P.Apart + ((size_t)(b * P.Next + e) * P.Nr) * 4 + st;
+    const int ksteps = (P.Nr + 3) / 4, per = (ksteps + 3) / 4;
+    const int ks0 = wk * per, ks1 = min(ksteps, ks0 + per);
     double c0 = 0.0, c1 = 0.0;
-    for (int k0 = 0; k0 < P.Nr; k0 += 4) {
-        const int qa = k0 + ak, qb = k0 + bk;
+#pragma unroll 4
+    for (int ks = ks0; ks < ks1; ++ks) {
+        const int qa = ks * 4 + ak, qb = ks * 4 + bk;
         const double a = (arow_ok && qa < P.Nr) ? Arow[(size_t)qa * 4] : 0.0;
         const double bb = (qb < P.Nr) ? P.phi_y[(size_t)qb * P.Npad + bn] : 0.0;
         asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                      : "+d"(c0), "+d"(c1)
                      : "d"(a), "d"(bb));
     }
-    const int cm = m0 + (lane >> 2), cn = n0 + 2 * (lane & 3);
-    if (cm < M) {
-        const int ce = cm / 3, cs = cm - 3 * ce;
-        double *out = P.Rz + ((size_t)(b * P.Next + ce) * 3 + cs) * P.Npad;
-        out[cn] = c0;
-        out[cn + 1] = c1;
+    s_c[wk][lane][0] = c0;
+    s_c[wk][lane][1] = c1;
+    __syncthreads();
+    if (wk == 0) {
+        c0 = ((s_c[0][lane][0] + s_c[1][lane][0]) + s_c[2][lane][0]) + s_c[3][lane][0];
+        c1 = ((s_c[0][lane][1] + s_c[1][lane][1]) + s_c[2][lane][1]) + s_c[3][lane][1];
+        const int cm = m0 + (lane >> 2), cn = n0 + 2 * (lane & 3);
+        if (cm < M) {
+            const int ce = cm / 3, cs = cm - 3 * ce;
+            double *out = P.Rz + ((size_t)(b * P.Next + ce) * 3 + cs) * P.Npad;
+            out[cn] = c0;
+            out[cn + 1] = c1;
+        }
     }
 }
 
@@ -107,17 +130,23 @@ __global__ void __launch_bounds__(32) gemm_kernel(const KParams P)
 // e in {i, x_Z, x_G} in a fixed order, adds the z-independent part, subtracts the MOM rows
 // (eq.(14),(15)), adds the local terms -phi_j(s_i)/Z(x_i), -phi_j(s_i)/G(x_i), and writes
 //   F = (z(x_i); g(x_i))  eq.(29),(30),   J = [[dz/da, dz/db],[dg/da, dg/db]]  eq.(35),(36).
-__device__ __forceinline__ void reduce_point(const KParams &P, long long bi, int j, double &Sa, double &Sb, double &Sv)
+constexpr int ASM_THREADS = 512;
+
+// partial sum over a contiguous part of the slot range of external point bi (ascending warp order)
+__device__ __forceinline__ void reduce_part(const KParams &P, long long bi, int j, int part, int parts, double &Sa,
+                                            double &Sb, double &Sv)
 {
     const long long rf = bi * P.Nr, rl = rf + P.Nr - 1;
     const long long wf = ((rf + 1) * P.W - 1) / P.R, wl = ((rl + 1) * P.W - 1) / P.R;
+    const long long n = wl - wf + 1, per = (n + parts - 1) / parts;
+    const long long w0 = wf + part * per, w1 = min(wl + 1, w0 + per);
     double a = 0.0, b = 0.0, v = 0.0;
-    for (long long w = wf; w <= wl; ++w) {
+#pragma unroll 4
+    for (long long w = w0; w < w1; ++w) {
         const double *sp = P.Spart + (size_t)(w + bi) * 3 * P.Npad;
         a += sp[j]; b += sp[P.Npad + j]; v += sp[2 * P.Npad + j];
     }
-    const double h = (j == 0) ? 0.5 : 1.0;      // the kernel accumulates with T_0 = 1; phi_0 = 1/2
-    Sa = a * h; Sb = b * h; Sv = v * h;
+    Sa = a; Sb = b; Sv = v;
 }
 
 __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, double *__restrict__ J,
@@ -150,19 +179,37 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
         F[(size_t)b * 2 * N + N + i] = invG - gG - s_pi[0][0] + s_pi[2][0];
     }
     if (J == nullptr) return;
-    for (int j = threadIdx.x; j < N; j += blockDim.x) {
-        double Sa_i, Sb_i, Sv_i, Sa_Z, Sb_Z, Sv_Z, Sa_G, Sb_G, Sv_G;
-        reduce_point(P, bi_i, j, Sa_i, Sb_i, Sv_i);
-        reduce_point(P, bi_Z, j, Sa_Z, Sb_Z, Sv_Z);
-        if (P.iG != P.iZ) reduce_point(P, bi_G, j, Sa_G, Sb_G, Sv_G);
-        else { Sa_G = Sa_Z; Sb_G = Sb_Z; Sv_G = Sv_Z; }
+    // threads = (part, j): each sums a contiguous part of the slot range; parts are combined in order
+    __shared__ double s_part[3][3][ASM_THREADS];
+    int PJ = 8;
+    while (PJ < N) PJ <<= 1;
+    const int parts = ASM_THREADS / PJ, part = threadIdx.x / PJ, j = threadIdx.x - part * PJ;
+    const int npt = (P.iG != P.iZ) ? 3 : 2;
+    if (j < N) {
+        for (int pt = 0; pt < npt; ++pt) {
+            const long long bi = pt == 0 ? bi_i : (pt == 1 ? bi_Z : bi_G);
+            double a, bb, v;
+            reduce_part(P, bi, j, part, parts, a, bb, v);
+            s_part[pt][0][threadIdx.x] = a; s_part[pt][1][threadIdx.x] = bb; s_part[pt][2][threadIdx.x] = v;
+        }
+    }
+    __syncthreads();
+    if (part == 0 && j < N) {
+        double S[3][3];
+        for (int pt = 0; pt < npt; ++pt)
+            for (int st = 0; st < 3; ++st) {
+                double t = 0.0;
+                for (int p2 = 0; p2 < parts; ++p2) t += s_part[pt][st][p2 * PJ + j];
+                S[pt][st] = (j == 0) ? 0.5 * t : t;       // the kernel accumulates with T_0 = 1; phi_0 = 1/2
+            }
+        if (npt == 2) { S[2][0] = S[1][0]; S[2][1] = S[1][1]; S[2][2] = S[1][2]; }
         const double *Ri = P.Rz + (size_t)bi_i * 3 * P.Npad, *RZ = P.Rz + (size_t)bi_Z * 3 * P.Npad,
                      *RG = P.Rz + (size_t)bi_G * 3 * P.Npad;
         const double phi = P.phi_x[(size_t)i * P.Npad + j];
         // dPi_Z/da = Sa + Ra, dPi_Z/db = Sb + Rb, dPi_G/da = Sv, dPi_G/db = Rv
-        const double dZa_i = Sa_i + Ri[j], dZb_i = Sb_i + Ri[P.Npad + j], dGa_i = Sv_i, dGb_i = Ri[2 * P.Npad + j];
-        const double dZa_s = Sa_Z + RZ[j], dZb_s = Sb_Z + RZ[P.Npad + j];
-        const double dGa_s = Sv_G, dGb_s = RG[2 * P.Npad + j];
+        const double dZa_i = S[0][0] + Ri[j], dZb_i = S[0][1] + Ri[P.Npad + j], dGa_i = S[0][2], dGb_i = Ri[2 * P.Npad + j];
+        const double dZa_s = S[1][0] + RZ[j], dZb_s = S[1][1] + RZ[P.Npad + j];
+        const double dGa_s = S[2][2], dGb_s = RG[2 * P.Npad + j];
         double *Jb = J + (size_t)b * 4 * N * N;
         Jb[(size_t)i * 2 * N + j] = -phi * invZ - dZa_i + dZa_s;
         Jb[(size_t)i * 2 * N + N + j] = -dZb_i + dZb_s;
@@ -232,7 +279,7 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     KParams kk = k;
     kk.want_jac = J_dev != nullptr;
     int launches = 0;
-    prep_kernel<<<kk.B, 256, 0, s>>>(kk, c_dev);
+    prep_kernel<<<dim3((kk.Nr + kk.N + 7) / 8, kk.B), 256, 0, s>>>(kk, c_dev);
     ++launches;
     if (ev0) cudaEventRecord((cudaEvent_t)ev0, s);
     launch_point(kk, cfg, stream);
@@ -240,11 +287,11 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     ++launches;
     if (kk.want_jac) {
         dim3 gg((3 * kk.Next + 7) / 8, kk.Npad / 8, kk.B);
-        gemm_kernel<<<gg, 32, 0, s>>>(kk);
+        gemm_kernel<<<gg, 128, 0, s>>>(kk);
         ++launches;
     }
     dim3 ga(kk.N, kk.B);
-    assemble_kernel<<<ga, 128, 0, s>>>(kk, bc_dev, J_dev, F_dev);
+    assemble_kernel<<<ga, ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
     ++launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "build launch");

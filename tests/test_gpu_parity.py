@@ -63,7 +63,7 @@ def test_configs_0_1_full_parity(orc, cfg, flags):
     check(J[0], F[0], Jo, Fo)
     # residual-only entry point gives the same F
     _, F2 = gpu_build(w, c, bc, flags, jac=False)
-    assert np.array_equal(F2, F)
+    assert np.allclose(F2, F, rtol=1e-12, atol=0)      # different template instance: same math, other rounding
 
 
 def test_tables_match_oracle(orc):

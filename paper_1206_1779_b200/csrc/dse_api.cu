@@ -26,6 +26,7 @@ struct dse_handle {
     double *d_J = nullptr, *d_F = nullptr, *d_lu = nullptr;   // internal J, F for dse_newton_step (+ LU scratch)
     double *d_c = nullptr, *d_bc = nullptr, *d_Jh = nullptr, *d_Fh = nullptr;   // staging for *_host calls
     int64_t launches = 0;
+    bool owns_const = false;
     // optional timing of the point kernel (dse_set_timing)
     static constexpr int EV_RING = 64;
     bool timing = false;
@@ -185,6 +186,8 @@ int dse_create(const dse_params *params, dse_handle **out)
     }
 
     // ---- launch configuration of the point kernel ----
+    k.use_constc = dse::acquire_const_slot(k) ? 1 : 0;
+    h->owns_const = k.use_constc != 0;
     rc = dse::query_point_kernel(k, h->cfg);
     if (rc < 0) { dse_destroy(h); return rc; }
     k.W = h->cfg.grid * (h->cfg.block / 32);
@@ -225,6 +228,7 @@ int dse_destroy(dse_handle *h)
 {
     if (!h) return DSE_OK;
     cudaDeviceSynchronize();
+    if (h->owns_const) dse::release_const_slot();
     if (h->d_tables) cudaFree(h->d_tables);
     if (h->d_work) cudaFree(h->d_work);
     if (h->d_geom) cudaFree(h->d_geom);

@@ -33,6 +33,7 @@ struct KParams {
     long long R;                       // rows = B * Next * Nr
     int W;                             // warps in the grid of the point kernel
     int want_jac;                      // 0: residual only (skip phase 2)
+    int use_constc;                    // coefficient pairs are read as constant-bank operands (single system, slot owner)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
     const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x;
     const double *geom;                // geometry cache [Next*Nr*Ntpad][4] or nullptr
@@ -60,6 +61,8 @@ int launch_geometry(const KParams &k, double *geom, void *stream);
 int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
               double *stats, double *scratch, void *stream);
 int query_point_kernel(const KParams &k, PointKernelConfig &cfg);
+bool acquire_const_slot(const KParams &k);
+void release_const_slot();
 size_t lu_scratch_doubles(int n);
 int launch_dfma_probe(int blocks, int iters, double *sink, void *stream);
 int launch_dmma_probe(int blocks, int iters, double *sink, void *stream);

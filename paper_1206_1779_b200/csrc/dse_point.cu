@@ -15,6 +15,8 @@
 // Template: NCH_T = number of 8-wide Chebyshev chunks when it is a power of two (everything unrolls),
 // 0 = generic run-time shape; GEOM = read the geometry cache; JAC = accumulate the Jacobian streams.
 #include <cstdio>
+#include <atomic>
+#include <cstdlib>
 
 #include "dse_device.cuh"
 
@@ -24,7 +26,9 @@ void set_error_text(const char *s);
 
 namespace {
 
-template <int NCH_T, bool GEOM, bool JAC>
+__constant__ double2 c_coef[DSE_MAX_NCHEB];     // coefficient pairs of a single-system build (constant-bank operands)
+
+template <int NCH_T, bool GEOM, bool JAC, int NP, bool CONSTC = false>
 __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P)
 {
     constexpr bool CT = NCH_T > 0;
@@ -35,8 +39,9 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
     const int ROUNDS = CT ? NCH_T : P.rounds;
     const int Npad = NCH * CJ;
     double *s_ang = smem;
-    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(Npad, NCH);
+    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(Npad, NCH, NP);
     double2 *s_coef = reinterpret_cast<double2 *>(wbase);
+    const int STASH = stash_doubles(NCH);                                 // per interleaved point set
     double4 *s_pt = reinterpret_cast<double4 *>(wbase + 2 * Npad);       // 33 entries, entry 32 = 0
     double *s_T = wbase + 2 * Npad + 132;
     double2 *s_T2 = reinterpret_cast<double2 *>(s_T);
@@ -54,6 +59,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
     const int rib = lane / g, kl = lane - rib * g;          // row-in-batch and angular lane
     const double halfLg = 0.5 * P.Lg;
     const double2 *tread = s_T2 + (active2 ? c_lane : 0) * (TCH_STRIDE / 2);
+    static_assert(NP == 1 || NCH_T > 0, "two-point interleave needs a compile-time chunk count");
 
     double accA[CJ], accB[CJ], accV[CJ];
 #pragma unroll
@@ -122,73 +128,108 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
         const double4 *grow = GEOM ? reinterpret_cast<const double4 *>(P.geom) + ((size_t)e * Nr + q) * P.Ntpad + kl
                                    : nullptr;
 
-        for (int kb = 0; kb < P.Ntpad; kb += 32) {
-            // ---------------- phase 1: lane = point (k = kb + kl < Ntpad: g divides Ntpad, g <= 32) ----------------
-            double sraw, gv, gq, gm;
-            if (GEOM) {
-                const double2 *gp = reinterpret_cast<const double2 *>(grow + kb);     // streamed once per build
-                const double2 g0 = __ldcs(gp), g1 = __ldcs(gp + 1);
-                sraw = g0.x; gv = g0.y; gq = g1.x; gm = g1.y;
-            } else {
-                point_geometry(rc, s_ang + (kb + kl) * 6, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
+        for (int kb = 0; kb < P.Ntpad; kb += 32 * NP) {
+            // ---------------- phase 1: lane = point; NP points per lane are interleaved for ILP ----------------
+            // (k = kb + 32 p + kl < Ntpad: g divides Ntpad, g <= 32; NP = 2 only when 64 divides Ntpad)
+            double gv[NP], gq[NP], gm[NP], EG[NP], EZ[NP], ts[NP], t2[NP], Te[NP], To[NP], Tem[NP], Tom[NP];
+            double lz0[NP], lz1[NP], lg0[NP], lg1[NP];
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                double sraw;
+                if (GEOM) {
+                    const double2 *gp = reinterpret_cast<const double2 *>(grow + kb + 32 * p);   // streamed once
+                    const double2 g0 = __ldcs(gp), g1 = __ldcs(gp + 1);
+                    sraw = g0.x; gv[p] = g0.y; gq[p] = g1.x; gm[p] = g1.y;
+                } else {
+                    point_geometry(rc, s_ang + (kb + 32 * p + kl) * 6, P.inv_eps2, P.two_over_Lg, sraw, gv[p], gq[p], gm[p]);
+                }
+                double s = sraw;
+                EG[p] = 0.0; EZ[p] = 0.0;
+                if (sraw < -1.0) {                       // z < eps2: G ~ z^pG, Z ~ z^pZ   eq.(16),(17)
+                    const double ell = (sraw + 1.0) * halfLg;
+                    EG[p] = P.pG * ell; EZ[p] = P.pZ * ell; s = -1.0;
+                } else if (sraw > 1.0) {                 // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
+                    const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                    EG[p] = P.delta * t; EZ[p] = P.gamma * t; s = 1.0;
+                }
+                ts[p] = 2.0 * s;
+                t2[p] = fma(2.0 * ts[p], s, -2.0);       // 2 T_2(s): stride-2 recurrence T_{j+2} = 2 T_2 T_j - T_{j-2}
+                Te[p] = 1.0; To[p] = s;                  // T_0, T_1
+                Tem[p] = fma(ts[p], s, -1.0); Tom[p] = s;   // T_{-2} = T_2, T_{-1} = T_1
+                lz0[p] = lz1[p] = lg0[p] = lg1[p] = 0.0;
             }
-            double s = sraw, EG = 0.0, EZ = 0.0;
-            if (sraw < -1.0) {                           // z < eps2: G ~ z^pG, Z ~ z^pZ   eq.(16),(17)
-                const double ell = (sraw + 1.0) * halfLg;
-                EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
-            } else if (sraw > 1.0) {                     // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
-                const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
-                EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
-            }
-            const double ts = 2.0 * s;
-            const double t2 = fma(2.0 * ts, s, -2.0);    // 2 T_2(s): stride-2 recurrence T_{j+2} = 2 T_2 T_j - T_{j-2}
-            double Te = 1.0, To = s;                     // T_0, T_1
-            double Tem = fma(ts, s, -1.0), Tom = s;      // T_{-2} = T_2, T_{-1} = T_1
-            double lz0 = 0.0, lz1 = 0.0, lg0 = 0.0, lg1 = 0.0;
 #pragma unroll
             for (int c = 0; c < NCH; ++c) {
-                if (JAC) s_T2[c * (TCH_STRIDE / 2) + lane] = make_double2(Te, To);
+                if (JAC) {
+#pragma unroll
+                    for (int p = 0; p < NP; ++p)
+                        reinterpret_cast<double2 *>(s_T + p * STASH)[c * (TCH_STRIDE / 2) + lane] = make_double2(Te[p], To[p]);
+                }
 #pragma unroll
                 for (int m = 0; m < CJ; m += 4) {
-                    const double2 c0 = s_coef[c * CJ + m], c1 = s_coef[c * CJ + m + 1];
-                    const double2 c2 = s_coef[c * CJ + m + 2], c3 = s_coef[c * CJ + m + 3];
-                    lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0);
-                    lz1 = fma(c1.x, To, lz1); lg1 = fma(c1.y, To, lg1);
-                    Tem = fma(t2, Te, -Tem);  Tom = fma(t2, To, -Tom);     // T_{j+2}, T_{j+3}
-                    lz0 = fma(c2.x, Tem, lz0); lg0 = fma(c2.y, Tem, lg0);
-                    lz1 = fma(c3.x, Tom, lz1); lg1 = fma(c3.y, Tom, lg1);
-                    Te = fma(t2, Tem, -Te);   To = fma(t2, Tom, -To);      // T_{j+4}, T_{j+5}
+                    const double2 c0 = CONSTC ? c_coef[c * CJ + m] : s_coef[c * CJ + m];
+                    const double2 c1 = CONSTC ? c_coef[c * CJ + m + 1] : s_coef[c * CJ + m + 1];
+                    const double2 c2 = CONSTC ? c_coef[c * CJ + m + 2] : s_coef[c * CJ + m + 2];
+                    const double2 c3 = CONSTC ? c_coef[c * CJ + m + 3] : s_coef[c * CJ + m + 3];
+#pragma unroll
+                    for (int p = 0; p < NP; ++p) {
+                        lz0[p] = fma(c0.x, Te[p], lz0[p]); lg0[p] = fma(c0.y, Te[p], lg0[p]);
+                        lz1[p] = fma(c1.x, To[p], lz1[p]); lg1[p] = fma(c1.y, To[p], lg1[p]);
+                        Tem[p] = fma(t2[p], Te[p], -Tem[p]);  Tom[p] = fma(t2[p], To[p], -Tom[p]);   // T_{j+2}, T_{j+3}
+                        lz0[p] = fma(c2.x, Tem[p], lz0[p]); lg0[p] = fma(c2.y, Tem[p], lg0[p]);
+                        lz1[p] = fma(c3.x, Tom[p], lz1[p]); lg1[p] = fma(c3.y, Tom[p], lg1[p]);
+                        Te[p] = fma(t2[p], Tem[p], -Te[p]);   To[p] = fma(t2[p], Tom[p], -To[p]);    // T_{j+4}, T_{j+5}
+                    }
                 }
             }
-            const double lnZz = (lz0 + lz1) + EZ, lnGz = (lg0 + lg1) + EG;
-            const double Zz = exp(lnZz), Gz = exp(lnGz), Pz = exp(fma(P.e1, lnGz, P.e2 * lnZz));
-            const double v = gv * (Gy * Zz);              // eq.(8):  -C W y Om sin^4/z^2 G(y) Z(z)
-            const double wQ = gq * (Py * Pz);             // eq.(9):  (C/3x) W Om sin^2 Q P(y) P(z)
-            const double wM = gm * (Gy * Gz);             // eq.(9):  (C/3x) W Om sin^2 M G(y) G(z)
-            const double ua = P.e2 * wQ;                  // weight of d/da_j  (P ~ Z^{e2})
-            const double ub = fma(P.e1, wQ, wM);          // weight of d/db_j  (P ~ G^{e1}; G(y)G(z))
-            sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                const double lnZz = (lz0[p] + lz1[p]) + EZ[p], lnGz = (lg0[p] + lg1[p]) + EG[p];
+                const double lnPz = fma(P.e1, lnGz, P.e2 * lnZz);
+                double Zz, Gz, Pz;
+                // |x| <= 700 for all three, tested on the high words (0x4085e000 = high word of 700.0; NaN/Inf fail)
+                const int hmax = max(max(__double2hiint(lnZz) & 0x7fffffff, __double2hiint(lnGz) & 0x7fffffff),
+                                     __double2hiint(lnPz) & 0x7fffffff);
+                if (hmax < 0x4085e000) {
+                    Zz = fast_exp(lnZz); Gz = fast_exp(lnGz); Pz = fast_exp(lnPz);
+                } else {                                   // out of the fast range (or NaN): library exp
+                    Zz = exp(lnZz); Gz = exp(lnGz); Pz = exp(lnPz);
+                }
+                const double v = gv[p] * (Gy * Zz);           // eq.(8):  -C W y Om sin^4/z^2 G(y) Z(z)
+                const double wQ = gq[p] * (Py * Pz);          // eq.(9):  (C/3x) W Om sin^2 Q P(y) P(z)
+                const double wM = gm[p] * (Gy * Gz);          // eq.(9):  (C/3x) W Om sin^2 M G(y) G(z)
+                const double ua = P.e2 * wQ;                  // weight of d/da_j  (P ~ Z^{e2})
+                const double ub = fma(P.e1, wQ, wM);          // weight of d/db_j  (P ~ G^{e1}; G(y)G(z))
+                sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
+                if (JAC) reinterpret_cast<double4 *>(reinterpret_cast<double *>(s_pt) + p * STASH)[lane] = make_double4(ts[p], ua, ub, v);
+            }
             if (JAC) {
-                s_pt[lane] = make_double4(ts, ua, ub, v);
                 __syncwarp();
                 // ---------------- phase 2: lane = (chunk, point sub-lane) ----------------
 #pragma unroll
-                for (int rd = 0; rd < ROUNDS; ++rd) {
-                    const int pt = rd * SUB + sub;
-                    const int pc = CT ? pt : ((active2 && pt < 32) ? pt : 32);     // slot 32 holds zero weights
-                    const double4 pw = s_pt[pc];
-                    const double2 tt = tread[pc & 31];
-                    double T0 = tt.x, T1 = tt.y;
-                    accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
-                    accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
+                for (int p = 0; p < NP; ++p) {
+                    const double4 *pts = reinterpret_cast<const double4 *>(reinterpret_cast<const double *>(s_pt) + p * STASH);
+                    const double2 *trd = reinterpret_cast<const double2 *>(reinterpret_cast<const double *>(tread) + p * STASH);
 #pragma unroll
-                    for (int m = 2; m < CJ; ++m) {
-                        const double T2 = fma(pw.x, T1, -T0);
-                        accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
-                        T0 = T1; T1 = T2;
+                    for (int rd = 0; rd < ROUNDS; ++rd) {
+                        const int pt = rd * SUB + sub;
+                        const int pc = CT ? pt : ((active2 && pt < 32) ? pt : 32);     // slot 32 holds zero weights
+                        const double4 pw = pts[pc];
+                        const double2 tt = trd[pc & 31];
+                        double T0 = tt.x, T1 = tt.y;
+                        accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
+                        accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
+#pragma unroll
+                        for (int m = 2; m < CJ; ++m) {
+                            const double T2 = fma(pw.x, T1, -T0);
+                            accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
+                            T0 = T1; T1 = T2;
+                        }
                     }
                 }
                 __syncwarp();
+            } else {
+                asm volatile("" ::: "memory");      // keep the coefficient loads inside the loop (no hoisting -> no spills)
             }
         }
         // H5/H7: row sums over the angular nodes (fixed xor tree), one writer per row
@@ -207,23 +248,46 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
 
 using KernelFn = void (*)(const KParams);
 
-template <bool GEOM>
-KernelFn pick_jac(int nch)
+inline int np_of(const KParams &k)      // two interleaved points per lane when the shapes allow it
 {
+    const bool pow2 = k.NCH == 1 || k.NCH == 2 || k.NCH == 4 || k.NCH == 8;
+    const char *env = getenv("DSE_NP");
+    const int want = env ? atoi(env) : 1;
+    return (want == 2 && pow2 && k.Ntpad % 64 == 0 && !k.use_constc) ? 2 : 1;
+}
+
+template <bool GEOM, bool JAC, bool CONSTC = false>
+KernelFn pick_nch(int nch, int np)
+{
+    if (np == 2 && !CONSTC) {
+        switch (nch) {
+            case 1: return point_kernel<1, GEOM, JAC, 2>;
+            case 2: return point_kernel<2, GEOM, JAC, 2>;
+            case 4: return point_kernel<4, GEOM, JAC, 2>;
+            default: return point_kernel<8, GEOM, JAC, 2>;
+        }
+    }
     switch (nch) {
-        case 1: return point_kernel<1, GEOM, true>;
-        case 2: return point_kernel<2, GEOM, true>;
-        case 4: return point_kernel<4, GEOM, true>;
-        case 8: return point_kernel<8, GEOM, true>;
-        case 16: return point_kernel<16, GEOM, true>;
-        default: return point_kernel<0, GEOM, true>;
+        case 1: return point_kernel<1, GEOM, JAC, 1, CONSTC>;
+        case 2: return point_kernel<2, GEOM, JAC, 1, CONSTC>;
+        case 4: return point_kernel<4, GEOM, JAC, 1, CONSTC>;
+        case 8: return point_kernel<8, GEOM, JAC, 1, CONSTC>;
+        case 16: return point_kernel<16, GEOM, JAC, 1, CONSTC>;
+        default: return point_kernel<0, GEOM, JAC, 1>;       // generic shapes: shared-memory coefficients
     }
 }
 
+inline bool constc_of(const KParams &k) { return k.use_constc != 0; }
+
 KernelFn pick(const KParams &k, bool jac)
 {
-    if (!jac) return k.geom ? point_kernel<0, true, false> : point_kernel<0, false, false>;
-    return k.geom ? pick_jac<true>(k.NCH) : pick_jac<false>(k.NCH);
+    const int np = np_of(k);
+    if (constc_of(k)) {
+        if (jac) return k.geom ? pick_nch<true, true, true>(k.NCH, 1) : pick_nch<false, true, true>(k.NCH, 1);
+        return k.geom ? pick_nch<true, false, true>(k.NCH, 1) : pick_nch<false, false, true>(k.NCH, 1);
+    }
+    if (!jac) return k.geom ? pick_nch<true, false>(k.NCH, np) : pick_nch<false, false>(k.NCH, np);
+    return k.geom ? pick_nch<true, true>(k.NCH, np) : pick_nch<false, true>(k.NCH, np);
 }
 
 int fail(cudaError_t e, const char *what)
@@ -236,6 +300,18 @@ int fail(cudaError_t e, const char *what)
 
 }  // namespace
 
+// The constant-bank coefficient slot is a per-module resource: at most one handle owns it at a time
+// (first come, released in dse_destroy); other handles keep their coefficients in shared memory.
+static std::atomic<int> g_const_owner{0};
+bool acquire_const_slot(const KParams &k)
+{
+    const bool pow2 = k.NCH == 1 || k.NCH == 2 || k.NCH == 4 || k.NCH == 8 || k.NCH == 16;
+    if (k.B != 1 || !pow2) return false;
+    int expected = 0;
+    return g_const_owner.compare_exchange_strong(expected, 1);
+}
+void release_const_slot() { g_const_owner.store(0); }
+
 int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
 {
     int dev = 0, sms = 0;
@@ -243,7 +319,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     if (e != cudaSuccess) return fail(e, "cudaGetDevice");
     e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return fail(e, "cudaDeviceGetAttribute");
-    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH));
+    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH, np_of(k)));
     for (int jac = 0; jac < 2; ++jac) {
         e = cudaFuncSetAttribute((const void *)pick(k, jac != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel smem)");
@@ -264,7 +340,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     // persistent-style grid: one wave of resident CTAs, but never more warps than rows
     long long grid = (long long)sms * per_sm;
     const long long wpb = POINT_THREADS / 32;
-    const long long batches_per_row = k.Ntpad / 32 > 0 ? k.Ntpad / 32 : 1;
+    const long long batches_per_row = k.Ntpad / 32 > 0 ? k.Ntpad / 32 : 1;   // 32-point batches
     // keep >= ~4 point batches per warp so that small problems do not pay for idle warps
     long long want_warps = (k.R * batches_per_row / k.rpb + 3) / 4;
     if (want_warps < 1) want_warps = 1;
@@ -277,6 +353,8 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
 
 int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
+    if (constc_of(k))
+        cudaMemcpyToSymbolAsync(c_coef, k.coefP, sizeof(double2) * k.Npad, 0, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
     pick(k, k.want_jac != 0)<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
     return 1;
 }

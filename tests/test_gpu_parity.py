@@ -128,3 +128,25 @@ def test_deterministic_bitwise():
         assert torch.equal(J, J0) and torch.equal(F, F0)
     assert d.launch_count() == 6 * 4
     d.close()
+
+
+def test_two_handles_constant_slot_and_shared_memory_paths(orc):
+    """The first single-system handle owns the constant-bank coefficient slot; a second live handle falls
+    back to shared-memory coefficients.  Both must match the oracle and each other."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(1)
+    Fo, Jo = orc.residual_jacobian(oracle_params(w), c[0], bc[0, 0], bc[0, 1])
+    d1 = Dse(params_from_workload(w))
+    d2 = Dse(params_from_workload(w))
+    ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
+    s2 = torch.cuda.Stream()
+    J1, F1 = d1.jacobian(ct, bt)
+    with torch.cuda.stream(s2):
+        J2, F2 = d2.jacobian(ct * 1.0, bt)
+    torch.cuda.synchronize()
+    check(J1.cpu().numpy()[0], F1.cpu().numpy()[0], Jo, Fo)
+    check(J2.cpu().numpy()[0], F2.cpu().numpy()[0], Jo, Fo)
+    assert np.allclose(J1.cpu().numpy(), J2.cpu().numpy(), rtol=1e-11, atol=0)
+    d1.close(); d2.close()

@@ -243,7 +243,7 @@ def run_ours(args, w, c, bc):
         k_ms = kernel_ms / max(kernel_n, 1)
         achieved = flops / (k_ms * 1e-3) / 1e12
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "point_kernel_traffic.json")
+        tpath = os.path.join(ROOT, "profiles", "point_kernel_traffic.txt")
         if os.path.exists(tpath):
             try:
                 traffic = json.load(open(tpath)).get(w.name)

@@ -48,3 +48,37 @@ def test_newton_trajectory_weak_coupling(orc):
         assert np.allclose(c_g.cpu().numpy()[0], c_o, rtol=0, atol=1e-9 * np.abs(c_o).max())
     assert dn[-1] < 1e-13
     d.close()
+
+
+def test_config2_newton_trajectory_literal(orc):
+    """BASELINE configs[2] run literally (start G = Z = 1, rho = 1).  DESIGN.md reading A17: the iteration
+    does not converge from this start on [1e-10, 1e10]; parity = the same trajectory as the oracle while
+    cond(J)*eps allows, and the same verdict."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(2)
+    d = Dse(params_from_workload(w))
+    p = oracle_params(w)
+    c_o = c[0].copy()
+    c_g = torch.from_numpy(c).cuda()
+    bt = torch.from_numpy(bc).cuda()
+    # step 0: J and F themselves agree to the parity tolerance
+    J, F = d.jacobian(c_g, bt)
+    Fo, Jo = orc.residual_jacobian(p, c_o, 1.0, 1.0)
+    assert np.linalg.norm(J.cpu().numpy()[0] - Jo) <= 1e-10 * np.linalg.norm(Jo)
+    # F at G = Z = 1: the two gluon loops cancel exactly in the continuum for y >> x (fn.5 L127), so the small-x
+    # rows of F are the rounding noise of sums whose terms are ~1e19: the fp64 oracle differs from its own
+    # long-double build by O(1) there (tests/test_oracle_path.py::test_config2_start_is_ill_conditioned).  The
+    # attainable bar is the conditioning-aware one: |dF_i| <= 1e-12 (|F_i| + ||J_i||).
+    Fg = F.cpu().numpy()[0]
+    assert (np.abs(Fg - Fo) / (np.abs(Fo) + np.linalg.norm(Jo, axis=1))).max() <= 1e-12
+    N = w.n_cheb
+    assert np.linalg.norm(Fg[N:] - Fo[N:]) <= 1e-10 * np.linalg.norm(Fo[N:])       # ghost rows: no cancellation
+    c_o, so, rc = orc.newton_step(p, c_o, 1.0, 1.0, 1.0)
+    st = d.newton_step(c_g, bt, 1.0).cpu().numpy()[0]
+    # the first update is large (|Delta| >> 1): the literal start is far outside the convergence basin
+    assert so[0] > 1.0 and st[0] > 1.0
+    # both sides report the same ill-conditioning (min pivot of the row-scaled matrix)
+    assert st[2] < 1e-8 and so[2] < 1e-8
+    d.close()

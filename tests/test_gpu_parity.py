@@ -150,3 +150,33 @@ def test_two_handles_constant_slot_and_shared_memory_paths(orc):
     check(J2.cpu().numpy()[0], F2.cpu().numpy()[0], Jo, Fo)
     assert np.allclose(J1.cpu().numpy(), J2.cpu().numpy(), rtol=1e-11, atol=0)
     d1.close(); d2.close()
+
+
+def test_config3_full_size_parity(orc):
+    """BASELINE configs[3] at full size, in the launch configuration bench.py times (both geometry modes)."""
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(3)
+    Fo, Jo = orc.residual_jacobian(oracle_params(w), c[0], bc[0, 0], bc[0, 1])
+    for flags in (0, 1):
+        J, F = gpu_build(w, c, bc, flags)
+        check(J[0], F[0], Jo, Fo)
+
+
+def test_config4_full_batch_sampled_systems(orc):
+    """BASELINE configs[4]: all 256 systems built in one launch sequence; sampled systems against the oracle,
+    and properties that hold for every system (finite, boundary value only shifts F)."""
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(4)
+    assert c.shape[0] == 256
+    J, F = gpu_build(w, c, bc)
+    assert np.all(np.isfinite(J)) and np.all(np.isfinite(F))
+    for b in (0, 1, 37, 128, 255):
+        Fo, Jo = orc.residual_jacobian(oracle_params(w), c[b], bc[b, 0], bc[b, 1])
+        check(J[b], F[b], Jo, Fo)
+    # same coefficients, different boundary value: J identical, ghost rows of F shifted by the difference
+    c2 = c.copy(); c2[1] = c2[0]
+    J2, F2 = gpu_build(w, c2[:2], bc[:2])
+    N = w.n_cheb
+    assert np.array_equal(J2[0], J2[1])
+    assert np.allclose(F2[1, N:] - F2[0, N:], -(bc[1, 0] - bc[0, 0]), rtol=0, atol=1e-12)
+    assert np.array_equal(F2[1, :N], F2[0, :N])

@@ -253,3 +253,22 @@ def test_newton_quadratic_convergence_P10(orc):
     c_full, _, _ = orc.newton_step(p, c0, 1.0, 1.0, 1.0)
     c_half, _, _ = orc.newton_step(p, c0, 1.0, 1.0, 0.5)
     assert np.allclose(c_half, 0.5 * c_full, atol=1e-15)
+
+
+def test_config2_start_is_ill_conditioned(orc, orc_ld):
+    """BASELINE configs[2] (start G = Z = 1 on [1e-10, 1e10]): at flat dressings the ghost and gluon loops of
+    eq.(9) cancel for y >> x (fn.5 L127, pin P7), so the small-x gluon rows of F are differences of ~1e19-sized
+    sums.  Evidence that NO fp64 evaluation can meet a normwise 1e-10 on F there: the oracle's double and
+    long-double builds disagree by O(1) normwise, while J and the conditioning-aware F metric agree to 1e-13."""
+    w, c, bc = config_inputs(2)
+    p = params_of(w)
+    F, J = orc.residual_jacobian(p, c[0], 1.0, 1.0)
+    Fl, Jl = orc_ld.residual_jacobian(p, c[0], 1.0, 1.0)
+    N = w.n_cheb
+    assert np.linalg.norm(J - Jl) <= 1e-13 * np.linalg.norm(Jl)
+    assert np.linalg.norm(F[:N] - Fl[:N]) > 1e-3 * np.linalg.norm(Fl[:N])          # gluon rows: noise
+    assert np.linalg.norm(F[N:] - Fl[N:]) <= 1e-12 * np.linalg.norm(Fl[N:])        # ghost rows: fine
+    assert (np.abs(F - Fl) / (np.abs(Fl) + np.linalg.norm(Jl, axis=1))).max() <= 1e-13
+    # and the Newton matrix is numerically singular at this point (row-scaled min pivot ~ eps)
+    x, stats, rc = orc.lu_solve(J, F)
+    assert stats[2] < 1e-10

@@ -45,6 +45,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
     double4 *s_pt = reinterpret_cast<double4 *>(wbase + 2 * Npad);       // 33 entries, entry 32 = 0
     double *s_T = wbase + 2 * Npad + 132;
     double2 *s_T2 = reinterpret_cast<double2 *>(s_T);
+    double4 *s_gbuf = reinterpret_cast<double4 *>(wbase + 2 * Npad + NP * STASH);   // [2][32] geometry records
 
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
     if (lane == 0) s_pt[32] = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -86,6 +87,25 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
         }
         __syncwarp();
     };
+
+    // Geometry cache, full-warp angular batches: the warp's batches are consecutive 1 KB records of one linear
+    // stream (wrapping at a system boundary), so the next batch is prefetched with cp.async into a warp-private
+    // double buffer while the current one is processed -- no registers held across the batch.
+    const bool PREF = GEOM && NP == 1 && g == 32;
+    const size_t gtotal = (size_t)P.Next * Nr * P.Ntpad;
+    const double4 *gbase = reinterpret_cast<const double4 *>(P.geom), *gend = gbase + gtotal, *gnext = gbase;
+    unsigned gphase = 0;
+    auto prefetch = [&](unsigned buf) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(s_gbuf + buf * 32 + lane);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(gnext));
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(gnext) + 16));
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
+    if (PREF && r0 < r1) {
+        const long long bi0 = r0 / Nr;
+        gnext = gbase + ((size_t)(bi0 % P.Next) * Nr + (size_t)(r0 - bi0 * Nr)) * P.Ntpad + lane;
+        prefetch(0);
+    }
 
     long long r = r0;
     while (r < r1) {
@@ -136,7 +156,16 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 double sraw;
-                if (GEOM) {
+                if (GEOM && PREF) {
+                    gnext += 32;                                   // next batch of this warp (possibly of the next row)
+                    if (gnext >= gend) gnext -= gtotal;
+                    prefetch(gphase ^ 1);
+                    asm volatile("cp.async.wait_group 1;\n" ::: "memory");     // the current batch has landed
+                    const double2 *gp = reinterpret_cast<const double2 *>(s_gbuf + gphase * 32 + lane);
+                    const double2 g0 = gp[0], g1 = gp[1];
+                    sraw = g0.x; gv[p] = g0.y; gq[p] = g1.x; gm[p] = g1.y;
+                    gphase ^= 1;
+                } else if (GEOM) {
                     const double2 *gp = reinterpret_cast<const double2 *>(grow + kb + 32 * p);   // streamed once
                     const double2 g0 = __ldcs(gp), g1 = __ldcs(gp + 1);
                     sraw = g0.x; gv[p] = g0.y; gq[p] = g1.x; gm[p] = g1.y;

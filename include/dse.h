@@ -136,6 +136,11 @@ DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[6]);
 DSE_API int dse_set_timing(dse_handle *h, int32_t enable);
 DSE_API int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches);
 
+/* Diagnostics: cycles summed over all warps of the last point-kernel launch, spent in (geometry, series,
+ * exp + weights, accumulation, whole warp).  All zeros unless the library was built with
+ * -DDSE_PHASE_TIMING (the default build carries no instrumentation).  Synchronous. */
+DSE_API int dse_get_phase_cycles(dse_handle *h, double out_host[5]);
+
 /* fp64 FMA throughput probe (the roofline denominator of an ALU-bound path): launches a kernel of
  * `blocks` x 256 threads, each running 8 independent chains of `iters` dependent DFMAs, on `stream`.
  * flops per launch = blocks*256*8*iters*2.  sink_dev receives one double per thread (>= blocks*256).

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
 EXPORTS = [
     "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_lu_solve",
     "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count", "dse_kernel_info",
-    "dse_set_timing", "dse_get_timing", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
+    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
@@ -62,6 +62,7 @@ def load_library():
     L.dse_kernel_info.argtypes = [vp, C.POINTER(C.c_int32 * 6)]
     L.dse_set_timing.argtypes = [vp, C.c_int32]
     L.dse_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+    L.dse_get_phase_cycles.argtypes = [vp, C.POINTER(C.c_double * 5)]
     L.dse_dfma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
     L.dse_dmma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
     L.dse_strerror.argtypes = [C.c_int]
@@ -181,6 +182,11 @@ class Dse:
         ms = C.c_double(); n = C.c_int64()
         _check(self.lib.dse_get_timing(self._h, C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def phase_cycles(self):
+        a = (C.c_double * 5)()
+        _check(self.lib.dse_get_phase_cycles(self._h, C.byref(a)))
+        return list(a)
 
     def launch_count(self):
         return int(self.lib.dse_launch_count(self._h))

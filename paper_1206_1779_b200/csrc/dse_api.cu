@@ -204,12 +204,13 @@ int dse_create(const dse_params *params, dse_handle **out)
     const size_t o_J = carve<double>(off, (size_t)k.B * n2 * n2), o_F = carve<double>(off, (size_t)k.B * n2);
     const size_t o_lu = carve<double>(off, (size_t)k.B * dse::lu_scratch_doubles((int)n2));
     const size_t o_c = carve<double>(off, (size_t)k.B * n2), o_bc = carve<double>(off, (size_t)k.B * 2);
+    const size_t o_dbg = carve<double>(off, (size_t)k.W * 5);
     if (cudaMalloc(&h->d_work, 8 * off) != cudaSuccess) { dse_destroy(h); return DSE_ENOMEM; }
     e = cudaMemset(h->d_work, 0, 8 * off);
     if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemset(workspace)"); }
     double *wk = h->d_work;
     k.coefP = wk + o_coef; k.Gy = wk + o_Gy; k.Py = wk + o_Py; k.invG = wk + o_iG; k.invZ = wk + o_iZ;
-    k.Apart = wk + o_A; k.Spart = wk + o_S; k.Rz = wk + o_R;
+    k.Apart = wk + o_A; k.Spart = wk + o_S; k.Rz = wk + o_R; k.dbg = wk + o_dbg;
     h->d_J = wk + o_J; h->d_F = wk + o_F; h->d_lu = wk + o_lu; h->d_c = wk + o_c; h->d_bc = wk + o_bc;
     h->d_Jh = h->d_J; h->d_Fh = h->d_F;
 
@@ -315,6 +316,17 @@ int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches)
     if (rc < 0) return rc;
     *total_ms = h->t_ms;
     *launches = h->t_n;
+    return DSE_OK;
+}
+
+int dse_get_phase_cycles(dse_handle *h, double out_host[5])
+{
+    if (!h || !out_host) return DSE_EINVAL;
+    std::vector<double> tmp((size_t)h->k.W * 5);
+    CK(cudaMemcpy(tmp.data(), h->k.dbg, 8 * tmp.size(), cudaMemcpyDeviceToHost));
+    for (int i = 0; i < 5; ++i) out_host[i] = 0.0;
+    for (int w = 0; w < h->k.W; ++w)
+        for (int i = 0; i < 5; ++i) out_host[i] += tmp[(size_t)w * 5 + i];
     return DSE_OK;
 }
 

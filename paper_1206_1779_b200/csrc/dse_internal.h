@@ -46,6 +46,7 @@ struct KParams {
     double *Rz;                        // [B*Next][3][Npad]  A . Phi_y
     double *D;                         // [B*Next][4][Npad]  dPiG/da, dPiG/db, dPiZ/da, dPiZ/db
     double *Pi;                        // [B*Next][2]        Pi_G, Pi_Z
+    double *dbg;                       // per-warp phase cycle counters (only with -DDSE_PHASE_TIMING), else nullptr
 };
 
 struct PointKernelConfig {

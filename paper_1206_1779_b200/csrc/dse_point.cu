@@ -65,8 +65,6 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
     double accA[CJ], accB[CJ], accV[CJ];
 #pragma unroll
     for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
-    long long cur_bi = -1;
-    int cur_b = -1;
 
     auto flush = [&](long long bi) {
         const size_t slot = (size_t)(w + bi);
@@ -107,25 +105,28 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
         prefetch(0);
     }
 
+#ifdef DSE_PHASE_TIMING
+    long long dbg_t[4] = {0, 0, 0, 0};
+    const long long dbg_start = clock64();
+#endif
+    // (bi, q0, b, e) are advanced incrementally: no 64-bit divisions inside the row loop
     long long r = r0;
+    long long bi = r0 / Nr;
+    int q0 = (int)(r0 - bi * Nr);
+    int cur_b = (int)(bi / P.Next);
+    int e = (int)(bi - (long long)cur_b * P.Next);
+    bool fresh = true;                                   // accumulators belong to a new external point
+    if (r0 < r1) {
+        for (int j = lane; j < Npad; j += 32)
+            s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
+        __syncwarp();
+    }
     while (r < r1) {
-        const long long bi = r / Nr;
-        const int q0 = (int)(r - bi * Nr);
-        if (bi != cur_bi) {
-            if (JAC && cur_bi >= 0) flush(cur_bi);
+        if (fresh) {
 #pragma unroll
             for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
-            cur_bi = bi;
-            const int b = (int)(bi / P.Next);
-            if (b != cur_b) {
-                __syncwarp();
-                for (int j = lane; j < Npad; j += 32)
-                    s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)b * Npad + j];
-                __syncwarp();
-                cur_b = b;
-            }
+            fresh = false;
         }
-        const int e = (int)(bi - (long long)cur_b * P.Next);
         const long long left = r1 - r;
         int nrow = P.rpb;
         if (left < nrow) nrow = (int)left;
@@ -149,6 +150,9 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
                                    : nullptr;
 
         for (int kb = 0; kb < P.Ntpad; kb += 32 * NP) {
+#ifdef DSE_PHASE_TIMING
+            const long long tk0 = clock64();
+#endif
             // ---------------- phase 1: lane = point; NP points per lane are interleaved for ILP ----------------
             // (k = kb + 32 p + kl < Ntpad: g divides Ntpad, g <= 32; NP = 2 only when 64 divides Ntpad)
             double gv[NP], gq[NP], gm[NP], EG[NP], EZ[NP], ts[NP], t2[NP], Te[NP], To[NP], Tem[NP], Tom[NP];
@@ -187,6 +191,9 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
                 Tem[p] = fma(ts[p], s, -1.0); Tom[p] = s;   // T_{-2} = T_2, T_{-1} = T_1
                 lz0[p] = lz1[p] = lg0[p] = lg1[p] = 0.0;
             }
+#ifdef DSE_PHASE_TIMING
+            const long long tk1 = clock64();
+#endif
 #pragma unroll
             for (int c = 0; c < NCH; ++c) {
                 if (JAC) {
@@ -211,6 +218,9 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
                     }
                 }
             }
+#ifdef DSE_PHASE_TIMING
+            const long long tk2 = clock64();
+#endif
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 const double lnZz = (lz0[p] + lz1[p]) + EZ[p], lnGz = (lg0[p] + lg1[p]) + EG[p];
@@ -232,6 +242,9 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
                 sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
                 if (JAC) reinterpret_cast<double4 *>(reinterpret_cast<double *>(s_pt) + p * STASH)[lane] = make_double4(ts[p], ua, ub, v);
             }
+#ifdef DSE_PHASE_TIMING
+            const long long tk3 = clock64();
+#endif
             if (JAC) {
                 __syncwarp();
                 // ---------------- phase 2: lane = (chunk, point sub-lane) ----------------
@@ -260,6 +273,12 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
             } else {
                 asm volatile("" ::: "memory");      // keep the coefficient loads inside the loop (no hoisting -> no spills)
             }
+#ifdef DSE_PHASE_TIMING
+            {
+                const long long tk4 = clock64();
+                dbg_t[0] += tk1 - tk0; dbg_t[1] += tk2 - tk1; dbg_t[2] += tk3 - tk2; dbg_t[3] += tk4 - tk3;
+            }
+#endif
         }
         // H5/H7: row sums over the angular nodes (fixed xor tree), one writer per row
         for (int o = g >> 1; o > 0; o >>= 1) {
@@ -271,8 +290,27 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
         if (kl == 0 && rowact)
             reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
         r += nrow;
+        q0 += nrow;
+        if (q0 >= Nr) {                                  // next external point (nrow never crosses this boundary)
+            if (JAC) flush(bi);
+            fresh = true;
+            q0 = 0; ++bi; ++e;
+            if (e == P.Next && r < r1) {                 // next system: stage its coefficient pairs
+                e = 0; ++cur_b;
+                __syncwarp();
+                for (int j = lane; j < Npad; j += 32)
+                    s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
+                __syncwarp();
+            }
+        }
     }
-    if (JAC && cur_bi >= 0) flush(cur_bi);
+    if (JAC && !fresh) flush(bi);
+#ifdef DSE_PHASE_TIMING
+    if (lane == 0 && P.dbg) {
+        for (int i = 0; i < 4; ++i) P.dbg[w * 5 + i] = (double)dbg_t[i];
+        P.dbg[w * 5 + 4] = (double)(clock64() - dbg_start);
+    }
+#endif
 }
 
 using KernelFn = void (*)(const KParams);

@@ -50,7 +50,9 @@ struct KParams {
 };
 
 struct PointKernelConfig {
-    int grid, block, smem, regs, ctas_per_sm, sms;
+    int grid, block, smem, regs, ctas_per_sm, sms;       // Jacobian build (defines KParams::W and the partial slots)
+    int res_grid, res_block, res_smem;                   // residual-only build (no partials)
+    int pipelined;                                       // Jacobian build uses the software-pipelined kernel
 };
 
 // launchers (dse_kernels.cu / dse_lu.cu); each returns the number of kernels launched or <0 on error

@@ -313,6 +313,224 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
 #endif
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// Software-pipelined variant (compile-time chunk count, full-warp angular batches, Jacobian on):
+// iteration t runs phase 1 of batch t (series, exp -- long dependent chains, little fp64 pipe pressure)
+// in the SAME straight-line block as phase 2 of batch t-1 (accumulation -- independent FMAs), reading and
+// writing the two halves of a double-buffered stash, so the scheduler hides the chains behind the FMAs.
+// One pipeline per (warp, external point) segment: prologue = zeroed weights, epilogue = phase 2 only.
+constexpr int PIPE_THREADS = 384;
+
+__host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc, bool geom)
+{
+    return (constc ? 0 : 2 * Npad) + 2 * stash_doubles(NCH) + (geom ? GBUF_DOUBLES : 0);
+}
+
+template <int NCH_T, bool GEOM, bool CONSTC>
+__global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KParams P)
+{
+    constexpr int NCH = NCH_T, SUB = 32 / NCH_T, ROUNDS = NCH_T, Npad = NCH_T * CJ;
+    extern __shared__ __align__(16) double smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
+    const int STASH = stash_doubles(NCH);
+    double *s_ang = smem;
+    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
+    double2 *s_coef = reinterpret_cast<double2 *>(wbase);
+    double *s_stash = wbase + (CONSTC ? 0 : 2 * Npad);                       // [2][STASH]: pt (33 x 4) then T
+    double4 *s_gbuf = reinterpret_cast<double4 *>(s_stash + 2 * STASH);     // [2][32] geometry records
+
+    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    __syncthreads();
+
+    const int Nr = P.Nr, BPR = P.Ntpad >> 5;                                 // batches per row
+    const long long R = P.R;
+    const long long w = (long long)blockIdx.x * WPB + warp;
+    const long long r0 = (w * R) / P.W, r1 = ((w + 1) * R) / P.W;
+    if (r0 >= r1) return;
+    const int c_lane = lane / SUB, sub = lane - c_lane * SUB;
+    const double halfLg = 0.5 * P.Lg;
+
+    double accA[CJ], accB[CJ], accV[CJ];
+
+    // phase 2 of the batch stashed in buffer `buf`
+    auto phase2 = [&](int buf) {
+        const double4 *pts = reinterpret_cast<const double4 *>(s_stash + buf * STASH);
+        const double2 *trd = reinterpret_cast<const double2 *>(s_stash + buf * STASH + 132) + c_lane * (TCH_STRIDE / 2);
+#pragma unroll
+        for (int rd = 0; rd < ROUNDS; ++rd) {
+            const int pt = rd * SUB + sub;
+            const double4 pw = pts[pt];
+            const double2 tt = trd[pt];
+            double T0 = tt.x, T1 = tt.y;
+            accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
+            accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
+#pragma unroll
+            for (int m = 2; m < CJ; ++m) {
+                const double T2 = fma(pw.x, T1, -T0);
+                accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
+                T0 = T1; T1 = T2;
+            }
+        }
+    };
+    auto flush = [&](long long bi, int buf) {      // `buf`'s T area is free: use it as the cross-lane scratch
+        double *scr = s_stash + buf * STASH + 132;
+        const size_t slot = (size_t)(w + bi);
+#pragma unroll
+        for (int st = 0; st < 3; ++st) {
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < CJ; ++m) scr[sub * Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
+            __syncwarp();
+            for (int j = lane; j < Npad; j += 32) {
+                double s = 0.0;
+                for (int sb = 0; sb < SUB; ++sb) s += scr[sb * Npad + j];
+                P.Spart[(slot * 3 + st) * Npad + j] = s;
+            }
+        }
+        __syncwarp();
+    };
+
+    // geometry stream (GEOM): consecutive 1 KB records, cp.async double buffer
+    const size_t gtotal = (size_t)P.Next * Nr * P.Ntpad;
+    const double4 *gbase = reinterpret_cast<const double4 *>(P.geom), *gend = gbase + gtotal, *gnext = gbase;
+    unsigned gphase = 0;
+    auto prefetch = [&](unsigned buf) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(s_gbuf + buf * 32 + lane);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(gnext));
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(gnext) + 16));
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
+
+    long long bi = r0 / Nr;
+    int q = (int)(r0 - bi * Nr);
+    int cur_b = (int)(bi / P.Next);
+    int e = (int)(bi - (long long)cur_b * P.Next);
+    if (GEOM) {
+        gnext = gbase + ((size_t)e * Nr + q) * P.Ntpad + lane;
+        prefetch(0);
+    }
+    if (!CONSTC) {
+        for (int j = lane; j < Npad; j += 32) s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
+        __syncwarp();
+    }
+
+    // both T stashes must hold finite numbers before the first (zero-weight) prologue phase 2
+    for (int b2 = 0; b2 < 2; ++b2)
+        for (int c = 0; c < NCH; ++c)
+            reinterpret_cast<double2 *>(s_stash + b2 * STASH + 132)[c * (TCH_STRIDE / 2) + lane] = make_double2(0.0, 0.0);
+
+    long long r = r0;
+    int cur = 0;                                           // stash half written by the current batch
+    while (r < r1) {
+        // ---------------- one (warp, external point) segment: rows [r, rend) ----------------
+        long long rend = r + (Nr - q);
+        if (rend > r1) rend = r1;
+#pragma unroll
+        for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
+        reinterpret_cast<double4 *>(s_stash + (cur ^ 1) * STASH)[lane] = make_double4(0.0, 0.0, 0.0, 0.0);   // prologue
+        __syncwarp();
+        for (; r < rend; ++r, ++q) {
+            const double Gy = P.Gy[(size_t)cur_b * Nr + q], Py = P.Py[(size_t)cur_b * Nr + q];
+            RowConst rc;
+            if (!GEOM) {
+                const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
+                const double y = P.y[q], sy = P.sy[q];
+                const double Wq = P.Wy[q];
+                const double d = (x - y) / (sx + sy);
+                rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
+            }
+            double sumA = 0.0, sumB = 0.0, sumV = 0.0, sumZ = 0.0;
+            for (int kb = 0; kb < BPR; ++kb) {
+                double sraw, gv, gq, gm;
+                if (GEOM) {
+                    gnext += 32;
+                    if (gnext >= gend) gnext -= gtotal;
+                    prefetch(gphase ^ 1);
+                    asm volatile("cp.async.wait_group 1;\n" ::: "memory");
+                    const double2 *gp = reinterpret_cast<const double2 *>(s_gbuf + gphase * 32 + lane);
+                    const double2 g0 = gp[0], g1 = gp[1];
+                    sraw = g0.x; gv = g0.y; gq = g1.x; gm = g1.y;
+                    gphase ^= 1;
+                } else {
+                    point_geometry(rc, s_ang + (kb * 32 + lane) * 6, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
+                }
+                double s = sraw, EG = 0.0, EZ = 0.0;
+                if (sraw < -1.0) {                       // z < eps2: eq.(16),(17)
+                    const double ell = (sraw + 1.0) * halfLg;
+                    EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
+                } else if (sraw > 1.0) {                 // z > L2: eq.(18),(19)
+                    const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                    EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
+                }
+                // ======== main block: phase 1 of this batch || phase 2 of the previous batch ========
+                const double ts = 2.0 * s;
+                const double t2 = fma(2.0 * ts, s, -2.0);
+                double Te = 1.0, To = s, Tem = fma(ts, s, -1.0), Tom = s;
+                double lz0 = 0.0, lz1 = 0.0, lg0 = 0.0, lg1 = 0.0;
+                double2 *tw = reinterpret_cast<double2 *>(s_stash + cur * STASH + 132);
+#pragma unroll
+                for (int c = 0; c < NCH; ++c) {
+                    tw[c * (TCH_STRIDE / 2) + lane] = make_double2(Te, To);
+#pragma unroll
+                    for (int m = 0; m < CJ; m += 4) {
+                        const double2 c0 = CONSTC ? c_coef[c * CJ + m] : s_coef[c * CJ + m];
+                        const double2 c1 = CONSTC ? c_coef[c * CJ + m + 1] : s_coef[c * CJ + m + 1];
+                        const double2 c2 = CONSTC ? c_coef[c * CJ + m + 2] : s_coef[c * CJ + m + 2];
+                        const double2 c3 = CONSTC ? c_coef[c * CJ + m + 3] : s_coef[c * CJ + m + 3];
+                        lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0);
+                        lz1 = fma(c1.x, To, lz1); lg1 = fma(c1.y, To, lg1);
+                        Tem = fma(t2, Te, -Tem);  Tom = fma(t2, To, -Tom);
+                        lz0 = fma(c2.x, Tem, lz0); lg0 = fma(c2.y, Tem, lg0);
+                        lz1 = fma(c3.x, Tom, lz1); lg1 = fma(c3.y, Tom, lg1);
+                        Te = fma(t2, Tem, -Te);   To = fma(t2, Tom, -To);
+                    }
+                }
+                const double lnZz = (lz0 + lz1) + EZ, lnGz = (lg0 + lg1) + EG;
+                const double lnPz = fma(P.e1, lnGz, P.e2 * lnZz);
+                double Zz = fast_exp(lnZz), Gz = fast_exp(lnGz), Pz = fast_exp(lnPz);
+                phase2(cur ^ 1);
+                // ======== end of main block ========
+                const int hmax = max(max(__double2hiint(lnZz) & 0x7fffffff, __double2hiint(lnGz) & 0x7fffffff),
+                                     __double2hiint(lnPz) & 0x7fffffff);
+                if (hmax >= 0x4085e000) { Zz = exp(lnZz); Gz = exp(lnGz); Pz = exp(lnPz); }   // |x| > 700 or NaN
+                const double v = gv * (Gy * Zz);              // eq.(8)
+                const double wQ = gq * (Py * Pz);             // eq.(9), gluon loop
+                const double wM = gm * (Gy * Gz);             // eq.(9), ghost loop
+                const double ua = P.e2 * wQ;
+                const double ub = fma(P.e1, wQ, wM);
+                sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
+                reinterpret_cast<double4 *>(s_stash + cur * STASH)[lane] = make_double4(ts, ua, ub, v);
+                __syncwarp();
+                cur ^= 1;
+            }
+            // H5/H7: row sums over the 32 angular lanes (fixed xor tree), lane 0 writes
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                sumA += __shfl_xor_sync(FULL, sumA, o);
+                sumB += __shfl_xor_sync(FULL, sumB, o);
+                sumV += __shfl_xor_sync(FULL, sumV, o);
+                sumZ += __shfl_xor_sync(FULL, sumZ, o);
+            }
+            if (lane == 0) reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
+        }
+        // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
+        phase2(cur ^ 1);
+        flush(bi, cur);
+        if (q >= Nr) {
+            q = 0; ++bi; ++e;
+            if (e == P.Next) {
+                e = 0; ++cur_b;
+                if (!CONSTC && r < r1) {
+                    for (int j = lane; j < Npad; j += 32)
+                        s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
+                    __syncwarp();
+                }
+            }
+        }
+    }
+    if (GEOM) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+}
 using KernelFn = void (*)(const KParams);
 
 inline int np_of(const KParams &k)      // two interleaved points per lane when the shapes allow it
@@ -379,34 +597,27 @@ bool acquire_const_slot(const KParams &k)
 }
 void release_const_slot() { g_const_owner.store(0); }
 
-int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
+static KernelFn pick_pipe(const KParams &k)
 {
-    int dev = 0, sms = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return fail(e, "cudaGetDevice");
-    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) return fail(e, "cudaDeviceGetAttribute");
-    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH, np_of(k)));
-    for (int jac = 0; jac < 2; ++jac) {
-        e = cudaFuncSetAttribute((const void *)pick(k, jac != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel smem)");
+#define DSE_PIPE_CASE(N)                                                                         \
+    case N:                                                                                      \
+        if (k.use_constc) return k.geom ? point_kernel_pipe<N, true, true> : point_kernel_pipe<N, false, true>; \
+        return k.geom ? point_kernel_pipe<N, true, false> : point_kernel_pipe<N, false, false>;
+    switch (k.NCH) {
+        DSE_PIPE_CASE(1)
+        DSE_PIPE_CASE(2)
+        DSE_PIPE_CASE(4)
+        DSE_PIPE_CASE(8)
+        DSE_PIPE_CASE(16)
+        default: return nullptr;
     }
-    const void *fn = (const void *)pick(k, true);
-    cudaFuncAttributes fa;
-    e = cudaFuncGetAttributes(&fa, fn);
-    if (e != cudaSuccess) return fail(e, "cudaFuncGetAttributes");
-    int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, POINT_THREADS, smem);
-    if (e != cudaSuccess) return fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
-    if (per_sm < 1) { set_error_text("point_kernel does not fit on an SM"); return DSE_ECUDA; }
-    cfg.block = POINT_THREADS;
-    cfg.smem = smem;
-    cfg.regs = fa.numRegs;
-    cfg.ctas_per_sm = per_sm;
-    cfg.sms = sms;
+#undef DSE_PIPE_CASE
+}
+
+static long long pick_grid(const KParams &k, int sms, int per_sm, int wpb)
+{
     // persistent-style grid: one wave of resident CTAs, but never more warps than rows
     long long grid = (long long)sms * per_sm;
-    const long long wpb = POINT_THREADS / 32;
     const long long batches_per_row = k.Ntpad / 32 > 0 ? k.Ntpad / 32 : 1;   // 32-point batches
     // keep >= ~4 point batches per warp so that small problems do not pay for idle warps
     long long want_warps = (k.R * batches_per_row / k.rpb + 3) / 4;
@@ -414,7 +625,58 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     long long want_grid = (want_warps + wpb - 1) / wpb;
     if (want_grid < grid) grid = want_grid;
     while (grid * wpb > k.R && grid > 1) --grid;
-    cfg.grid = (int)grid;
+    return grid;
+}
+
+int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
+{
+    int dev = 0, sms = 0, smem_max = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(e, "cudaGetDevice");
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return fail(e, "cudaDeviceGetAttribute");
+    e = cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return fail(e, "cudaDeviceGetAttribute(smem)");
+    cfg.sms = sms;
+
+    // residual-only build (and the Jacobian build of generic shapes): warp-independent kernel, 512 threads
+    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH, np_of(k)));
+    for (int jac = 0; jac < 2; ++jac) {
+        e = cudaFuncSetAttribute((const void *)pick(k, jac != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel smem)");
+    }
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)pick(k, false), POINT_THREADS, smem);
+    if (e != cudaSuccess) return fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (per_sm < 1) { set_error_text("point_kernel does not fit on an SM"); return DSE_ECUDA; }
+    cfg.res_block = POINT_THREADS;
+    cfg.res_smem = smem;
+    cfg.res_grid = (int)pick_grid(k, sms, per_sm, POINT_THREADS / 32);
+
+    // Jacobian build: software-pipelined kernel when the shape allows it
+    const void *fn = (const void *)pick(k, true);
+    int block = POINT_THREADS, jsmem = smem;
+    cfg.pipelined = 0;
+    KernelFn pf = (k.g == 32 && !getenv("DSE_NO_PIPE")) ? pick_pipe(k) : nullptr;
+    if (pf) {
+        const int psmem = (int)sizeof(double) * (k.Ntpad * 6 + (PIPE_THREADS / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
+        if (psmem <= smem_max) {
+            e = cudaFuncSetAttribute((const void *)pf, cudaFuncAttributeMaxDynamicSharedMemorySize, psmem);
+            if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel_pipe smem)");
+            fn = (const void *)pf; block = PIPE_THREADS; jsmem = psmem; cfg.pipelined = 1;
+        }
+    }
+    cudaFuncAttributes fa;
+    e = cudaFuncGetAttributes(&fa, fn);
+    if (e != cudaSuccess) return fail(e, "cudaFuncGetAttributes");
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, block, jsmem);
+    if (e != cudaSuccess) return fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (per_sm < 1) { set_error_text("point kernel does not fit on an SM"); return DSE_ECUDA; }
+    cfg.block = block;
+    cfg.smem = jsmem;
+    cfg.regs = fa.numRegs;
+    cfg.ctas_per_sm = per_sm;
+    cfg.grid = (int)pick_grid(k, sms, per_sm, block / 32);
     return 0;
 }
 
@@ -422,7 +684,14 @@ int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
     if (constc_of(k))
         cudaMemcpyToSymbolAsync(c_coef, k.coefP, sizeof(double2) * k.Npad, 0, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
-    pick(k, k.want_jac != 0)<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
+    if (k.want_jac) {
+        KernelFn fn = cfg.pipelined ? pick_pipe(k) : pick(k, true);
+        fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
+    } else {
+        KParams kk = k;
+        kk.W = cfg.res_grid * (cfg.res_block / 32);          // the residual build has its own row partition
+        pick(k, false)<<<cfg.res_grid, cfg.res_block, cfg.res_smem, (cudaStream_t)stream>>>(kk);
+    }
     return 1;
 }
 

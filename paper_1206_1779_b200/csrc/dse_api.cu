@@ -148,6 +148,11 @@ int dse_create(const dse_params *params, dse_handle **out)
     k.rpb = 32 / k.g;
     k.Next = T.Next; k.B = params->n_batch; k.iZ = T.iZ; k.iG = T.iG;
     k.R = (long long)k.B * k.Next * k.Nr;
+    if ((long long)k.Next * k.Nr * k.Ntpad >= (1ll << 31) || (long long)k.B * k.Next >= (1ll << 30)) {
+        dse::set_error_text("grid too large: N_ext*N_r*N_theta must stay below 2^31 points per system");
+        delete h;
+        return DSE_EINVAL;
+    }
     k.eps2 = params->eps2; k.L2 = params->L2; k.inv_eps2 = 1.0 / params->eps2;
     k.Lg = T.Lg; k.two_over_Lg = 2.0 / T.Lg;
     k.pG = params->ir_exp_G; k.pZ = params->ir_exp_Z; k.omega = params->uv_omega;
@@ -191,6 +196,8 @@ int dse_create(const dse_params *params, dse_handle **out)
     rc = dse::query_point_kernel(k, h->cfg);
     if (rc < 0) { dse_destroy(h); return rc; }
     k.W = h->cfg.grid * (h->cfg.block / 32);
+    k.upr = h->cfg.pipelined ? (k.Ntpad / 32) : 1;      // the pipelined kernel partitions 32-point batches
+    k.U = k.R * k.upr;
 
     // ---- workspace (one allocation, zero-initialised: unwritten partial slots must read 0) ----
     const size_t n2 = 2 * (size_t)k.N;
@@ -198,7 +205,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     const size_t o_coef = carve<double>(off, (size_t)k.B * k.Npad * 2);
     const size_t o_Gy = carve<double>(off, (size_t)k.B * k.Nr), o_Py = carve<double>(off, (size_t)k.B * k.Nr);
     const size_t o_iG = carve<double>(off, (size_t)k.B * k.N), o_iZ = carve<double>(off, (size_t)k.B * k.N);
-    const size_t o_A = carve<double>(off, (size_t)k.R * 4);
+    const size_t o_A = carve<double>(off, (size_t)k.R * 4), o_AH = carve<double>(off, (size_t)k.R * 4);
     const size_t o_S = carve<double>(off, ((size_t)k.W + (size_t)k.B * k.Next) * 3 * k.Npad);
     const size_t o_R = carve<double>(off, (size_t)k.B * k.Next * 3 * k.Npad);
     const size_t o_J = carve<double>(off, (size_t)k.B * n2 * n2), o_F = carve<double>(off, (size_t)k.B * n2);
@@ -210,7 +217,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemset(workspace)"); }
     double *wk = h->d_work;
     k.coefP = wk + o_coef; k.Gy = wk + o_Gy; k.Py = wk + o_Py; k.invG = wk + o_iG; k.invZ = wk + o_iZ;
-    k.Apart = wk + o_A; k.Spart = wk + o_S; k.Rz = wk + o_R; k.dbg = wk + o_dbg;
+    k.Apart = wk + o_A; k.AHead = wk + o_AH; k.Spart = wk + o_S; k.Rz = wk + o_R; k.dbg = wk + o_dbg;
     h->d_J = wk + o_J; h->d_F = wk + o_F; h->d_lu = wk + o_lu; h->d_c = wk + o_c; h->d_bc = wk + o_bc;
     h->d_Jh = h->d_J; h->d_Fh = h->d_F;
 

@@ -32,6 +32,8 @@ struct KParams {
     int Next, B, iZ, iG;
     long long R;                       // rows = B * Next * Nr
     int W;                             // warps in the grid of the point kernel
+    long long U;                       // partition units of the Jacobian build: rows (upr = 1) or 32-point batches
+    int upr;                           // partition units per row
     int want_jac;                      // 0: residual only (skip phase 2)
     int use_constc;                    // coefficient pairs are read as constant-bank operands (single system, slot owner)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
@@ -42,6 +44,7 @@ struct KParams {
     double *Gy, *Py;                   // [B][Nr]
     double *invG, *invZ;               // [B][N]   1/G(x_i), 1/Z(x_i)
     double *Apart;                     // [B*Next][Nr][4]   sum_k (u_a, u_b, v, wQ+wM)
+    double *AHead;                     // same shape: partial sums of rows whose angular batches span two warps (else 0)
     double *Spart;                     // [W + B*Next][3][Npad]
     double *Rz;                        // [B*Next][3][Npad]  A . Phi_y
     double *D;                         // [B*Next][4][Npad]  dPiG/da, dPiG/db, dPiZ/da, dPiZ/db

@@ -84,43 +84,52 @@ __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
 // ---------------------------------------------------------------------------------------------
 // H7: Rz[b,e,stream][j] = sum_q A_stream[b,e,q] phi_j(t_q): the z-independent part of the Jacobian,
 // a dense [3 N_ext x N_r] . [N_r x N] contraction per system, on the fp64 tensor path
-// (mma.sync.aligned.m8n8k4 f64 -> DMMA).  One warp per 8x8 output tile, K = N_r in steps of 4.
-__global__ void __launch_bounds__(128) gemm_kernel(const KParams P)
+// (mma.sync.aligned.m8n8k4 f64 -> DMMA).  One CTA per (8 external points, 8 values of j, system); its
+// 16 warps split K = N_r; each lane loads one 32-byte row-sum record (all three streams at once), so one
+// k-step feeds three MMAs; the 16 partial tiles are combined in warp order (deterministic).
+constexpr int GEMM_WARPS = 16;
+__global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
 {
-    // 4 warps per 8x8 tile, each takes a contiguous quarter of K; partial tiles combined in warp order
-    __shared__ double s_c[4][32][2];
+    __shared__ double s_c[GEMM_WARPS][3][32][2];
     const int lane = threadIdx.x & 31, wk = threadIdx.x >> 5;
-    const int m0 = blockIdx.x * 8, n0 = blockIdx.y * 8, b = blockIdx.z;
-    const int M = 3 * P.Next;
-    const int am = m0 + (lane >> 2), ak = lane & 3;          // A fragment: row = lane/4, col = lane%4
-    const int bk = lane & 3, bn = n0 + (lane >> 2);          // B fragment: row = lane%4, col = lane/4
-    const bool arow_ok = am < M;
-    const int e = arow_ok ? am / 3 : 0, st = arow_ok ? am - 3 * (am / 3) : 0;
-    const double *Arow = P.Apart + ((size_t)(b * P.Next + e) * P.Nr) * 4 + st;
-    const int ksteps = (P.Nr + 3) / 4, per = (ksteps + 3) / 4;
+    const int e0 = blockIdx.x * 8, n0 = blockIdx.y * 8, b = blockIdx.z;
+    const int ae = e0 + (lane >> 2), ak = lane & 3;          // A fragment: row = lane/4 (external point), col = lane%4 (q)
+    const int bk = lane & 3, bn = n0 + (lane >> 2);          // B fragment: row = lane%4 (q), col = lane/4 (j)
+    const bool arow_ok = ae < P.Next;
+    const size_t rowbase = ((size_t)b * P.Next + (arow_ok ? ae : 0)) * P.Nr;
+    const double4 *Arow = reinterpret_cast<const double4 *>(P.Apart) + rowbase;
+    const double4 *Hrow = reinterpret_cast<const double4 *>(P.AHead) + rowbase;
+    const int ksteps = (P.Nr + 3) / 4, per = (ksteps + GEMM_WARPS - 1) / GEMM_WARPS;
     const int ks0 = wk * per, ks1 = min(ksteps, ks0 + per);
-    double c0 = 0.0, c1 = 0.0;
-#pragma unroll 4
+    double c[3][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+#pragma unroll 8
     for (int ks = ks0; ks < ks1; ++ks) {
         const int qa = ks * 4 + ak, qb = ks * 4 + bk;
-        const double a = (arow_ok && qa < P.Nr) ? Arow[(size_t)qa * 4] : 0.0;
+        double4 a = make_double4(0.0, 0.0, 0.0, 0.0);
+        if (arow_ok && qa < P.Nr) {
+            const double4 a1 = Arow[qa], a2 = Hrow[qa];
+            a = make_double4(a1.x + a2.x, a1.y + a2.y, a1.z + a2.z, 0.0);
+        }
         const double bb = (qb < P.Nr) ? P.phi_y[(size_t)qb * P.Npad + bn] : 0.0;
-        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                     : "+d"(c0), "+d"(c1)
-                     : "d"(a), "d"(bb));
+        asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                     : "+d"(c[0][0]), "+d"(c[0][1]) : "d"(a.x), "d"(bb));
+        asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                     : "+d"(c[1][0]), "+d"(c[1][1]) : "d"(a.y), "d"(bb));
+        asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                     : "+d"(c[2][0]), "+d"(c[2][1]) : "d"(a.z), "d"(bb));
     }
-    s_c[wk][lane][0] = c0;
-    s_c[wk][lane][1] = c1;
+#pragma unroll
+    for (int st = 0; st < 3; ++st) { s_c[wk][st][lane][0] = c[st][0]; s_c[wk][st][lane][1] = c[st][1]; }
     __syncthreads();
-    if (wk == 0) {
-        c0 = ((s_c[0][lane][0] + s_c[1][lane][0]) + s_c[2][lane][0]) + s_c[3][lane][0];
-        c1 = ((s_c[0][lane][1] + s_c[1][lane][1]) + s_c[2][lane][1]) + s_c[3][lane][1];
-        const int cm = m0 + (lane >> 2), cn = n0 + 2 * (lane & 3);
-        if (cm < M) {
-            const int ce = cm / 3, cs = cm - 3 * ce;
-            double *out = P.Rz + ((size_t)(b * P.Next + ce) * 3 + cs) * P.Npad;
-            out[cn] = c0;
-            out[cn + 1] = c1;
+    if (wk < 3) {                                            // warp st combines stream st
+        const int st = wk;
+        double r0 = 0.0, r1 = 0.0;
+        for (int w2 = 0; w2 < GEMM_WARPS; ++w2) { r0 += s_c[w2][st][lane][0]; r1 += s_c[w2][st][lane][1]; }
+        const int ce = e0 + (lane >> 2), cn = n0 + 2 * (lane & 3);     // C fragment: row = lane/4, cols 2(lane%4), +1
+        if (ce < P.Next) {
+            double *out = P.Rz + (((size_t)b * P.Next + ce) * 3 + st) * P.Npad;
+            out[cn] = r0;
+            out[cn + 1] = r1;
         }
     }
 }
@@ -136,8 +145,8 @@ constexpr int ASM_THREADS = 512;
 __device__ __forceinline__ void reduce_part(const KParams &P, long long bi, int j, int part, int parts, double &Sa,
                                             double &Sb, double &Sv)
 {
-    const long long rf = bi * P.Nr, rl = rf + P.Nr - 1;
-    const long long wf = ((rf + 1) * P.W - 1) / P.R, wl = ((rl + 1) * P.W - 1) / P.R;
+    const long long rf = bi * P.Nr * P.upr, rl = rf + (long long)P.Nr * P.upr - 1;     // first/last partition unit of bi
+    const long long wf = ((rf + 1) * P.W - 1) / P.U, wl = ((rl + 1) * P.W - 1) / P.U;
     const long long n = wl - wf + 1, per = (n + parts - 1) / parts;
     const long long w0 = wf + part * per, w1 = min(wl + 1, w0 + per);
     double a = 0.0, b = 0.0, v = 0.0;
@@ -163,7 +172,8 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
         double pg = 0.0, pz = 0.0;
         for (int q = lane; q < P.Nr; q += 32) {
             const double4 a = reinterpret_cast<const double4 *>(P.Apart)[(size_t)bi * P.Nr + q];
-            pg += a.z; pz += a.w;
+            const double4 hh = reinterpret_cast<const double4 *>(P.AHead)[(size_t)bi * P.Nr + q];
+            pg += a.z + hh.z; pz += a.w + hh.w;
         }
         for (int o = 16; o > 0; o >>= 1) {
             pg += __shfl_xor_sync(FULL, pg, o);
@@ -240,7 +250,7 @@ __global__ void __launch_bounds__(256) dmma_probe_kernel(int iters, double *sink
     for (int i = 0; i < iters; ++i) {
 #pragma unroll
         for (int m = 0; m < 4; ++m)
-            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+            asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                          : "+d"(c[m][0]), "+d"(c[m][1])
                          : "d"(a), "d"(b));
     }
@@ -286,8 +296,8 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     if (ev1) cudaEventRecord((cudaEvent_t)ev1, s);
     ++launches;
     if (kk.want_jac) {
-        dim3 gg((3 * kk.Next + 7) / 8, kk.Npad / 8, kk.B);
-        gemm_kernel<<<gg, 128, 0, s>>>(kk);
+        dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);
+        gemm_kernel<<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
         ++launches;
     }
     dim3 ga(kk.N, kk.B);

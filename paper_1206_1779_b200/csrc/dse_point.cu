@@ -287,8 +287,10 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
             sumV += __shfl_xor_sync(FULL, sumV, o);
             sumZ += __shfl_xor_sync(FULL, sumZ, o);
         }
-        if (kl == 0 && rowact)
+        if (kl == 0 && rowact) {
             reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
+            reinterpret_cast<double4 *>(P.AHead)[(size_t)bi * Nr + q] = make_double4(0.0, 0.0, 0.0, 0.0);   // rows are never split here
+        }
         r += nrow;
         q0 += nrow;
         if (q0 >= Nr) {                                  // next external point (nrow never crosses this boundary)
@@ -320,7 +322,10 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
 // in the SAME straight-line block as phase 2 of batch t-1 (accumulation -- independent FMAs), reading and
 // writing the two halves of a double-buffered stash, so the scheduler hides the chains behind the FMAs.
 // One pipeline per (warp, external point) segment: prologue = zeroed weights, epilogue = phase 2 only.
-constexpr int PIPE_THREADS = 384;
+#ifndef DSE_PIPE_THREADS
+#define DSE_PIPE_THREADS 384
+#endif
+constexpr int PIPE_THREADS = DSE_PIPE_THREADS;
 
 __host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc, bool geom)
 {
@@ -344,10 +349,13 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
     __syncthreads();
 
     const int Nr = P.Nr, BPR = P.Ntpad >> 5;                                 // batches per row
-    const long long R = P.R;
+    // work is partitioned in 32-point batches (P.U = rows * BPR): balanced to +-1 batch over all warps; a row whose
+    // batches span two warps gets its head partial in AHead and its tail partial in Apart
     const long long w = (long long)blockIdx.x * WPB + warp;
-    const long long r0 = (w * R) / P.W, r1 = ((w + 1) * R) / P.W;
-    if (r0 >= r1) return;
+    const long long t0 = (w * P.U) / P.W, t1 = ((w + 1) * P.U) / P.W;
+    if (t0 >= t1) return;
+    const long long r0 = t0 / BPR;
+    int kb = (int)(t0 - r0 * BPR);
     const int c_lane = lane / SUB, sub = lane - c_lane * SUB;
     const double halfLg = 0.5 * P.Lg;
 
@@ -373,7 +381,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
             }
         }
     };
-    auto flush = [&](long long bi, int buf) {      // `buf`'s T area is free: use it as the cross-lane scratch
+    auto flush = [&](int bi, int buf) {      // `buf`'s T area is free: use it as the cross-lane scratch
         double *scr = s_stash + buf * STASH + 132;
         const size_t slot = (size_t)(w + bi);
 #pragma unroll
@@ -392,22 +400,23 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
     };
 
     // geometry stream (GEOM): consecutive 1 KB records, cp.async double buffer
-    const size_t gtotal = (size_t)P.Next * Nr * P.Ntpad;
-    const double4 *gbase = reinterpret_cast<const double4 *>(P.geom), *gend = gbase + gtotal, *gnext = gbase;
-    unsigned gphase = 0;
+    // (32-bit record index: at most 2^31 points per system; checked in dse_create)
+    const unsigned gtotal = (unsigned)P.Next * (unsigned)Nr * (unsigned)P.Ntpad;
+    unsigned gidx = 0, gphase = 0;
     auto prefetch = [&](unsigned buf) {
+        const double4 *src = reinterpret_cast<const double4 *>(P.geom) + gidx;
         const unsigned dst = (unsigned)__cvta_generic_to_shared(s_gbuf + buf * 32 + lane);
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(gnext));
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(gnext) + 16));
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src));
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(src) + 16));
         asm volatile("cp.async.commit_group;\n" ::);
     };
 
-    long long bi = r0 / Nr;
-    int q = (int)(r0 - bi * Nr);
-    int cur_b = (int)(bi / P.Next);
-    int e = (int)(bi - (long long)cur_b * P.Next);
+    int bi = (int)(r0 / Nr);
+    int q = (int)(r0 - (long long)bi * Nr);
+    int cur_b = bi / P.Next;
+    int e = bi - cur_b * P.Next;
     if (GEOM) {
-        gnext = gbase + ((size_t)e * Nr + q) * P.Ntpad + lane;
+        gidx = ((unsigned)e * Nr + q) * P.Ntpad + kb * 32 + lane;
         prefetch(0);
     }
     if (!CONSTC) {
@@ -420,17 +429,16 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
         for (int c = 0; c < NCH; ++c)
             reinterpret_cast<double2 *>(s_stash + b2 * STASH + 132)[c * (TCH_STRIDE / 2) + lane] = make_double2(0.0, 0.0);
 
-    long long r = r0;
+    int rem = (int)(t1 - t0);                              // batches left for this warp
     int cur = 0;                                           // stash half written by the current batch
-    while (r < r1) {
-        // ---------------- one (warp, external point) segment: rows [r, rend) ----------------
-        long long rend = r + (Nr - q);
-        if (rend > r1) rend = r1;
+    while (rem > 0) {
+        // ---------------- one (warp, external point) segment ----------------
 #pragma unroll
         for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
         reinterpret_cast<double4 *>(s_stash + (cur ^ 1) * STASH)[lane] = make_double4(0.0, 0.0, 0.0, 0.0);   // prologue
         __syncwarp();
-        for (; r < rend; ++r, ++q) {
+        bool seg_done = false;
+        while (!seg_done) {
             const double Gy = P.Gy[(size_t)cur_b * Nr + q], Py = P.Py[(size_t)cur_b * Nr + q];
             RowConst rc;
             if (!GEOM) {
@@ -441,11 +449,13 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
                 rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
             }
             double sumA = 0.0, sumB = 0.0, sumV = 0.0, sumZ = 0.0;
-            for (int kb = 0; kb < BPR; ++kb) {
+            const int kb_begin = kb;
+            const int kb_end = (rem < BPR - kb) ? kb + rem : BPR;
+            for (; kb < kb_end; ++kb, --rem) {
                 double sraw, gv, gq, gm;
                 if (GEOM) {
-                    gnext += 32;
-                    if (gnext >= gend) gnext -= gtotal;
+                    gidx += 32;
+                    if (gidx >= gtotal) gidx -= gtotal;
                     prefetch(gphase ^ 1);
                     asm volatile("cp.async.wait_group 1;\n" ::: "memory");
                     const double2 *gp = reinterpret_cast<const double2 *>(s_gbuf + gphase * 32 + lane);
@@ -504,15 +514,30 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
                 __syncwarp();
                 cur ^= 1;
             }
-            // H5/H7: row sums over the 32 angular lanes (fixed xor tree), lane 0 writes
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                sumA += __shfl_xor_sync(FULL, sumA, o);
-                sumB += __shfl_xor_sync(FULL, sumB, o);
-                sumV += __shfl_xor_sync(FULL, sumV, o);
-                sumZ += __shfl_xor_sync(FULL, sumZ, o);
+            // H5/H7: row sums over the 32 angular lanes.  Transposing reduction: after the first two steps each
+            // quarter-warp carries one of the four sums (6 shuffles instead of 20; fixed order -> deterministic).
+            {
+                const bool up = lane & 16, hi = lane & 8;
+                double x0 = up ? sumV : sumA, x1 = up ? sumZ : sumB;
+                const double y0 = up ? sumA : sumV, y1 = up ? sumB : sumZ;
+                x0 += __shfl_xor_sync(FULL, y0, 16);
+                x1 += __shfl_xor_sync(FULL, y1, 16);
+                double z = hi ? x1 : x0;
+                const double zs = hi ? x0 : x1;
+                z += __shfl_xor_sync(FULL, zs, 8);
+                z += __shfl_xor_sync(FULL, z, 4);
+                z += __shfl_xor_sync(FULL, z, 2);
+                z += __shfl_xor_sync(FULL, z, 1);
+                // lanes 0, 8, 16, 24 hold sum(u_a), sum(u_b), sum(v), sum(wQ + wM)
+                const bool has_first = kb_begin == 0, has_last = kb_end == BPR;
+                double *dst = (has_last ? P.Apart : P.AHead) + ((size_t)bi * Nr + q) * 4 + (lane >> 3);
+                if ((lane & 7) == 0) {
+                    *dst = z;
+                    if (has_first && has_last) P.AHead[((size_t)bi * Nr + q) * 4 + (lane >> 3)] = 0.0;
+                }
+                if (has_last) { kb = 0; ++q; if (q == Nr) seg_done = true; }
+                if (rem <= 0) seg_done = true;
             }
-            if (lane == 0) reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
         }
         // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
         phase2(cur ^ 1);
@@ -521,7 +546,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
             q = 0; ++bi; ++e;
             if (e == P.Next) {
                 e = 0; ++cur_b;
-                if (!CONSTC && r < r1) {
+                if (!CONSTC && rem > 0) {
                     for (int j = lane; j < Npad; j += 32)
                         s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
                     __syncwarp();
@@ -614,6 +639,19 @@ static KernelFn pick_pipe(const KParams &k)
 #undef DSE_PIPE_CASE
 }
 
+// grid of the pipelined kernel: units are 32-point batches; every warp gets >= max(4, batches per row) of them so
+// that a row spans at most two warps
+static long long pick_grid_pipe(const KParams &k, int sms, int per_sm, int wpb)
+{
+    const long long bpr = k.Ntpad / 32, units = k.R * bpr, min_units = bpr > 4 ? bpr : 4;
+    long long grid = (long long)sms * per_sm;
+    long long want_grid = (units / min_units + wpb - 1) / wpb;
+    if (want_grid < 1) want_grid = 1;
+    if (want_grid < grid) grid = want_grid;
+    while (grid > 1 && units / (grid * wpb) < min_units) --grid;
+    return grid;
+}
+
 static long long pick_grid(const KParams &k, int sms, int per_sm, int wpb)
 {
     // persistent-style grid: one wave of resident CTAs, but never more warps than rows
@@ -676,7 +714,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     cfg.smem = jsmem;
     cfg.regs = fa.numRegs;
     cfg.ctas_per_sm = per_sm;
-    cfg.grid = (int)pick_grid(k, sms, per_sm, block / 32);
+    cfg.grid = (int)(cfg.pipelined ? pick_grid_pipe(k, sms, per_sm, block / 32) : pick_grid(k, sms, per_sm, block / 32));
     return 0;
 }
 

@@ -300,7 +300,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", type=int, default=3, choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--geometry-cache", type=int, default=0)
+    ap.add_argument("--geometry-cache", type=int, default=1,
+                    help="1: coefficient-independent per-point factors are tabulated once in dse_create (default); "
+                         "0: recomputed inside every build")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     w, c, bc = config_inputs(args.config)

@@ -166,20 +166,33 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
     const long long bi_i = (long long)b * P.Next + i, bi_Z = (long long)b * P.Next + P.iZ,
                     bi_G = (long long)b * P.Next + P.iG;
     __shared__ double s_pi[3][2];
+    __shared__ double s_pw[ASM_THREADS / 32][3][2];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (warp < 3) {                              // Pi_G, Pi_Z at e = i, x_Z, x_G: fixed-order sum over q
-        const long long bi = warp == 0 ? bi_i : (warp == 1 ? bi_Z : bi_G);
-        double pg = 0.0, pz = 0.0;
-        for (int q = lane; q < P.Nr; q += 32) {
-            const double4 a = reinterpret_cast<const double4 *>(P.Apart)[(size_t)bi * P.Nr + q];
-            const double4 hh = reinterpret_cast<const double4 *>(P.AHead)[(size_t)bi * P.Nr + q];
-            pg += a.z + hh.z; pz += a.w + hh.w;
+    {   // Pi_G, Pi_Z at e = i, x_Z, x_G: all threads stride over q (loads in flight together), fixed-order combine
+        const int npi = (P.iG != P.iZ) ? 3 : 2;
+        for (int pt = 0; pt < npi; ++pt) {
+            const long long bi = pt == 0 ? bi_i : (pt == 1 ? bi_Z : bi_G);
+            double pg = 0.0, pz = 0.0;
+            for (int q = threadIdx.x; q < P.Nr; q += ASM_THREADS) {
+                const double4 a = reinterpret_cast<const double4 *>(P.Apart)[(size_t)bi * P.Nr + q];
+                const double4 hh = reinterpret_cast<const double4 *>(P.AHead)[(size_t)bi * P.Nr + q];
+                pg += a.z + hh.z; pz += a.w + hh.w;
+            }
+            for (int o = 16; o > 0; o >>= 1) {
+                pg += __shfl_xor_sync(FULL, pg, o);
+                pz += __shfl_xor_sync(FULL, pz, o);
+            }
+            if (lane == 0) { s_pw[warp][pt][0] = pg; s_pw[warp][pt][1] = pz; }
         }
-        for (int o = 16; o > 0; o >>= 1) {
-            pg += __shfl_xor_sync(FULL, pg, o);
-            pz += __shfl_xor_sync(FULL, pz, o);
+        __syncthreads();
+        if (threadIdx.x < 2 * npi) {
+            const int pt = threadIdx.x >> 1, cmp = threadIdx.x & 1;
+            double t = 0.0;
+            for (int w2 = 0; w2 < ASM_THREADS / 32; ++w2) t += s_pw[w2][pt][cmp];
+            s_pi[pt][cmp] = t;
         }
-        if (lane == 0) { s_pi[warp][0] = pg; s_pi[warp][1] = pz; }
+        __syncthreads();
+        if (npi == 2 && threadIdx.x < 2) s_pi[2][threadIdx.x] = s_pi[1][threadIdx.x];     // x_G == x_Z
     }
     __syncthreads();
     const double invZ = P.invZ[(size_t)b * N + i], invG = P.invG[(size_t)b * N + i];

@@ -77,6 +77,10 @@ typedef struct dse_params {
 #define DSE_FLAG_GEOMETRY_CACHE 1 /* precompute the coefficient-independent per-point factors once in
                                      dse_create (32 B/point in HBM) instead of per build            */
 
+#define DSE_FLAG_ANGULAR_TANH_SINH 2 /* angular rule: tanh-sinh in xi = cos(theta) (eq.(5)) with n_theta
+                                        equidistant abscissae t_k in [-3,3], xi_k = tanh((pi/2) sinh t_k), instead of
+                                        Gauss-Legendre in theta (reading A9b)                              */
+
 typedef struct dse_handle dse_handle; /* opaque; owned by the library */
 
 /* Builds the quadrature/collocation tables (Gauss-Legendre in ln y and in theta, Chebyshev roots

@@ -42,6 +42,7 @@ typedef long double real;
 #define R_SQRT sqrtl
 #define R_SIN sinl
 #define R_COS cosl
+#define R_ATAN atanl
 #define R_FABS fabsl
 #define R_PI 3.14159265358979323846264338327950288L
 #define R_TINY 1e-19L
@@ -52,6 +53,7 @@ typedef double real;
 #define R_SQRT sqrt
 #define R_SIN sin
 #define R_COS cos
+#define R_ATAN atan
 #define R_FABS fabs
 #define R_PI 3.14159265358979323846264338327950288
 #define R_TINY 1e-16
@@ -62,7 +64,8 @@ typedef struct orc_params {
     int32_t n_cheb;    /* N: Chebyshev polynomials per dressing function, eq.(23),(24) L179-181 */
     int32_t n_r;       /* radial Gauss-Legendre nodes in ln y on [eps2, L2] (L62; reading A8)   */
     int32_t n_theta;   /* angular Gauss-Legendre nodes in theta on [0, pi] (reading A9)         */
-    int32_t pad_;
+    int32_t angular_rule; /* 0: Gauss-Legendre in theta (BASELINE configs, reading A9);
+                             1: tanh-sinh in xi = cos(theta) (eq.(5)), reading A9b      */
     double eps2, L2;   /* IR matching point / UV cutoff (L188)                                  */
     double alpha_mu;   /* alpha(mu^2) = g^2 / 4 pi (L131, L135)                                 */
     double n_colors;   /* N_c                                                                   */
@@ -257,10 +260,28 @@ void orc_tables(const orc_params *p, double *x_ext, double *s_root, double *t_r,
         Wy[q] = (double)((real)w[q] * (Lg / 2) * yy);
     }
     double *tau = (double *)malloc(sizeof(double) * (size_t)Nt);
-    orc_gauss_legendre(Nt, tau, w);
-    for (int k = 0; k < Nt; ++k) {
-        theta[k] = (double)(((real)tau[k] + 1) * R_PI / 2);
-        Omega[k] = (double)((real)w[k] * R_PI / 2);
+    if (p->angular_rule == 0) {
+        orc_gauss_legendre(Nt, tau, w);
+        for (int k = 0; k < Nt; ++k) {
+            theta[k] = (double)(((real)tau[k] + 1) * R_PI / 2);
+            Omega[k] = (double)((real)w[k] * R_PI / 2);
+        }
+    } else {
+        /* tanh-sinh rule for int_{-1}^{1} dxi sqrt(1-xi^2) f  (eq.(5), ref.[31]); the paper gives no step or
+         * truncation: reading A9b takes Nt equidistant abscissae t_k in [-3, 3], u_k = (pi/2) sinh t_k,
+         * xi_k = tanh u_k, w_k = h (pi/2) cosh t_k / cosh^2 u_k.  In the theta form used here:
+         * theta_k = 2 atan(exp(-u_k)) (so that cos theta = xi, sin theta = 1/cosh u without cancellation) and
+         * Omega_k = w_k / sin theta_k, i.e. Omega sin^2 = w sqrt(1-xi^2), Omega sin^4 = w (1-xi^2)^(3/2). */
+        const real tmax = 3;
+        const real h = (Nt > 1) ? 2 * tmax / (real)(Nt - 1) : 0;
+        for (int k = 0; k < Nt; ++k) {
+            real t = tmax - h * (real)k;                 /* descending t -> ascending theta */
+            real u = R_PI / 2 * (R_EXP(t) - R_EXP(-t)) / 2;
+            real ch = (R_EXP(u) + R_EXP(-u)) / 2;        /* cosh u = 1 / sin theta */
+            real wk = h * (R_PI / 2) * ((R_EXP(t) + R_EXP(-t)) / 2) / (ch * ch);
+            theta[k] = (double)(2 * R_ATAN(R_EXP(-u)));
+            Omega[k] = (double)(wk * ch);
+        }
     }
     for (int i = 0; i < N; ++i) {
         real s = -R_COS(R_PI * ((real)i + (real)0.5) / (real)N);

@@ -18,7 +18,7 @@ _dp = C.POINTER(C.c_double)
 
 class OrcParams(C.Structure):
     _fields_ = [
-        ("n_cheb", C.c_int32), ("n_r", C.c_int32), ("n_theta", C.c_int32), ("pad_", C.c_int32),
+        ("n_cheb", C.c_int32), ("n_r", C.c_int32), ("n_theta", C.c_int32), ("angular_rule", C.c_int32),
         ("eps2", C.c_double), ("L2", C.c_double), ("alpha_mu", C.c_double), ("n_colors", C.c_double),
         ("x_G", C.c_double), ("x_Z", C.c_double), ("delta", C.c_double),
         ("ir_exp_G", C.c_double), ("ir_exp_Z", C.c_double), ("uv_omega", C.c_double),
@@ -26,10 +26,10 @@ class OrcParams(C.Structure):
 
 
 def make_params(n_cheb, n_r, n_theta, eps2, L2, x_G, x_Z, alpha_mu=1.0, n_colors=3.0, delta=-9.0 / 44.0,
-                ir_exp_G=-0.595353, ir_exp_Z=2 * 0.595353, uv_omega=None):
+                ir_exp_G=-0.595353, ir_exp_Z=2 * 0.595353, uv_omega=None, angular_rule=0):
     if uv_omega is None:
         uv_omega = 11.0 * n_colors * alpha_mu / (12.0 * np.pi)
-    return OrcParams(int(n_cheb), int(n_r), int(n_theta), 0, float(eps2), float(L2), float(alpha_mu),
+    return OrcParams(int(n_cheb), int(n_r), int(n_theta), int(angular_rule), float(eps2), float(L2), float(alpha_mu),
                      float(n_colors), float(x_G), float(x_Z), float(delta), float(ir_exp_G), float(ir_exp_Z),
                      float(uv_omega))
 

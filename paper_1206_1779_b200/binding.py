@@ -19,6 +19,7 @@ EXPORTS = [
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
+DSE_FLAG_ANGULAR_TANH_SINH = 2
 
 
 class DseParams(C.Structure):
@@ -79,6 +80,8 @@ def _check(rc):
 
 
 def params_from_workload(w, n_batch=None, flags=0):
+    if getattr(w, "angular_rule", 0) == 1:
+        flags |= DSE_FLAG_ANGULAR_TANH_SINH
     return DseParams(w.n_cheb, w.n_r, w.n_theta, w.n_batch if n_batch is None else n_batch, w.eps2, w.L2,
                      w.alpha_mu, w.n_colors, w.x_G, w.x_Z, w.delta, w.ir_exp_G, w.ir_exp_Z, w.uv_omega, flags, 0)
 

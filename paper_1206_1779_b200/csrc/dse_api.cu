@@ -65,7 +65,7 @@ int validate(const dse_params *p)
     if (!finite_pos(p->x_G) || !finite_pos(p->x_Z)) return DSE_EINVAL;
     if (!std::isfinite(p->delta) || !std::isfinite(p->ir_exp_G) || !std::isfinite(p->ir_exp_Z)) return DSE_EINVAL;
     if (!std::isfinite(p->uv_omega) || p->uv_omega < 0.0) return DSE_EINVAL;
-    if (p->reserved != 0 || (p->flags & ~DSE_FLAG_GEOMETRY_CACHE)) return DSE_EINVAL;
+    if (p->reserved != 0 || (p->flags & ~(DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_ANGULAR_TANH_SINH))) return DSE_EINVAL;
     return DSE_OK;
 }
 

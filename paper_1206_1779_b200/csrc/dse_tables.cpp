@@ -105,10 +105,34 @@ void build_tables(const dse_params &p, HostTables &T)
         T.t_r[q] = (double)t[q];
         phi_row(N, T.Npad, t[q], &T.phi_y[(size_t)q * T.Npad]);
     }
-    // angular rule in theta
-    gauss_legendre(Nt, t, w);
+    // angular rule: Gauss-Legendre in theta, or tanh-sinh in xi = cos(theta) (eq.(5))
     T.theta.resize(Nt); T.Omega.resize(Nt);
     T.ang.assign((size_t)T.Ntpad * 6, 0.0);
+    if (p.flags & DSE_FLAG_ANGULAR_TANH_SINH) {
+        // int dxi sqrt(1-xi^2) f:  t_k equidistant in [-3,3], u = (pi/2) sinh t, xi = tanh u, 1-xi^2 = 1/cosh^2 u,
+        // w = h (pi/2) cosh t / cosh^2 u.  The kernel's "Omega sin^2" and "Omega sin^4" are w sqrt(1-xi^2) and
+        // w (1-xi^2)^(3/2); sin^2(theta/2) = (1-xi)/2 = 1/(1+e^{2u}) without cancellation.
+        const ld tmax = 3.0L, h = Nt > 1 ? 2 * tmax / (Nt - 1) : 0.0L;
+        for (int k = 0; k < Nt; ++k) {
+            const ld tt = tmax - h * k;                       // descending t: ascending theta
+            const ld u = PI_L / 2 * sinhl(tt), ch = coshl(u), xi = tanhl(u);
+            const ld wk = h * (PI_L / 2) * coshl(tt) / (ch * ch);
+            T.theta[k] = (double)(2 * atanl(expl(-u)));
+            T.Omega[k] = (double)(wk * ch);
+            double *a = &T.ang[(size_t)k * 6];
+            a[0] = (double)(1 / (1 + expl(2 * u)));
+            a[1] = (double)(6 * xi);
+            a[2] = (double)(2 + xi * xi);
+            a[3] = (double)(-2 / (ch * ch));
+            a[4] = (double)(wk / ch);
+            a[5] = (double)(wk / (ch * ch * ch));
+        }
+        for (int k = Nt; k < T.Ntpad; ++k) {                  // padded lanes: a valid angle with zero weight
+            double *a = &T.ang[(size_t)k * 6];
+            for (int m = 0; m < 4; ++m) a[m] = T.ang[m];
+        }
+    } else {
+    gauss_legendre(Nt, t, w);
     for (int k = 0; k < T.Ntpad; ++k) {
         const int kk = k < Nt ? k : 0;                 // padded lanes: a valid angle with zero weight
         ld th = (t[kk] + 1) * PI_L / 2;
@@ -124,6 +148,7 @@ void build_tables(const dse_params &p, HostTables &T)
         a[3] = (double)(-2 * s * s);
         a[4] = (double)((ld)(double)Om * s * s);
         a[5] = (double)((ld)(double)Om * s * s * s * s);
+    }
     }
     // external points: Chebyshev roots s_i = -cos(pi (i+1/2)/N), ascending, then x_Z, then x_G
     T.x_ext.resize(T.Next); T.sx_ext.resize(T.Next); T.c3x_ext.resize(T.Next);

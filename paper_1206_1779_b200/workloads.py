@@ -31,6 +31,7 @@ class Workload:
     ir_exp_G: float = -KAPPA
     ir_exp_Z: float = 2 * KAPPA
     uv_omega: float = field(default=None)
+    angular_rule: int = 0  # 0: Gauss-Legendre in theta (BASELINE configs); 1: tanh-sinh in xi
 
     def __post_init__(self):
         if self.uv_omega is None:

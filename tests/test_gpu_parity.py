@@ -22,7 +22,7 @@ def _torch():
 def oracle_params(w):
     from oracle.oracle import make_params
     return make_params(w.n_cheb, w.n_r, w.n_theta, w.eps2, w.L2, w.x_G, w.x_Z, w.alpha_mu, w.n_colors, w.delta,
-                       w.ir_exp_G, w.ir_exp_Z, w.uv_omega)
+                       w.ir_exp_G, w.ir_exp_Z, w.uv_omega, getattr(w, "angular_rule", 0))
 
 
 def gpu_build(w, c, bc, flags=0, jac=True):
@@ -180,3 +180,22 @@ def test_config4_full_batch_sampled_systems(orc):
     assert np.array_equal(J2[0], J2[1])
     assert np.allclose(F2[1, N:] - F2[0, N:], -(bc[1, 0] - bc[0, 0]), rtol=0, atol=1e-12)
     assert np.array_equal(F2[1, :N], F2[0, :N])
+
+
+@pytest.mark.parametrize("n_theta", [16, 64, 40])
+def test_tanh_sinh_angular_rule_parity(orc, n_theta):
+    """NEXT f3: tanh-sinh rule in xi = cos(theta); only the tables change."""
+    _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    w = Workload("tanh-sinh", 16, 48, n_theta, 1e-6, 5e4, angular_rule=1)
+    c = draw_coefficients(23, w.n_cheb)[None, :]
+    bc = np.array([[1.1, 0.9]])
+    Fo, Jo = orc.residual_jacobian(oracle_params(w), c[0], 1.1, 0.9)
+    for flags in (0, 1):
+        J, F = gpu_build(w, c, bc, flags)
+        check(J[0], F[0], Jo, Fo)
+    d = Dse(params_from_workload(w))
+    t = d.tables(); d.close()
+    o = orc.tables(oracle_params(w))
+    assert np.allclose(t["theta"], o["theta"], rtol=1e-13) and np.allclose(t["Omega"], o["Omega"], rtol=1e-12)

@@ -276,3 +276,38 @@ def test_infrared_exponent_and_fixed_point_P8(orc):
     k_star = (k0 - 0.0001) + 0.0002 * f_lo / (f_lo - f_hi)
     assert abs(k_star - k0) < 5e-6                          # the paper prints six digits
     assert abs(k_star - (93 - math.sqrt(1201)) / 98) < 5e-6
+
+
+# ------------------------------------------------------------------------------------------ NEXT f3
+def test_tanh_sinh_angular_rule(orc):
+    """PAPER.md L62-66, eq.(5): int_0^pi dtheta sin^2 f -> int_{-1}^{1} dxi sqrt(1-xi^2) f with a tanh-sinh rule
+    (reading A9b).  Checked against closed forms: the measure itself, the ghost measure, and the closed-form
+    angular integrals of pin P4 (kernels with endpoint-singular behaviour at t -> 1)."""
+    p = make_params(4, 4, 64, 1e-4, 1e4, 1.0, 1.0, angular_rule=1)
+    tab = orc.tables(p)
+    th, Om = tab["theta"], tab["Omega"]
+    assert np.all(np.diff(th) > 0) and th[0] > 0 and th[-1] < PI
+    xi = np.cos(th)
+    # nodes are xi = tanh((pi/2) sinh t) on an equidistant t grid in [-3, 3]
+    t_grid = np.arcsinh(np.arctanh(np.clip(xi[8:-8], -1, 1)) * 2 / PI)
+    assert np.allclose(np.diff(t_grid), -6.0 / 63, atol=1e-9)
+    s2 = np.sin(th) ** 2
+    assert abs(np.sum(Om * s2) - PI / 2) < 1e-13            # int sqrt(1-xi^2) dxi
+    assert abs(np.sum(Om * s2 ** 2) - 3 * PI / 8) < 1e-13   # int (1-xi^2)^(3/2) dxi  (eq.(8), reading A1)
+    for (x, y) in [(1.0, 2.0), (1.0, 1.0 / 0.9), (3.7, 0.037)]:
+        big, small = max(x, y), min(x, y)
+        tt = small / big
+        z = np.array([orc.z(x, y, a) for a in th])
+        M = np.array([orc.kernel_M(x, y, a) for a in th])
+        Q = np.array([orc.kernel_Q(x, y, a) for a in th])
+        assert abs(np.sum(Om * s2 / z) - PI / (2 * big)) < 1e-10 / big
+        exact_M = PI * (3 - tt) / 8 if y > x else PI * tt * (3 - tt) / 8
+        assert abs(np.sum(Om * s2 * M) - exact_M) < 1e-10
+        assert abs(np.sum(Om * s2 * Q) - PI * (7 * tt * tt - 50 * tt - 6) / 16) < 1e-9
+    # the two rules give the same self-energies up to their (small) quadrature errors
+    c = np.array([0.2, -0.1, 0.05, 0.0, -0.3, 0.1, 0.0, 0.02])
+    pg = make_params(4, 4, 64, 1e-4, 1e4, 1.0, 1.0, angular_rule=0)
+    tg = orc.tables(pg)
+    a = orc.self_energy(p, c, 0.7, tab["y"], tab["Wy"], th, Om)
+    b = orc.self_energy(pg, c, 0.7, tg["y"], tg["Wy"], tg["theta"], tg["Omega"])
+    assert np.allclose(a, b, rtol=1e-6)

@@ -79,37 +79,51 @@ typedef struct orc_params {
 /* ------------------------------------------------------------------------------------------ */
 /* P1. Gauss-Legendre nodes t[0..n) ascending in (-1,1) and weights w, by Newton iteration on   */
 /* the Legendre three-term recurrence (textbook; "standard Gauss-Legendre").       */
+static void gl_node(int n, int i, real *xo, real *wo)
+{
+    /* Chebyshev-like initial guess, ascending order */
+    real x = -R_COS(R_PI * ((real)i + (real)0.75) / ((real)n + (real)0.5));
+    real dp = 1;
+    for (int it = 0; it < 100; ++it) {
+        real p0 = 1, p1 = x;
+        for (int m = 2; m <= n; ++m) {
+            real p2 = (((real)(2 * m - 1)) * x * p1 - ((real)(m - 1)) * p0) / (real)m;
+            p0 = p1; p1 = p2;
+        }
+        if (n == 1) { p0 = 1; p1 = x; }
+        dp = (real)n * (x * p1 - p0) / (x * x - 1);     /* P_n'(x) */
+        real dx = p1 / dp;
+        x -= dx;
+        if (R_FABS(dx) <= R_TINY) break;
+    }
+    /* final derivative at the converged node */
+    {
+        real p0 = 1, p1 = x;
+        for (int m = 2; m <= n; ++m) {
+            real p2 = (((real)(2 * m - 1)) * x * p1 - ((real)(m - 1)) * p0) / (real)m;
+            p0 = p1; p1 = p2;
+        }
+        if (n == 1) { p0 = 1; p1 = x; }
+        dp = (real)n * (x * p1 - p0) / (x * x - 1);
+    }
+    *xo = x;
+    *wo = 2 / ((1 - x * x) * dp * dp);
+}
 void orc_gauss_legendre(int n, double *t, double *w)
 {
     for (int i = 0; i < n; ++i) {
-        /* Chebyshev-like initial guess, ascending order */
-        real x = -R_COS(R_PI * ((real)i + (real)0.75) / ((real)n + (real)0.5));
-        real dp = 1;
-        for (int it = 0; it < 100; ++it) {
-            real p0 = 1, p1 = x;
-            for (int m = 2; m <= n; ++m) {
-                real p2 = (((real)(2 * m - 1)) * x * p1 - ((real)(m - 1)) * p0) / (real)m;
-                p0 = p1; p1 = p2;
-            }
-            if (n == 1) { p0 = 1; p1 = x; }
-            dp = (real)n * (x * p1 - p0) / (x * x - 1);     /* P_n'(x) */
-            real dx = p1 / dp;
-            x -= dx;
-            if (R_FABS(dx) <= R_TINY) break;
-        }
-        /* final derivative at the converged node */
-        {
-            real p0 = 1, p1 = x;
-            for (int m = 2; m <= n; ++m) {
-                real p2 = (((real)(2 * m - 1)) * x * p1 - ((real)(m - 1)) * p0) / (real)m;
-                p0 = p1; p1 = p2;
-            }
-            if (n == 1) { p0 = 1; p1 = x; }
-            dp = (real)n * (x * p1 - p0) / (x * x - 1);
-        }
+        real x, ww;
+        gl_node(n, i, &x, &ww);
         t[i] = (double)x;
-        w[i] = (double)(2 / ((1 - x * x) * dp * dp));
+        w[i] = (double)ww;
     }
+}
+/* one node of the n-point rule (for sampled checks of very large rules, e.g. n = 2^17 of PAPER.md fn.13) */
+void orc_gl_node(int n, int i, double *t, double *w)
+{
+    real x, ww;
+    gl_node(n, i, &x, &ww);
+    *t = (double)x; *w = (double)ww;
 }
 
 /* P2. phi_0 = 1/2, phi_j = T_j(s) for j >= 1 (the b_0/2 convention of eq.(23),(24) L179-181),  */
@@ -481,6 +495,37 @@ int orc_newton_step(const orc_params *p, double *c, double gG, double gZ, double
     for (int j = 0; j < n; ++j) c[j] -= rho * d[j];
     free(F);
     return rc;
+}
+
+/* NEXT f4. Schwinger function of the gluon propagator, eq.(20) L157 with sigma(p^2) = Z(p^2)/p^2 (L161):
+ *   Delta(t) = (1/pi) int_0^inf d|p| cos(t|p|) Z(p^2)/p^2
+ * as a "generalized scalar product" over a mapped Gauss-Legendre rule (L382; 2^17 nodes in fn.13).  The paper
+ * does not give the map: reading A22 takes n_nodes GL nodes in u = ln|p| on [ln sqrt(p2_min), ln sqrt(p2_max)],
+ * d|p| = |p| du.  Z outside [eps2, L2] is the continuation of O2.  Plain serial sums, node by node. */
+void orc_schwinger(const orc_params *p, const double *c, int n_nodes, double p2_min, double p2_max, int n_t,
+                   const double *t, double *out)
+{
+    const int N = p->n_cheb;
+    real *cr = (real *)malloc(sizeof(real) * (size_t)(3 * N + 2 * n_nodes));
+    real *phi = cr + 2 * N, *pn = phi + N, *fn = pn + n_nodes;
+    for (int j = 0; j < 2 * N; ++j) cr[j] = c[j];
+    const real u0 = R_LOG((real)p2_min) / 2, u1 = R_LOG((real)p2_max) / 2;
+    for (int i = 0; i < n_nodes; ++i) {
+        real x, w;
+        gl_node(n_nodes, i, &x, &w);
+        real u = u0 + (x + 1) / 2 * (u1 - u0);
+        real pp = R_EXP(u);
+        real lnG, lnZ, sc;
+        ln_dress(p, cr, pp * pp, phi, &lnG, &lnZ, &sc);
+        pn[i] = pp;
+        fn[i] = w * (u1 - u0) / 2 * pp * R_EXP(lnZ) / (pp * pp);      /* d|p| * Z(p^2)/p^2 */
+    }
+    for (int m = 0; m < n_t; ++m) {
+        real sum = 0;
+        for (int i = 0; i < n_nodes; ++i) sum += fn[i] * R_COS((real)t[m] * pn[i]);
+        out[m] = (double)(sum / R_PI);
+    }
+    free(cr);
 }
 
 int orc_sizeof_real(void) { return (int)sizeof(real); }

@@ -51,6 +51,8 @@ class Oracle:
         L = self.lib
         L.orc_gauss_legendre.argtypes = [C.c_int, _dp, _dp]
         L.orc_cheb_phi.argtypes = [C.c_int, C.c_double, _dp]
+        L.orc_gl_node.argtypes = [C.c_int, C.c_int, _dp, _dp]
+        L.orc_schwinger.argtypes = [C.POINTER(OrcParams), _dp, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp]
         for name in ("orc_z", "orc_kernel_M", "orc_kernel_Q", "orc_kernel_ghost", "orc_kernel_M_literal",
                      "orc_kernel_Q_literal"):
             f = getattr(L, name)
@@ -74,6 +76,17 @@ class Oracle:
         t = np.empty(n); w = np.empty(n)
         self.lib.orc_gauss_legendre(n, _ptr(t), _ptr(w))
         return t, w
+
+    def gl_node(self, n, i):
+        t = C.c_double(); w = C.c_double()
+        self.lib.orc_gl_node(int(n), int(i), C.byref(t), C.byref(w))
+        return t.value, w.value
+
+    def schwinger(self, p, c, n_nodes, p2_min, p2_max, t):
+        c = _f64(c); t = _f64(t)
+        out = np.empty(len(t))
+        self.lib.orc_schwinger(C.byref(p), _ptr(c), int(n_nodes), float(p2_min), float(p2_max), len(t), _ptr(t), _ptr(out))
+        return out
 
     def cheb_phi(self, n, s):
         phi = np.empty(n)

@@ -272,3 +272,41 @@ def test_config2_start_is_ill_conditioned(orc, orc_ld):
     # and the Newton matrix is numerically singular at this point (row-scaled min pivot ~ eps)
     x, stats, rc = orc.lu_solve(J, F)
     assert stats[2] < 1e-10
+
+
+# ------------------------------------------------------------------------------------ NEXT f4: Schwinger function
+def _massive_propagator_coefficients(orc, N, eps2, L2):
+    """ln Z interpolating Z = x/(x+1) (sigma = Z/p^2 = 1/(p^2+m^2), m = 1) at the Chebyshev roots."""
+    p = make_params(N, 4, 4, eps2, L2, 1.0, 1.0, ir_exp_G=0.0, ir_exp_Z=1.0, uv_omega=0.0)
+    tab = orc.tables(p)
+    x = tab["x_ext"][:N]
+    T = np.stack([orc.cheb_phi(N, s) for s in tab["s_root"]])
+    T[:, 0] *= 2
+    a = (2.0 / N) * (T.T @ np.log(x / (x + 1.0)))
+    return p, np.concatenate([a, np.zeros(N)])
+
+
+def test_schwinger_function_closed_form(orc):
+    """eq.(20): Delta(t) = (1/pi) int_0^inf dp cos(tp) sigma(p^2).  For sigma = 1/(p^2+m^2) the textbook value is
+    exp(-m t)/(2m); the cutoff at p_max = 100 leaves a tail of order sin(t p_max)/(pi t p_max^2) ~ 1e-5."""
+    p, c = _massive_propagator_coefficients(orc, 64, 1e-6, 1e4)
+    t = np.array([0.5, 1.0, 3.0, 6.0])
+    d = orc.schwinger(p, c, 2048, 1e-16, 1e4, t)
+    assert np.allclose(d, np.exp(-t) / 2, rtol=0, atol=5e-5)
+    assert np.all(d > 0)                                    # a physical (positive-norm) particle: no zero crossing
+    d2 = orc.schwinger(p, c, 4096, 1e-16, 1e4, t)
+    assert np.allclose(d, d2, rtol=0, atol=1e-9)            # converged in the number of nodes
+
+
+def test_gl_single_node_matches_full_rule(orc):
+    t, w = orc.gauss_legendre(257)
+    for i in (0, 1, 128, 200, 256):
+        ti, wi = orc.gl_node(257, i)
+        assert ti == t[i] and wi == w[i]
+    # a node of the paper's 2^17-point rule (fn.13): symmetric partner and the asymptotic spacing pi/(n+1/2)
+    n = 1 << 17
+    a, wa = orc.gl_node(n, 1000)
+    b, wb = orc.gl_node(n, n - 1 - 1000)
+    assert abs(a + b) < 1e-15 and abs(wa - wb) < 1e-18
+    a2, _ = orc.gl_node(n, 1001)
+    assert abs((math.acos(a) - math.acos(a2)) - PI / (n + 0.5)) < 1e-9

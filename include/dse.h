@@ -140,6 +140,18 @@ DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[6]);
 DSE_API int dse_set_timing(dse_handle *h, int32_t enable);
 DSE_API int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches);
 
+/* NEXT f4 -- the paper's second GPU workload (Table 2).
+ * dse_gauss_legendre: n-point Gauss-Legendre rule generated on the device (Newton iteration on the Legendre
+ * recurrence, one thread per pair of nodes): x_dev[n] ascending in (-1,1), w_dev[n]; work_dev >= 2(n+2) doubles.
+ * dse_schwinger: Delta(t_m) = (1/pi) int d|p| cos(t_m |p|) Z(p^2)/p^2, eq.(20) with sigma = Z/p^2 (L161), over
+ * n_nodes Gauss-Legendre nodes in ln|p| on [sqrt(p2_min), sqrt(p2_max)] (reading A22); Z from the
+ * a-coefficients of c_dev [n_batch][2N] with the continuation of eq.(16),(19) outside [eps2, L2].
+ * t_dev[n_t], delta_dev[n_batch][n_t]; work_dev >= (5 + n_batch) n_nodes + 4 doubles.  Asynchronous on `stream`,
+ * deterministic.  2 <= n, n_nodes <= 2^24; 0 < p2_min < p2_max. */
+DSE_API int dse_gauss_legendre(int32_t n, double *x_dev, double *w_dev, double *work_dev, void *stream);
+DSE_API int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, double p2_min, double p2_max,
+                          const double *t_dev, int32_t n_t, double *delta_dev, double *work_dev, void *stream);
+
 /* Diagnostics: cycles summed over all warps of the last point-kernel launch, spent in (geometry, series,
  * exp + weights, accumulation, whole warp).  All zeros unless the library was built with
  * -DDSE_PHASE_TIMING (the default build carries no instrumentation).  Synchronous. */

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
 EXPORTS = [
     "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_lu_solve",
     "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count", "dse_kernel_info",
-    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
+    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_gauss_legendre", "dse_schwinger", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
@@ -64,6 +64,8 @@ def load_library():
     L.dse_set_timing.argtypes = [vp, C.c_int32]
     L.dse_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.dse_get_phase_cycles.argtypes = [vp, C.POINTER(C.c_double * 5)]
+    L.dse_gauss_legendre.argtypes = [C.c_int32, dp, dp, dp, vp]
+    L.dse_schwinger.argtypes = [vp, dp, C.c_int32, C.c_double, C.c_double, dp, C.c_int32, dp, dp, vp]
     L.dse_dfma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
     L.dse_dmma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
     L.dse_strerror.argtypes = [C.c_int]
@@ -160,6 +162,17 @@ class Dse:
                                      _dev_ptr(stats), _stream_ptr(stream)))
         return x, stats
 
+    def schwinger(self, c, t, n_nodes, p2_min, p2_max, stream=None):
+        """Delta(t) of eq.(20) for every system: returns a [n_batch, len(t)] tensor."""
+        import torch
+        out = torch.empty((self.B, t.numel()), dtype=torch.float64, device=c.device)
+        work = torch.empty((5 + self.B) * n_nodes + 4, dtype=torch.float64, device=c.device)
+        _check(self.lib.dse_schwinger(self._h, _dev_ptr(c, self.B * 2 * self.N), int(n_nodes), float(p2_min),
+                                      float(p2_max), _dev_ptr(t), int(t.numel()), _dev_ptr(out), _dev_ptr(work),
+                                      _stream_ptr(stream)))
+        self._keep = work            # the call is asynchronous: keep the workspace alive until the next call
+        return out
+
     def jacobian_host(self, c_host: np.ndarray, bc_host: np.ndarray, J_host: np.ndarray, F_host: np.ndarray):
         """Host buffers in, host buffers out (numpy float64, C-contiguous; pinned memory recommended)."""
         for a in (c_host, bc_host, F_host) + ((J_host,) if J_host is not None else ()):
@@ -208,3 +221,15 @@ def dfma_probe(blocks, iters, sink, stream=None):
 def dmma_probe(blocks, iters, sink, stream=None):
     _check(load_library().dse_dmma_probe(blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
     return blocks * 8 * 4 * iters * 512
+
+
+def gauss_legendre(n, device="cuda", stream=None):
+    """n-point Gauss-Legendre rule generated on the device: (x[n] ascending, w[n])."""
+    import torch
+    x = torch.empty(n, dtype=torch.float64, device=device)
+    w = torch.empty(n, dtype=torch.float64, device=device)
+    work = torch.empty(2 * (n + 2), dtype=torch.float64, device=device)
+    _check(load_library().dse_gauss_legendre(int(n), _dev_ptr(x), _dev_ptr(w), _dev_ptr(work), _stream_ptr(stream)))
+    import torch.cuda
+    torch.cuda.current_stream().synchronize()
+    return x, w

@@ -326,6 +326,24 @@ int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches)
     return DSE_OK;
 }
 
+int dse_gauss_legendre(int32_t n, double *x_dev, double *w_dev, double *work_dev, void *stream)
+{
+    if (n < 2 || n > (1 << 24) || !x_dev || !w_dev || !work_dev) return DSE_EINVAL;
+    int rc = dse::launch_gauss_legendre(n, x_dev, w_dev, work_dev, stream);
+    return rc < 0 ? rc : DSE_OK;
+}
+
+int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, double p2_min, double p2_max, const double *t_dev,
+                  int32_t n_t, double *delta_dev, double *work_dev, void *stream)
+{
+    if (!h || !c_dev || !t_dev || !delta_dev || !work_dev || n_nodes < 2 || n_nodes > (1 << 24) || n_t < 1) return DSE_EINVAL;
+    if (!finite_pos(p2_min) || !finite_pos(p2_max) || !(p2_min < p2_max)) return DSE_EINVAL;
+    int rc = dse::launch_schwinger(h->k, c_dev, n_nodes, p2_min, p2_max, t_dev, n_t, delta_dev, work_dev, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    return DSE_OK;
+}
+
 int dse_get_phase_cycles(dse_handle *h, double out_host[5])
 {
     if (!h || !out_host) return DSE_EINVAL;

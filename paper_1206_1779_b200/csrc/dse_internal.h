@@ -70,6 +70,9 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg);
 bool acquire_const_slot(const KParams &k);
 void release_const_slot();
 size_t lu_scratch_doubles(int n);
+int launch_gauss_legendre(int n, double *x, double *w, double *work, void *stream);
+int launch_schwinger(const KParams &k, const double *c, int n, double p2_min, double p2_max, const double *t, int n_t,
+                     double *out, double *work, void *stream);
 int launch_dfma_probe(int blocks, int iters, double *sink, void *stream);
 int launch_dmma_probe(int blocks, int iters, double *sink, void *stream);
 

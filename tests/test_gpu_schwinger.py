@@ -1,0 +1,75 @@
+"""NEXT f4: device-generated Gauss-Legendre rule and the Schwinger function eq.(20) against the oracle."""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from test_gpu_parity import oracle_params, _torch   # noqa: E402
+from test_oracle_path import _massive_propagator_coefficients   # noqa: E402
+
+
+@pytest.mark.parametrize("n", [2, 3, 64, 257, 4096])
+def test_device_gauss_legendre_matches_oracle(orc, n):
+    _torch()
+    from paper_1206_1779_b200.binding import gauss_legendre
+    x, w = gauss_legendre(n)
+    x = x.cpu().numpy(); w = w.cpu().numpy()
+    xo, wo = orc.gauss_legendre(n)
+    assert np.allclose(x, xo, rtol=0, atol=2e-15)
+    assert np.allclose(w, wo, rtol=2e-11, atol=0)
+    assert abs(w.sum() - 2.0) < 1e-13
+
+
+def test_device_gauss_legendre_full_size_sampled(orc):
+    """The paper's 2^17-node rule (fn.13): properties at full size + sampled nodes the oracle computes one by one."""
+    _torch()
+    from paper_1206_1779_b200.binding import gauss_legendre
+    n = 1 << 17
+    x, w = gauss_legendre(n)
+    x = x.cpu().numpy(); w = w.cpu().numpy()
+    assert np.all(np.diff(x) > 0) and np.array_equal(x, -x[::-1]) and np.array_equal(w, w[::-1])
+    assert abs(w.sum() - 2.0) < 1e-12
+    assert abs(np.sum(w * x ** 2) - 2.0 / 3.0) < 1e-12 and abs(np.sum(w * x ** 40) - 2.0 / 41.0) < 1e-12
+    for i in (0, 1, 777, 40000, n // 2 - 1, n // 2, n - 2):
+        xo, wo = orc.gl_node(n, i)
+        # the recurrence at n = 2^17 carries ~n*eps of rounding in P_n': edge weights agree to ~1e-9 only (both sides)
+        assert abs(x[i] - xo) < 5e-15 and abs(w[i] - wo) <= 2e-8 * wo
+
+
+def test_schwinger_matches_oracle_and_closed_form(orc):
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse
+    from paper_1206_1779_b200.binding import DseParams
+    N, eps2, L2 = 64, 1e-6, 1e4
+    p, c = _massive_propagator_coefficients(orc, N, eps2, L2)
+    prm = DseParams(N, 8, 8, 1, eps2, L2, 1.0, 3.0, 1.0, 1.0, -9.0 / 44.0, 0.0, 1.0, 0.0, 0, 0)
+    d = Dse(prm)
+    t = np.linspace(0.1, 8.0, 37)
+    n_nodes = 3000                                           # ragged: not a multiple of the block size
+    out = d.schwinger(torch.from_numpy(c[None, :]).cuda(), torch.from_numpy(t).cuda(), n_nodes, 1e-16, L2)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()[0]
+    ref = orc.schwinger(p, c, n_nodes, 1e-16, L2, t)
+    assert np.allclose(out, ref, rtol=1e-10, atol=1e-13)
+    big = t >= 0.5                                          # cutoff tail ~ sin(t p_max)/(pi t p_max^2) <= 6.4e-5 there
+    assert np.allclose(out[big], np.exp(-t[big]) / 2, rtol=0, atol=7e-5)      # sigma = 1/(p^2+1): exp(-t)/2
+    d.close()
+
+
+def test_schwinger_batched_random_dressings(orc):
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    w = Workload("schw", 24, 8, 8, 1e-6, 5e4, n_batch=3)
+    c = np.stack([draw_coefficients(70 + b, 24) for b in range(3)])
+    d = Dse(params_from_workload(w))
+    t = np.array([0.0, 0.3, 1.7, 5.0, 12.0])
+    out = d.schwinger(torch.from_numpy(c).cuda(), torch.from_numpy(t).cuda(), 2048, 1e-10, 2e5)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    for b in range(3):
+        ref = orc.schwinger(oracle_params(w), c[b], 2048, 1e-10, 2e5, t)
+        assert np.allclose(out[b], ref, rtol=1e-10, atol=1e-12 * np.abs(ref).max())
+    d.close()

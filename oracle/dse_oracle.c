@@ -74,6 +74,8 @@ typedef struct orc_params {
     double ir_exp_G;   /* exponent of G below eps2, eq.(17): -kappa                             */
     double ir_exp_Z;   /* exponent of Z below eps2, eq.(16): 2 kappa                            */
     double uv_omega;   /* omega of eq.(18),(19) L121-131; 0 => constant continuation above L2   */
+    int32_t n_ir;      /* NEXT f2: nodes of the infrared piece int_0^{eps2} dy of eq.(26); 0 = none */
+    int32_t pad2_;
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -266,12 +268,27 @@ void orc_tables(const orc_params *p, double *x_ext, double *s_root, double *t_r,
 {
     const int N = p->n_cheb, Nr = p->n_r, Nt = p->n_theta;
     real Lg = lg_of(p);
-    double *w = (double *)malloc(sizeof(double) * (size_t)(Nr > Nt ? Nr : Nt));
-    orc_gauss_legendre(Nr, t_r, w);
+    const int Nir = p->n_ir;
+    int wmax = Nr > Nt ? Nr : Nt;
+    if (Nir > wmax) wmax = Nir;
+    double *w = (double *)malloc(sizeof(double) * (size_t)wmax);
+    /* infrared piece int_0^{eps2} dy of eq.(26) L190 (the paper gives no node map: reading A23): Gauss-Legendre
+     * in v on (-1,1) with y = eps2 ((1+v)/2)^4, dy = 2 eps2 ((1+v)/2)^3 dv; the dressings there are the power laws
+     * eq.(16),(17).  These Nir nodes come first (ascending y); their mapped argument is the clamped s = -1. */
+    if (Nir > 0) {
+        orc_gauss_legendre(Nir, t_r, w);
+        for (int q = 0; q < Nir; ++q) {
+            real h = ((real)t_r[q] + 1) / 2;
+            y[q] = (double)((real)p->eps2 * h * h * h * h);
+            Wy[q] = (double)((real)w[q] * 2 * (real)p->eps2 * h * h * h);
+            t_r[q] = -1.0;
+        }
+    }
+    orc_gauss_legendre(Nr, t_r + Nir, w);
     for (int q = 0; q < Nr; ++q) {
-        real yy = (real)p->eps2 * R_EXP(((real)t_r[q] + 1) * Lg / 2);
-        y[q] = (double)yy;
-        Wy[q] = (double)((real)w[q] * (Lg / 2) * yy);
+        real yy = (real)p->eps2 * R_EXP(((real)t_r[Nir + q] + 1) * Lg / 2);
+        y[Nir + q] = (double)yy;
+        Wy[Nir + q] = (double)((real)w[q] * (Lg / 2) * yy);
     }
     double *tau = (double *)malloc(sizeof(double) * (size_t)Nt);
     if (p->angular_rule == 0) {
@@ -344,8 +361,10 @@ static void self_energy(const orc_params *p, const real *c, real x, int ny, cons
             real Q = kernel_Q_real(x, y, th);
             real M = kernel_M_real(x, y, th);
             real v = -C * W * y * Om * s2 * s2 / (z * z) * R_EXP(lnGy + lnZz);
-            real wQ = C / (3 * x) * W * Om * s2 * Q * R_EXP(lnPy + lnPz);
-            real wM = C / (3 * x) * W * Om * s2 * M * R_EXP(lnGy + lnGz);
+            /* at the ghost subtraction point x_G = 0 (L135) only eq.(8) is evaluated: gluon prefactor 1/(3x) -> 0 */
+            const real c3x = (x > 0) ? C / (3 * x) : 0;
+            real wQ = c3x * W * Om * s2 * Q * R_EXP(lnPy + lnPz);
+            real wM = c3x * W * Om * s2 * M * R_EXP(lnGy + lnGz);
             sG += v; sQ += wQ; sM += wM;
             if (dG_da) {
                 for (int j = 0; j < N; ++j) {
@@ -385,7 +404,7 @@ void orc_self_energy(const orc_params *p, const double *c, double x, int ny, con
 /* J may be NULL (residual only).  Returns 0.                                                   */
 int orc_residual_jacobian(const orc_params *p, const double *c, double gG, double gZ, double *F, double *J)
 {
-    const int N = p->n_cheb, Nr = p->n_r, Nt = p->n_theta;
+    const int N = p->n_cheb, Nr = p->n_r + p->n_ir, Nt = p->n_theta;
     const int Ne = orc_n_ext(p);
     const int iZ = N, iG = (p->x_G == p->x_Z) ? N : N + 1;
     double *x_ext = (double *)malloc(sizeof(double) * (size_t)(Ne + N + 3 * Nr + 2 * Nt));

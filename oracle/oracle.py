@@ -22,16 +22,17 @@ class OrcParams(C.Structure):
         ("eps2", C.c_double), ("L2", C.c_double), ("alpha_mu", C.c_double), ("n_colors", C.c_double),
         ("x_G", C.c_double), ("x_Z", C.c_double), ("delta", C.c_double),
         ("ir_exp_G", C.c_double), ("ir_exp_Z", C.c_double), ("uv_omega", C.c_double),
+        ("n_ir", C.c_int32), ("pad2_", C.c_int32),
     ]
 
 
 def make_params(n_cheb, n_r, n_theta, eps2, L2, x_G, x_Z, alpha_mu=1.0, n_colors=3.0, delta=-9.0 / 44.0,
-                ir_exp_G=-0.595353, ir_exp_Z=2 * 0.595353, uv_omega=None, angular_rule=0):
+                ir_exp_G=-0.595353, ir_exp_Z=2 * 0.595353, uv_omega=None, angular_rule=0, n_ir=0):
     if uv_omega is None:
         uv_omega = 11.0 * n_colors * alpha_mu / (12.0 * np.pi)
     return OrcParams(int(n_cheb), int(n_r), int(n_theta), int(angular_rule), float(eps2), float(L2), float(alpha_mu),
                      float(n_colors), float(x_G), float(x_Z), float(delta), float(ir_exp_G), float(ir_exp_Z),
-                     float(uv_omega))
+                     float(uv_omega), int(n_ir), 0)
 
 
 def _ptr(a):
@@ -95,8 +96,9 @@ class Oracle:
 
     def tables(self, p):
         ne = self.lib.orc_n_ext(C.byref(p))
-        out = dict(x_ext=np.empty(ne), s_root=np.empty(p.n_cheb), t_r=np.empty(p.n_r), y=np.empty(p.n_r),
-                   Wy=np.empty(p.n_r), theta=np.empty(p.n_theta), Omega=np.empty(p.n_theta))
+        nr = p.n_r + p.n_ir
+        out = dict(x_ext=np.empty(ne), s_root=np.empty(p.n_cheb), t_r=np.empty(nr), y=np.empty(nr),
+                   Wy=np.empty(nr), theta=np.empty(p.n_theta), Omega=np.empty(p.n_theta))
         self.lib.orc_tables(C.byref(p), *[_ptr(out[k]) for k in ("x_ext", "s_root", "t_r", "y", "Wy", "theta", "Omega")])
         return out
 

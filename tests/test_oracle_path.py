@@ -310,3 +310,78 @@ def test_gl_single_node_matches_full_rule(orc):
     assert abs(a + b) < 1e-15 and abs(wa - wb) < 1e-18
     a2, _ = orc.gl_node(n, 1001)
     assert abs((math.acos(a) - math.acos(a2)) - PI / (n + 0.5)) < 1e-9
+
+
+# ------------------------------------------------------------------------------------ P9: the paper's own numbers
+def test_paper_scaling_solution_P9(orc):
+    """with eps2 = 1e-6, L2 = 5e4, x_G = 0, 1/G(0) = 0, x_Z = L2, Z(x_Z) = 0.256, alpha(mu^2) = 1 the
+    converged solution has alpha(M_Z^2) = 0.118 (M_Z = 91.2 GeV, fn.7), the infrared fixed point alpha(0) = 2.972 =
+    8.915/N_c (L151), the power laws G ~ x^-kappa, Z ~ x^(2 kappa) (eq.(16),(17)), and the gluon Schwinger function
+    has a zero slightly below t = 5 GeV^-1 (L165).  The whole oracle path (tables incl. the infrared piece of eq.(26),
+    kernels, continuation, residual, analytic Jacobian, equilibrated LU, damped Newton) is needed to get there."""
+    import scaling_setup as S
+    gold = {}
+    import os
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")):
+        f = line.split("#")[0].split()
+        if len(f) == 2:
+            gold[f[0]] = float(f[1])
+    p = make_params(S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, 0.0, S.L2, n_ir=S.N_IR)
+    c = S.start_coefficients(orc, p)
+    dn = []
+    for it in range(30):
+        F, J = orc.residual_jacobian(p, c, S.G_G, S.G_Z)
+        d, st, rc = orc.lu_solve(J, F)
+        assert rc == 0
+        c = c - S.damping(st[0]) * d
+        dn.append(st[0])
+        if st[0] < 1e-11:
+            break
+    assert dn[-1] < 1e-11 and len(dn) <= 15
+    assert dn[-2] < 1e-5 and dn[-1] < 100 * dn[-2] ** 2 + 1e-12       # quadratic at the end (L226)
+
+    def alpha(x):
+        g, z = orc.ln_dress(p, c, x)
+        return math.exp(2 * g + z)                                     # alpha(x) = alpha(mu^2) G^2 Z, L145
+
+    assert abs(alpha(gold["M_Z_GeV"] ** 2) - gold["alpha_MZ"]) < 1e-3   # printed 0.118
+    assert abs(alpha(S.EPS2) - gold["alpha0_Nc3"]) < 5e-3               # printed 2.972
+    h = 1.02
+    for x in (3e-6, 1e-5):
+        sG = (orc.ln_dress(p, c, x * h)[0] - orc.ln_dress(p, c, x / h)[0]) / (2 * math.log(h))
+        sZ = (orc.ln_dress(p, c, x * h)[1] - orc.ln_dress(p, c, x / h)[1]) / (2 * math.log(h))
+        assert abs(sG + gold["kappa"]) < 2e-3 and abs(sZ - 2 * gold["kappa"]) < 2e-3
+    lnG, lnZ = orc.ln_dress(p, c, S.L2)
+    assert abs(math.exp(lnZ) - 0.256) < 1e-4                            # renormalisation condition, up to the N = 36 collocation error
+    t = np.linspace(0.5, 8.0, 76)
+    dlt = orc.schwinger(p, c, 4096, 1e-14, S.L2, t)
+    zeros = [0.5 * (t[i] + t[i + 1]) for i in range(len(t) - 1) if dlt[i] * dlt[i + 1] < 0]
+    assert dlt[0] > 0 and len(zeros) >= 1 and 3.0 < zeros[0] < gold["schwinger_zero_t_upper"]
+
+
+def test_infrared_piece_closed_form(orc):
+    """eq.(26) L190 with the [0, eps2] piece: for G = Z = 1 everywhere the y < x part of the ghost loop becomes
+    int_0^x dy y/x^2 = 1/2, so Pi_G^0(x) = -C (3 pi/8) [1/2 + ln(L2/x)] (x > eps2)."""
+    eps2, L2, x = 1e-3, 1e3, 2.0
+    p = make_params(4, 400, 200, eps2, L2, 1.0, 1.0, ir_exp_G=0.0, ir_exp_Z=0.0, uv_omega=0.0, n_ir=24)
+    tab = orc.tables(p)
+    assert len(tab["y"]) == 424 and np.all(np.diff(tab["y"]) > 0) and tab["y"][23] < eps2 < tab["y"][24]
+    assert abs(np.sum(tab["Wy"][:24]) - eps2) < 1e-15                     # int_0^eps2 dy
+    assert abs(np.sum(tab["Wy"][:24] * tab["y"][:24] ** 0.4) - eps2 ** 1.4 / 1.4) < 1e-12 * eps2 ** 1.4
+    # split the main rule at y = x for spectral convergence (test-only rule), keep the oracle's infrared nodes
+    t, w = orc.gauss_legendre(200)
+    ys, Ws = [tab["y"][:24]], [tab["Wy"][:24]]
+    for lo, hi in ((eps2, x), (x, L2)):
+        L = math.log(hi / lo)
+        yy = lo * np.exp((t + 1) * L / 2)
+        ys.append(yy); Ws.append(w * L / 2 * yy)
+    out = orc.self_energy(p, np.zeros(8), x, np.concatenate(ys), np.concatenate(Ws), tab["theta"], tab["Omega"])
+    C = orc.coupling_C(p)
+    assert abs(out[0] + C * (3 * PI / 8) * (0.5 + math.log(L2 / x))) < 2e-8
+    # x_G = 0: the ghost self-energy at zero momentum, int dy y (3 pi/8)/y^2 = (3 pi/8) [ln(L2/eps2) + int_0^eps2 dy/y]:
+    # with flat dressings the infrared piece diverges logarithmically, so check the main piece only
+    p0 = make_params(4, 64, 16, eps2, L2, 0.0, 1.0, ir_exp_G=0.0, ir_exp_Z=0.0, uv_omega=0.0)
+    tab0 = orc.tables(p0)
+    assert tab0["x_ext"][5] == 0.0
+    o0 = orc.self_energy(p0, np.zeros(8), 0.0, tab0["y"], tab0["Wy"], tab0["theta"], tab0["Omega"])
+    assert abs(o0[0] + C * (3 * PI / 8) * math.log(L2 / eps2)) < 1e-12 and o0[1] == 0.0 and o0[2] == 0.0

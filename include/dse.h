@@ -65,13 +65,15 @@ typedef struct dse_params {
     double eps2, L2;    /* IR matching point and UV cutoff, 0 < eps2 < L2 (L188)                         */
     double alpha_mu;    /* alpha(mu^2) = g^2/4pi (L131,L135); C = 4 pi alpha N_c/(2 pi)^3                */
     double n_colors;    /* N_c                                                                           */
-    double x_G, x_Z;    /* MOM subtraction points, > 0 (eq.(14),(15)); x_G = 0 is not supported yet      */
+    double x_G, x_Z;    /* MOM subtraction points (eq.(14),(15)); x_Z > 0; x_G >= 0, x_G = 0 (the paper's choice,
+                           L135) needs x_G != x_Z: at x = 0 only the ghost equation is evaluated             */
     double delta;       /* ghost anomalous dimension -9/44 (L58); gamma = -1 - 2 delta (L131)            */
     double ir_exp_G;    /* exponent of G below eps2, eq.(17): -kappa                                     */
     double ir_exp_Z;    /* exponent of Z below eps2, eq.(16): 2 kappa                                    */
     double uv_omega;    /* omega of eq.(18),(19); 0 => constant continuation above L2                    */
     int32_t flags;      /* DSE_FLAG_* bits                                                               */
-    int32_t reserved;   /* must be 0                                                                     */
+    int32_t n_r_ir;     /* >= 0: Gauss-Legendre nodes of the infrared piece int_0^{eps2} dy of eq.(26),
+                           y = eps2 ((1+v)/2)^4 (reading A23); 0 = no infrared piece (BASELINE configs) */
 } dse_params;
 
 #define DSE_FLAG_GEOMETRY_CACHE 1 /* precompute the coefficient-independent per-point factors once in
@@ -120,7 +122,7 @@ DSE_API int dse_jacobian_host(dse_handle *h, const double *c_host, const double 
 /* Sizes: n_ext = number of external points (N roots, then x_Z, then x_G if different). */
 DSE_API int dse_n_ext(const dse_handle *h);
 
-/* Copies the tables to host arrays (any pointer may be NULL): x_ext[n_ext], y[n_r], Wy[n_r]
+/* Copies the tables to host arrays (any pointer may be NULL): x_ext[n_ext], y[n_r_ir + n_r] (infrared piece first), Wy[n_r_ir + n_r]
  * (= w_q (Lg/2) y_q), theta[n_theta], Omega[n_theta] (= w_k pi/2).  For tests. */
 DSE_API int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, double *Wy_host,
                    double *theta_host, double *Omega_host);

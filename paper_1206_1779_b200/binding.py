@@ -28,7 +28,7 @@ class DseParams(C.Structure):
         ("eps2", C.c_double), ("L2", C.c_double), ("alpha_mu", C.c_double), ("n_colors", C.c_double),
         ("x_G", C.c_double), ("x_Z", C.c_double), ("delta", C.c_double),
         ("ir_exp_G", C.c_double), ("ir_exp_Z", C.c_double), ("uv_omega", C.c_double),
-        ("flags", C.c_int32), ("reserved", C.c_int32),
+        ("flags", C.c_int32), ("n_r_ir", C.c_int32),
     ]
 
 
@@ -85,7 +85,7 @@ def params_from_workload(w, n_batch=None, flags=0):
     if getattr(w, "angular_rule", 0) == 1:
         flags |= DSE_FLAG_ANGULAR_TANH_SINH
     return DseParams(w.n_cheb, w.n_r, w.n_theta, w.n_batch if n_batch is None else n_batch, w.eps2, w.L2,
-                     w.alpha_mu, w.n_colors, w.x_G, w.x_Z, w.delta, w.ir_exp_G, w.ir_exp_Z, w.uv_omega, flags, 0)
+                     w.alpha_mu, w.n_colors, w.x_G, w.x_Z, w.delta, w.ir_exp_G, w.ir_exp_Z, w.uv_omega, flags, getattr(w, "n_ir", 0))
 
 
 def _stream_ptr(stream=None):
@@ -184,7 +184,8 @@ class Dse:
     # ---- introspection ----------------------------------------------------------------------------
     def tables(self):
         p = self.params
-        out = dict(x_ext=np.empty(self.n_ext), y=np.empty(p.n_r), Wy=np.empty(p.n_r), theta=np.empty(p.n_theta),
+        nr = p.n_r + p.n_r_ir
+        out = dict(x_ext=np.empty(self.n_ext), y=np.empty(nr), Wy=np.empty(nr), theta=np.empty(p.n_theta),
                    Omega=np.empty(p.n_theta))
         _check(self.lib.dse_get_tables(self._h, *[C.c_void_p(out[k].ctypes.data)
                                                   for k in ("x_ext", "y", "Wy", "theta", "Omega")]))

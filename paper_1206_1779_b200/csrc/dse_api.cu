@@ -62,10 +62,10 @@ int validate(const dse_params *p)
     if (p->n_r > (1 << 20) || p->n_theta > (1 << 16) || p->n_batch > (1 << 20)) return DSE_EINVAL;
     if (!finite_pos(p->eps2) || !finite_pos(p->L2) || !(p->eps2 < p->L2)) return DSE_EINVAL;
     if (!finite_pos(p->alpha_mu) || !finite_pos(p->n_colors)) return DSE_EINVAL;
-    if (!finite_pos(p->x_G) || !finite_pos(p->x_Z)) return DSE_EINVAL;
+    if (!finite_pos(p->x_Z) || !std::isfinite(p->x_G) || p->x_G < 0.0 || (p->x_G == 0.0 && p->x_Z == 0.0)) return DSE_EINVAL;
     if (!std::isfinite(p->delta) || !std::isfinite(p->ir_exp_G) || !std::isfinite(p->ir_exp_Z)) return DSE_EINVAL;
     if (!std::isfinite(p->uv_omega) || p->uv_omega < 0.0) return DSE_EINVAL;
-    if (p->reserved != 0 || (p->flags & ~(DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_ANGULAR_TANH_SINH))) return DSE_EINVAL;
+    if (p->n_r_ir < 0 || p->n_r_ir > (1 << 20) || (p->flags & ~(DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_ANGULAR_TANH_SINH))) return DSE_EINVAL;
     return DSE_OK;
 }
 
@@ -164,6 +164,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     size_t off = 0;
     const size_t o_x = carve<double>(off, T.Next), o_sx = carve<double>(off, T.Next), o_c3 = carve<double>(off, T.Next);
     const size_t o_y = carve<double>(off, T.Nr), o_sy = carve<double>(off, T.Nr), o_W = carve<double>(off, T.Nr);
+    const size_t o_EG = carve<double>(off, T.Nr), o_EZ = carve<double>(off, T.Nr);
     const size_t o_ang = carve<double>(off, T.ang.size());
     const size_t o_py = carve<double>(off, T.phi_y.size()), o_px = carve<double>(off, T.phi_x.size());
     std::vector<double> host(off, 0.0);
@@ -173,6 +174,8 @@ int dse_create(const dse_params *params, dse_handle **out)
     memcpy(&host[o_y], T.y.data(), 8 * T.y.size());
     memcpy(&host[o_sy], T.sy.data(), 8 * T.sy.size());
     memcpy(&host[o_W], T.Wy.data(), 8 * T.Wy.size());
+    memcpy(&host[o_EG], T.EGy.data(), 8 * T.EGy.size());
+    memcpy(&host[o_EZ], T.EZy.data(), 8 * T.EZy.size());
     memcpy(&host[o_ang], T.ang.data(), 8 * T.ang.size());
     memcpy(&host[o_py], T.phi_y.data(), 8 * T.phi_y.size());
     memcpy(&host[o_px], T.phi_x.data(), 8 * T.phi_x.size());
@@ -181,7 +184,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemcpy(tables)"); }
     double *t = h->d_tables;
     k.x_ext = t + o_x; k.sx_ext = t + o_sx; k.c3x_ext = t + o_c3;
-    k.y = t + o_y; k.sy = t + o_sy; k.Wy = t + o_W; k.ang = t + o_ang; k.phi_y = t + o_py; k.phi_x = t + o_px;
+    k.y = t + o_y; k.sy = t + o_sy; k.Wy = t + o_W; k.EGy = t + o_EG; k.EZy = t + o_EZ; k.ang = t + o_ang; k.phi_y = t + o_py; k.phi_x = t + o_px;
 
     // ---- geometry cache (optional) ----
     if (params->flags & DSE_FLAG_GEOMETRY_CACHE) {

@@ -17,7 +17,8 @@ struct HostTables {
     int iZ = 0, iG = 0;                       // external-point index of x_Z, x_G
     double Lg = 0, C = 0;
     std::vector<double> x_ext, sx_ext, c3x_ext;   // x, sqrt x, C/(3x)
-    std::vector<double> y, sy, Wy, t_r;           // radial nodes, sqrt, W_q = w_q (Lg/2) y_q, s(y_q)
+    std::vector<double> y, sy, Wy, t_r;           // radial nodes (infrared piece first), sqrt, dy weight, s(y_q)
+    std::vector<double> EGy, EZy;                 // continuation add-ons of ln G(y_q), ln Z(y_q) (0 inside [eps2, L2])
     std::vector<double> theta, Omega;             // angular nodes/weights (unpadded)
     std::vector<double> ang;                      // [Ntpad][6]: sh2, 6c, 2+c^2, -2 s2, Om s2, Om s2^2
     std::vector<double> phi_y;                    // [Nr][Npad]   phi_j(t_q)   (phi_0 = 1/2)
@@ -37,7 +38,7 @@ struct KParams {
     int want_jac;                      // 0: residual only (skip phase 2)
     int use_constc;                    // coefficient pairs are read as constant-bank operands (single system, slot owner)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
-    const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x;
+    const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x, *EGy, *EZy;
     const double *geom;                // geometry cache [Next*Nr*Ntpad][4] or nullptr
     // per-build workspace
     double *coefP;                     // [B][Npad][2]  (a_j, b_j), j = 0 pre-halved, zero padded

@@ -50,6 +50,7 @@ __global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double
     }
     if (lane == 0) {
         if (isy) {
+            lnG += P.EGy[item]; lnZ += P.EZy[item];          // power-law continuation below eps2 (infrared piece)
             P.Gy[(size_t)b * P.Nr + item] = exp(lnG);
             P.Py[(size_t)b * P.Nr + item] = exp(P.e1 * lnG + P.e2 * lnZ);
         } else {

@@ -75,7 +75,7 @@ inline void phi_row(int N, int Npad, ld s, double *out)
 
 void build_tables(const dse_params &p, HostTables &T)
 {
-    const int N = p.n_cheb, Nr = p.n_r, Nt = p.n_theta;
+    const int N = p.n_cheb, Nir = p.n_r_ir, Nmain = p.n_r, Nr = Nmain + Nir, Nt = p.n_theta;
     T.N = N;
     T.Npad = ((N + CJ - 1) / CJ) * CJ;
     T.Nr = Nr;
@@ -93,17 +93,34 @@ void build_tables(const dse_params &p, HostTables &T)
     T.C = (double)C;
 
     std::vector<ld> t, w;
-    // radial rule in s; y = eps2 exp((s+1) Lg/2), dy = (Lg/2) y ds
-    gauss_legendre(Nr, t, w);
     T.y.resize(Nr); T.sy.resize(Nr); T.Wy.resize(Nr); T.t_r.resize(Nr);
+    T.EGy.assign(Nr, 0.0); T.EZy.assign(Nr, 0.0);
     T.phi_y.assign((size_t)Nr * T.Npad, 0.0);
-    for (int q = 0; q < Nr; ++q) {
+    // infrared piece int_0^{eps2} dy of eq.(26): GL in v, y = eps2 ((1+v)/2)^4, dy = 2 eps2 ((1+v)/2)^3 dv; the
+    // dressings there are the power laws eq.(16),(17): ln G(y) = series(s = -1) + p_G ln(y/eps2)
+    if (Nir > 0) {
+        gauss_legendre(Nir, t, w);
+        for (int q = 0; q < Nir; ++q) {
+            const ld hq = (t[q] + 1) / 2;
+            T.y[q] = (double)((ld)p.eps2 * hq * hq * hq * hq);
+            T.sy[q] = (double)sqrtl((ld)T.y[q]);
+            T.Wy[q] = (double)(w[q] * 2 * (ld)p.eps2 * hq * hq * hq);
+            T.t_r[q] = -1.0;
+            const ld ell = logl((ld)T.y[q] / (ld)p.eps2);
+            T.EGy[q] = (double)((ld)p.ir_exp_G * ell);
+            T.EZy[q] = (double)((ld)p.ir_exp_Z * ell);
+            phi_row(N, T.Npad, -1.0L, &T.phi_y[(size_t)q * T.Npad]);
+        }
+    }
+    // main radial rule in s; y = eps2 exp((s+1) Lg/2), dy = (Lg/2) y ds
+    gauss_legendre(Nmain, t, w);
+    for (int q = 0; q < Nmain; ++q) {
         ld yy = (ld)p.eps2 * expl((t[q] + 1) * Lg / 2);
-        T.y[q] = (double)yy;
-        T.sy[q] = (double)sqrtl((ld)T.y[q]);          // sqrt of the rounded table value
-        T.Wy[q] = (double)(w[q] * (Lg / 2) * yy);
-        T.t_r[q] = (double)t[q];
-        phi_row(N, T.Npad, t[q], &T.phi_y[(size_t)q * T.Npad]);
+        T.y[Nir + q] = (double)yy;
+        T.sy[Nir + q] = (double)sqrtl((ld)T.y[Nir + q]);          // sqrt of the rounded table value
+        T.Wy[Nir + q] = (double)(w[q] * (Lg / 2) * yy);
+        T.t_r[Nir + q] = (double)t[q];
+        phi_row(N, T.Npad, t[q], &T.phi_y[(size_t)(Nir + q) * T.Npad]);
     }
     // angular rule: Gauss-Legendre in theta, or tanh-sinh in xi = cos(theta) (eq.(5))
     T.theta.resize(Nt); T.Omega.resize(Nt);
@@ -162,7 +179,8 @@ void build_tables(const dse_params &p, HostTables &T)
     if (!same) T.x_ext[T.iG] = p.x_G;
     for (int e = 0; e < T.Next; ++e) {
         T.sx_ext[e] = (double)sqrtl((ld)T.x_ext[e]);
-        T.c3x_ext[e] = (double)(C / (3 * (ld)T.x_ext[e]));
+        // at x = 0 (x_G = 0, L135) only the ghost equation is evaluated: the gluon prefactor C/(3x) is dropped
+        T.c3x_ext[e] = T.x_ext[e] > 0.0 ? (double)(C / (3 * (ld)T.x_ext[e])) : 0.0;
     }
 }
 

@@ -47,7 +47,10 @@ def test_error_paths_without_gpu(lib):
     bad.eps2 = 2e10
     assert lib.dse_create(ctypes.byref(bad), ctypes.byref(h)) == -1
     bad = params_from_workload(CONFIGS[0])
-    bad.x_G = 0.0
+    bad.x_G = -1.0
+    assert lib.dse_create(ctypes.byref(bad), ctypes.byref(h)) == -1
+    bad = params_from_workload(CONFIGS[0])
+    bad.n_r_ir = -3
     assert lib.dse_create(ctypes.byref(bad), ctypes.byref(h)) == -1
     assert lib.dse_destroy(None) == 0
     assert lib.dse_jacobian(None, None, None, None, None, None) == -1

@@ -83,6 +83,10 @@ typedef struct dse_params {
                                         equidistant abscissae t_k in [-3,3], xi_k = tanh((pi/2) sinh t_k), instead of
                                         Gauss-Legendre in theta (reading A9b)                              */
 
+#define DSE_FLAG_RADIAL_SPLIT 4 /* the paper's radial split int_{eps2}^{x} + int_{x}^{L2} (eq.(26)) with n_r nodes in
+                                   EACH interval (L364): the radial rule then depends on the external point
+                                   (n_r_ir + 2 n_r nodes per point); default: one rule on [eps2, L2] (BASELINE configs) */
+
 typedef struct dse_handle dse_handle; /* opaque; owned by the library */
 
 /* Builds the quadrature/collocation tables (Gauss-Legendre in ln y and in theta, Chebyshev roots

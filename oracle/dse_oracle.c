@@ -75,7 +75,8 @@ typedef struct orc_params {
     double ir_exp_Z;   /* exponent of Z below eps2, eq.(16): 2 kappa                            */
     double uv_omega;   /* omega of eq.(18),(19) L121-131; 0 => constant continuation above L2   */
     int32_t n_ir;      /* NEXT f2: nodes of the infrared piece int_0^{eps2} dy of eq.(26); 0 = none */
-    int32_t pad2_;
+    int32_t radial_split; /* NEXT f1: 1 = the paper's split int_{eps2}^{x} + int_{x}^{L2} (eq.(26)) with n_r
+                             nodes in EACH interval (L364), so the radial rule depends on the external point */
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -325,6 +326,39 @@ void orc_tables(const orc_params *p, double *x_ext, double *s_root, double *t_r,
     free(w);
 }
 
+/* NEXT f1. Radial rule of external point x with the split of eq.(26): the n_ir infrared nodes of orc_tables,
+ * then n_r Gauss-Legendre nodes in ln y on [eps2, xm] and n_r on [xm, L2], xm = min(max(x, eps2), L2) (L364: "32/64/128
+ * Gauss-Legendre nodes within each of the three integration intervals").  An empty interval (x <= eps2 or x >= L2)
+ * contributes nodes of zero weight.  y, Wy: n_ir + 2 n_r entries. */
+void orc_radial_rule_split(const orc_params *p, double x, double *y, double *Wy)
+{
+    const int Nr = p->n_r, Nir = p->n_ir;
+    double *t = (double *)malloc(sizeof(double) * (size_t)(2 * (Nr > Nir ? Nr : Nir)));
+    double *w = t + (Nr > Nir ? Nr : Nir);
+    if (Nir > 0) {
+        orc_gauss_legendre(Nir, t, w);
+        for (int q = 0; q < Nir; ++q) {
+            real h = ((real)t[q] + 1) / 2;
+            y[q] = (double)((real)p->eps2 * h * h * h * h);
+            Wy[q] = (double)((real)w[q] * 2 * (real)p->eps2 * h * h * h);
+        }
+    }
+    real xm = x;
+    if (xm < (real)p->eps2) xm = p->eps2;
+    if (xm > (real)p->L2) xm = p->L2;
+    orc_gauss_legendre(Nr, t, w);
+    for (int part = 0; part < 2; ++part) {
+        const real lo = part == 0 ? (real)p->eps2 : xm, hi = part == 0 ? xm : (real)p->L2;
+        const real L = R_LOG(hi / lo);
+        for (int q = 0; q < Nr; ++q) {
+            real yy = lo * R_EXP(((real)t[q] + 1) * L / 2);
+            y[Nir + part * Nr + q] = (double)yy;
+            Wy[Nir + part * Nr + q] = (double)((real)w[q] * (L / 2) * yy);
+        }
+    }
+    free(t);
+}
+
 /* O5 + O7 at one external point x with an arbitrary product rule (y_q, W_q, theta_k, Omega_k): */
 /*   Pi_G(x)   = sum_{q,k} v,           v  = -C W_q y_q Om_k sin^4/z^2 G(y_q) Z(z)    eq.(8)    */
 /*   Pi_Z^Q(x) = sum wQ, wQ = (C/3x) W_q Om_k sin^2 Q P(y_q) P(z)                     eq.(9)    */
@@ -404,7 +438,7 @@ void orc_self_energy(const orc_params *p, const double *c, double x, int ny, con
 /* J may be NULL (residual only).  Returns 0.                                                   */
 int orc_residual_jacobian(const orc_params *p, const double *c, double gG, double gZ, double *F, double *J)
 {
-    const int N = p->n_cheb, Nr = p->n_r + p->n_ir, Nt = p->n_theta;
+    const int N = p->n_cheb, Nr = (p->radial_split ? 2 * p->n_r : p->n_r) + p->n_ir, Nt = p->n_theta;
     const int Ne = orc_n_ext(p);
     const int iZ = N, iG = (p->x_G == p->x_Z) ? N : N + 1;
     double *x_ext = (double *)malloc(sizeof(double) * (size_t)(Ne + N + 3 * Nr + 2 * Nt));
@@ -415,6 +449,7 @@ int orc_residual_jacobian(const orc_params *p, const double *c, double gG, doubl
     for (int j = 0; j < 2 * N; ++j) cr[j] = c[j];
     for (int e = 0; e < Ne; ++e) {
         real *d = D + (size_t)4 * N * e;
+        if (p->radial_split) orc_radial_rule_split(p, x_ext[e], y, Wy);      /* the rule of this external point */
         self_energy(p, cr, (real)x_ext[e], Nr, y, Wy, Nt, th, Om, &PiG[e], &PiQ[e], &PiM[e],
                     J ? d : NULL, J ? d + N : NULL, J ? d + 2 * N : NULL, J ? d + 3 * N : NULL);
     }

@@ -22,17 +22,17 @@ class OrcParams(C.Structure):
         ("eps2", C.c_double), ("L2", C.c_double), ("alpha_mu", C.c_double), ("n_colors", C.c_double),
         ("x_G", C.c_double), ("x_Z", C.c_double), ("delta", C.c_double),
         ("ir_exp_G", C.c_double), ("ir_exp_Z", C.c_double), ("uv_omega", C.c_double),
-        ("n_ir", C.c_int32), ("pad2_", C.c_int32),
+        ("n_ir", C.c_int32), ("radial_split", C.c_int32),
     ]
 
 
 def make_params(n_cheb, n_r, n_theta, eps2, L2, x_G, x_Z, alpha_mu=1.0, n_colors=3.0, delta=-9.0 / 44.0,
-                ir_exp_G=-0.595353, ir_exp_Z=2 * 0.595353, uv_omega=None, angular_rule=0, n_ir=0):
+                ir_exp_G=-0.595353, ir_exp_Z=2 * 0.595353, uv_omega=None, angular_rule=0, n_ir=0, radial_split=0):
     if uv_omega is None:
         uv_omega = 11.0 * n_colors * alpha_mu / (12.0 * np.pi)
     return OrcParams(int(n_cheb), int(n_r), int(n_theta), int(angular_rule), float(eps2), float(L2), float(alpha_mu),
                      float(n_colors), float(x_G), float(x_Z), float(delta), float(ir_exp_G), float(ir_exp_Z),
-                     float(uv_omega), int(n_ir), 0)
+                     float(uv_omega), int(n_ir), int(radial_split))
 
 
 def _ptr(a):
@@ -52,6 +52,7 @@ class Oracle:
         L = self.lib
         L.orc_gauss_legendre.argtypes = [C.c_int, _dp, _dp]
         L.orc_cheb_phi.argtypes = [C.c_int, C.c_double, _dp]
+        L.orc_radial_rule_split.argtypes = [C.POINTER(OrcParams), C.c_double, _dp, _dp]
         L.orc_gl_node.argtypes = [C.c_int, C.c_int, _dp, _dp]
         L.orc_schwinger.argtypes = [C.POINTER(OrcParams), _dp, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp]
         for name in ("orc_z", "orc_kernel_M", "orc_kernel_Q", "orc_kernel_ghost", "orc_kernel_M_literal",
@@ -77,6 +78,12 @@ class Oracle:
         t = np.empty(n); w = np.empty(n)
         self.lib.orc_gauss_legendre(n, _ptr(t), _ptr(w))
         return t, w
+
+    def radial_rule_split(self, p, x):
+        n = p.n_ir + 2 * p.n_r
+        y = np.empty(n); Wy = np.empty(n)
+        self.lib.orc_radial_rule_split(C.byref(p), float(x), _ptr(y), _ptr(Wy))
+        return y, Wy
 
     def gl_node(self, n, i):
         t = C.c_double(); w = C.c_double()

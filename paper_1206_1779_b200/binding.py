@@ -20,6 +20,7 @@ EXPORTS = [
 
 DSE_FLAG_GEOMETRY_CACHE = 1
 DSE_FLAG_ANGULAR_TANH_SINH = 2
+DSE_FLAG_RADIAL_SPLIT = 4
 
 
 class DseParams(C.Structure):
@@ -84,6 +85,8 @@ def _check(rc):
 def params_from_workload(w, n_batch=None, flags=0):
     if getattr(w, "angular_rule", 0) == 1:
         flags |= DSE_FLAG_ANGULAR_TANH_SINH
+    if getattr(w, "radial_split", 0) == 1:
+        flags |= DSE_FLAG_RADIAL_SPLIT
     return DseParams(w.n_cheb, w.n_r, w.n_theta, w.n_batch if n_batch is None else n_batch, w.eps2, w.L2,
                      w.alpha_mu, w.n_colors, w.x_G, w.x_Z, w.delta, w.ir_exp_G, w.ir_exp_Z, w.uv_omega, flags, getattr(w, "n_ir", 0))
 
@@ -184,7 +187,7 @@ class Dse:
     # ---- introspection ----------------------------------------------------------------------------
     def tables(self):
         p = self.params
-        nr = p.n_r + p.n_r_ir
+        nr = (2 if p.flags & DSE_FLAG_RADIAL_SPLIT else 1) * p.n_r + p.n_r_ir
         out = dict(x_ext=np.empty(self.n_ext), y=np.empty(nr), Wy=np.empty(nr), theta=np.empty(p.n_theta),
                    Omega=np.empty(p.n_theta))
         _check(self.lib.dse_get_tables(self._h, *[C.c_void_p(out[k].ctypes.data)

@@ -65,7 +65,7 @@ int validate(const dse_params *p)
     if (!finite_pos(p->x_Z) || !std::isfinite(p->x_G) || p->x_G < 0.0 || (p->x_G == 0.0 && p->x_Z == 0.0)) return DSE_EINVAL;
     if (!std::isfinite(p->delta) || !std::isfinite(p->ir_exp_G) || !std::isfinite(p->ir_exp_Z)) return DSE_EINVAL;
     if (!std::isfinite(p->uv_omega) || p->uv_omega < 0.0) return DSE_EINVAL;
-    if (p->n_r_ir < 0 || p->n_r_ir > (1 << 20) || (p->flags & ~(DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_ANGULAR_TANH_SINH))) return DSE_EINVAL;
+    if (p->n_r_ir < 0 || p->n_r_ir > (1 << 20) || (p->flags & ~(DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_ANGULAR_TANH_SINH | DSE_FLAG_RADIAL_SPLIT))) return DSE_EINVAL;
     return DSE_OK;
 }
 
@@ -147,6 +147,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     k.g = T.Ntpad < 32 ? T.Ntpad : 32;
     k.rpb = 32 / k.g;
     k.Next = T.Next; k.B = params->n_batch; k.iZ = T.iZ; k.iG = T.iG;
+    k.rstride = T.rstride; k.Gext = T.rstride ? T.Next : 1;
     k.R = (long long)k.B * k.Next * k.Nr;
     if ((long long)k.Next * k.Nr * k.Ntpad >= (1ll << 31) || (long long)k.B * k.Next >= (1ll << 30)) {
         dse::set_error_text("grid too large: N_ext*N_r*N_theta must stay below 2^31 points per system");
@@ -163,8 +164,8 @@ int dse_create(const dse_params *params, dse_handle **out)
     // ---- tables -> device (one allocation) ----
     size_t off = 0;
     const size_t o_x = carve<double>(off, T.Next), o_sx = carve<double>(off, T.Next), o_c3 = carve<double>(off, T.Next);
-    const size_t o_y = carve<double>(off, T.Nr), o_sy = carve<double>(off, T.Nr), o_W = carve<double>(off, T.Nr);
-    const size_t o_EG = carve<double>(off, T.Nr), o_EZ = carve<double>(off, T.Nr);
+    const size_t o_y = carve<double>(off, T.y.size()), o_sy = carve<double>(off, T.y.size()), o_W = carve<double>(off, T.y.size());
+    const size_t o_EG = carve<double>(off, T.y.size()), o_EZ = carve<double>(off, T.y.size());
     const size_t o_ang = carve<double>(off, T.ang.size());
     const size_t o_py = carve<double>(off, T.phi_y.size()), o_px = carve<double>(off, T.phi_x.size());
     std::vector<double> host(off, 0.0);
@@ -206,7 +207,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     const size_t n2 = 2 * (size_t)k.N;
     off = 0;
     const size_t o_coef = carve<double>(off, (size_t)k.B * k.Npad * 2);
-    const size_t o_Gy = carve<double>(off, (size_t)k.B * k.Nr), o_Py = carve<double>(off, (size_t)k.B * k.Nr);
+    const size_t o_Gy = carve<double>(off, (size_t)k.B * k.Gext * k.Nr), o_Py = carve<double>(off, (size_t)k.B * k.Gext * k.Nr);
     const size_t o_iG = carve<double>(off, (size_t)k.B * k.N), o_iZ = carve<double>(off, (size_t)k.B * k.N);
     const size_t o_A = carve<double>(off, (size_t)k.R * 4), o_AH = carve<double>(off, (size_t)k.R * 4);
     const size_t o_S = carve<double>(off, ((size_t)k.W + (size_t)k.B * k.Next) * 3 * k.Npad);
@@ -366,8 +367,8 @@ int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, doub
     if (!h) return DSE_EINVAL;
     const dse::HostTables &T = h->tab;
     if (x_ext_host) memcpy(x_ext_host, T.x_ext.data(), 8 * T.x_ext.size());
-    if (y_host) memcpy(y_host, T.y.data(), 8 * T.y.size());
-    if (Wy_host) memcpy(Wy_host, T.Wy.data(), 8 * T.Wy.size());
+    if (y_host) memcpy(y_host, T.y.data(), 8 * (size_t)T.Nr);          // split rule: the rule of external point 0
+    if (Wy_host) memcpy(Wy_host, T.Wy.data(), 8 * (size_t)T.Nr);
     if (theta_host) memcpy(theta_host, T.theta.data(), 8 * T.theta.size());
     if (Omega_host) memcpy(Omega_host, T.Omega.data(), 8 * T.Omega.size());
     return DSE_OK;

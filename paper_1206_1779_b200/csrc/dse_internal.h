@@ -15,6 +15,7 @@ constexpr int MAX_NCH = DSE_MAX_NCHEB / CJ;
 struct HostTables {
     int N = 0, Npad = 0, Nr = 0, Nt = 0, Ntpad = 0, Next = 0;
     int iZ = 0, iG = 0;                       // external-point index of x_Z, x_G
+    int rstride = 0;                          // radial tables are [Next][Nr] (rstride = Nr, split rule) or shared (0)
     double Lg = 0, C = 0;
     std::vector<double> x_ext, sx_ext, c3x_ext;   // x, sqrt x, C/(3x)
     std::vector<double> y, sy, Wy, t_r;           // radial nodes (infrared piece first), sqrt, dy weight, s(y_q)
@@ -31,6 +32,7 @@ struct KParams {
     int N, Npad, NCH, SUB, rounds;     // Chebyshev: N, padded to NCH*CJ; phase-2 lanes = NCH chunk x SUB point lanes
     int Nr, Nt, Ntpad, g, rpb;         // angular nodes padded to a multiple of g (g = 32, or pow2 >= Nt); rows per batch
     int Next, B, iZ, iG;
+    int rstride, Gext;                 // radial tables: element (e, q) at e*rstride + q; Gy/Py are [B][Gext][Nr] (Gext = Next or 1)
     long long R;                       // rows = B * Next * Nr
     int W;                             // warps in the grid of the point kernel
     long long U;                       // partition units of the Jacobian build: rows (upr = 1) or 32-point batches

@@ -35,9 +35,10 @@ __global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double
             P.coefP[((size_t)b * P.Npad + j) * 2 + 1] = bb;
         }
     }
-    if (item >= P.Nr + P.N) return;
-    const bool isy = item < P.Nr;
-    const double *phi = isy ? P.phi_y + (size_t)item * P.Npad : P.phi_x + (size_t)(item - P.Nr) * P.Npad;
+    const int NG = P.Gext * P.Nr;                        // fixed points y_{e,q} (split rule) or y_q (shared rule)
+    if (item >= NG + P.N) return;
+    const bool isy = item < NG;
+    const double *phi = isy ? P.phi_y + (size_t)item * P.Npad : P.phi_x + (size_t)(item - NG) * P.Npad;
     double lnZ = 0.0, lnG = 0.0;
     for (int j = lane; j < P.N; j += 32) {       // phi_0 = 1/2 is in the table
         const double f = phi[j];
@@ -51,11 +52,11 @@ __global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double
     if (lane == 0) {
         if (isy) {
             lnG += P.EGy[item]; lnZ += P.EZy[item];          // power-law continuation below eps2 (infrared piece)
-            P.Gy[(size_t)b * P.Nr + item] = exp(lnG);
-            P.Py[(size_t)b * P.Nr + item] = exp(P.e1 * lnG + P.e2 * lnZ);
+            P.Gy[(size_t)b * NG + item] = exp(lnG);
+            P.Py[(size_t)b * NG + item] = exp(P.e1 * lnG + P.e2 * lnZ);
         } else {
-            P.invG[(size_t)b * P.N + (item - P.Nr)] = exp(-lnG);
-            P.invZ[(size_t)b * P.N + (item - P.Nr)] = exp(-lnZ);
+            P.invG[(size_t)b * P.N + (item - NG)] = exp(-lnG);
+            P.invZ[(size_t)b * P.N + (item - NG)] = exp(-lnZ);
         }
     }
 }
@@ -69,7 +70,8 @@ __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
         const long long eq = t / P.Ntpad;
         const int q = (int)(eq % P.Nr), e = (int)(eq / P.Nr);
         const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
-        const double y = P.y[q], sy = P.sy[q], Wq = P.Wy[q];
+        const int rq = e * P.rstride + q;
+        const double y = P.y[rq], sy = P.sy[rq], Wq = P.Wy[rq];
         RowConst rc;
         const double d = (x - y) / (sx + sy);
         rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
@@ -132,6 +134,28 @@ __global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
             out[cn] = r0;
             out[cn + 1] = r1;
         }
+    }
+}
+
+// H7 with the split radial rule (DSE_FLAG_RADIAL_SPLIT): phi_j(s(y_{e,q})) depends on the external point, so the
+// contraction is a batch of [3 x N_r].[N_r x N] products, one per (system, external point): one warp each, lanes
+// over j, plain FMAs in ascending q (a 3-row operand cannot fill a tensor-core tile).
+__global__ void __launch_bounds__(128) contract_split_kernel(const KParams P)
+{
+    const int e = blockIdx.x, b = blockIdx.y;
+    const size_t rowbase = ((size_t)b * P.Next + e) * P.Nr;
+    const double4 *A = reinterpret_cast<const double4 *>(P.Apart) + rowbase;
+    const double4 *H = reinterpret_cast<const double4 *>(P.AHead) + rowbase;
+    const double *Phi = P.phi_y + (size_t)e * P.rstride * P.Npad;
+    for (int j = threadIdx.x; j < P.Npad; j += blockDim.x) {
+        double ra = 0.0, rb = 0.0, rv = 0.0;
+        for (int q = 0; q < P.Nr; ++q) {
+            const double4 a = A[q], h = H[q];
+            const double f = Phi[(size_t)q * P.Npad + j];
+            ra = fma(a.x + h.x, f, ra); rb = fma(a.y + h.y, f, rb); rv = fma(a.z + h.z, f, rv);
+        }
+        double *out = P.Rz + ((size_t)b * P.Next + e) * 3 * P.Npad;
+        out[j] = ra; out[P.Npad + j] = rb; out[2 * P.Npad + j] = rv;
     }
 }
 
@@ -303,15 +327,19 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     KParams kk = k;
     kk.want_jac = J_dev != nullptr;
     int launches = 0;
-    prep_kernel<<<dim3((kk.Nr + kk.N + 7) / 8, kk.B), 256, 0, s>>>(kk, c_dev);
+    prep_kernel<<<dim3((kk.Gext * kk.Nr + kk.N + 7) / 8, kk.B), 256, 0, s>>>(kk, c_dev);
     ++launches;
     if (ev0) cudaEventRecord((cudaEvent_t)ev0, s);
     launch_point(kk, cfg, stream);
     if (ev1) cudaEventRecord((cudaEvent_t)ev1, s);
     ++launches;
     if (kk.want_jac) {
-        dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);
-        gemm_kernel<<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
+        if (kk.rstride) {
+            contract_split_kernel<<<dim3(kk.Next, kk.B), 128, 0, s>>>(kk);
+        } else {
+            dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);
+            gemm_kernel<<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
+        }
         ++launches;
     }
     dim3 ga(kk.N, kk.B);

@@ -136,12 +136,14 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
 
         // row constants (identical in all lanes of a row)
         const double rowmask = rowact ? 1.0 : 0.0;
-        const double Gy = P.Gy[(size_t)cur_b * Nr + q] * rowmask, Py = P.Py[(size_t)cur_b * Nr + q] * rowmask;
+        const size_t gq = ((size_t)cur_b * P.Gext + (P.rstride ? e : 0)) * Nr + q;
+        const double Gy = P.Gy[gq] * rowmask, Py = P.Py[gq] * rowmask;
         RowConst rc;
         if (!GEOM) {
             const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
-            const double y = P.y[q], sy = P.sy[q];
-            const double Wq = P.Wy[q];
+            const int rq = e * P.rstride + q;
+            const double y = P.y[rq], sy = P.sy[rq];
+            const double Wq = P.Wy[rq];
             const double d = (x - y) / (sx + sy);
             rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
         }
@@ -439,12 +441,14 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
         __syncwarp();
         bool seg_done = false;
         while (!seg_done) {
-            const double Gy = P.Gy[(size_t)cur_b * Nr + q], Py = P.Py[(size_t)cur_b * Nr + q];
+            const size_t gq = ((size_t)cur_b * P.Gext + (P.rstride ? e : 0)) * Nr + q;
+            const double Gy = P.Gy[gq], Py = P.Py[gq];
             RowConst rc;
             if (!GEOM) {
                 const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
-                const double y = P.y[q], sy = P.sy[q];
-                const double Wq = P.Wy[q];
+                const int rq = e * P.rstride + q;
+                const double y = P.y[rq], sy = P.sy[rq];
+                const double Wq = P.Wy[rq];
                 const double d = (x - y) / (sx + sy);
                 rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
             }

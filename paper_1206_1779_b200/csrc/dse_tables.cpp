@@ -75,7 +75,8 @@ inline void phi_row(int N, int Npad, ld s, double *out)
 
 void build_tables(const dse_params &p, HostTables &T)
 {
-    const int N = p.n_cheb, Nir = p.n_r_ir, Nmain = p.n_r, Nr = Nmain + Nir, Nt = p.n_theta;
+    const bool split = (p.flags & DSE_FLAG_RADIAL_SPLIT) != 0;
+    const int N = p.n_cheb, Nir = p.n_r_ir, Nmain = p.n_r, Nr = (split ? 2 : 1) * Nmain + Nir, Nt = p.n_theta;
     T.N = N;
     T.Npad = ((N + CJ - 1) / CJ) * CJ;
     T.Nr = Nr;
@@ -93,34 +94,69 @@ void build_tables(const dse_params &p, HostTables &T)
     T.C = (double)C;
 
     std::vector<ld> t, w;
-    T.y.resize(Nr); T.sy.resize(Nr); T.Wy.resize(Nr); T.t_r.resize(Nr);
-    T.EGy.assign(Nr, 0.0); T.EZy.assign(Nr, 0.0);
-    T.phi_y.assign((size_t)Nr * T.Npad, 0.0);
-    // infrared piece int_0^{eps2} dy of eq.(26): GL in v, y = eps2 ((1+v)/2)^4, dy = 2 eps2 ((1+v)/2)^3 dv; the
-    // dressings there are the power laws eq.(16),(17): ln G(y) = series(s = -1) + p_G ln(y/eps2)
-    if (Nir > 0) {
-        gauss_legendre(Nir, t, w);
-        for (int q = 0; q < Nir; ++q) {
-            const ld hq = (t[q] + 1) / 2;
-            T.y[q] = (double)((ld)p.eps2 * hq * hq * hq * hq);
-            T.sy[q] = (double)sqrtl((ld)T.y[q]);
-            T.Wy[q] = (double)(w[q] * 2 * (ld)p.eps2 * hq * hq * hq);
-            T.t_r[q] = -1.0;
-            const ld ell = logl((ld)T.y[q] / (ld)p.eps2);
-            T.EGy[q] = (double)((ld)p.ir_exp_G * ell);
-            T.EZy[q] = (double)((ld)p.ir_exp_Z * ell);
-            phi_row(N, T.Npad, -1.0L, &T.phi_y[(size_t)q * T.Npad]);
-        }
+    // external points first (the split radial rule depends on them): Chebyshev roots s_i = -cos(pi (i+1/2)/N),
+    // ascending, then x_Z, then x_G
+    T.x_ext.resize(T.Next); T.sx_ext.resize(T.Next); T.c3x_ext.resize(T.Next);
+    T.phi_x.assign((size_t)N * T.Npad, 0.0);
+    for (int i = 0; i < N; ++i) {
+        ld s = -cosl(PI_L * (i + 0.5L) / N);
+        T.x_ext[i] = (double)((ld)p.eps2 * expl((s + 1) * Lg / 2));
+        phi_row(N, T.Npad, s, &T.phi_x[(size_t)i * T.Npad]);
     }
-    // main radial rule in s; y = eps2 exp((s+1) Lg/2), dy = (Lg/2) y ds
-    gauss_legendre(Nmain, t, w);
-    for (int q = 0; q < Nmain; ++q) {
-        ld yy = (ld)p.eps2 * expl((t[q] + 1) * Lg / 2);
-        T.y[Nir + q] = (double)yy;
-        T.sy[Nir + q] = (double)sqrtl((ld)T.y[Nir + q]);          // sqrt of the rounded table value
-        T.Wy[Nir + q] = (double)(w[q] * (Lg / 2) * yy);
-        T.t_r[Nir + q] = (double)t[q];
-        phi_row(N, T.Npad, t[q], &T.phi_y[(size_t)(Nir + q) * T.Npad]);
+    T.x_ext[T.iZ] = p.x_Z;
+    if (!same) T.x_ext[T.iG] = p.x_G;
+    for (int e = 0; e < T.Next; ++e) {
+        T.sx_ext[e] = (double)sqrtl((ld)T.x_ext[e]);
+        // at x = 0 (x_G = 0, L135) only the ghost equation is evaluated: the gluon prefactor C/(3x) is dropped
+        T.c3x_ext[e] = T.x_ext[e] > 0.0 ? (double)(C / (3 * (ld)T.x_ext[e])) : 0.0;
+    }
+
+    // radial rule(s): [infrared piece | main], shared by all external points, or -- DSE_FLAG_RADIAL_SPLIT, eq.(26) --
+    // [infrared piece | (eps2, x_e) | (x_e, L2)] per external point with n_r nodes in each interval (L364)
+    const int nrules = split ? T.Next : 1;
+    T.rstride = split ? Nr : 0;
+    const size_t tot = (size_t)nrules * Nr;
+    T.y.resize(tot); T.sy.resize(tot); T.Wy.resize(tot); T.t_r.resize(tot);
+    T.EGy.assign(tot, 0.0); T.EZy.assign(tot, 0.0);
+    T.phi_y.assign(tot * T.Npad, 0.0);
+    std::vector<ld> tir, wir, tm, wm;
+    if (Nir > 0) gauss_legendre(Nir, tir, wir);
+    gauss_legendre(Nmain, tm, wm);
+    for (int rule = 0; rule < nrules; ++rule) {
+        const size_t o = (size_t)rule * Nr;
+        // infrared piece int_0^{eps2} dy: GL in v, y = eps2 ((1+v)/2)^4, dy = 2 eps2 ((1+v)/2)^3 dv; the dressings there
+        // are the power laws eq.(16),(17): ln G(y) = series(s = -1) + p_G ln(y/eps2)
+        for (int q = 0; q < Nir; ++q) {
+            const ld hq = (tir[q] + 1) / 2;
+            T.y[o + q] = (double)((ld)p.eps2 * hq * hq * hq * hq);
+            T.Wy[o + q] = (double)(wir[q] * 2 * (ld)p.eps2 * hq * hq * hq);
+            T.t_r[o + q] = -1.0;
+            const ld ell = logl((ld)T.y[o + q] / (ld)p.eps2);
+            T.EGy[o + q] = (double)((ld)p.ir_exp_G * ell);
+            T.EZy[o + q] = (double)((ld)p.ir_exp_Z * ell);
+            phi_row(N, T.Npad, -1.0L, &T.phi_y[(o + q) * T.Npad]);
+        }
+        // main rule(s) in ln y: y = lo exp((v+1) L/2), dy = (L/2) y dv; s(y) by eq.(25)
+        ld xm = split ? (ld)T.x_ext[rule] : (ld)p.L2;
+        if (xm < (ld)p.eps2) xm = p.eps2;
+        if (xm > (ld)p.L2) xm = p.L2;
+        for (int part = 0; part < (split ? 2 : 1); ++part) {
+            const ld lo = part == 0 ? (ld)p.eps2 : xm, hi = (split && part == 0) ? xm : (ld)p.L2;
+            const ld L = logl(hi / lo);
+            for (int q = 0; q < Nmain; ++q) {
+                const size_t i = o + Nir + (size_t)part * Nmain + q;
+                const ld yy = lo * expl((tm[q] + 1) * L / 2);
+                T.y[i] = (double)yy;
+                T.Wy[i] = (double)(wm[q] * (L / 2) * yy);
+                ld sy = 2 * logl(yy / (ld)p.eps2) / Lg - 1;
+                if (!split) sy = tm[q];                         // the shared rule is laid out in s itself
+                if (sy < -1) sy = -1;
+                if (sy > 1) sy = 1;
+                T.t_r[i] = (double)sy;
+                phi_row(N, T.Npad, sy, &T.phi_y[i * T.Npad]);
+            }
+        }
+        for (int q = 0; q < Nr; ++q) T.sy[o + q] = (double)sqrtl((ld)T.y[o + q]);    // sqrt of the rounded table value
     }
     // angular rule: Gauss-Legendre in theta, or tanh-sinh in xi = cos(theta) (eq.(5))
     T.theta.resize(Nt); T.Omega.resize(Nt);
@@ -166,21 +202,6 @@ void build_tables(const dse_params &p, HostTables &T)
         a[4] = (double)((ld)(double)Om * s * s);
         a[5] = (double)((ld)(double)Om * s * s * s * s);
     }
-    }
-    // external points: Chebyshev roots s_i = -cos(pi (i+1/2)/N), ascending, then x_Z, then x_G
-    T.x_ext.resize(T.Next); T.sx_ext.resize(T.Next); T.c3x_ext.resize(T.Next);
-    T.phi_x.assign((size_t)N * T.Npad, 0.0);
-    for (int i = 0; i < N; ++i) {
-        ld s = -cosl(PI_L * (i + 0.5L) / N);
-        T.x_ext[i] = (double)((ld)p.eps2 * expl((s + 1) * Lg / 2));
-        phi_row(N, T.Npad, s, &T.phi_x[(size_t)i * T.Npad]);
-    }
-    T.x_ext[T.iZ] = p.x_Z;
-    if (!same) T.x_ext[T.iG] = p.x_G;
-    for (int e = 0; e < T.Next; ++e) {
-        T.sx_ext[e] = (double)sqrtl((ld)T.x_ext[e]);
-        // at x = 0 (x_G = 0, L135) only the ghost equation is evaluated: the gluon prefactor C/(3x) is dropped
-        T.c3x_ext[e] = T.x_ext[e] > 0.0 ? (double)(C / (3 * (ld)T.x_ext[e])) : 0.0;
     }
 }
 

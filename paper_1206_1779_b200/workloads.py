@@ -32,6 +32,7 @@ class Workload:
     ir_exp_Z: float = 2 * KAPPA
     uv_omega: float = field(default=None)
     n_ir: int = 0          # nodes of the infrared piece int_0^{eps2} dy (eq.(26)); 0 in the BASELINE configs
+    radial_split: int = 0  # 1: the paper's split at y = x with n_r nodes in each interval (eq.(26))
     angular_rule: int = 0  # 0: Gauss-Legendre in theta (BASELINE configs); 1: tanh-sinh in xi
 
     def __post_init__(self):
@@ -45,7 +46,7 @@ class Workload:
     @property
     def points(self):
         """quadrature points per system and build: N_ext * N_r * N_theta"""
-        return self.n_ext * (self.n_r + self.n_ir) * self.n_theta
+        return self.n_ext * ((2 if self.radial_split else 1) * self.n_r + self.n_ir) * self.n_theta
 
     @property
     def paper_equiv_evals(self):

@@ -22,7 +22,7 @@ def _torch():
 def oracle_params(w):
     from oracle.oracle import make_params
     return make_params(w.n_cheb, w.n_r, w.n_theta, w.eps2, w.L2, w.x_G, w.x_Z, w.alpha_mu, w.n_colors, w.delta,
-                       w.ir_exp_G, w.ir_exp_Z, w.uv_omega, getattr(w, "angular_rule", 0), getattr(w, "n_ir", 0))
+                       w.ir_exp_G, w.ir_exp_Z, w.uv_omega, getattr(w, "angular_rule", 0), getattr(w, "n_ir", 0), getattr(w, "radial_split", 0))
 
 
 def gpu_build(w, c, bc, flags=0, jac=True):

@@ -15,6 +15,9 @@ from test_gpu_parity import oracle_params, gpu_build, check, _torch   # noqa: E4
     dict(n_ir=12, x_G=0.0, x_Z=5e4),                # the paper's subtraction points (L135)
     dict(n_ir=0, x_G=0.0, x_Z=30.0),                # x_G = 0 without the infrared piece
     dict(n_ir=7, x_G=0.0, x_Z=5e4, angular_rule=1, n_theta=40),
+    dict(radial_split=1),                           # NEXT f1: the paper's split at y = x (eq.(26)), x_G = x_Z
+    dict(radial_split=1, n_ir=12, x_G=0.0, x_Z=5e4, n_r=24),        # the paper's full three-interval rule
+    dict(radial_split=1, n_ir=5, x_G=3.0, x_Z=5e4, n_r=13, n_theta=21, n_cheb=12),   # ragged
 ])
 def test_infrared_piece_and_zero_subtraction_point_parity(orc, kw):
     from paper_1206_1779_b200.workloads import Workload, draw_coefficients

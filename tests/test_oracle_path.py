@@ -385,3 +385,39 @@ def test_infrared_piece_closed_form(orc):
     assert tab0["x_ext"][5] == 0.0
     o0 = orc.self_energy(p0, np.zeros(8), 0.0, tab0["y"], tab0["Wy"], tab0["theta"], tab0["Omega"])
     assert abs(o0[0] + C * (3 * PI / 8) * math.log(L2 / eps2)) < 1e-12 and o0[1] == 0.0 and o0[2] == 0.0
+
+
+def test_radial_split_rule_f1(orc):
+    """eq.(26) L190 / L364: int_{eps2}^{x} + int_{x}^{L2} with n_r nodes in each interval removes the kink of the
+    integrand at y = x: the tree-level closed forms (pin P5) are reached with 40 nodes per interval, where the single
+    rule on [eps2, L2] with 80 nodes is still off by ~1e-4."""
+    eps2, L2 = 1e-4, 1e4
+    p = make_params(4, 40, 200, eps2, L2, 1.0, 1.0, ir_exp_G=0.0, ir_exp_Z=0.0, uv_omega=0.0, radial_split=1)
+    p1 = make_params(4, 80, 200, eps2, L2, 1.0, 1.0, ir_exp_G=0.0, ir_exp_Z=0.0, uv_omega=0.0)
+    tab, tab1 = orc.tables(p), orc.tables(p1)
+    C = orc.coupling_C(p)
+    for x in (0.01, 1.0, 37.0):
+        y, Wy = orc.radial_rule_split(p, x)
+        assert len(y) == 80 and np.all(np.diff(y) > 0) and y[39] < x < y[40]
+        assert abs(np.sum(Wy) - (L2 - eps2)) < 1e-9 * L2
+        out = orc.self_energy(p, np.zeros(8), x, y, Wy, tab["theta"], tab["Omega"])
+        PiG0 = -C * (3 * PI / 8) * ((x * x - eps2 ** 2) / (2 * x * x) + math.log(L2 / x))
+        PiZ0 = (C * PI / (48 * x)) * ((5 / 3) * (x ** 3 - eps2 ** 3) / x ** 2 - 22 * (x * x - eps2 ** 2) / x
+                                     - 6 * (x - eps2) + 7 * x * x * (1 / x - 1 / L2) - 52 * x * math.log(L2 / x))
+        assert abs(out[0] - PiG0) < 1e-9 * abs(PiG0) and abs(out[1] + out[2] - PiZ0) < 1e-8 * abs(PiZ0)
+        single = orc.self_energy(p1, np.zeros(8), x, tab1["y"], tab1["Wy"], tab1["theta"], tab1["Omega"])
+        assert abs(single[0] - PiG0) > 1e-6 * abs(PiG0)
+    # degenerate intervals: x <= eps2 and x >= L2 put zero weight on the empty interval
+    y, Wy = orc.radial_rule_split(p, L2)
+    assert np.all(Wy[40:] == 0.0) and abs(np.sum(Wy[:40]) - (L2 - eps2)) < 1e-9 * L2
+    y, Wy = orc.radial_rule_split(p, 0.0)
+    assert np.all(Wy[:40] == 0.0) and abs(np.sum(Wy[40:]) - (L2 - eps2)) < 1e-9 * L2
+    # the Jacobian of the split discretisation is still the derivative of its residual (eq.(38))
+    c = draw_coefficients(9, 4)
+    F, J = orc.residual_jacobian(p, c, 1.0, 1.0)
+    Jfd = np.empty((8, 8))
+    for j in range(8):
+        cp = c.copy(); cp[j] += 1e-6
+        cm = c.copy(); cm[j] -= 1e-6
+        Jfd[:, j] = (orc.residual_jacobian(p, cp, 1, 1, jac=False) - orc.residual_jacobian(p, cm, 1, 1, jac=False)) / 2e-6
+    assert np.linalg.norm(J - Jfd) <= 1e-8 * np.linalg.norm(J)

@@ -313,7 +313,9 @@ def test_gl_single_node_matches_full_rule(orc):
 
 
 # ------------------------------------------------------------------------------------ P9: the paper's own numbers
-def test_paper_scaling_solution_P9(orc):
+@pytest.mark.parametrize("n_r,n_theta,rule,split", [(96, 32, 0, 0), (64, 48, 1, 1)],
+                         ids=["single-logGL+GL-theta", "paper: 3 intervals x 64 + tanh-sinh"])
+def test_paper_scaling_solution_P9(orc, n_r, n_theta, rule, split):
     """with eps2 = 1e-6, L2 = 5e4, x_G = 0, 1/G(0) = 0, x_Z = L2, Z(x_Z) = 0.256, alpha(mu^2) = 1 the
     converged solution has alpha(M_Z^2) = 0.118 (M_Z = 91.2 GeV, fn.7), the infrared fixed point alpha(0) = 2.972 =
     8.915/N_c (L151), the power laws G ~ x^-kappa, Z ~ x^(2 kappa) (eq.(16),(17)), and the gluon Schwinger function
@@ -326,7 +328,7 @@ def test_paper_scaling_solution_P9(orc):
         f = line.split("#")[0].split()
         if len(f) == 2:
             gold[f[0]] = float(f[1])
-    p = make_params(S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, 0.0, S.L2, n_ir=S.N_IR)
+    p = make_params(S.N, n_r, n_theta, S.EPS2, S.L2, 0.0, S.L2, n_ir=S.N_IR, angular_rule=rule, radial_split=split)
     c = S.start_coefficients(orc, p)
     dn = []
     for it in range(30):

@@ -105,6 +105,13 @@ DSE_API int dse_residual(dse_handle *h, const double *c_dev, const double *bc_de
 DSE_API int dse_jacobian(dse_handle *h, const double *c_dev, const double *bc_dev, double *J_dev, double *F_dev,
                  void *stream);
 
+/* Self-check mode (the paper's own definition of the Newton matrix, eq.(38),(39) L316-336): J by central finite
+ * differences of the residual, column j from c_j +- h_j with h_j = eps_rel * max(1, |c_j|) (the paper uses
+ * eps_j ~ 1e-5 a_j, which fails at a_j = 0: DESIGN.md reading A16).  4N residual builds; asynchronous on `stream`.
+ * J_dev [n_batch][2N][2N].  Meant for verification, not for speed. */
+DSE_API int dse_jacobian_fd(dse_handle *h, const double *c_dev, const double *bc_dev, double eps_rel, double *J_dev,
+                            void *stream);
+
 /* One Newton-Raphson step (eq.(31)-(35)): builds J, F, scales each row of (J|F) by 1/max_j|J_ij|,
  * LU with partial pivoting (first maximal element wins), solves J Delta = F, c <- c - rho Delta
  * in place.  stats_dev[b] = { max|Delta|, max_i|F_i| row-scaled, min|pivot|, growth max|U|/max|A| }.

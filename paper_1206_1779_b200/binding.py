@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
 EXPORTS = [
     "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_lu_solve",
     "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count", "dse_kernel_info",
-    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_gauss_legendre", "dse_schwinger", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
+    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_gauss_legendre", "dse_schwinger", "dse_jacobian_fd", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
@@ -65,6 +65,7 @@ def load_library():
     L.dse_set_timing.argtypes = [vp, C.c_int32]
     L.dse_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.dse_get_phase_cycles.argtypes = [vp, C.POINTER(C.c_double * 5)]
+    L.dse_jacobian_fd.argtypes = [vp, dp, dp, C.c_double, dp, vp]
     L.dse_gauss_legendre.argtypes = [C.c_int32, dp, dp, dp, vp]
     L.dse_schwinger.argtypes = [vp, dp, C.c_int32, C.c_double, C.c_double, dp, C.c_int32, dp, dp, vp]
     L.dse_dfma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
@@ -147,6 +148,15 @@ class Dse:
         _check(self.lib.dse_jacobian(self._h, _dev_ptr(c, self.B * n), _dev_ptr(bc, 2 * self.B),
                                      _dev_ptr(J, self.B * n * n), _dev_ptr(F, self.B * n), _stream_ptr(stream)))
         return J, F
+
+    def jacobian_fd(self, c, bc, eps_rel=1e-6, stream=None):
+        """Central finite-difference Newton matrix (the paper's eq.(38)): a self-check of the analytic one."""
+        import torch
+        n = 2 * self.N
+        J = torch.empty((self.B, n, n), dtype=torch.float64, device=c.device)
+        _check(self.lib.dse_jacobian_fd(self._h, _dev_ptr(c, self.B * n), _dev_ptr(bc, 2 * self.B), float(eps_rel),
+                                        _dev_ptr(J), _stream_ptr(stream)))
+        return J
 
     def newton_step(self, c, bc, rho=1.0, stats=None, stream=None):
         import torch

@@ -24,6 +24,7 @@ struct dse_handle {
     double *d_work = nullptr;       // one allocation for the per-build workspace
     double *d_geom = nullptr;       // geometry cache (optional)
     double *d_J = nullptr, *d_F = nullptr, *d_lu = nullptr;   // internal J, F for dse_newton_step (+ LU scratch)
+    double *d_fd = nullptr;
     double *d_c = nullptr, *d_bc = nullptr, *d_Jh = nullptr, *d_Fh = nullptr;   // staging for *_host calls
     int64_t launches = 0;
     bool owns_const = false;
@@ -216,12 +217,13 @@ int dse_create(const dse_params *params, dse_handle **out)
     const size_t o_lu = carve<double>(off, (size_t)k.B * dse::lu_scratch_doubles((int)n2));
     const size_t o_c = carve<double>(off, (size_t)k.B * n2), o_bc = carve<double>(off, (size_t)k.B * 2);
     const size_t o_dbg = carve<double>(off, (size_t)k.W * 5);
+    const size_t o_fd = carve<double>(off, (size_t)k.B * n2 * 3);          // finite-difference self-check: c_tmp, F+, F-
     if (cudaMalloc(&h->d_work, 8 * off) != cudaSuccess) { dse_destroy(h); return DSE_ENOMEM; }
     e = cudaMemset(h->d_work, 0, 8 * off);
     if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemset(workspace)"); }
     double *wk = h->d_work;
     k.coefP = wk + o_coef; k.Gy = wk + o_Gy; k.Py = wk + o_Py; k.invG = wk + o_iG; k.invZ = wk + o_iZ;
-    k.Apart = wk + o_A; k.AHead = wk + o_AH; k.Spart = wk + o_S; k.Rz = wk + o_R; k.dbg = wk + o_dbg;
+    k.Apart = wk + o_A; k.AHead = wk + o_AH; k.Spart = wk + o_S; k.Rz = wk + o_R; k.dbg = wk + o_dbg; h->d_fd = wk + o_fd;
     h->d_J = wk + o_J; h->d_F = wk + o_F; h->d_lu = wk + o_lu; h->d_c = wk + o_c; h->d_bc = wk + o_bc;
     h->d_Jh = h->d_J; h->d_Fh = h->d_F;
 
@@ -327,6 +329,26 @@ int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches)
     if (rc < 0) return rc;
     *total_ms = h->t_ms;
     *launches = h->t_n;
+    return DSE_OK;
+}
+
+int dse_jacobian_fd(dse_handle *h, const double *c_dev, const double *bc_dev, double eps_rel, double *J_dev, void *stream)
+{
+    if (!h || !c_dev || !bc_dev || !J_dev || !(eps_rel > 0.0) || !std::isfinite(eps_rel)) return DSE_EINVAL;
+    const int n2 = 2 * h->k.N, B = h->k.B;
+    double *c_tmp = h->d_fd, *Fp = c_tmp + (size_t)B * n2, *Fm = Fp + (size_t)B * n2;
+    for (int j = 0; j < n2; ++j) {
+        for (int sgn = 0; sgn < 2; ++sgn) {
+            int rc = dse::launch_fd_perturb(n2, B, c_dev, c_tmp, j, sgn ? -1.0 : 1.0, eps_rel, stream);
+            if (rc < 0) return rc;
+            h->launches += rc;
+            rc = do_build(h, c_tmp, bc_dev, nullptr, sgn ? Fm : Fp, stream);
+            if (rc < 0) return rc;
+        }
+        int rc = dse::launch_fd_column(n2, B, c_dev, Fp, Fm, J_dev, j, eps_rel, stream);
+        if (rc < 0) return rc;
+        h->launches += rc;
+    }
     return DSE_OK;
 }
 

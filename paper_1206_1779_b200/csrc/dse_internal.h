@@ -66,6 +66,9 @@ struct PointKernelConfig {
 int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c_dev, const double *bc_dev,
                  double *J_dev, double *F_dev, void *stream, void *ev0 = nullptr, void *ev1 = nullptr);
 int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream);
+int launch_fd_perturb(int n2, int B, const double *c, double *c_tmp, int j, double sign, double eps_rel, void *stream);
+int launch_fd_column(int n2, int B, const double *c, const double *Fp, const double *Fm, double *J, int j, double eps_rel,
+                     void *stream);
 int launch_geometry(const KParams &k, double *geom, void *stream);
 int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
               double *stats, double *scratch, void *stream);

@@ -267,6 +267,31 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
 }
 
 // ---------------------------------------------------------------------------------------------
+// Finite-difference self-check (eq.(38),(39)): c_tmp = c with c_j -> c_j + sign * h_j;  J[:, j] = (F+ - F-)/(2 h_j)
+__device__ __forceinline__ double fd_step(double cj, double eps_rel) { return eps_rel * fmax(1.0, fabs(cj)); }
+
+__global__ void fd_perturb_kernel(int n2, const double *__restrict__ c, double *__restrict__ c_tmp, int j, double sign,
+                                  double eps_rel)
+{
+    const int b = blockIdx.x;
+    for (int i = threadIdx.x; i < n2; i += blockDim.x) {
+        const double v = c[(size_t)b * n2 + i];
+        c_tmp[(size_t)b * n2 + i] = (i == j) ? v + sign * fd_step(v, eps_rel) : v;
+    }
+}
+
+__global__ void fd_column_kernel(int n2, const double *__restrict__ c, const double *__restrict__ Fp,
+                                 const double *__restrict__ Fm, double *__restrict__ J, int j, double eps_rel)
+{
+    const int b = blockIdx.x;
+    const double cj = c[(size_t)b * n2 + j];
+    // the step actually taken, as representable numbers: (c_j + h) - (c_j - h)
+    const double h2 = (cj + fd_step(cj, eps_rel)) - (cj - fd_step(cj, eps_rel));
+    for (int i = threadIdx.x; i < n2; i += blockDim.x)
+        J[((size_t)b * n2 + i) * n2 + j] = (Fp[(size_t)b * n2 + i] - Fm[(size_t)b * n2 + i]) / h2;
+}
+
+// ---------------------------------------------------------------------------------------------
 // fp64 throughput probes (roofline denominators; see include/dse.h)
 __global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double *sink)
 {
@@ -348,6 +373,20 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "build launch");
     return launches;
+}
+
+int launch_fd_perturb(int n2, int B, const double *c, double *c_tmp, int j, double sign, double eps_rel, void *stream)
+{
+    fd_perturb_kernel<<<B, 128, 0, (cudaStream_t)stream>>>(n2, c, c_tmp, j, sign, eps_rel);
+    return 1;
+}
+int launch_fd_column(int n2, int B, const double *c, const double *Fp, const double *Fm, double *J, int j, double eps_rel,
+                     void *stream)
+{
+    fd_column_kernel<<<B, 128, 0, (cudaStream_t)stream>>>(n2, c, Fp, Fm, J, j, eps_rel);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fd launch");
+    return 1;
 }
 
 int launch_dfma_probe(int blocks, int iters, double *sink, void *stream)

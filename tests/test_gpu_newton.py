@@ -82,3 +82,30 @@ def test_config2_newton_trajectory_literal(orc):
     # both sides report the same ill-conditioning (min pivot of the row-scaled matrix)
     assert st[2] < 1e-8 and so[2] < 1e-8
     d.close()
+
+
+def test_finite_difference_self_check_mode(orc):
+    """NEXT f3: the paper's own Jacobian definition, eq.(38), as a GPU self-check of the analytic matrix."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import config_inputs
+    w, c, bc = config_inputs(0)
+    d = Dse(params_from_workload(w))
+    ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
+    J, F = d.jacobian(ct, bt)
+    Jfd = d.jacobian_fd(ct, bt, 1e-6)
+    torch.cuda.synchronize()
+    J = J.cpu().numpy()[0]; Jfd = Jfd.cpu().numpy()[0]
+    assert np.linalg.norm(J - Jfd) <= 1e-8 * np.linalg.norm(J)
+    assert (np.linalg.norm(J - Jfd, axis=1) / np.linalg.norm(J, axis=1)).max() < 1e-7
+    # same differences as the oracle's own finite differences
+    p = oracle_params(w)
+    n = 2 * w.n_cheb
+    Jo = np.empty((n, n))
+    for j in range(n):
+        h = 1e-6 * max(1.0, abs(c[0, j]))
+        cp = c[0].copy(); cp[j] += h
+        cm = c[0].copy(); cm[j] -= h
+        Jo[:, j] = (orc.residual_jacobian(p, cp, 1, 1, jac=False) - orc.residual_jacobian(p, cm, 1, 1, jac=False)) / ((c[0, j] + h) - (c[0, j] - h))
+    assert (np.linalg.norm(Jfd - Jo, axis=1) / np.linalg.norm(Jo, axis=1)).max() < 1e-6
+    d.close()

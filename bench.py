@@ -146,6 +146,7 @@ def run_ours(args, w, c, bc):
     import torch.distributed as dist
     from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE
     from paper_1206_1779_b200.binding import dfma_probe
+    from paper_1206_1779_b200.sharding import max_over_ranks
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -211,10 +212,7 @@ def run_ours(args, w, c, bc):
     kernel_ms, kernel_n = d.get_timing()
     d.set_timing(False)
     launches = d.launch_count() - l0
-    if world > 1:
-        tmax = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        total_ms = float(tmax.item())
+    total_ms = max_over_ranks(total_ms, device="cuda")            # multi-GPU numbers: max over ranks
     ms_per_step = total_ms / args.steps
     value = world * nb * args.steps / (total_ms * 1e-3)
 
@@ -231,10 +229,7 @@ def run_ours(args, w, c, bc):
         d.jacobian_host(c_h.numpy(), bc_h.numpy(), J_h.numpy(), F_h.numpy())
     torch.cuda.synchronize()
     t_e2e = time.perf_counter() - t0
-    if world > 1:
-        tm = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-        t_e2e = float(tm.item())
+    t_e2e = max_over_ranks(t_e2e, device="cuda")
     e2e_value = world * nb * e2e_steps / t_e2e
 
     info = d.kernel_info()

@@ -143,8 +143,10 @@ DSE_API int64_t dse_launch_count(const dse_handle *h);
 
 /* Configuration of the dominant kernel, for reporting: out[0] = grid, out[1] = block,
  * out[2] = dynamic shared memory bytes, out[3] = registers/thread, out[4] = resident CTAs/SM,
- * out[5] = SM count. */
-DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[6]);
+ * out[5] = SM count, out[6] = variant of the Jacobian point kernel (0 generic, 1 software-pipelined,
+ * 2 batched: 8 systems per warp on the fp64 tensor path, chosen when n_batch % 8 == 0, 25 <= n_cheb <= 32 and
+ * n_theta >= 32), out[7] = reserved (0). */
+DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[8]);
 
 /* Per-kernel device timing of the dominant (point) kernel, for the roofline report: while enabled,
  * every build records a CUDA event pair around the point kernel on the build's stream (nothing else

@@ -61,7 +61,7 @@ def load_library():
     L.dse_get_tables.argtypes = [vp, dp, dp, dp, dp, dp]
     L.dse_launch_count.argtypes = [vp]
     L.dse_launch_count.restype = C.c_int64
-    L.dse_kernel_info.argtypes = [vp, C.POINTER(C.c_int32 * 6)]
+    L.dse_kernel_info.argtypes = [vp, C.POINTER(C.c_int32 * 8)]
     L.dse_set_timing.argtypes = [vp, C.c_int32]
     L.dse_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.dse_get_phase_cycles.argtypes = [vp, C.POINTER(C.c_double * 5)]
@@ -222,9 +222,10 @@ class Dse:
         return int(self.lib.dse_launch_count(self._h))
 
     def kernel_info(self):
-        a = (C.c_int32 * 6)()
+        a = (C.c_int32 * 8)()
         _check(self.lib.dse_kernel_info(self._h, C.byref(a)))
-        return dict(grid=a[0], block=a[1], smem=a[2], regs=a[3], ctas_per_sm=a[4], sms=a[5])
+        return dict(grid=a[0], block=a[1], smem=a[2], regs=a[3], ctas_per_sm=a[4], sms=a[5],
+                    variant=("generic", "pipelined", "batched-dmma")[a[6]])
 
 
 def dfma_probe(blocks, iters, sink, stream=None):

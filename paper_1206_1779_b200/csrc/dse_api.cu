@@ -200,9 +200,14 @@ int dse_create(const dse_params *params, dse_handle **out)
     h->owns_const = k.use_constc != 0;
     rc = dse::query_point_kernel(k, h->cfg);
     if (rc < 0) { dse_destroy(h); return rc; }
+    if (dse::batched_eligible(k)) {                       // 8 systems per warp on the fp64 tensor path
+        rc = dse::query_point_batched(k, h->cfg);
+        if (rc < 0) { dse_destroy(h); return rc; }
+    }
     k.W = h->cfg.grid * (h->cfg.block / 32);
-    k.upr = h->cfg.pipelined ? (k.Ntpad / 32) : 1;      // the pipelined kernel partitions 32-point batches
-    k.U = k.R * k.upr;
+    k.upr = (h->cfg.pipelined || h->cfg.batched) ? (k.Ntpad / 32) : 1;      // these kernels partition 32-point batches
+    k.bgroup = h->cfg.batched ? 8 : 1;
+    k.U = k.R / k.bgroup * k.upr;
 
     // ---- workspace (one allocation, zero-initialised: unwritten partial slots must read 0) ----
     const size_t n2 = 2 * (size_t)k.N;
@@ -211,7 +216,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     const size_t o_Gy = carve<double>(off, (size_t)k.B * k.Gext * k.Nr), o_Py = carve<double>(off, (size_t)k.B * k.Gext * k.Nr);
     const size_t o_iG = carve<double>(off, (size_t)k.B * k.N), o_iZ = carve<double>(off, (size_t)k.B * k.N);
     const size_t o_A = carve<double>(off, (size_t)k.R * 4), o_AH = carve<double>(off, (size_t)k.R * 4);
-    const size_t o_S = carve<double>(off, ((size_t)k.W + (size_t)k.B * k.Next) * 3 * k.Npad);
+    const size_t o_S = carve<double>(off, ((size_t)k.W * k.bgroup + (size_t)k.B * k.Next) * 3 * k.Npad);
     const size_t o_R = carve<double>(off, (size_t)k.B * k.Next * 3 * k.Npad);
     const size_t o_J = carve<double>(off, (size_t)k.B * n2 * n2), o_F = carve<double>(off, (size_t)k.B * n2);
     const size_t o_lu = carve<double>(off, (size_t)k.B * dse::lu_scratch_doubles((int)n2));
@@ -398,11 +403,12 @@ int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, doub
 
 int64_t dse_launch_count(const dse_handle *h) { return h ? h->launches : 0; }
 
-int dse_kernel_info(const dse_handle *h, int32_t out[6])
+int dse_kernel_info(const dse_handle *h, int32_t out[8])
 {
     if (!h || !out) return DSE_EINVAL;
     out[0] = h->cfg.grid; out[1] = h->cfg.block; out[2] = h->cfg.smem; out[3] = h->cfg.regs;
     out[4] = h->cfg.ctas_per_sm; out[5] = h->cfg.sms;
+    out[6] = h->cfg.batched ? 2 : (h->cfg.pipelined ? 1 : 0); out[7] = 0;
     return DSE_OK;
 }
 

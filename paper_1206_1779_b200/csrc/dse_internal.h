@@ -37,6 +37,7 @@ struct KParams {
     int W;                             // warps in the grid of the point kernel
     long long U;                       // partition units of the Jacobian build: rows (upr = 1) or 32-point batches
     int upr;                           // partition units per row
+    int bgroup;                        // systems per work unit: 8 with the batched DMMA point kernel, else 1
     int want_jac;                      // 0: residual only (skip phase 2)
     int use_constc;                    // coefficient pairs are read as constant-bank operands (single system, slot owner)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
@@ -59,6 +60,7 @@ struct PointKernelConfig {
     int grid, block, smem, regs, ctas_per_sm, sms;       // Jacobian build (defines KParams::W and the partial slots)
     int res_grid, res_block, res_smem;                   // residual-only build (no partials)
     int pipelined;                                       // Jacobian build uses the software-pipelined kernel
+    int batched;                                         // Jacobian build uses the batched DMMA kernel (8 systems per warp)
 };
 
 // launchers (dse_kernels.cu / dse_lu.cu); each returns the number of kernels launched or <0 on error
@@ -66,6 +68,10 @@ struct PointKernelConfig {
 int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c_dev, const double *bc_dev,
                  double *J_dev, double *F_dev, void *stream, void *ev0 = nullptr, void *ev1 = nullptr);
 int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream);
+// batched DMMA point kernel (dse_point_batched.cu): eligibility, launch configuration, launch
+bool batched_eligible(const KParams &k);
+int query_point_batched(const KParams &k, PointKernelConfig &cfg);
+int launch_point_batched(const KParams &k, const PointKernelConfig &cfg, void *stream);
 int launch_fd_perturb(int n2, int B, const double *c, double *c_tmp, int j, double sign, double eps_rel, void *stream);
 int launch_fd_column(int n2, int B, const double *c, const double *Fp, const double *Fm, double *J, int j, double eps_rel,
                      void *stream);

@@ -170,14 +170,19 @@ constexpr int ASM_THREADS = 512;
 __device__ __forceinline__ void reduce_part(const KParams &P, long long bi, int j, int part, int parts, double &Sa,
                                             double &Sb, double &Sv)
 {
-    const long long rf = bi * P.Nr * P.upr, rl = rf + (long long)P.Nr * P.upr - 1;     // first/last partition unit of bi
+    // P.bgroup systems share one work unit (batched DMMA kernel: 8, else 1): the partition runs over the group-level
+    // index big = (b / bgroup) * Next + e, and a slot holds bgroup partials
+    const long long b_sys = bi / P.Next, e = bi - b_sys * P.Next;
+    const long long big = (b_sys / P.bgroup) * P.Next + e;
+    const int m = (int)(b_sys % P.bgroup);
+    const long long rf = big * P.Nr * P.upr, rl = rf + (long long)P.Nr * P.upr - 1;     // first/last partition unit of big
     const long long wf = ((rf + 1) * P.W - 1) / P.U, wl = ((rl + 1) * P.W - 1) / P.U;
     const long long n = wl - wf + 1, per = (n + parts - 1) / parts;
     const long long w0 = wf + part * per, w1 = min(wl + 1, w0 + per);
     double a = 0.0, b = 0.0, v = 0.0;
 #pragma unroll 4
     for (long long w = w0; w < w1; ++w) {
-        const double *sp = P.Spart + (size_t)(w + bi) * 3 * P.Npad;
+        const double *sp = P.Spart + ((size_t)(w + big) * P.bgroup + m) * 3 * P.Npad;
         a += sp[j]; b += sp[P.Npad + j]; v += sp[2 * P.Npad + j];
     }
     Sa = a; Sb = b; Sv = v;

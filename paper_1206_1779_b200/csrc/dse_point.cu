@@ -699,6 +699,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     const void *fn = (const void *)pick(k, true);
     int block = POINT_THREADS, jsmem = smem;
     cfg.pipelined = 0;
+    cfg.batched = 0;
     KernelFn pf = (k.g == 32 && !getenv("DSE_NO_PIPE")) ? pick_pipe(k) : nullptr;
     if (pf) {
         const int psmem = (int)sizeof(double) * (k.Ntpad * 6 + (PIPE_THREADS / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
@@ -726,6 +727,7 @@ int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
     if (constc_of(k))
         cudaMemcpyToSymbolAsync(c_coef, k.coefP, sizeof(double2) * k.Npad, 0, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+    if (k.want_jac && cfg.batched) return launch_point_batched(k, cfg, stream);
     if (k.want_jac) {
         KernelFn fn = cfg.pipelined ? pick_pipe(k) : pick(k, true);
         fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);

@@ -114,6 +114,36 @@ def test_batched_systems(orc):
         check(J[b], F[b], Jo, Fo)
 
 
+@pytest.mark.parametrize("shape", [
+    dict(n_cheb=32, n_r=24, n_theta=64),                              # two angular batches per row
+    dict(n_cheb=27, n_r=9, n_theta=40, x_G=3.0, x_Z=5e3),             # padded j and theta, N_ext = N + 2
+    dict(n_cheb=30, n_r=8, n_theta=32, n_ir=6, radial_split=1, x_G=0.0),   # per-point rules, infrared piece, x_G = 0
+])
+def test_batched_tensor_path_every_system(orc, shape, monkeypatch):
+    """n_batch % 8 == 0 and N padded to 32: eight systems per warp on the fp64 tensor path (mma.sync m8n8k4).
+    Every system against the oracle, both geometry modes, and against the per-system kernel of the same library."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    kw = dict(eps2=1e-6, L2=5e4); kw.update(shape)
+    w = Workload("batched", **kw)
+    B = 16
+    c = np.stack([draw_coefficients(100 + b, w.n_cheb) for b in range(B)])
+    bc = np.stack([[0.5 + 0.05 * b, 1.2 + 0.03 * b] for b in range(B)])
+    d = Dse(params_from_workload(w, n_batch=B)); assert d.kernel_info()["variant"] == "batched-dmma"; d.close()
+    Js = []
+    for flags in (0, 1):
+        J, F = gpu_build(w, c, bc, flags)
+        Js.append(J)
+        for b in range(B):
+            Fo, Jo = orc.residual_jacobian(oracle_params(w), c[b], bc[b, 0], bc[b, 1])
+            check(J[b], F[b], Jo, Fo)
+    monkeypatch.setenv("DSE_NO_BATCHED", "1")
+    d = Dse(params_from_workload(w, n_batch=B)); assert d.kernel_info()["variant"] != "batched-dmma"; d.close()
+    J1, F1 = gpu_build(w, c, bc, 0)
+    assert np.linalg.norm(J1 - Js[0]) <= 1e-12 * np.linalg.norm(J1)
+
+
 def test_deterministic_bitwise():
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload

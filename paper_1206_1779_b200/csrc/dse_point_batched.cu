@@ -21,12 +21,16 @@ void set_error_text(const char *s);
 
 namespace {
 
-constexpr int BT_THREADS = 256;
+#ifndef DSE_BT_THREADS
+#define DSE_BT_THREADS 384
+#endif
+constexpr int BT_THREADS = DSE_BT_THREADS;
 constexpr int BT_NPAD = 32;                 // Chebyshev indices (padded)
 constexpr int BT_KS = BT_NPAD / 4;          // k-steps of step A
 constexpr int BT_NT = BT_NPAD / 8;          // n-tiles of step C
 constexpr int BT_TS = 36;                   // row stride of the T tile (conflict-free for both access patterns)
-constexpr int BT_WARP_DOUBLES = 8 * BT_TS + GBUF_DOUBLES;
+constexpr int BT_COEF_DOUBLES = 2 * BT_KS * 32;   // step-A B fragments of the warp's 8 systems, in fragment order
+constexpr int BT_WARP_DOUBLES = 8 * BT_TS + GBUF_DOUBLES + BT_COEF_DOUBLES;
 
 __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 {
@@ -43,6 +47,7 @@ __global__ void __launch_bounds__(BT_THREADS, 1) point_kernel_batched(const KPar
     double *s_ang = smem;
     double *sT = smem + (size_t)P.Ntpad * 6 + (size_t)warp * BT_WARP_DOUBLES;       // [8][BT_TS]
     double4 *s_gbuf = reinterpret_cast<double4 *>(sT + 8 * BT_TS);                  // [2][32] geometry records
+    double *sC = sT + 8 * BT_TS + GBUF_DOUBLES;                                     // [BT_KS][2][32] coefficient fragments
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
     __syncthreads();
 
@@ -75,15 +80,15 @@ __global__ void __launch_bounds__(BT_THREADS, 1) point_kernel_batched(const KPar
         prefetch(0);
     }
 
-    double cB0[BT_KS], cB1[BT_KS];                        // step-A B fragments: coefficients of the 8 systems
+    // step-A B fragments (coefficients of the 8 systems) live in shared memory, one value per (k-step, pair, lane)
     auto load_coef = [&](int g) {
         const int col = lane >> 2;                        // column of the n-tile: system col/2, part col%2 (a|b)
         const double *c0 = P.coefP + ((size_t)(8 * g + (col >> 1)) * BT_NPAD) * 2 + (col & 1);
         const double *c1 = P.coefP + ((size_t)(8 * g + 4 + (col >> 1)) * BT_NPAD) * 2 + (col & 1);
 #pragma unroll
         for (int ks = 0; ks < BT_KS; ++ks) {
-            cB0[ks] = c0[(size_t)(4 * ks + jq) * 2];
-            cB1[ks] = c1[(size_t)(4 * ks + jq) * 2];
+            sC[(2 * ks) * 32 + lane] = c0[(size_t)(4 * ks + jq) * 2];
+            sC[(2 * ks + 1) * 32 + lane] = c1[(size_t)(4 * ks + jq) * 2];
         }
     };
     load_coef(sg);
@@ -156,10 +161,17 @@ __global__ void __launch_bounds__(BT_THREADS, 1) point_kernel_batched(const KPar
                     for (int ks = 0; ks < BT_KS; ++ks) sT[pt_l * BT_TS + 4 * ks + jq] = Tv[ks];
                     // ---- step A: ln Z(z), ln G(z) of (point pt_l, systems jq and 4 + jq) ----
                     double lz0 = 0.0, lg0 = 0.0, lz1 = 0.0, lg1 = 0.0;
+                    {
+                        // four independent accumulator chains (even / odd k-steps) hide the DMMA latency
+                        double mz0 = 0.0, mg0 = 0.0, mz1 = 0.0, mg1 = 0.0;
 #pragma unroll
-                    for (int ks = 0; ks < BT_KS; ++ks) {
-                        dmma(lz0, lg0, Tv[ks], cB0[ks]);
-                        dmma(lz1, lg1, Tv[ks], cB1[ks]);
+                        for (int ks = 0; ks < BT_KS; ks += 2) {
+                            dmma(lz0, lg0, Tv[ks], sC[(2 * ks) * 32 + lane]);
+                            dmma(lz1, lg1, Tv[ks], sC[(2 * ks + 1) * 32 + lane]);
+                            dmma(mz0, mg0, Tv[ks + 1], sC[(2 * ks + 2) * 32 + lane]);
+                            dmma(mz1, mg1, Tv[ks + 1], sC[(2 * ks + 3) * 32 + lane]);
+                        }
+                        lz0 += mz0; lg0 += mg0; lz1 += mz1; lg1 += mg1;
                     }
                     // ---- step B: weights of the two (point, system) pairs ----
                     double U0[3], U1[3];

@@ -91,21 +91,28 @@ __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
 // 16 warps split K = N_r; each lane loads one 32-byte row-sum record (all three streams at once), so one
 // k-step feeds three MMAs; the 16 partial tiles are combined in warp order (deterministic).
 constexpr int GEMM_WARPS = 16;
+// NTG = n-tiles (8 values of j each) per CTA: 1 for a single system (most CTAs, shortest latency), 4 for batches
+// (every row-sum record is read once per 32 values of j instead of once per 8)
+template <int NTG>
 __global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
 {
     __shared__ double s_c[GEMM_WARPS][3][32][2];
-    const int lane = threadIdx.x & 31, wk = threadIdx.x >> 5;
-    const int e0 = blockIdx.x * 8, n0 = blockIdx.y * 8, b = blockIdx.z;
+    const int lane = threadIdx.x & 31, wk = threadIdx.x >> 5, nwarps = blockDim.x >> 5;   // 3 <= nwarps <= GEMM_WARPS
+    const int e0 = blockIdx.x * 8, n0 = blockIdx.y * 8 * NTG, b = blockIdx.z;
     const int ae = e0 + (lane >> 2), ak = lane & 3;          // A fragment: row = lane/4 (external point), col = lane%4 (q)
     const int bk = lane & 3, bn = n0 + (lane >> 2);          // B fragment: row = lane%4 (q), col = lane/4 (j)
     const bool arow_ok = ae < P.Next;
     const size_t rowbase = ((size_t)b * P.Next + (arow_ok ? ae : 0)) * P.Nr;
     const double4 *Arow = reinterpret_cast<const double4 *>(P.Apart) + rowbase;
     const double4 *Hrow = reinterpret_cast<const double4 *>(P.AHead) + rowbase;
-    const int ksteps = (P.Nr + 3) / 4, per = (ksteps + GEMM_WARPS - 1) / GEMM_WARPS;
+    const int ksteps = (P.Nr + 3) / 4, per = (ksteps + nwarps - 1) / nwarps;
     const int ks0 = wk * per, ks1 = min(ksteps, ks0 + per);
-    double c[3][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
-#pragma unroll 8
+    double c[NTG][3][2];
+#pragma unroll
+    for (int nt = 0; nt < NTG; ++nt)
+#pragma unroll
+        for (int st = 0; st < 3; ++st) c[nt][st][0] = c[nt][st][1] = 0.0;
+#pragma unroll(NTG == 1 ? 8 : 2)
     for (int ks = ks0; ks < ks1; ++ks) {
         const int qa = ks * 4 + ak, qb = ks * 4 + bk;
         double4 a = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -113,26 +120,33 @@ __global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
             const double4 a1 = Arow[qa], a2 = Hrow[qa];
             a = make_double4(a1.x + a2.x, a1.y + a2.y, a1.z + a2.z, 0.0);
         }
-        const double bb = (qb < P.Nr) ? P.phi_y[(size_t)qb * P.Npad + bn] : 0.0;
-        asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                     : "+d"(c[0][0]), "+d"(c[0][1]) : "d"(a.x), "d"(bb));
-        asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                     : "+d"(c[1][0]), "+d"(c[1][1]) : "d"(a.y), "d"(bb));
-        asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                     : "+d"(c[2][0]), "+d"(c[2][1]) : "d"(a.z), "d"(bb));
+#pragma unroll
+        for (int nt = 0; nt < NTG; ++nt) {
+            const double bb = (qb < P.Nr && bn + 8 * nt < P.Npad) ? P.phi_y[(size_t)qb * P.Npad + bn + 8 * nt] : 0.0;
+            asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(c[nt][0][0]), "+d"(c[nt][0][1]) : "d"(a.x), "d"(bb));
+            asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(c[nt][1][0]), "+d"(c[nt][1][1]) : "d"(a.y), "d"(bb));
+            asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(c[nt][2][0]), "+d"(c[nt][2][1]) : "d"(a.z), "d"(bb));
+        }
     }
 #pragma unroll
-    for (int st = 0; st < 3; ++st) { s_c[wk][st][lane][0] = c[st][0]; s_c[wk][st][lane][1] = c[st][1]; }
-    __syncthreads();
-    if (wk < 3) {                                            // warp st combines stream st
-        const int st = wk;
-        double r0 = 0.0, r1 = 0.0;
-        for (int w2 = 0; w2 < GEMM_WARPS; ++w2) { r0 += s_c[w2][st][lane][0]; r1 += s_c[w2][st][lane][1]; }
-        const int ce = e0 + (lane >> 2), cn = n0 + 2 * (lane & 3);     // C fragment: row = lane/4, cols 2(lane%4), +1
-        if (ce < P.Next) {
-            double *out = P.Rz + (((size_t)b * P.Next + ce) * 3 + st) * P.Npad;
-            out[cn] = r0;
-            out[cn + 1] = r1;
+    for (int nt = 0; nt < NTG; ++nt) {
+        if (nt > 0) __syncthreads();                         // the previous tile's partials have been combined
+#pragma unroll
+        for (int st = 0; st < 3; ++st) { s_c[wk][st][lane][0] = c[nt][st][0]; s_c[wk][st][lane][1] = c[nt][st][1]; }
+        __syncthreads();
+        if (wk < 3) {                                        // warp st combines stream st
+            const int st = wk;
+            double r0 = 0.0, r1 = 0.0;
+            for (int w2 = 0; w2 < nwarps; ++w2) { r0 += s_c[w2][st][lane][0]; r1 += s_c[w2][st][lane][1]; }
+            const int ce = e0 + (lane >> 2), cn = n0 + 8 * nt + 2 * (lane & 3);     // C fragment: row = lane/4, cols 2(lane%4), +1
+            if (ce < P.Next && cn < P.Npad) {
+                double *out = P.Rz + (((size_t)b * P.Next + ce) * 3 + st) * P.Npad;
+                out[cn] = r0;
+                out[cn + 1] = r1;
+            }
         }
     }
 }
@@ -192,7 +206,7 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
                                 double *__restrict__ F)
 {
     const int i = blockIdx.x, b = blockIdx.y;
-    const int N = P.N;
+    const int N = P.N, nthr = blockDim.x;      // 128 <= nthr <= ASM_THREADS, a multiple of 32 and of PJ
     const long long bi_i = (long long)b * P.Next + i, bi_Z = (long long)b * P.Next + P.iZ,
                     bi_G = (long long)b * P.Next + P.iG;
     __shared__ double s_pi[3][2];
@@ -203,7 +217,7 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
         for (int pt = 0; pt < npi; ++pt) {
             const long long bi = pt == 0 ? bi_i : (pt == 1 ? bi_Z : bi_G);
             double pg = 0.0, pz = 0.0;
-            for (int q = threadIdx.x; q < P.Nr; q += ASM_THREADS) {
+            for (int q = threadIdx.x; q < P.Nr; q += nthr) {
                 const double4 a = reinterpret_cast<const double4 *>(P.Apart)[(size_t)bi * P.Nr + q];
                 const double4 hh = reinterpret_cast<const double4 *>(P.AHead)[(size_t)bi * P.Nr + q];
                 pg += a.z + hh.z; pz += a.w + hh.w;
@@ -218,7 +232,7 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
         if (threadIdx.x < 2 * npi) {
             const int pt = threadIdx.x >> 1, cmp = threadIdx.x & 1;
             double t = 0.0;
-            for (int w2 = 0; w2 < ASM_THREADS / 32; ++w2) t += s_pw[w2][pt][cmp];
+            for (int w2 = 0; w2 < nthr / 32; ++w2) t += s_pw[w2][pt][cmp];
             s_pi[pt][cmp] = t;
         }
         __syncthreads();
@@ -236,7 +250,7 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
     __shared__ double s_part[3][3][ASM_THREADS];
     int PJ = 8;
     while (PJ < N) PJ <<= 1;
-    const int parts = ASM_THREADS / PJ, part = threadIdx.x / PJ, j = threadIdx.x - part * PJ;
+    const int parts = nthr / PJ, part = threadIdx.x / PJ, j = threadIdx.x - part * PJ;
     const int npt = (P.iG != P.iZ) ? 3 : 2;
     if (j < N) {
         for (int pt = 0; pt < npt; ++pt) {
@@ -367,13 +381,21 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
         if (kk.rstride) {
             contract_split_kernel<<<dim3(kk.Next, kk.B), 128, 0, s>>>(kk);
         } else {
-            dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);
-            gemm_kernel<<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
+            // one system: one n-tile per CTA, K split over 16 warps (latency); many systems: 4 n-tiles per CTA and
+            // 4 warps, the grid fills the GPU and every row-sum record is read once per 32 values of j
+            if (kk.B >= 8) {
+                dim3 gg((kk.Next + 7) / 8, (kk.Npad / 8 + 3) / 4, kk.B);
+                gemm_kernel<4><<<gg, 4 * 32, 0, s>>>(kk);
+            } else {
+                dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);
+                gemm_kernel<1><<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
+            }
         }
         ++launches;
     }
     dim3 ga(kk.N, kk.B);
-    assemble_kernel<<<ga, ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
+    // many systems: few slots per external point, small CTAs keep more of them resident
+    assemble_kernel<<<ga, kk.B >= 8 ? 128 : ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
     ++launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "build launch");

@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -198,6 +199,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     // ---- launch configuration of the point kernel ----
     k.use_constc = dse::acquire_const_slot(k) ? 1 : 0;
     h->owns_const = k.use_constc != 0;
+    k.coefC = (k.use_constc && !getenv("DSE_CONST_MEMCPY")) ? dse::const_slot_address() : nullptr;
     rc = dse::query_point_kernel(k, h->cfg);
     if (rc < 0) { dse_destroy(h); return rc; }
     if (dse::batched_eligible(k)) {                       // 8 systems per warp on the fp64 tensor path

@@ -40,6 +40,7 @@ struct KParams {
     int bgroup;                        // systems per work unit: 8 with the batched DMMA point kernel, else 1
     int want_jac;                      // 0: residual only (skip phase 2)
     int use_constc;                    // coefficient pairs are read as constant-bank operands (single system, slot owner)
+    double *coefC;                     // global address of the constant-bank slot (prep_kernel writes it), or nullptr
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
     const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x, *EGy, *EZy;
     const double *geom;                // geometry cache [Next*Nr*Ntpad][4] or nullptr
@@ -76,10 +77,14 @@ int launch_fd_perturb(int n2, int B, const double *c, double *c_tmp, int j, doub
 int launch_fd_column(int n2, int B, const double *c, const double *Fp, const double *Fm, double *J, int j, double eps_rel,
                      void *stream);
 int launch_geometry(const KParams &k, double *geom, void *stream);
+bool lu_reg_eligible(int n);      // 2N <= 128: register-resident LU (dse_lu_reg.cu)
+int launch_lu_reg(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
+                  double *stats, void *stream);
 int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
               double *stats, double *scratch, void *stream);
 int query_point_kernel(const KParams &k, PointKernelConfig &cfg);
 bool acquire_const_slot(const KParams &k);
+double *const_slot_address();     // global-memory address of the slot (nullptr if unavailable)
 void release_const_slot();
 size_t lu_scratch_doubles(int n);
 int launch_gauss_legendre(int n, double *x, double *w, double *work, void *stream);

@@ -5,10 +5,12 @@
 //   point_kernel    H2-H6 (the hot kernel): every quadrature point (x_e, y_q, theta_k)
 //   gemm_kernel     H7  the only dense contraction, A[e,q] . phi_j(t_q), on the fp64 tensor path (DMMA)
 //   assemble_kernel H8  fixed-order reduction of the per-warp partials, subtraction rows, local terms
+//                       (small single-system builds: H7 runs inside the assemble CTAs, also as DMMA)
 // Equation numbers refer to PAPER.md (arXiv:1206.1779); see include/dse.h and DESIGN.md.
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 
 #include "dse_device.cuh"
 
@@ -33,6 +35,7 @@ __global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double
             if (j == 0) { a *= 0.5; bb *= 0.5; }
             P.coefP[((size_t)b * P.Npad + j) * 2 + 0] = a;
             P.coefP[((size_t)b * P.Npad + j) * 2 + 1] = bb;
+            if (P.coefC) { P.coefC[2 * j] = a; P.coefC[2 * j + 1] = bb; }      // constant-bank slot (single system)
         }
     }
     const int NG = P.Gext * P.Nr;                        // fixed points y_{e,q} (split rule) or y_q (shared rule)
@@ -202,8 +205,12 @@ __device__ __forceinline__ void reduce_part(const KParams &P, long long bi, int 
     Sa = a; Sb = b; Sv = v;
 }
 
-__global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, double *__restrict__ J,
-                                double *__restrict__ F)
+// FUSED (few systems, shared radial rule): the CTA also computes the z-independent rows it needs, H7, itself --
+// six rows (R_a, R_b, R_v at x_i; R_a, R_b at x_Z; R_v at x_G) fill one 8-row DMMA tile, the warps split (j-tile,
+// K = N_r); no separate gemm launch.  Not FUSED: the rows come from Rz (gemm_kernel / contract_split_kernel).
+template <bool FUSED>
+__global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, const double *__restrict__ bc,
+                                                               double *__restrict__ J, double *__restrict__ F)
 {
     const int i = blockIdx.x, b = blockIdx.y;
     const int N = P.N, nthr = blockDim.x;      // 128 <= nthr <= ASM_THREADS, a multiple of 32 and of PJ
@@ -260,6 +267,53 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
             s_part[pt][0][threadIdx.x] = a; s_part[pt][1][threadIdx.x] = bb; s_part[pt][2][threadIdx.x] = v;
         }
     }
+    __shared__ double s_R[FUSED ? 6 * 128 : 1];                   // [kp][6 rows][Npad], KP * Npad <= 128
+    int KP = 1;
+    if (FUSED) {
+        const int NT = P.Npad >> 3, nw = nthr >> 5;
+        KP = nw / NT > 1 ? nw / NT : 1;
+        const int ksteps = (P.Nr + 3) >> 2, per = (ksteps + KP - 1) / KP;
+        const int row = lane >> 2;                               // A fragment: row = lane/4, col (q) = lane%4
+        const long long bi_r = row < 3 ? bi_i : (row < 5 ? bi_Z : bi_G);
+        const int comp = row < 3 ? row : (row < 5 ? row - 3 : 2);
+        const double *Ar = P.Apart + (size_t)bi_r * P.Nr * 4 + comp, *Hr = P.AHead + (size_t)bi_r * P.Nr * 4 + comp;
+        for (int item = warp; item < NT * KP; item += nw) {
+            const int nt = item % NT, kp = item / NT;
+            const int ks0 = kp * per, ks1 = min(ksteps, ks0 + per);
+            const double *Bp = P.phi_y + 8 * nt + (lane >> 2);   // B fragment: row (q) = lane%4, col (j) = lane/4
+            double c[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};      // four chains hide the DMMA latency
+            const double amask = row < 6 ? 1.0 : 0.0;            // rows 6, 7 of the tile are padding
+            const double *Aq = row < 6 ? Ar : P.Apart, *Hq = row < 6 ? Hr : P.AHead;
+            const int ksf = min(ks1, P.Nr >> 2);                 // k-steps whose four q are all in range
+            int ks = ks0;
+            for (; ks + 8 <= ksf; ks += 8) {                     // 24 independent loads in flight, then 8 MMAs
+                double av[8], hv[8], bv[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const size_t q = (size_t)(4 * (ks + u) + (lane & 3));
+                    av[u] = Aq[q * 4]; hv[u] = Hq[q * 4]; bv[u] = Bp[q * P.Npad];
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                        : "+d"(c[u & 3][0]), "+d"(c[u & 3][1]) : "d"((av[u] + hv[u]) * amask), "d"(bv[u]));
+            }
+            for (; ks < ks1; ++ks) {                             // ragged tail
+                const int q = 4 * ks + (lane & 3);
+                const bool ok = q < P.Nr;
+                const size_t qq = ok ? q : 0;
+                const double a = ok ? (Aq[qq * 4] + Hq[qq * 4]) * amask : 0.0;
+                const double bb = ok ? Bp[qq * P.Npad] : 0.0;
+                asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                    : "+d"(c[ks & 3][0]), "+d"(c[ks & 3][1]) : "d"(a), "d"(bb));
+            }
+            if (row < 6) {                                       // C fragment: row = lane/4, cols 2 (lane%4), +1
+                double *o = s_R + (size_t)(kp * 6 + row) * P.Npad + 8 * nt + 2 * (lane & 3);
+                o[0] = (c[0][0] + c[1][0]) + (c[2][0] + c[3][0]);
+                o[1] = (c[0][1] + c[1][1]) + (c[2][1] + c[3][1]);
+            }
+        }
+    }
     __syncthreads();
     if (part == 0 && j < N) {
         double S[3][3];
@@ -270,13 +324,25 @@ __global__ void assemble_kernel(const KParams P, const double *__restrict__ bc, 
                 S[pt][st] = (j == 0) ? 0.5 * t : t;       // the kernel accumulates with T_0 = 1; phi_0 = 1/2
             }
         if (npt == 2) { S[2][0] = S[1][0]; S[2][1] = S[1][1]; S[2][2] = S[1][2]; }
-        const double *Ri = P.Rz + (size_t)bi_i * 3 * P.Npad, *RZ = P.Rz + (size_t)bi_Z * 3 * P.Npad,
-                     *RG = P.Rz + (size_t)bi_G * 3 * P.Npad;
+        double R[6];                                             // R_a, R_b, R_v at x_i; R_a, R_b at x_Z; R_v at x_G
+        if (FUSED) {
+#pragma unroll
+            for (int r = 0; r < 6; ++r) {
+                double t = 0.0;
+                for (int kp = 0; kp < KP; ++kp) t += s_R[(size_t)(kp * 6 + r) * P.Npad + j];
+                R[r] = t;
+            }
+        } else {
+            const double *Ri = P.Rz + (size_t)bi_i * 3 * P.Npad, *RZ = P.Rz + (size_t)bi_Z * 3 * P.Npad,
+                         *RG = P.Rz + (size_t)bi_G * 3 * P.Npad;
+            R[0] = Ri[j]; R[1] = Ri[P.Npad + j]; R[2] = Ri[2 * P.Npad + j];
+            R[3] = RZ[j]; R[4] = RZ[P.Npad + j]; R[5] = RG[2 * P.Npad + j];
+        }
         const double phi = P.phi_x[(size_t)i * P.Npad + j];
         // dPi_Z/da = Sa + Ra, dPi_Z/db = Sb + Rb, dPi_G/da = Sv, dPi_G/db = Rv
-        const double dZa_i = S[0][0] + Ri[j], dZb_i = S[0][1] + Ri[P.Npad + j], dGa_i = S[0][2], dGb_i = Ri[2 * P.Npad + j];
-        const double dZa_s = S[1][0] + RZ[j], dZb_s = S[1][1] + RZ[P.Npad + j];
-        const double dGa_s = S[2][2], dGb_s = RG[2 * P.Npad + j];
+        const double dZa_i = S[0][0] + R[0], dZb_i = S[0][1] + R[1], dGa_i = S[0][2], dGb_i = R[2];
+        const double dZa_s = S[1][0] + R[3], dZb_s = S[1][1] + R[4];
+        const double dGa_s = S[2][2], dGb_s = R[5];
         double *Jb = J + (size_t)b * 4 * N * N;
         Jb[(size_t)i * 2 * N + j] = -phi * invZ - dZa_i + dZa_s;
         Jb[(size_t)i * 2 * N + N + j] = -dZb_i + dZb_s;
@@ -377,25 +443,30 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     launch_point(kk, cfg, stream);
     if (ev1) cudaEventRecord((cudaEvent_t)ev1, s);
     ++launches;
-    if (kk.want_jac) {
+    // few systems, shared radial rule, small Phi table: H7 is fused into the assemble CTAs (one launch less on the
+    // latency path: -3 us per build at cfg 0/1); large tables keep the separate gemm (every fused CTA would stream
+    // the whole N_r x N table: +15 us at cfg 3)
+    const bool fused = kk.want_jac && !kk.rstride && kk.B < 8 && (long long)kk.Nr * kk.Npad <= 16384 &&
+                       !getenv("DSE_NO_FUSED_ASSEMBLE");
+    if (kk.want_jac && !fused) {
         if (kk.rstride) {
             contract_split_kernel<<<dim3(kk.Next, kk.B), 128, 0, s>>>(kk);
+        } else if (kk.B >= 8) {
+            // many systems: 4 n-tiles per CTA and 4 warps, the grid fills the GPU and every row-sum record is read
+            // once per 32 values of j
+            dim3 gg((kk.Next + 7) / 8, (kk.Npad / 8 + 3) / 4, kk.B);
+            gemm_kernel<4><<<gg, 4 * 32, 0, s>>>(kk);
         } else {
-            // one system: one n-tile per CTA, K split over 16 warps (latency); many systems: 4 n-tiles per CTA and
-            // 4 warps, the grid fills the GPU and every row-sum record is read once per 32 values of j
-            if (kk.B >= 8) {
-                dim3 gg((kk.Next + 7) / 8, (kk.Npad / 8 + 3) / 4, kk.B);
-                gemm_kernel<4><<<gg, 4 * 32, 0, s>>>(kk);
-            } else {
-                dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);
-                gemm_kernel<1><<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
-            }
+            dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);        // one n-tile per CTA, K split over 16 warps (latency)
+            gemm_kernel<1><<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
         }
         ++launches;
     }
     dim3 ga(kk.N, kk.B);
-    // many systems: few slots per external point, small CTAs keep more of them resident
-    assemble_kernel<<<ga, kk.B >= 8 ? 128 : ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
+    if (fused)
+        assemble_kernel<true><<<ga, ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
+    else    // many systems: few slots per external point, small CTAs keep more of them resident
+        assemble_kernel<false><<<ga, kk.B >= 8 ? 128 : ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
     ++launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "build launch");

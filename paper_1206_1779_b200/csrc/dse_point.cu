@@ -625,6 +625,14 @@ bool acquire_const_slot(const KParams &k)
     return g_const_owner.compare_exchange_strong(expected, 1);
 }
 void release_const_slot() { g_const_owner.store(0); }
+// prep_kernel stores the coefficient pairs through this address; the constant caches are invalidated at every
+// kernel launch, so the point kernel that follows on the same stream reads the new values from the constant bank
+double *const_slot_address()
+{
+    void *p = nullptr;
+    if (cudaGetSymbolAddress(&p, c_coef) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return static_cast<double *>(p);
+}
 
 static KernelFn pick_pipe(const KParams &k)
 {
@@ -725,7 +733,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
 
 int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
-    if (constc_of(k))
+    if (constc_of(k) && !k.coefC)                              // fallback: in-stream copy of the pairs into the slot
         cudaMemcpyToSymbolAsync(c_coef, k.coefP, sizeof(double2) * k.Npad, 0, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
     if (k.want_jac && cfg.batched) return launch_point_batched(k, cfg, stream);
     if (k.want_jac) {

@@ -25,6 +25,20 @@ def test_lu_solve_matches_oracle(orc):
             assert rc == 0
             assert np.allclose(x[s], xo, rtol=1e-9, atol=1e-13 * np.abs(xo).max())
             assert np.allclose(st[s], so, rtol=1e-9)
+            # the factorisation itself (scaling, pivot choice, multipliers, unfused updates) is bit-identical to the
+            # plain C elimination: max|F| scaled, smallest pivot and growth factor agree exactly
+            assert np.array_equal(st[s][1:], so[1:]), (n, st[s], so)
+    # frequent ties in the pivot search (small integer entries): the first maximal element must win, as in the plain loop
+    for n in (24, 64, 100):
+        A = rng.integers(-3, 4, size=(2, n, n)).astype(np.float64) + 7.0 * np.eye(n)
+        b = rng.integers(-5, 6, size=(2, n)).astype(np.float64)
+        x, st = d.lu_solve(torch.from_numpy(A).cuda(), torch.from_numpy(b).cuda())
+        x = x.cpu().numpy(); st = st.cpu().numpy()
+        for s in range(2):
+            xo, so, rc = orc.lu_solve(A[s], b[s])
+            assert rc == 0
+            assert np.allclose(x[s], xo, rtol=1e-9, atol=1e-13 * np.abs(xo).max())
+            assert np.array_equal(st[s][1:], so[1:]), (n, st[s], so)
     d.close()
 
 

@@ -156,7 +156,7 @@ def test_deterministic_bitwise():
     for _ in range(5):
         J, F = d.jacobian(ct, bt)
         assert torch.equal(J, J0) and torch.equal(F, F0)
-    assert d.launch_count() == 6 * 4
+    assert d.launch_count() == 6 * 3      # cfg 1: prep, point, assemble (H7 fused into it) per build
     d.close()
 
 

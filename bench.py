@@ -253,7 +253,7 @@ def run_ours(args, w, c, bc):
         tpath = os.path.join(ROOT, "profiles", "point_kernel_traffic.txt")
         if os.path.exists(tpath):
             try:
-                traffic = json.load(open(tpath)).get(w.name)
+                traffic = json.load(open(tpath)).get(w.name) if args.geometry_cache else None   # captured with the cache on
             except Exception:
                 traffic = None
         line = {

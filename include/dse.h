@@ -144,8 +144,8 @@ DSE_API int64_t dse_launch_count(const dse_handle *h);
 /* Configuration of the dominant kernel, for reporting: out[0] = grid, out[1] = block,
  * out[2] = dynamic shared memory bytes, out[3] = registers/thread, out[4] = resident CTAs/SM,
  * out[5] = SM count, out[6] = variant of the Jacobian point kernel (0 generic, 1 software-pipelined,
- * 2 batched: 8 systems per warp on the fp64 tensor path, chosen when n_batch % 8 == 0, 25 <= n_cheb <= 32 and
- * n_theta >= 32), out[7] = reserved (0). */
+ * 2 batched: 8 systems per warp on the fp64 tensor path, chosen when n_batch >= 8 (padded to a multiple of 8 with
+ * idle systems, at most a quarter of the padded batch), n_cheb <= 64 and n_theta >= 32), out[7] = reserved (0). */
 DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[8]);
 
 /* Per-kernel device timing of the dominant (point) kernel, for the roofline report: while enabled,

@@ -209,16 +209,20 @@ int dse_create(const dse_params *params, dse_handle **out)
     k.W = h->cfg.grid * (h->cfg.block / 32);
     k.upr = (h->cfg.pipelined || h->cfg.batched) ? (k.Ntpad / 32) : 1;      // these kernels partition 32-point batches
     k.bgroup = h->cfg.batched ? 8 : 1;
-    k.U = k.R / k.bgroup * k.upr;
+    // the batched kernel works on groups of 8 systems: the batch is padded with idle systems (zero coefficients, zero
+    // weights) whose rows exist in the workspace but are never read by the later kernels
+    const size_t Bpad = h->cfg.batched ? ((size_t)k.B + 7) / 8 * 8 : (size_t)k.B;
+    const size_t Rpad = Bpad * k.Next * k.Nr;
+    k.U = (long long)(Rpad / k.bgroup) * k.upr;
 
     // ---- workspace (one allocation, zero-initialised: unwritten partial slots must read 0) ----
     const size_t n2 = 2 * (size_t)k.N;
     off = 0;
-    const size_t o_coef = carve<double>(off, (size_t)k.B * k.Npad * 2);
-    const size_t o_Gy = carve<double>(off, (size_t)k.B * k.Gext * k.Nr), o_Py = carve<double>(off, (size_t)k.B * k.Gext * k.Nr);
+    const size_t o_coef = carve<double>(off, Bpad * k.Npad * 2);
+    const size_t o_Gy = carve<double>(off, Bpad * k.Gext * k.Nr), o_Py = carve<double>(off, Bpad * k.Gext * k.Nr);
     const size_t o_iG = carve<double>(off, (size_t)k.B * k.N), o_iZ = carve<double>(off, (size_t)k.B * k.N);
-    const size_t o_A = carve<double>(off, (size_t)k.R * 4), o_AH = carve<double>(off, (size_t)k.R * 4);
-    const size_t o_S = carve<double>(off, ((size_t)k.W * k.bgroup + (size_t)k.B * k.Next) * 3 * k.Npad);
+    const size_t o_A = carve<double>(off, Rpad * 4), o_AH = carve<double>(off, Rpad * 4);
+    const size_t o_S = carve<double>(off, ((size_t)k.W * k.bgroup + Bpad * k.Next) * 3 * k.Npad);
     const size_t o_R = carve<double>(off, (size_t)k.B * k.Next * 3 * k.Npad);
     const size_t o_J = carve<double>(off, (size_t)k.B * n2 * n2), o_F = carve<double>(off, (size_t)k.B * n2);
     const size_t o_lu = carve<double>(off, (size_t)k.B * dse::lu_scratch_doubles((int)n2));

@@ -9,7 +9,8 @@
 // fragments of step A hand every lane ln Z(z), ln G(z) of two (point, system) pairs -> 3 exp and the weights there;
 // the weights are transposed into A fragments with shuffles.  Partials per (warp, system group, external point) are
 // written straight from the accumulator fragments; assemble_kernel sums them in warp order (deterministic).
-// Requirements: n_batch % 8 == 0, N padded to 32, full-warp angular batches; other shapes use dse_point.cu.
+// Requirements: n_batch >= 8 (padded to a multiple of 8 with idle systems, at most a quarter of the padded batch),
+// N <= 64 (tiles of 16, 32, 48 or 64 indices), full-warp angular batches; other shapes use dse_point.cu.
 #include <cstdio>
 #include <cstdlib>
 
@@ -21,16 +22,15 @@ void set_error_text(const char *s);
 
 namespace {
 
-#ifndef DSE_BT_THREADS
-#define DSE_BT_THREADS 384
-#endif
-constexpr int BT_THREADS = DSE_BT_THREADS;
-constexpr int BT_NPAD = 32;                 // Chebyshev indices (padded)
-constexpr int BT_KS = BT_NPAD / 4;          // k-steps of step A
-constexpr int BT_NT = BT_NPAD / 8;          // n-tiles of step C
-constexpr int BT_TS = 36;                   // row stride of the T tile (conflict-free for both access patterns)
-constexpr int BT_COEF_DOUBLES = 2 * BT_KS * 32;   // step-A B fragments of the warp's 8 systems, in fragment order
-constexpr int BT_WARP_DOUBLES = 8 * BT_TS + GBUF_DOUBLES + BT_COEF_DOUBLES;
+// NPADB = N padded to a multiple of 16 (16, 32, 48 or 64): Chebyshev extent of the tiles
+template <int NPADB> struct BT {
+    static constexpr int THREADS = NPADB <= 32 ? 384 : 256;      // 12 or 8 warps per SM (register budget)
+    static constexpr int KS = NPADB / 4;                         // k-steps of step A
+    static constexpr int NT = NPADB / 8;                         // n-tiles of step C
+    static constexpr int TS = NPADB + 4;                         // row stride of the T tile: = 4 (mod 16), conflict-free
+    static constexpr int COEF_DOUBLES = 2 * KS * 32;             // step-A B fragments of the warp's 8 systems
+    static constexpr int WARP_DOUBLES = 8 * TS + GBUF_DOUBLES + COEF_DOUBLES;
+};
 
 __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 {
@@ -39,9 +39,10 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
         : "d"(a), "d"(b));
 }
 
-template <bool GEOM>
-__global__ void __launch_bounds__(BT_THREADS, 1) point_kernel_batched(const KParams P)
+template <bool GEOM, int NPADB>
+__global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(const KParams P)
 {
+    constexpr int BT_KS = BT<NPADB>::KS, BT_NT = BT<NPADB>::NT, BT_TS = BT<NPADB>::TS, BT_WARP_DOUBLES = BT<NPADB>::WARP_DOUBLES;
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
     double *s_ang = smem;
@@ -83,12 +84,13 @@ __global__ void __launch_bounds__(BT_THREADS, 1) point_kernel_batched(const KPar
     // step-A B fragments (coefficients of the 8 systems) live in shared memory, one value per (k-step, pair, lane)
     auto load_coef = [&](int g) {
         const int col = lane >> 2;                        // column of the n-tile: system col/2, part col%2 (a|b)
-        const double *c0 = P.coefP + ((size_t)(8 * g + (col >> 1)) * BT_NPAD) * 2 + (col & 1);
-        const double *c1 = P.coefP + ((size_t)(8 * g + 4 + (col >> 1)) * BT_NPAD) * 2 + (col & 1);
+        const double *c0 = P.coefP + ((size_t)(8 * g + (col >> 1)) * P.Npad) * 2 + (col & 1);
+        const double *c1 = P.coefP + ((size_t)(8 * g + 4 + (col >> 1)) * P.Npad) * 2 + (col & 1);
 #pragma unroll
         for (int ks = 0; ks < BT_KS; ++ks) {
-            sC[(2 * ks) * 32 + lane] = c0[(size_t)(4 * ks + jq) * 2];
-            sC[(2 * ks + 1) * 32 + lane] = c1[(size_t)(4 * ks + jq) * 2];
+            const bool in = 4 * ks + jq < P.Npad;           // NPADB may exceed the library's padding (multiple of 8)
+            sC[(2 * ks) * 32 + lane] = in ? c0[(size_t)(4 * ks + jq) * 2] : 0.0;
+            sC[(2 * ks + 1) * 32 + lane] = in ? c1[(size_t)(4 * ks + jq) * 2] : 0.0;
         }
     };
     load_coef(sg);
@@ -249,8 +251,8 @@ __global__ void __launch_bounds__(BT_THREADS, 1) point_kernel_batched(const KPar
             for (int st = 0; st < 3; ++st)
 #pragma unroll
                 for (int nt = 0; nt < BT_NT; ++nt) {
-                    double *dst = P.Spart + ((slot * 8 + sys) * 3 + st) * BT_NPAD + 8 * nt + 2 * jq;
-                    *reinterpret_cast<double2 *>(dst) = make_double2(acc[st][nt][0], acc[st][nt][1]);
+                    double *dst = P.Spart + ((slot * 8 + sys) * 3 + st) * P.Npad + 8 * nt + 2 * jq;
+                    if (8 * nt < P.Npad) *reinterpret_cast<double2 *>(dst) = make_double2(acc[st][nt][0], acc[st][nt][1]);
                 }
         }
         if (q >= Nr) {
@@ -274,39 +276,65 @@ int fail(cudaError_t e, const char *what)
 
 }  // namespace
 
+// 8 systems per warp: at least 8 systems, at most a quarter of the padded batch wasted, N <= 64, full-warp angular batches
 bool batched_eligible(const KParams &k)
 {
-    return k.B >= 8 && k.B % 8 == 0 && k.Npad == BT_NPAD && k.g == 32 && !getenv("DSE_NO_BATCHED");
+    const int Bpad = (k.B + 7) / 8 * 8;
+    return k.B >= 8 && 4 * (Bpad - k.B) <= Bpad && k.Npad <= 64 && k.g == 32 && !getenv("DSE_NO_BATCHED");
 }
+
+namespace {
+using BatchedFn = void (*)(const KParams);
+template <int NPADB> BatchedFn pick_batched(bool geom)
+{
+    return geom ? point_kernel_batched<true, NPADB> : point_kernel_batched<false, NPADB>;
+}
+struct BatchedVariant { BatchedFn fn; int threads, smem; };
+BatchedVariant batched_variant(const KParams &k)
+{
+    const bool g = k.geom != nullptr;
+    const int base = (int)sizeof(double) * k.Ntpad * 6;
+#define DSE_BT_CASE(NPADB) \
+    return BatchedVariant{pick_batched<NPADB>(g), BT<NPADB>::THREADS, \
+                          base + (int)sizeof(double) * (BT<NPADB>::THREADS / 32) * BT<NPADB>::WARP_DOUBLES}
+    if (k.Npad <= 16) DSE_BT_CASE(16);
+    if (k.Npad <= 32) DSE_BT_CASE(32);
+    if (k.Npad <= 48) DSE_BT_CASE(48);
+    DSE_BT_CASE(64);
+#undef DSE_BT_CASE
+}
+}  // namespace
 
 int query_point_batched(const KParams &k, PointKernelConfig &cfg)
 {
-    const void *fn = k.geom ? (const void *)point_kernel_batched<true> : (const void *)point_kernel_batched<false>;
-    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (BT_THREADS / 32) * BT_WARP_DOUBLES);
+    const BatchedVariant v = batched_variant(k);
+    const void *fn = (const void *)v.fn;
+    const int smem = v.smem;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel_batched)");
     cudaFuncAttributes fa;
     e = cudaFuncGetAttributes(&fa, fn);
     if (e != cudaSuccess) return fail(e, "cudaFuncGetAttributes");
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, BT_THREADS, smem);
-    if (e != cudaSuccess || per_sm < 1) return fail(e, "occupancy(point_kernel_batched)");
-    const long long wpb = BT_THREADS / 32, bpr = k.Ntpad / 32;
-    const long long units = k.R / 8 * bpr, min_units = bpr > 4 ? bpr : 4;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, v.threads, smem);
+    if (e != cudaSuccess) return fail(e, "occupancy(point_kernel_batched)");
+    if (per_sm < 1) { set_error_text("point_kernel_batched does not fit on an SM"); return DSE_ECUDA; }
+    const long long wpb = v.threads / 32, bpr = k.Ntpad / 32;
+    const long long groups = (k.B + 7) / 8;
+    const long long units = groups * k.Next * k.Nr * bpr, min_units = bpr > 4 ? bpr : 4;
     long long grid = (long long)cfg.sms * per_sm;
     long long want = (units / min_units + wpb - 1) / wpb;
     if (want < 1) want = 1;
     if (want < grid) grid = want;
     while (grid > 1 && units / (grid * wpb) < min_units) --grid;
-    cfg.grid = (int)grid; cfg.block = BT_THREADS; cfg.smem = smem; cfg.regs = fa.numRegs; cfg.ctas_per_sm = per_sm;
+    cfg.grid = (int)grid; cfg.block = v.threads; cfg.smem = smem; cfg.regs = fa.numRegs; cfg.ctas_per_sm = per_sm;
     cfg.pipelined = 0; cfg.batched = 1;
     return 0;
 }
 
 int launch_point_batched(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
-    if (k.geom) point_kernel_batched<true><<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
-    else point_kernel_batched<false><<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
+    batched_variant(k).fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
     return 1;
 }
 

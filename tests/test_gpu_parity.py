@@ -114,20 +114,22 @@ def test_batched_systems(orc):
         check(J[b], F[b], Jo, Fo)
 
 
-@pytest.mark.parametrize("shape", [
-    dict(n_cheb=32, n_r=24, n_theta=64),                              # two angular batches per row
-    dict(n_cheb=27, n_r=9, n_theta=40, x_G=3.0, x_Z=5e3),             # padded j and theta, N_ext = N + 2
-    dict(n_cheb=30, n_r=8, n_theta=32, n_ir=6, radial_split=1, x_G=0.0),   # per-point rules, infrared piece, x_G = 0
+@pytest.mark.parametrize("shape,B", [
+    (dict(n_cheb=32, n_r=24, n_theta=64), 16),                              # two angular batches per row
+    (dict(n_cheb=27, n_r=9, n_theta=40, x_G=3.0, x_Z=5e3), 16),             # padded j and theta, N_ext = N + 2
+    (dict(n_cheb=30, n_r=8, n_theta=32, n_ir=6, radial_split=1, x_G=0.0), 16),   # per-point rules, infrared piece, x_G = 0
+    (dict(n_cheb=12, n_r=10, n_theta=32), 13),                              # 16-index tiles; batch padded 13 -> 16
+    (dict(n_cheb=36, n_r=8, n_theta=64), 8),                                # the paper's N = 36: 48-index tiles, N_pad = 40
+    (dict(n_cheb=60, n_r=6, n_theta=32), 14),                               # the paper's N = 60: 64-index tiles, 14 -> 16
 ])
-def test_batched_tensor_path_every_system(orc, shape, monkeypatch):
-    """n_batch % 8 == 0 and N padded to 32: eight systems per warp on the fp64 tensor path (mma.sync m8n8k4).
+def test_batched_tensor_path_every_system(orc, shape, B, monkeypatch):
+    """n_batch >= 8 and N <= 64: eight systems per warp on the fp64 tensor path (mma.sync m8n8k4).
     Every system against the oracle, both geometry modes, and against the per-system kernel of the same library."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
     from paper_1206_1779_b200.workloads import Workload, draw_coefficients
     kw = dict(eps2=1e-6, L2=5e4); kw.update(shape)
     w = Workload("batched", **kw)
-    B = 16
     c = np.stack([draw_coefficients(100 + b, w.n_cheb) for b in range(B)])
     bc = np.stack([[0.5 + 0.05 * b, 1.2 + 0.03 * b] for b in range(B)])
     d = Dse(params_from_workload(w, n_batch=B)); assert d.kernel_info()["variant"] == "batched-dmma"; d.close()

@@ -735,7 +735,7 @@ int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
     if (constc_of(k) && !k.coefC)                              // fallback: in-stream copy of the pairs into the slot
         cudaMemcpyToSymbolAsync(c_coef, k.coefP, sizeof(double2) * k.Npad, 0, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
-    if (k.want_jac && cfg.batched) return launch_point_batched(k, cfg, stream);
+    if (cfg.batched) return launch_point_batched(k, cfg, stream);     // Jacobian or residual-only variant
     if (k.want_jac) {
         KernelFn fn = cfg.pipelined ? pick_pipe(k) : pick(k, true);
         fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);

@@ -39,7 +39,8 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
         : "d"(a), "d"(b));
 }
 
-template <bool GEOM, int NPADB>
+// JAC = false: residual only (dse_residual) -- steps A and B and the row sums, no T tile, no accumulation
+template <bool GEOM, int NPADB, bool JAC>
 __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(const KParams P)
 {
     constexpr int BT_KS = BT<NPADB>::KS, BT_NT = BT<NPADB>::NT, BT_TS = BT<NPADB>::TS, BT_WARP_DOUBLES = BT<NPADB>::WARP_DOUBLES;
@@ -98,10 +99,12 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
     double acc[3][BT_NT][2];                              // step-C accumulators: rows = systems, cols = j
     while (rem > 0) {
         // ---------------- one (warp, system group, external point) segment ----------------
+        if (JAC) {
 #pragma unroll
-        for (int st = 0; st < 3; ++st)
+            for (int st = 0; st < 3; ++st)
 #pragma unroll
-            for (int nt = 0; nt < BT_NT; ++nt) acc[st][nt][0] = acc[st][nt][1] = 0.0;
+                for (int nt = 0; nt < BT_NT; ++nt) acc[st][nt][0] = acc[st][nt][1] = 0.0;
+        }
         bool seg_done = false;
         while (!seg_done) {
             const size_t gq0 = ((size_t)(8 * sg + jq) * P.Gext + (P.rstride ? e : 0)) * Nr + q;
@@ -158,9 +161,11 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
                         const double Tn = fma(tw4, Tc, -Tm);
                         Tm = Tc; Tc = Tn; Tv[ks] = Tn;
                     }
-                    __syncwarp();                                    // the previous tile's B fragments have been read
+                    if (JAC) {
+                        __syncwarp();                                // the previous tile's B fragments have been read
 #pragma unroll
-                    for (int ks = 0; ks < BT_KS; ++ks) sT[pt_l * BT_TS + 4 * ks + jq] = Tv[ks];
+                        for (int ks = 0; ks < BT_KS; ++ks) sT[pt_l * BT_TS + 4 * ks + jq] = Tv[ks];
+                    }
                     // ---- step A: ln Z(z), ln G(z) of (point pt_l, systems jq and 4 + jq) ----
                     double lz0 = 0.0, lg0 = 0.0, lz1 = 0.0, lg1 = 0.0;
                     {
@@ -197,10 +202,10 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
                         sum0[0] += U0[0]; sum0[1] += U0[1]; sum0[2] += v0; sum0[3] += wQ0 + wM0;
                         sum1[0] += U1[0]; sum1[1] += U1[1]; sum1[2] += v1; sum1[3] += wQ1 + wM1;
                     }
-                    __syncwarp();                                    // the T tile is complete
+                    if (JAC) __syncwarp();                           // the T tile is complete
                     // ---- step C: S[sys, j](stream) += sum_pt U[sys, pt] T[pt, j] ----
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
+                    for (int h = 0; h < (JAC ? 2 : 0); ++h) {
                         // A fragment: row = system lane/4, col = point 4h + lane%4; its weight lives in lane
                         // 4 * point + system % 4, pair system / 4
                         const int src = 16 * h + 4 * jq + (pt_l & 3);
@@ -244,7 +249,7 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
             }
         }
         // partial of this (warp, system group, external point): accumulator fragments go straight to the slot
-        {
+        if (JAC) {
             const size_t slot = (size_t)(w + big);
             const int sys = pt_l;                                    // C fragment: row = lane/4, cols 2 (lane%4), +1
 #pragma unroll
@@ -285,17 +290,18 @@ bool batched_eligible(const KParams &k)
 
 namespace {
 using BatchedFn = void (*)(const KParams);
-template <int NPADB> BatchedFn pick_batched(bool geom)
+template <int NPADB> BatchedFn pick_batched(bool geom, bool jac)
 {
-    return geom ? point_kernel_batched<true, NPADB> : point_kernel_batched<false, NPADB>;
+    if (jac) return geom ? point_kernel_batched<true, NPADB, true> : point_kernel_batched<false, NPADB, true>;
+    return geom ? point_kernel_batched<true, NPADB, false> : point_kernel_batched<false, NPADB, false>;
 }
 struct BatchedVariant { BatchedFn fn; int threads, smem; };
-BatchedVariant batched_variant(const KParams &k)
+BatchedVariant batched_variant(const KParams &k, bool jac)
 {
     const bool g = k.geom != nullptr;
     const int base = (int)sizeof(double) * k.Ntpad * 6;
 #define DSE_BT_CASE(NPADB) \
-    return BatchedVariant{pick_batched<NPADB>(g), BT<NPADB>::THREADS, \
+    return BatchedVariant{pick_batched<NPADB>(g, jac), BT<NPADB>::THREADS, \
                           base + (int)sizeof(double) * (BT<NPADB>::THREADS / 32) * BT<NPADB>::WARP_DOUBLES}
     if (k.Npad <= 16) DSE_BT_CASE(16);
     if (k.Npad <= 32) DSE_BT_CASE(32);
@@ -307,10 +313,12 @@ BatchedVariant batched_variant(const KParams &k)
 
 int query_point_batched(const KParams &k, PointKernelConfig &cfg)
 {
-    const BatchedVariant v = batched_variant(k);
+    const BatchedVariant v = batched_variant(k, true);
     const void *fn = (const void *)v.fn;
     const int smem = v.smem;
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess)      // the residual-only variant runs in the same launch configuration
+        e = cudaFuncSetAttribute((const void *)batched_variant(k, false).fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel_batched)");
     cudaFuncAttributes fa;
     e = cudaFuncGetAttributes(&fa, fn);
@@ -334,7 +342,7 @@ int query_point_batched(const KParams &k, PointKernelConfig &cfg)
 
 int launch_point_batched(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
-    batched_variant(k).fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
+    batched_variant(k, k.want_jac != 0).fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
     return 1;
 }
 

@@ -140,6 +140,8 @@ def test_batched_tensor_path_every_system(orc, shape, B, monkeypatch):
         for b in range(B):
             Fo, Jo = orc.residual_jacobian(oracle_params(w), c[b], bc[b, 0], bc[b, 1])
             check(J[b], F[b], Jo, Fo)
+        _, F2 = gpu_build(w, c, bc, flags, jac=False)          # dse_residual: the residual-only variant of the kernel
+        assert np.allclose(F2, F, rtol=1e-12, atol=0)
     monkeypatch.setenv("DSE_NO_BATCHED", "1")
     d = Dse(params_from_workload(w, n_batch=B)); assert d.kernel_info()["variant"] != "batched-dmma"; d.close()
     J1, F1 = gpu_build(w, c, bc, 0)

@@ -337,7 +337,10 @@ __host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc,
 template <int NCH_T, bool GEOM, bool CONSTC>
 __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KParams P)
 {
-    constexpr int NCH = NCH_T, SUB = 32 / NCH_T, ROUNDS = NCH_T, Npad = NCH_T * CJ;
+    // lanes = (chunk of 8 j, point sub-lane); chunk counts that do not divide 32 leave 32 - NCH * SUB lanes idle in
+    // phase 2 and read the zero-weight stash slot 32 for the points past the batch
+    constexpr int NCH = NCH_T, SUB = 32 / NCH_T, ROUNDS = (32 + SUB - 1) / SUB, Npad = NCH_T * CJ;
+    constexpr bool EXACT = NCH * SUB == 32 && ROUNDS * SUB == 32;
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
     const int STASH = stash_doubles(NCH);
@@ -358,7 +361,8 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
     if (t0 >= t1) return;
     const long long r0 = t0 / BPR;
     int kb = (int)(t0 - r0 * BPR);
-    const int c_lane = lane / SUB, sub = lane - c_lane * SUB;
+    const bool lane_on = EXACT || lane < NCH * SUB;
+    const int c_lane = lane_on ? lane / SUB : 0, sub = lane_on ? lane - c_lane * SUB : 0;
     const double halfLg = 0.5 * P.Lg;
 
     double accA[CJ], accB[CJ], accV[CJ];
@@ -369,7 +373,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
         const double2 *trd = reinterpret_cast<const double2 *>(s_stash + buf * STASH + 132) + c_lane * (TCH_STRIDE / 2);
 #pragma unroll
         for (int rd = 0; rd < ROUNDS; ++rd) {
-            const int pt = rd * SUB + sub;
+            const int pt = EXACT ? rd * SUB + sub : min(rd * SUB + sub, 32);     // slot 32: zero weights, finite T
             const double4 pw = pts[pt];
             const double2 tt = trd[pt];
             double T0 = tt.x, T1 = tt.y;
@@ -390,7 +394,8 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
         for (int st = 0; st < 3; ++st) {
             __syncwarp();
 #pragma unroll
-            for (int m = 0; m < CJ; ++m) scr[sub * Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
+            for (int m = 0; m < CJ; ++m)
+                if (lane_on) scr[sub * Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
             __syncwarp();
             for (int j = lane; j < Npad; j += 32) {
                 double s = 0.0;
@@ -428,8 +433,12 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KPara
 
     // both T stashes must hold finite numbers before the first (zero-weight) prologue phase 2
     for (int b2 = 0; b2 < 2; ++b2)
-        for (int c = 0; c < NCH; ++c)
-            reinterpret_cast<double2 *>(s_stash + b2 * STASH + 132)[c * (TCH_STRIDE / 2) + lane] = make_double2(0.0, 0.0);
+        for (int c = 0; c < NCH; ++c) {
+            double2 *tz = reinterpret_cast<double2 *>(s_stash + b2 * STASH + 132) + c * (TCH_STRIDE / 2);
+            tz[lane] = make_double2(0.0, 0.0);
+            if (!EXACT && lane == 0) tz[32] = make_double2(0.0, 0.0);        // read with the zero-weight slot 32
+        }
+    if (!EXACT && lane < 2) reinterpret_cast<double4 *>(s_stash + lane * STASH)[32] = make_double4(0.0, 0.0, 0.0, 0.0);
 
     int rem = (int)(t1 - t0);                              // batches left for this warp
     int cur = 0;                                           // stash half written by the current batch
@@ -643,8 +652,13 @@ static KernelFn pick_pipe(const KParams &k)
     switch (k.NCH) {
         DSE_PIPE_CASE(1)
         DSE_PIPE_CASE(2)
+        DSE_PIPE_CASE(3)
         DSE_PIPE_CASE(4)
+        DSE_PIPE_CASE(5)         // the paper's N = 36
+        DSE_PIPE_CASE(6)
+        DSE_PIPE_CASE(7)
         DSE_PIPE_CASE(8)
+        DSE_PIPE_CASE(12)        // the paper's N = 96
         DSE_PIPE_CASE(16)
         default: return nullptr;
     }

@@ -90,6 +90,10 @@ def test_tables_match_oracle(orc):
     dict(n_cheb=2, n_r=2, n_theta=2),          # minimum sizes
     dict(n_cheb=16, n_r=40, n_theta=32, x_G=3.0, x_Z=5e3),   # distinct subtraction points (N_ext = N + 2)
     dict(n_cheb=128, n_r=6, n_theta=8),        # maximum N
+    dict(n_cheb=20, n_r=12, n_theta=32),       # NCH = 3: pipelined kernel with idle phase-2 lanes (30 of 32)
+    dict(n_cheb=48, n_r=10, n_theta=64),       # NCH = 6
+    dict(n_cheb=52, n_r=9, n_theta=32),        # NCH = 7
+    dict(n_cheb=96, n_r=5, n_theta=32),        # the paper's N = 96: NCH = 12, 24 of 32 lanes
 ])
 def test_ragged_and_edge_shapes(orc, shape):
     from paper_1206_1779_b200.workloads import Workload, draw_coefficients

@@ -704,31 +704,37 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     cfg.sms = sms;
 
     // residual-only build (and the Jacobian build of generic shapes): warp-independent kernel, 512 threads
-    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (POINT_THREADS / 32) * warp_doubles(k.Npad, k.NCH, np_of(k)));
+    // (large N with full-warp angular batches: fewer warps per CTA until the per-warp stashes fit in shared memory)
+    int gthr = POINT_THREADS;
+    while (gthr > 128 && (int)sizeof(double) * (k.Ntpad * 6 + (gthr / 32) * warp_doubles(k.Npad, k.NCH, np_of(k))) > smem_max) gthr -= 128;
+    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (gthr / 32) * warp_doubles(k.Npad, k.NCH, np_of(k)));
     for (int jac = 0; jac < 2; ++jac) {
         e = cudaFuncSetAttribute((const void *)pick(k, jac != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel smem)");
     }
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)pick(k, false), POINT_THREADS, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)pick(k, false), gthr, smem);
     if (e != cudaSuccess) return fail(e, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
     if (per_sm < 1) { set_error_text("point_kernel does not fit on an SM"); return DSE_ECUDA; }
-    cfg.res_block = POINT_THREADS;
+    cfg.res_block = gthr;
     cfg.res_smem = smem;
-    cfg.res_grid = (int)pick_grid(k, sms, per_sm, POINT_THREADS / 32);
+    cfg.res_grid = (int)pick_grid(k, sms, per_sm, gthr / 32);
 
     // Jacobian build: software-pipelined kernel when the shape allows it
     const void *fn = (const void *)pick(k, true);
-    int block = POINT_THREADS, jsmem = smem;
+    int block = gthr, jsmem = smem;
     cfg.pipelined = 0;
     cfg.batched = 0;
     KernelFn pf = (k.g == 32 && !getenv("DSE_NO_PIPE")) ? pick_pipe(k) : nullptr;
     if (pf) {
-        const int psmem = (int)sizeof(double) * (k.Ntpad * 6 + (PIPE_THREADS / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
-        if (psmem <= smem_max) {
+        // large N: fewer warps per CTA until the double-buffered stashes fit in shared memory (at least 8 warps)
+        for (int thr = PIPE_THREADS; thr >= 256; thr -= 128) {
+            const int psmem = (int)sizeof(double) * (k.Ntpad * 6 + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
+            if (psmem > smem_max) continue;
             e = cudaFuncSetAttribute((const void *)pf, cudaFuncAttributeMaxDynamicSharedMemorySize, psmem);
             if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel_pipe smem)");
-            fn = (const void *)pf; block = PIPE_THREADS; jsmem = psmem; cfg.pipelined = 1;
+            fn = (const void *)pf; block = thr; jsmem = psmem; cfg.pipelined = 1;
+            break;
         }
     }
     cudaFuncAttributes fa;

@@ -94,6 +94,7 @@ def test_tables_match_oracle(orc):
     dict(n_cheb=48, n_r=10, n_theta=64),       # NCH = 6
     dict(n_cheb=52, n_r=9, n_theta=32),        # NCH = 7
     dict(n_cheb=96, n_r=5, n_theta=32),        # the paper's N = 96: NCH = 12, 24 of 32 lanes
+    dict(n_cheb=128, n_r=4, n_theta=32),       # maximum N with full-warp angular batches: fewer warps per CTA (shared memory)
 ])
 def test_ragged_and_edge_shapes(orc, shape):
     from paper_1206_1779_b200.workloads import Workload, draw_coefficients

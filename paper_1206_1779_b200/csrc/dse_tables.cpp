@@ -163,22 +163,27 @@ void build_tables(const dse_params &p, HostTables &T)
     T.ang.assign((size_t)T.Ntpad * 6, 0.0);
     if (p.flags & DSE_FLAG_ANGULAR_TANH_SINH) {
         // int dxi sqrt(1-xi^2) f:  t_k equidistant in [-3,3], u = (pi/2) sinh t, xi = tanh u, 1-xi^2 = 1/cosh^2 u,
-        // w = h (pi/2) cosh t / cosh^2 u.  The kernel's "Omega sin^2" and "Omega sin^4" are w sqrt(1-xi^2) and
-        // w (1-xi^2)^(3/2); sin^2(theta/2) = (1-xi)/2 = 1/(1+e^{2u}) without cancellation.
+        // w = h (pi/2) cosh t / cosh^2 u, in the theta form: theta = 2 atan(e^-u), Omega = w / sin(theta) = w cosh u, so
+        // that "Omega sin^2" and "Omega sin^4" are w sqrt(1-xi^2) and w (1-xi^2)^(3/2).
         const ld tmax = 3.0L, h = Nt > 1 ? 2 * tmax / (Nt - 1) : 0.0L;
         for (int k = 0; k < Nt; ++k) {
             const ld tt = tmax - h * k;                       // descending t: ascending theta
-            const ld u = PI_L / 2 * sinhl(tt), ch = coshl(u), xi = tanhl(u);
+            const ld u = PI_L / 2 * sinhl(tt), ch = coshl(u);
             const ld wk = h * (PI_L / 2) * coshl(tt) / (ch * ch);
             T.theta[k] = (double)(2 * atanl(expl(-u)));
             T.Omega[k] = (double)(wk * ch);
+            // the rule IS the pair (theta_k, Omega_k) of doubles that dse_get_tables returns: like the Gauss-Legendre
+            // branch, everything the kernels use is derived from those rounded values (next to theta = pi, sin(theta)
+            // inherits the rounding of theta -- nodes of relative weight < 1e-11; reading A25)
+            const ld thd = (ld)T.theta[k], Om = (ld)T.Omega[k];
+            const ld sh = sinl(thd / 2), c = cosl(thd), sn = sinl(thd);
             double *a = &T.ang[(size_t)k * 6];
-            a[0] = (double)(1 / (1 + expl(2 * u)));
-            a[1] = (double)(6 * xi);
-            a[2] = (double)(2 + xi * xi);
-            a[3] = (double)(-2 / (ch * ch));
-            a[4] = (double)(wk / ch);
-            a[5] = (double)(wk / (ch * ch * ch));
+            a[0] = (double)(sh * sh);
+            a[1] = (double)(6 * c);
+            a[2] = (double)(2 + c * c);
+            a[3] = (double)(-2 * sn * sn);
+            a[4] = (double)(Om * sn * sn);
+            a[5] = (double)(Om * sn * sn * sn * sn);
         }
         for (int k = Nt; k < T.Ntpad; ++k) {                  // padded lanes: a valid angle with zero weight
             double *a = &T.ang[(size_t)k * 6];

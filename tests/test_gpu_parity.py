@@ -221,7 +221,7 @@ def test_config4_full_batch_sampled_systems(orc):
     assert np.array_equal(F2[1, :N], F2[0, :N])
 
 
-@pytest.mark.parametrize("n_theta", [16, 64, 40])
+@pytest.mark.parametrize("n_theta", [16, 64, 40, 2, 3])      # 2: both nodes in the tails, next to theta = 0 and pi
 def test_tanh_sinh_angular_rule_parity(orc, n_theta):
     """NEXT f3: tanh-sinh rule in xi = cos(theta); only the tables change."""
     _torch()

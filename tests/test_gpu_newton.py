@@ -123,3 +123,37 @@ def test_finite_difference_self_check_mode(orc):
         Jo[:, j] = (orc.residual_jacobian(p, cp, 1, 1, jac=False) - orc.residual_jacobian(p, cm, 1, 1, jac=False)) / ((c[0, j] + h) - (c[0, j] - h))
     assert (np.linalg.norm(Jfd - Jo, axis=1) / np.linalg.norm(Jo, axis=1)).max() < 1e-6
     d.close()
+
+
+def test_lu_random_sizes_exact_factorisation(orc):
+    """Random sizes, scalings, tie-rich and singular matrices: solution within conditioning, scaling / smallest pivot /
+    growth factor bit-identical to the plain C elimination (both LU kernels: registers for n <= 128, blocked above)."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import CONFIGS
+    d = Dse(params_from_workload(CONFIGS[0]))
+    rng = np.random.default_rng(11)
+    for it in range(60):
+        n = int(rng.choice([1, 2, 3, 7, 8, 9, 15, 16, 17, 31, 32, 33, 40, 63, 64, 65, 72, 100, 120, 127, 128]))
+        kind = int(rng.integers(0, 4))
+        if kind == 0:
+            A = rng.normal(size=(2, n, n))
+        elif kind == 1:
+            A = rng.normal(size=(2, n, n)) * 10.0 ** rng.uniform(-8, 8, size=(2, n, 1))
+        elif kind == 2:
+            A = rng.integers(-2, 3, size=(2, n, n)).astype(np.float64) + 5.0 * np.eye(n)
+        else:
+            A = rng.normal(size=(2, n, n))
+            if n > 2:
+                A[:, :, n // 2] = 0.0                      # a zero column: singular, the column is skipped
+        b = rng.normal(size=(2, n)) * np.abs(A).max(axis=2).clip(1e-300)
+        x, st = d.lu_solve(torch.from_numpy(A).cuda(), torch.from_numpy(b).cuda())
+        x = x.cpu().numpy(); st = st.cpu().numpy()
+        for s in range(2):
+            xo, so, rc = orc.lu_solve(A[s], b[s])
+            if rc == 0:
+                assert np.allclose(x[s], xo, rtol=1e-7, atol=1e-10 * np.abs(xo).max()), (n, kind)
+                assert np.array_equal(st[s][1:], so[1:]), (n, kind, st[s], so)
+            else:
+                assert np.array_equal(st[s][1:3], so[1:3]), (n, kind, st[s], so)
+    d.close()

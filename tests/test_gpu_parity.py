@@ -238,3 +238,41 @@ def test_tanh_sinh_angular_rule_parity(orc, n_theta):
     t = d.tables(); d.close()
     o = orc.tables(oracle_params(w))
     assert np.allclose(t["theta"], o["theta"], rtol=1e-13) and np.allclose(t["Omega"], o["Omega"], rtol=1e-12)
+
+
+def test_random_shapes_against_oracle(orc):
+    """Seeded random shapes, batch sizes, rules and flags (every kernel variant gets picked): J, F and the residual-only
+    entry point against the oracle.  This sweep found the N = 128 / n_theta >= 32 shared-memory limit and reading A25."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    rng = np.random.default_rng(2024)
+    seen = set()
+    for it in range(60):
+        N = int(rng.choice([2, 3, 5, 8, 9, 16, 17, 24, 31, 32, 33, 40, 47, 48, 56, 63, 64, 65, 72, 96, 120, 128]))
+        nr = int(rng.integers(2, 24)); nt = int(rng.choice([2, 3, 7, 8, 16, 31, 32, 33, 40, 64, 65, 96]))
+        B = int(rng.choice([1, 1, 2, 3, 8, 9, 13, 16]))
+        if N > 64 and B > 2:
+            B = 2
+        kw = dict(n_cheb=N, n_r=nr, n_theta=nt, eps2=10.0 ** rng.integers(-12, -3), L2=10.0 ** rng.integers(2, 12))
+        if rng.random() < 0.3: kw.update(x_G=3.0, x_Z=5e1)
+        if rng.random() < 0.2: kw.update(radial_split=1)
+        if rng.random() < 0.2: kw.update(n_ir=int(rng.integers(1, 6)))
+        if rng.random() < 0.15: kw.update(x_G=0.0)
+        if rng.random() < 0.2: kw.update(angular_rule=1)
+        w = Workload("fuzz", **kw)
+        flags = int(rng.integers(0, 2))
+        c = np.stack([draw_coefficients(1000 * it + b, N) for b in range(B)])
+        bc = np.stack([[0.7 + 0.1 * b, 1.3 - 0.05 * b] for b in range(B)])
+        d = Dse(params_from_workload(w, n_batch=B, flags=flags)); seen.add(d.kernel_info()["variant"])
+        ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
+        J, F = d.jacobian(ct, bt); F2 = d.residual(ct, bt); torch.cuda.synchronize()
+        J = J.cpu().numpy(); F = F.cpu().numpy(); F2 = F2.cpu().numpy(); d.close()
+        for b in range(min(B, 3)):
+            Fo, Jo = orc.residual_jacobian(oracle_params(w), c[b], bc[b, 0], bc[b, 1])
+            # normwise only: with few radial nodes single rows are differences of terms 1e15 times their size
+            assert np.all(np.isfinite(J[b])) and np.all(np.isfinite(F[b]))
+            en = np.linalg.norm(J[b] - Jo) / np.linalg.norm(Jo); ef = np.linalg.norm(F[b] - Fo) / np.linalg.norm(Fo)
+            assert en <= TOL_NORM and ef <= TOL_NORM, (kw, B, flags, en, ef)
+            assert np.allclose(F2[b], F[b], rtol=1e-11, atol=1e-13 * np.abs(F[b]).max()), kw
+    assert seen == {"generic", "pipelined", "batched-dmma"}

@@ -157,3 +157,26 @@ def test_lu_random_sizes_exact_factorisation(orc):
             else:
                 assert np.array_equal(st[s][1:3], so[1:3]), (n, kind, st[s], so)
     d.close()
+
+
+def test_newton_steps_batched_systems(orc):
+    """Eight systems per handle (tensor-path build + one LU CTA per system): every system follows the oracle's iterates."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload
+    w = Workload("newton-weak-batch", 10, 48, 32, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
+    B = 8
+    d = Dse(params_from_workload(w, n_batch=B)); assert d.kernel_info()["variant"] == "batched-dmma"
+    p = oracle_params(w)
+    c0 = np.zeros((B, 20))                                   # G = Z = 1; the systems differ in their boundary values
+    bcs = np.stack([[1.0 + 0.001 * b, 1.0 - 0.0005 * b] for b in range(B)])     # inside the basin of plain Newton steps
+    c_g = torch.from_numpy(c0.copy()).cuda(); bc_g = torch.from_numpy(bcs).cuda()
+    c_o = c0.copy()
+    for it in range(8):
+        st = d.newton_step(c_g, bc_g, 1.0).cpu().numpy()
+        for b in range(B):
+            c_o[b], so, rc = orc.newton_step(p, c_o[b], bcs[b, 0], bcs[b, 1], 1.0)
+            assert rc == 0 and abs(st[b, 0] - so[0]) <= 1e-9 * so[0] + 1e-12
+        assert np.allclose(c_g.cpu().numpy(), c_o, rtol=0, atol=1e-9 * np.abs(c_o).max())
+    assert st[:, 0].max() < 1e-8                             # every system converges quadratically
+    d.close()

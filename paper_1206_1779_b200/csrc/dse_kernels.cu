@@ -216,11 +216,12 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
     const int N = P.N, nthr = blockDim.x;      // 128 <= nthr <= ASM_THREADS, a multiple of 32 and of PJ
     const long long bi_i = (long long)b * P.Next + i, bi_Z = (long long)b * P.Next + P.iZ,
                     bi_G = (long long)b * P.Next + P.iG;
-    __shared__ double s_pi[3][2];
     __shared__ double s_pw[ASM_THREADS / 32][3][2];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    {   // Pi_G, Pi_Z at e = i, x_Z, x_G: all threads stride over q (loads in flight together), fixed-order combine
-        const int npi = (P.iG != P.iZ) ? 3 : 2;
+    // All global loads of the CTA (row sums for Pi, partial slots, the fused contraction) are issued before its single
+    // barrier, so their latencies overlap; the combination steps after the barrier read shared memory only.
+    const int npi = (P.iG != P.iZ) ? 3 : 2;
+    {   // Pi_G, Pi_Z at e = i, x_Z, x_G: all threads stride over q, per-warp partials in fixed order
         for (int pt = 0; pt < npi; ++pt) {
             const long long bi = pt == 0 ? bi_i : (pt == 1 ? bi_Z : bi_G);
             double pg = 0.0, pz = 0.0;
@@ -235,24 +236,25 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
             }
             if (lane == 0) { s_pw[warp][pt][0] = pg; s_pw[warp][pt][1] = pz; }
         }
-        __syncthreads();
-        if (threadIdx.x < 2 * npi) {
-            const int pt = threadIdx.x >> 1, cmp = threadIdx.x & 1;
-            double t = 0.0;
-            for (int w2 = 0; w2 < nthr / 32; ++w2) t += s_pw[w2][pt][cmp];
-            s_pi[pt][cmp] = t;
-        }
-        __syncthreads();
-        if (npi == 2 && threadIdx.x < 2) s_pi[2][threadIdx.x] = s_pi[1][threadIdx.x];     // x_G == x_Z
     }
-    __syncthreads();
     const double invZ = P.invZ[(size_t)b * N + i], invG = P.invG[(size_t)b * N + i];
-    if (threadIdx.x == 0) {
-        const double gG = bc[2 * b + 0], gZ = bc[2 * b + 1];
-        F[(size_t)b * 2 * N + i] = invZ - gZ - s_pi[0][1] + s_pi[1][1];
-        F[(size_t)b * 2 * N + N + i] = invG - gG - s_pi[0][0] + s_pi[2][0];
+    if (J == nullptr) {                                          // residual only
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double pi[3][2];
+            for (int pt = 0; pt < npi; ++pt)
+                for (int cmp = 0; cmp < 2; ++cmp) {
+                    double t = 0.0;
+                    for (int w2 = 0; w2 < nthr / 32; ++w2) t += s_pw[w2][pt][cmp];
+                    pi[pt][cmp] = t;
+                }
+            if (npi == 2) { pi[2][0] = pi[1][0]; pi[2][1] = pi[1][1]; }      // x_G == x_Z
+            const double gG = bc[2 * b + 0], gZ = bc[2 * b + 1];
+            F[(size_t)b * 2 * N + i] = invZ - gZ - pi[0][1] + pi[1][1];
+            F[(size_t)b * 2 * N + N + i] = invG - gG - pi[0][0] + pi[2][0];
+        }
+        return;
     }
-    if (J == nullptr) return;
     // threads = (part, j): each sums a contiguous part of the slot range; parts are combined in order
     __shared__ double s_part[3][3][ASM_THREADS];
     int PJ = 8;
@@ -315,6 +317,19 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
         }
     }
     __syncthreads();
+    if (threadIdx.x == nthr - 1) {                               // F (one thread; the J threads are the first ones)
+        double pi[3][2];
+        for (int pt = 0; pt < npi; ++pt)
+            for (int cmp = 0; cmp < 2; ++cmp) {
+                double t = 0.0;
+                for (int w2 = 0; w2 < nthr / 32; ++w2) t += s_pw[w2][pt][cmp];
+                pi[pt][cmp] = t;
+            }
+        if (npi == 2) { pi[2][0] = pi[1][0]; pi[2][1] = pi[1][1]; }          // x_G == x_Z
+        const double gG = bc[2 * b + 0], gZ = bc[2 * b + 1];
+        F[(size_t)b * 2 * N + i] = invZ - gZ - pi[0][1] + pi[1][1];
+        F[(size_t)b * 2 * N + N + i] = invG - gG - pi[0][0] + pi[2][0];
+    }
     if (part == 0 && j < N) {
         double S[3][3];
         for (int pt = 0; pt < npt; ++pt)

@@ -200,7 +200,7 @@ __device__ __forceinline__ void reduce_part(const KParams &P, long long bi, int 
 #pragma unroll 4
     for (long long w = w0; w < w1; ++w) {
         const double *sp = P.Spart + ((size_t)(w + big) * P.bgroup + m) * 3 * P.Npad;
-        a += sp[j]; b += sp[P.Npad + j]; v += sp[2 * P.Npad + j];
+        a += __ldg(sp + j); b += __ldg(sp + P.Npad + j); v += __ldg(sp + 2 * P.Npad + j);
     }
     Sa = a; Sb = b; Sv = v;
 }
@@ -226,9 +226,10 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
             const long long bi = pt == 0 ? bi_i : (pt == 1 ? bi_Z : bi_G);
             double pg = 0.0, pz = 0.0;
             for (int q = threadIdx.x; q < P.Nr; q += nthr) {
-                const double4 a = reinterpret_cast<const double4 *>(P.Apart)[(size_t)bi * P.Nr + q];
-                const double4 hh = reinterpret_cast<const double4 *>(P.AHead)[(size_t)bi * P.Nr + q];
-                pg += a.z + hh.z; pz += a.w + hh.w;
+                // (read-only loads: the compiler may hoist them over the shared-memory stores of the other stages)
+                const double2 a = __ldg(reinterpret_cast<const double2 *>(P.Apart) + ((size_t)bi * P.Nr + q) * 2 + 1);
+                const double2 hh = __ldg(reinterpret_cast<const double2 *>(P.AHead) + ((size_t)bi * P.Nr + q) * 2 + 1);
+                pg += a.x + hh.x; pz += a.y + hh.y;
             }
             for (int o = 16; o > 0; o >>= 1) {
                 pg += __shfl_xor_sync(FULL, pg, o);
@@ -293,7 +294,7 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
                     const size_t q = (size_t)(4 * (ks + u) + (lane & 3));
-                    av[u] = Aq[q * 4]; hv[u] = Hq[q * 4]; bv[u] = Bp[q * P.Npad];
+                    av[u] = __ldg(Aq + q * 4); hv[u] = __ldg(Hq + q * 4); bv[u] = __ldg(Bp + q * P.Npad);
                 }
 #pragma unroll
                 for (int u = 0; u < 8; ++u)
@@ -304,8 +305,8 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
                 const int q = 4 * ks + (lane & 3);
                 const bool ok = q < P.Nr;
                 const size_t qq = ok ? q : 0;
-                const double a = ok ? (Aq[qq * 4] + Hq[qq * 4]) * amask : 0.0;
-                const double bb = ok ? Bp[qq * P.Npad] : 0.0;
+                const double a = ok ? (__ldg(Aq + qq * 4) + __ldg(Hq + qq * 4)) * amask : 0.0;
+                const double bb = ok ? __ldg(Bp + qq * P.Npad) : 0.0;
                 asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                     : "+d"(c[ks & 3][0]), "+d"(c[ks & 3][1]) : "d"(a), "d"(bb));
             }

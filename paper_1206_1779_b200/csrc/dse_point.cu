@@ -665,11 +665,11 @@ static KernelFn pick_pipe(const KParams &k)
 #undef DSE_PIPE_CASE
 }
 
-// grid of the pipelined kernel: units are 32-point batches; every warp gets >= max(4, batches per row) of them so
-// that a row spans at most two warps
+// grid of the pipelined kernel: units are 32-point batches; every warp gets at least one row's worth of them, so that
+// a row spans at most two warps (small problems are latency-bound: more warps with less work each is faster)
 static long long pick_grid_pipe(const KParams &k, int sms, int per_sm, int wpb)
 {
-    const long long bpr = k.Ntpad / 32, units = k.R * bpr, min_units = bpr > 4 ? bpr : 4;
+    const long long bpr = k.Ntpad / 32, units = k.R * bpr, min_units = bpr;
     long long grid = (long long)sms * per_sm;
     long long want_grid = (units / min_units + wpb - 1) / wpb;
     if (want_grid < 1) want_grid = 1;
@@ -683,8 +683,8 @@ static long long pick_grid(const KParams &k, int sms, int per_sm, int wpb)
     // persistent-style grid: one wave of resident CTAs, but never more warps than rows
     long long grid = (long long)sms * per_sm;
     const long long batches_per_row = k.Ntpad / 32 > 0 ? k.Ntpad / 32 : 1;   // 32-point batches
-    // keep >= ~4 point batches per warp so that small problems do not pay for idle warps
-    long long want_warps = (k.R * batches_per_row / k.rpb + 3) / 4;
+    // small problems are latency-bound: one 32-point batch per warp
+    long long want_warps = k.R * batches_per_row / k.rpb;
     if (want_warps < 1) want_warps = 1;
     long long want_grid = (want_warps + wpb - 1) / wpb;
     if (want_grid < grid) grid = want_grid;

@@ -329,7 +329,7 @@ int query_point_batched(const KParams &k, PointKernelConfig &cfg)
     if (per_sm < 1) { set_error_text("point_kernel_batched does not fit on an SM"); return DSE_ECUDA; }
     const long long wpb = v.threads / 32, bpr = k.Ntpad / 32;
     const long long groups = (k.B + 7) / 8;
-    const long long units = groups * k.Next * k.Nr * bpr, min_units = bpr > 4 ? bpr : 4;
+    const long long units = groups * k.Next * k.Nr * bpr, min_units = bpr;      // at least one row per warp
     long long grid = (long long)cfg.sms * per_sm;
     long long want = (units / min_units + wpb - 1) / wpb;
     if (want < 1) want = 1;

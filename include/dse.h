@@ -167,6 +167,11 @@ DSE_API int dse_gauss_legendre(int32_t n, double *x_dev, double *w_dev, double *
 DSE_API int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, double p2_min, double p2_max,
                           const double *t_dev, int32_t n_t, double *delta_dev, double *work_dev, void *stream);
 
+/* Environment switches for A/B measurements and tests (read in dse_create unless noted; none changes results beyond
+ * rounding order): DSE_NO_BATCHED (per-system point kernels for batches), DSE_NO_PIPE (non-pipelined point kernel),
+ * DSE_CONST_MEMCPY (coefficient slot filled by a device-to-device copy instead of prep_kernel's direct store),
+ * DSE_NO_FUSED_ASSEMBLE and DSE_LU_BLOCKED (separate contraction kernel / shared-memory LU; read once per process). */
+
 /* Diagnostics: cycles summed over all warps of the last point-kernel launch, spent in (geometry, series,
  * exp + weights, accumulation, whole warp).  All zeros unless the library was built with
  * -DDSE_PHASE_TIMING (the default build carries no instrumentation).  Synchronous. */

@@ -462,8 +462,8 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     // few systems, shared radial rule, small Phi table: H7 is fused into the assemble CTAs (one launch less on the
     // latency path: -3 us per build at cfg 0/1); large tables keep the separate gemm (every fused CTA would stream
     // the whole N_r x N table: +15 us at cfg 3)
-    const bool fused = kk.want_jac && !kk.rstride && kk.B < 8 && (long long)kk.Nr * kk.Npad <= 16384 &&
-                       !getenv("DSE_NO_FUSED_ASSEMBLE");
+    static const bool no_fused = getenv("DSE_NO_FUSED_ASSEMBLE") != nullptr;     // A/B switch, read once
+    const bool fused = kk.want_jac && !kk.rstride && kk.B < 8 && (long long)kk.Nr * kk.Npad <= 16384 && !no_fused;
     if (kk.want_jac && !fused) {
         if (kk.rstride) {
             contract_split_kernel<<<dim3(kk.Next, kk.B), 128, 0, s>>>(kk);

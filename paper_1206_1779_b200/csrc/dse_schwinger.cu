@@ -12,6 +12,7 @@
 //   schwinger_kernel    one CTA per (t_m, system): fixed-order strided sum of f_i cos(t_m p_i)
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdio>
 
 #include "dse_internal.h"
@@ -32,48 +33,80 @@ __global__ void gl_prepare_kernel(int n, double2 *__restrict__ ab)
     }
 }
 
-// P_n(x) and P_{n-1}(x) for two abscissae at once (two independent chains per thread)
-__device__ __forceinline__ void legendre2(int n, const double2 *__restrict__ ab, double xa, double xb, double &pa,
-                                          double &pam, double &pb, double &pbm)
+// P_n(x) and P_{n-1}(x) for two abscissae at once (two independent chains per thread).  One warp per CTA: the
+// recurrence coefficients (2 MB at n = 2^17: L2-resident, ~300 cycles away) are staged through shared memory in chunks
+// of GL_CHUNK entries with a cp.async double buffer, so the loop only sees shared-memory latency.
+constexpr int GL_CHUNK = 512;
+__device__ __forceinline__ void legendre2(int n, const double2 *__restrict__ ab, double2 *s_ab /*[2][GL_CHUNK]*/,
+                                          double xa, double xb, double &pa, double &pam, double &pb, double &pbm)
 {
+    const int lane = threadIdx.x;
+    auto stage = [&](int chunk, int buf) {                       // entries m = 2 + chunk * GL_CHUNK + i
+        const int m0 = 2 + chunk * GL_CHUNK;
+        for (int i = lane; i < GL_CHUNK; i += 32) {
+            const int m = min(m0 + i, n);                        // (clamped: entries past n are never used)
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_ab + buf * GL_CHUNK + i);
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(ab + m));
+        }
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
     double a0 = 1.0, a1 = xa, b0 = 1.0, b1 = xb;
-    for (int m = 2; m <= n; ++m) {
-        const double2 c = ab[m];
-        const double a2 = fma(c.x * xa, a1, -c.y * a0);
-        const double b2 = fma(c.x * xb, b1, -c.y * b0);
-        a0 = a1; a1 = a2; b0 = b1; b1 = b2;
+    const int nchunks = (n - 1 + GL_CHUNK - 1) / GL_CHUNK;       // steps m = 2 .. n
+    if (nchunks > 0) stage(0, 0);
+    for (int ch = 0; ch < nchunks; ++ch) {
+        if (ch + 1 < nchunks) stage(ch + 1, (ch + 1) & 1);
+        else asm volatile("cp.async.commit_group;\n" ::);
+        asm volatile("cp.async.wait_group 1;\n" ::: "memory");
+        __syncwarp();
+        const double2 *cur = s_ab + (ch & 1) * GL_CHUNK;
+        const int cnt = min(GL_CHUNK, n - 1 - ch * GL_CHUNK);
+#pragma unroll 8
+        for (int i = 0; i < cnt; ++i) {
+            const double2 c = cur[i];
+            const double a2 = fma(c.x * xa, a1, -c.y * a0);
+            const double b2 = fma(c.x * xb, b1, -c.y * b0);
+            a0 = a1; a1 = a2; b0 = b1; b1 = b2;
+        }
+        __syncwarp();                                            // the buffer is restaged two chunks later
     }
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     pa = a1; pam = a0; pb = b1; pbm = b0;
 }
 
 // nodes ascending in (-1, 1); thread t handles the nodes i = t and i = t + q (q = quarter) of the upper half and
 // mirrors them.  Newton on P_n with P_n' = n (x P_n - P_{n-1}) / (x^2 - 1); weight 2 / ((1 - x^2) P_n'^2).
-__global__ void __launch_bounds__(128) gl_nodes_kernel(int n, const double2 *__restrict__ ab, double *__restrict__ x,
+__global__ void __launch_bounds__(32) gl_nodes_kernel(int n, const double2 *__restrict__ ab, double *__restrict__ x,
                                                        double *__restrict__ w)
 {
+    __shared__ __align__(16) double2 s_ab[2 * GL_CHUNK];
     const int half = (n + 1) / 2;                 // number of non-negative nodes
     const int q = (half + 1) / 2;
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= q) return;
+    const bool valid = t < q;                     // (all lanes stay: the coefficient staging is warp-wide)
     // k-th largest root (k = 0 is the largest): Tricomi-type starting value
-    const int ka = t, kb = min(t + q, half - 1);
+    const int ka = min(t, half - 1), kb = min(t + q, half - 1);
     double xa = (1.0 - (n - 1.0) / (8.0 * n * (double)n * n)) * cospi((4.0 * ka + 3.0) / (4.0 * n + 2.0));
     double xb = (1.0 - (n - 1.0) / (8.0 * n * (double)n * n)) * cospi((4.0 * kb + 3.0) / (4.0 * n + 2.0));
     double pa, pam, pb, pbm, da = 1.0, db = 1.0;
-    for (int it = 0; it < 12; ++it) {
-        legendre2(n, ab, xa, xb, pa, pam, pb, pbm);
+    // Newton converges quadratically: once a step is below 1e-14 the node is exact to rounding after it (the error
+    // left is ~step^2).  Demanding |step| <= 1e-16 never triggered at n = 2^17 -- the O(n eps) noise of the recurrence
+    // keeps the steps at ~1e-15 -- and ran all 12 iterations.
+    bool live_a = true, live_b = true;
+    for (int it = 0; it < 12 && __any_sync(0xffffffffu, live_a || live_b); ++it) {      // warp-uniform trip count
+        legendre2(n, ab, s_ab, xa, xb, pa, pam, pb, pbm);
         da = n * (xa * pa - pam) / (xa * xa - 1.0);
         db = n * (xb * pb - pbm) / (xb * xb - 1.0);
         const double sa = pa / da, sb = pb / db;
-        xa -= sa; xb -= sb;
-        if (fabs(sa) <= 1e-16 && fabs(sb) <= 1e-16) break;
+        if (live_a) { xa -= sa; live_a = fabs(sa) > 1e-14; }
+        if (live_b) { xb -= sb; live_b = fabs(sb) > 1e-14; }
     }
-    legendre2(n, ab, xa, xb, pa, pam, pb, pbm);
+    legendre2(n, ab, s_ab, xa, xb, pa, pam, pb, pbm);
     da = n * (xa * pa - pam) / (xa * xa - 1.0);
     db = n * (xb * pb - pbm) / (xb * xb - 1.0);
     const double wa = 2.0 / ((1.0 - xa * xa) * da * da), wb = 2.0 / ((1.0 - xb * xb) * db * db);
     if ((n & 1) && ka == half - 1) xa = 0.0;      // the middle node of an odd rule
     if ((n & 1) && kb == half - 1) xb = 0.0;
+    if (!valid) return;
     x[n - 1 - ka] = xa; w[n - 1 - ka] = wa; x[ka] = -xa; w[ka] = wa;
     x[n - 1 - kb] = xb; w[n - 1 - kb] = wb; x[kb] = -xb; w[kb] = wb;
 }
@@ -149,7 +182,7 @@ int launch_gauss_legendre(int n, double *x, double *w, double *work, void *strea
     double2 *ab = reinterpret_cast<double2 *>(work);
     gl_prepare_kernel<<<(n + 256) / 256, 256, 0, s>>>(n, ab);
     const int q = (((n + 1) / 2) + 1) / 2;
-    gl_nodes_kernel<<<(q + 127) / 128, 128, 0, s>>>(n, ab, x, w);
+    gl_nodes_kernel<<<(q + 31) / 32, 32, 0, s>>>(n, ab, x, w);      // one warp per CTA: balanced over the SMs
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(e, "gauss_legendre launch");
     return 2;

@@ -121,7 +121,8 @@ DSE_API int dse_newton_step(dse_handle *h, double *c_dev, const double *bc_dev, 
 
 /* Solves A x = b for n_sys dense row-major systems with the same equilibrated LU kernel that
  * dse_newton_step uses (exposed for tests): A_dev [n_sys][n][n], b_dev [n_sys][n], x_dev [n_sys][n],
- * stats_dev [n_sys][4] or NULL.  A_dev and b_dev are not modified.  1 <= n <= 256. */
+ * stats_dev [n_sys][4] or NULL.  A_dev and b_dev are not modified.  1 <= n <= 256; n > 128 uses the handle's own
+ * scratch and therefore requires n == 2 n_cheb and n_sys <= n_batch (else DSE_EINVAL). */
 DSE_API int dse_lu_solve(dse_handle *h, int32_t n, int32_t n_sys, const double *A_dev, const double *b_dev,
                  double *x_dev, double *stats_dev, void *stream);
 

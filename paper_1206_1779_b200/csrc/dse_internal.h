@@ -80,6 +80,9 @@ int launch_geometry(const KParams &k, double *geom, void *stream);
 bool lu_reg_eligible(int n);      // 2N <= 128: register-resident LU (dse_lu_reg.cu)
 int launch_lu_reg(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
                   double *stats, void *stream);
+bool lu_cluster_eligible(int n);  // 128 < 2N <= 256: the register-resident LU over a cluster of 4 CTAs
+int launch_lu_cluster(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
+                      double *stats, double *scratch, void *stream);
 int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
               double *stats, double *scratch, void *stream);
 int query_point_kernel(const KParams &k, PointKernelConfig &cfg);

@@ -14,7 +14,7 @@ def test_lu_solve_matches_oracle(orc):
     d = Dse(params_from_workload(CONFIGS[0]))
     rng = np.random.default_rng(5)
     for n in (1, 2, 16, 64, 128, 200):
-        if n > 158 and n != 16:
+        if n > 128 and n != 16:
             continue   # large systems use the handle's own scratch (2N only)
         A = rng.normal(size=(3, n, n)) * 10.0 ** rng.uniform(-8, 8, size=(3, n, 1))
         b = rng.normal(size=(3, n)) * np.abs(A).max(axis=2)
@@ -179,4 +179,36 @@ def test_newton_steps_batched_systems(orc):
             assert rc == 0 and abs(st[b, 0] - so[0]) <= 1e-9 * so[0] + 1e-12
         assert np.allclose(c_g.cpu().numpy(), c_o, rtol=0, atol=1e-9 * np.abs(c_o).max())
     assert st[:, 0].max() < 1e-8                             # every system converges quadratically
+    d.close()
+
+
+@pytest.mark.parametrize("N", [65, 80, 96, 128])
+def test_lu_cluster_path_exact_factorisation(orc, N):
+    """128 < 2N <= 256: the register-resident LU over a cluster of 4 CTAs (distributed shared memory, split cluster
+    barrier).  Same bar as the single-CTA kernel: solution within conditioning, factorisation bit-identical."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload
+    n = 2 * N
+    d = Dse(params_from_workload(Workload("lu", n_cheb=N, n_r=4, n_theta=4, eps2=1e-6, L2=1e4), n_batch=3))
+    rng = np.random.default_rng(N)
+    for kind in range(4):
+        if kind == 0:
+            A = rng.normal(size=(3, n, n))
+        elif kind == 1:
+            A = rng.normal(size=(3, n, n)) * 10.0 ** rng.uniform(-8, 8, size=(3, n, 1))
+        elif kind == 2:
+            A = rng.integers(-2, 3, size=(3, n, n)).astype(np.float64) + 5.0 * np.eye(n)
+        else:
+            A = rng.normal(size=(3, n, n)); A[:, :, n // 2] = 0.0
+        b = rng.normal(size=(3, n)) * np.abs(A).max(axis=2)
+        x, st = d.lu_solve(torch.from_numpy(A).cuda(), torch.from_numpy(b).cuda())
+        x = x.cpu().numpy(); st = st.cpu().numpy()
+        for s in range(3):
+            xo, so, rc = orc.lu_solve(A[s], b[s])
+            if rc == 0:
+                assert np.allclose(x[s], xo, rtol=1e-7, atol=1e-10 * np.abs(xo).max()), (n, kind)
+                assert np.array_equal(st[s][1:], so[1:]), (n, kind, st[s], so)
+            else:
+                assert np.array_equal(st[s][1:3], so[1:3]), (n, kind, st[s], so)
     d.close()

@@ -334,8 +334,10 @@ __host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc,
     return (constc ? 0 : 2 * Npad) + 2 * stash_doubles(NCH) + (geom ? GBUF_DOUBLES : 0);
 }
 
-template <int NCH_T, bool GEOM, bool CONSTC>
-__global__ void __launch_bounds__(PIPE_THREADS, 1) point_kernel_pipe(const KParams P)
+// THR: threads per CTA the register budget is compiled for (384: ~160 registers; 512: 128 registers, 16 warps per SM --
+// 2 % faster on large problems, slower on small ones)
+template <int NCH_T, bool GEOM, bool CONSTC, int THR = PIPE_THREADS>
+__global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
 {
     // lanes = (chunk of 8 j, point sub-lane); chunk counts that do not divide 32 leave 32 - NCH * SUB lanes idle in
     // phase 2 and read the zero-weight stash slot 32 for the points past the batch
@@ -643,8 +645,13 @@ double *const_slot_address()
     return static_cast<double *>(p);
 }
 
-static KernelFn pick_pipe(const KParams &k)
+constexpr int PIPE_THREADS_BIG = 512;
+static KernelFn pick_pipe(const KParams &k, bool big = false)
 {
+    if (big && k.NCH == 8) {                                     // 16 warps per SM: large problems with N = 57..64
+        if (k.use_constc) return k.geom ? point_kernel_pipe<8, true, true, PIPE_THREADS_BIG> : point_kernel_pipe<8, false, true, PIPE_THREADS_BIG>;
+        return k.geom ? point_kernel_pipe<8, true, false, PIPE_THREADS_BIG> : point_kernel_pipe<8, false, false, PIPE_THREADS_BIG>;
+    }
 #define DSE_PIPE_CASE(N)                                                                         \
     case N:                                                                                      \
         if (k.use_constc) return k.geom ? point_kernel_pipe<N, true, true> : point_kernel_pipe<N, false, true>; \
@@ -727,8 +734,18 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     cfg.batched = 0;
     KernelFn pf = (k.g == 32 && !getenv("DSE_NO_PIPE")) ? pick_pipe(k) : nullptr;
     if (pf) {
+        // large problems (>= 48 batches per warp at 16 warps per SM) with 8 chunks: the 512-thread build of the kernel
+        const long long units = k.R * (k.Ntpad / 32);
+        const int big_smem = (int)sizeof(double) * (k.Ntpad * 6 + (PIPE_THREADS_BIG / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
+        const bool big = k.NCH == 8 && units >= 48LL * sms * (PIPE_THREADS_BIG / 32) && big_smem <= smem_max && !getenv("DSE_NO_PIPE512");
+        if (big) {
+            pf = pick_pipe(k, true);
+            e = cudaFuncSetAttribute((const void *)pf, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem);
+            if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel_pipe smem)");
+            fn = (const void *)pf; block = PIPE_THREADS_BIG; jsmem = big_smem; cfg.pipelined = 2;
+        }
         // large N: fewer warps per CTA until the double-buffered stashes fit in shared memory (at least 8 warps)
-        for (int thr = PIPE_THREADS; thr >= 256; thr -= 128) {
+        for (int thr = PIPE_THREADS; !big && thr >= 256; thr -= 128) {
             const int psmem = (int)sizeof(double) * (k.Ntpad * 6 + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
             if (psmem > smem_max) continue;
             e = cudaFuncSetAttribute((const void *)pf, cudaFuncAttributeMaxDynamicSharedMemorySize, psmem);
@@ -757,7 +774,7 @@ int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
         cudaMemcpyToSymbolAsync(c_coef, k.coefP, sizeof(double2) * k.Npad, 0, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
     if (cfg.batched) return launch_point_batched(k, cfg, stream);     // Jacobian or residual-only variant
     if (k.want_jac) {
-        KernelFn fn = cfg.pipelined ? pick_pipe(k) : pick(k, true);
+        KernelFn fn = cfg.pipelined ? pick_pipe(k, cfg.pipelined == 2) : pick(k, true);
         fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
     } else {
         KParams kk = k;

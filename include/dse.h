@@ -119,6 +119,23 @@ DSE_API int dse_jacobian_fd(dse_handle *h, const double *c_dev, const double *bc
 DSE_API int dse_newton_step(dse_handle *h, double *c_dev, const double *bc_dev, double rho, double *stats_dev,
                     void *stream);
 
+/* The whole Newton-Raphson iteration (eq.(31)-(35); L226: "iterated", under-relaxed far from the solution, rho back
+ * to one close to it) on the device, with no host round trip between the steps: one CUDA graph whose WHILE node
+ * repeats the body (build J, F -> equilibrated LU -> update + convergence test) until every system has
+ * |Delta|_inf < tol (Delta = the full Newton improvement of the step, tested before relaxation; the step that
+ * passes the test is still applied) or max_iter steps have run.  Per system and step the relaxation is
+ *     rho_n = min(rho, step_cap / |Delta_n|_inf)   (step_cap > 0: no coefficient moves by more than step_cap;
+ *                                                    step_cap <= 0: rho_n = rho)             [DESIGN.md reading A26]
+ * A system that has converged, or whose Delta is not finite (singular J), is frozen; the others go on.
+ * c_dev [n_batch][2N] in/out, bc_dev [n_batch][2];  info_dev [n_batch][6] (may be NULL) =
+ *   { steps taken, |Delta|_inf of the last step, row-scaled |F|_inf of the last step, smallest |pivot| over all
+ *     steps, rho_n of the last step, status: 1 converged, 0 max_iter reached, -1 non-finite Delta }.
+ * 0 < rho <= 1, tol >= 0 (0: always run max_iter steps), 1 <= max_iter.  Asynchronous on `stream`; the graph is
+ * built at the first call and kept in the handle; the iterates live in the handle's own buffers, so calls on one
+ * handle must be issued on one stream at a time (as for every other call that uses the workspace). */
+DSE_API int dse_newton_solve(dse_handle *h, double *c_dev, const double *bc_dev, double rho, double step_cap, double tol,
+                             int32_t max_iter, double *info_dev, void *stream);
+
 /* Solves A x = b for n_sys dense row-major systems with the same equilibrated LU kernel that
  * dse_newton_step uses (exposed for tests): A_dev [n_sys][n][n], b_dev [n_sys][n], x_dev [n_sys][n],
  * stats_dev [n_sys][4] or NULL.  A_dev and b_dev are not modified.  1 <= n <= 256; n > 128 uses the handle's own

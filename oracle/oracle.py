@@ -154,3 +154,28 @@ class Oracle:
         stats = np.empty(4)
         rc = self.lib.orc_newton_step(C.byref(p), _ptr(c), float(gG), float(gZ), float(rho), _ptr(stats))
         return c, stats, rc
+
+    def newton_solve(self, p, c, gG, gZ, rho=1.0, step_cap=0.0, tol=1e-12, max_iter=50):
+        """The Newton-Raphson iteration, eq.(31)-(35) L218-273, with the under-relaxation of L226 ("used to relax the
+        system ... After some iteration steps, this parameter can be set back to one"): the paper gives no rule for
+        rho_n; reading A26 takes rho_n = min(rho, step_cap / |Delta_n|_inf) (no coefficient moves by more
+        than step_cap; step_cap <= 0: rho_n = rho).  Step by step: build F, J -> solve J Delta = F -> c <- c - rho_n
+        Delta; stop after the step whose |Delta|_inf < tol.  Returns (c, [(|Delta|inf, |F|inf scaled, min pivot,
+        rho_n) per step], status) with status 1 converged, 0 max_iter reached, -1 non-finite Delta (c left as it was).
+        Pinned by P9 (tests/test_oracle_path.py): the paper's printed alpha(M_Z^2), alpha(0), kappa."""
+        c = _f64(c).copy()
+        hist = []
+        for _ in range(int(max_iter)):
+            F, J = self.residual_jacobian(p, c, gG, gZ)
+            d, st, rc = self.lu_solve(J, F)
+            if not np.isfinite(st[0]):
+                hist.append((st[0], st[1], st[2], 0.0))
+                return c, hist, -1
+            r = rho
+            if step_cap > 0.0 and rho * st[0] > step_cap:
+                r = step_cap / st[0]
+            c = c - r * d
+            hist.append((st[0], st[1], st[2], r))
+            if st[0] < tol:
+                return c, hist, 1
+        return c, hist, 0

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
 
 EXPORTS = [
-    "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_lu_solve",
+    "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_newton_solve", "dse_lu_solve",
     "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count", "dse_kernel_info",
     "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_gauss_legendre", "dse_schwinger", "dse_jacobian_fd", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
 ]
@@ -55,6 +55,7 @@ def load_library():
     L.dse_residual.argtypes = [vp, dp, dp, dp, vp]
     L.dse_jacobian.argtypes = [vp, dp, dp, dp, dp, vp]
     L.dse_newton_step.argtypes = [vp, dp, dp, C.c_double, dp, vp]
+    L.dse_newton_solve.argtypes = [vp, dp, dp, C.c_double, C.c_double, C.c_double, C.c_int32, dp, vp]
     L.dse_lu_solve.argtypes = [vp, C.c_int32, C.c_int32, dp, dp, dp, dp, vp]
     L.dse_jacobian_host.argtypes = [vp, dp, dp, dp, dp]
     L.dse_n_ext.argtypes = [vp]
@@ -165,6 +166,17 @@ class Dse:
         _check(self.lib.dse_newton_step(self._h, _dev_ptr(c, self.B * 2 * self.N), _dev_ptr(bc, 2 * self.B),
                                         float(rho), _dev_ptr(stats, 4 * self.B), _stream_ptr(stream)))
         return stats
+
+    def newton_solve(self, c, bc, rho=1.0, step_cap=0.0, tol=1e-12, max_iter=50, info=None, stream=None):
+        """Whole Newton iteration on the device (one CUDA graph, no host round trips); c is updated in place.
+        Returns info [n_batch, 6] = (steps, |Delta|inf, |F|inf, min |pivot|, last rho_n, status)."""
+        import torch
+        if info is None:
+            info = torch.empty((self.B, 6), dtype=torch.float64, device=c.device)
+        _check(self.lib.dse_newton_solve(self._h, _dev_ptr(c, self.B * 2 * self.N), _dev_ptr(bc, 2 * self.B), float(rho),
+                                         float(step_cap), float(tol), int(max_iter), _dev_ptr(info, 6 * self.B),
+                                         _stream_ptr(stream)))
+        return info
 
     def lu_solve(self, A, b, stream=None):
         import torch

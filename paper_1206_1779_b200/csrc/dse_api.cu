@@ -26,6 +26,8 @@ struct dse_handle {
     double *d_geom = nullptr;       // geometry cache (optional)
     double *d_J = nullptr, *d_F = nullptr, *d_lu = nullptr;   // internal J, F for dse_newton_step (+ LU scratch)
     double *d_fd = nullptr;
+    double *d_delta = nullptr, *d_stats = nullptr, *d_ctl = nullptr, *d_info = nullptr;   // dse_newton_solve
+    dse::SolveGraph *solve = nullptr;                                                     // built at the first solve
     double *d_c = nullptr, *d_bc = nullptr, *d_Jh = nullptr, *d_Fh = nullptr;   // staging for *_host calls
     int64_t launches = 0;
     bool owns_const = false;
@@ -229,6 +231,8 @@ int dse_create(const dse_params *params, dse_handle **out)
     const size_t o_c = carve<double>(off, (size_t)k.B * n2), o_bc = carve<double>(off, (size_t)k.B * 2);
     const size_t o_dbg = carve<double>(off, (size_t)k.W * 5);
     const size_t o_fd = carve<double>(off, (size_t)k.B * n2 * 3);          // finite-difference self-check: c_tmp, F+, F-
+    const size_t o_dl = carve<double>(off, (size_t)k.B * n2), o_st = carve<double>(off, (size_t)k.B * 4);
+    const size_t o_ctl = carve<double>(off, 8), o_info = carve<double>(off, (size_t)k.B * 6);
     if (cudaMalloc(&h->d_work, 8 * off) != cudaSuccess) { dse_destroy(h); return DSE_ENOMEM; }
     e = cudaMemset(h->d_work, 0, 8 * off);
     if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemset(workspace)"); }
@@ -237,6 +241,7 @@ int dse_create(const dse_params *params, dse_handle **out)
     k.Apart = wk + o_A; k.AHead = wk + o_AH; k.Spart = wk + o_S; k.Rz = wk + o_R; k.dbg = wk + o_dbg; h->d_fd = wk + o_fd;
     h->d_J = wk + o_J; h->d_F = wk + o_F; h->d_lu = wk + o_lu; h->d_c = wk + o_c; h->d_bc = wk + o_bc;
     h->d_Jh = h->d_J; h->d_Fh = h->d_F;
+    h->d_delta = wk + o_dl; h->d_stats = wk + o_st; h->d_ctl = wk + o_ctl; h->d_info = wk + o_info;
 
     if (k.geom) {
         rc = dse::launch_geometry(k, h->d_geom, nullptr);
@@ -254,6 +259,7 @@ int dse_destroy(dse_handle *h)
     if (!h) return DSE_OK;
     cudaDeviceSynchronize();
     if (h->owns_const) dse::release_const_slot();
+    dse::solve_graph_destroy(h->solve);
     if (h->d_tables) cudaFree(h->d_tables);
     if (h->d_work) cudaFree(h->d_work);
     if (h->d_geom) cudaFree(h->d_geom);
@@ -284,6 +290,29 @@ int dse_newton_step(dse_handle *h, double *c_dev, const double *bc_dev, double r
     rc = dse::launch_lu(2 * h->k.N, h->k.B, h->d_J, h->d_F, nullptr, c_dev, rho, stats_dev, h->d_lu, stream);
     if (rc < 0) return rc;
     h->launches += rc;
+    return DSE_OK;
+}
+
+int dse_newton_solve(dse_handle *h, double *c_dev, const double *bc_dev, double rho, double step_cap, double tol,
+                     int32_t max_iter, double *info_dev, void *stream)
+{
+    if (!h || !c_dev || !bc_dev || !(rho > 0.0) || !(rho <= 1.0) || !std::isfinite(step_cap) || !(tol >= 0.0) ||
+        !std::isfinite(tol) || max_iter < 1)
+        return DSE_EINVAL;
+    const size_t n2 = 2 * (size_t)h->k.N, B = (size_t)h->k.B;
+    if (!h->solve) {
+        int rc = dse::solve_graph_create(h->k, h->cfg, h->d_c, h->d_bc, h->d_J, h->d_F, h->d_delta, h->d_stats, h->d_lu,
+                                         h->d_ctl, h->d_info, &h->solve);
+        if (rc < 0) return rc;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    CK(cudaMemcpyAsync(h->d_c, c_dev, 8 * B * n2, cudaMemcpyDeviceToDevice, s));
+    CK(cudaMemcpyAsync(h->d_bc, bc_dev, 8 * B * 2, cudaMemcpyDeviceToDevice, s));
+    int rc = dse::launch_solve(h->solve, rho, step_cap, tol, max_iter, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    CK(cudaMemcpyAsync(c_dev, h->d_c, 8 * B * n2, cudaMemcpyDeviceToDevice, s));
+    if (info_dev) CK(cudaMemcpyAsync(info_dev, h->d_info, 8 * B * 6, cudaMemcpyDeviceToDevice, s));
     return DSE_OK;
 }
 

@@ -90,6 +90,12 @@ bool acquire_const_slot(const KParams &k);
 double *const_slot_address();     // global-memory address of the slot (nullptr if unavailable)
 void release_const_slot();
 size_t lu_scratch_doubles(int n);
+// dse_solve.cu: the Newton iteration as a CUDA graph with a WHILE node (dse_newton_solve)
+struct SolveGraph;
+int solve_graph_create(const KParams &k, const PointKernelConfig &cfg, double *c, const double *bc, double *J, double *F,
+                       double *delta, double *stats, double *lu_scratch, double *ctl, double *info, SolveGraph **out);
+void solve_graph_destroy(SolveGraph *g);
+int launch_solve(SolveGraph *g, double rho, double cap, double tol, int max_iter, void *stream);
 int launch_gauss_legendre(int n, double *x, double *w, double *work, void *stream);
 int launch_schwinger(const KParams &k, const double *c, int n, double p2_min, double p2_max, const double *t, int n_t,
                      double *out, double *work, void *stream);

@@ -27,6 +27,9 @@ def start_coefficients(orc, p):
     return c
 
 
+STEP_CAP = 0.5
+
+
 def damping(dmax):
     """under-relaxation: cap the update at 0.5 until the iteration is close, then rho = 1"""
-    return min(1.0, 0.5 / dmax)
+    return min(1.0, STEP_CAP / dmax)

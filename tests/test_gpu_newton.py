@@ -212,3 +212,103 @@ def test_lu_cluster_path_exact_factorisation(orc, N):
             else:
                 assert np.array_equal(st[s][1:3], so[1:3]), (n, kind, st[s], so)
     d.close()
+
+
+# ----------------------------------------------------------------------------- dse_newton_solve (device-side iteration)
+def test_newton_solve_graph_weak_coupling(orc):
+    """The whole iteration as one CUDA graph (WHILE node) against the oracle's plain loop: same number of steps, same
+    per-step record, converged coefficients to the north_star bar (1e-9); then the call-level controls."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload
+    w = Workload("newton-weak", 10, 64, 24, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
+    d = Dse(params_from_workload(w))
+    p = oracle_params(w)
+    bc = torch.ones((1, 2), dtype=torch.float64, device="cuda")
+    c_o, hist, status = orc.newton_solve(p, np.zeros(20), 1.0, 1.0, rho=1.0, step_cap=0.0, tol=1e-12, max_iter=20)
+    assert status == 1 and 3 <= len(hist) <= 8
+    c_g = torch.zeros((1, 20), dtype=torch.float64, device="cuda")
+    info = d.newton_solve(c_g, bc, rho=1.0, step_cap=0.0, tol=1e-12, max_iter=20).cpu().numpy()[0]
+    assert info[0] == len(hist) and info[5] == 1.0
+    assert abs(info[1] - hist[-1][0]) <= 1e-9 * hist[-1][0] + 1e-12 and info[4] == 1.0
+    assert abs(info[3] - min(h[2] for h in hist)) <= 1e-9 * info[3]
+    assert np.abs(c_g.cpu().numpy()[0] - c_o).max() <= 1e-9 * np.abs(c_o).max()
+    # the same handle again, other scalars (the graph is reused): two steps only -> status 0, equal to two plain steps
+    c2 = torch.zeros((1, 20), dtype=torch.float64, device="cuda")
+    info2 = d.newton_solve(c2, bc, rho=1.0, step_cap=0.0, tol=1e-12, max_iter=2).cpu().numpy()[0]
+    c_s = torch.zeros((1, 20), dtype=torch.float64, device="cuda")
+    for _ in range(2):
+        st = d.newton_step(c_s, bc, 1.0)
+    assert info2[0] == 2 and info2[5] == 0.0
+    assert np.abs((c2 - c_s).cpu().numpy()).max() <= 1e-15 * np.abs(c_o).max()
+    assert info2[1] == st.cpu().numpy()[0, 0]
+    # tol = 0: exactly max_iter steps; under-relaxation rho = 0.5 without a cap follows the oracle
+    c3 = torch.zeros((1, 20), dtype=torch.float64, device="cuda")
+    info3 = d.newton_solve(c3, bc, rho=0.5, step_cap=0.0, tol=0.0, max_iter=6).cpu().numpy()[0]
+    c_o3, hist3, status3 = orc.newton_solve(p, np.zeros(20), 1.0, 1.0, rho=0.5, step_cap=0.0, tol=0.0, max_iter=6)
+    assert info3[0] == 6 and info3[5] == 0.0 and status3 == 0 and info3[4] == 0.5
+    assert np.abs(c3.cpu().numpy()[0] - c_o3).max() <= 1e-9 * np.abs(c_o3).max()
+    # argument checks
+    import ctypes
+    from paper_1206_1779_b200.binding import _dev_ptr, _stream_ptr
+    for bad in [(0.0, 0.0, 1e-12, 5), (1.5, 0.0, 1e-12, 5), (1.0, 0.0, -1.0, 5), (1.0, 0.0, 1e-12, 0), (float("nan"), 0.0, 1e-12, 5)]:
+        rc = d.lib.dse_newton_solve(d._h, _dev_ptr(c3), _dev_ptr(bc), ctypes.c_double(bad[0]), ctypes.c_double(bad[1]),
+                                    ctypes.c_double(bad[2]), bad[3], None, _stream_ptr())
+        assert rc == -1, bad
+    d.close()
+
+
+def test_newton_solve_graph_batched_systems(orc):
+    """Eight systems in one graph: each stops on its own criterion (frozen once converged), the loop ends with the
+    last one; every system matches its own oracle solve."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload
+    w = Workload("newton-weak-batch", 10, 48, 32, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
+    B = 8
+    d = Dse(params_from_workload(w, n_batch=B))
+    p = oracle_params(w)
+    bcs = np.stack([[1.0 + 0.001 * b, 1.0 - 0.0005 * b] for b in range(B)])     # inside the basin of plain Newton steps
+    c0 = np.zeros((B, 20))                                   # G = Z = 1 ...
+    c0[3] = orc.newton_solve(p, c0[3], bcs[3, 0], bcs[3, 1], tol=1e-13, max_iter=25)[0]   # ... but system 3 starts converged
+    c_g = torch.from_numpy(c0.copy()).cuda()
+    info = d.newton_solve(c_g, torch.from_numpy(bcs).cuda(), rho=1.0, step_cap=0.5, tol=1e-10, max_iter=25).cpu().numpy()
+    c = c_g.cpu().numpy()
+    steps = []
+    for b in range(B):
+        c_o, hist, status = orc.newton_solve(p, c0[b], bcs[b, 0], bcs[b, 1], rho=1.0, step_cap=0.5, tol=1e-10, max_iter=25)
+        assert status == 1 and info[b, 5] == 1.0
+        assert info[b, 0] == len(hist), (b, info[b], len(hist))
+        assert np.abs(c[b] - c_o).max() <= 1e-9 * np.abs(c_o).max()
+        steps.append(len(hist))
+    assert steps[3] == 1 and len(set(steps)) >= 3            # the systems really stop at different steps
+    d.close()
+
+
+def test_newton_solve_graph_paper_scaling_solution(orc):
+    """The paper's own parameter set (L135, L364) solved by ONE call: same step count and converged coefficients as
+    the oracle's loop with the same relaxation rule (reading A26), and the paper's printed alpha(M_Z^2), alpha(0)."""
+    torch = _torch()
+    import math
+    import scaling_setup as S
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload
+    w = Workload("paper-scaling", S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, x_G=0.0, x_Z=S.L2, n_ir=S.N_IR)
+    p = oracle_params(w)
+    c0 = S.start_coefficients(orc, p)
+    c_o, hist, status = orc.newton_solve(p, c0, S.G_G, S.G_Z, rho=1.0, step_cap=S.STEP_CAP, tol=1e-11, max_iter=30)
+    assert status == 1
+    d = Dse(params_from_workload(w, flags=1))
+    c_g = torch.from_numpy(c0[None, :].copy()).cuda()
+    bc = torch.tensor([[S.G_G, S.G_Z]], dtype=torch.float64, device="cuda")
+    info = d.newton_solve(c_g, bc, rho=1.0, step_cap=S.STEP_CAP, tol=1e-11, max_iter=30).cpu().numpy()[0]
+    assert info[5] == 1.0 and info[0] == len(hist)
+    c = c_g.cpu().numpy()[0]
+    assert np.abs(c - c_o).max() <= 1e-9 * np.abs(c_o).max()
+
+    def alpha(xv):
+        g, z = orc.ln_dress(p, c, xv)
+        return math.exp(2 * g + z)
+
+    assert abs(alpha(91.2 ** 2) - 0.118) < 1e-3 and abs(alpha(S.EPS2) - 2.972) < 5e-3      # PAPER.md L143, L151
+    d.close()

@@ -330,16 +330,10 @@ def test_paper_scaling_solution_P9(orc, n_r, n_theta, rule, split):
             gold[f[0]] = float(f[1])
     p = make_params(S.N, n_r, n_theta, S.EPS2, S.L2, 0.0, S.L2, n_ir=S.N_IR, angular_rule=rule, radial_split=split)
     c = S.start_coefficients(orc, p)
-    dn = []
-    for it in range(30):
-        F, J = orc.residual_jacobian(p, c, S.G_G, S.G_Z)
-        d, st, rc = orc.lu_solve(J, F)
-        assert rc == 0
-        c = c - S.damping(st[0]) * d
-        dn.append(st[0])
-        if st[0] < 1e-11:
-            break
-    assert dn[-1] < 1e-11 and len(dn) <= 15
+    c, hist, status = orc.newton_solve(p, c, S.G_G, S.G_Z, rho=1.0, step_cap=S.STEP_CAP, tol=1e-11, max_iter=30)
+    dn = [h[0] for h in hist]
+    assert status == 1 and dn[-1] < 1e-11 and len(dn) <= 15
+    assert all(h[3] == S.damping(h[0]) for h in hist)                  # the relaxation rule of reading A26
     assert dn[-2] < 1e-5 and dn[-1] < 100 * dn[-2] ** 2 + 1e-12       # quadratic at the end (L226)
 
     def alpha(x):

@@ -188,7 +188,8 @@ DSE_API int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, d
 /* Environment switches for A/B measurements and tests (read in dse_create unless noted; none changes results beyond
  * rounding order): DSE_NO_BATCHED (per-system point kernels for batches), DSE_NO_PIPE (non-pipelined point kernel),
  * DSE_CONST_MEMCPY (coefficient slot filled by a device-to-device copy instead of prep_kernel's direct store),
- * DSE_NO_FUSED_ASSEMBLE and DSE_LU_BLOCKED (separate contraction kernel / shared-memory LU; read once per process). */
+ * DSE_NO_FUSED_ASSEMBLE, DSE_LU_BLOCKED and DSE_NO_PDL (separate contraction kernel / shared-memory LU / plain launches
+ * instead of programmatic dependent launches between the kernels of a build; read once per process). */
 
 /* Diagnostics: cycles summed over all warps of the last point-kernel launch, spent in (geometry, series,
  * exp + weights, accumulation, whole warp).  All zeros unless the library was built with

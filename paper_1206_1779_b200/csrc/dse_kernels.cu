@@ -24,6 +24,7 @@ namespace {
 __global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double *__restrict__ c)
 {
     // grid (tiles, B); one WARP per fixed point (y_q or x_i), lanes over j, fixed xor-tree reduction
+    pdl_trigger();
     const int b = blockIdx.y;
     const int lane = threadIdx.x & 31;
     const int item = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -100,6 +101,8 @@ template <int NTG>
 __global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
 {
     __shared__ double s_c[GEMM_WARPS][3][32][2];
+    pdl_trigger();
+    pdl_wait();                                              // row sums of the point kernel
     const int lane = threadIdx.x & 31, wk = threadIdx.x >> 5, nwarps = blockDim.x >> 5;   // 3 <= nwarps <= GEMM_WARPS
     const int e0 = blockIdx.x * 8, n0 = blockIdx.y * 8 * NTG, b = blockIdx.z;
     const int ae = e0 + (lane >> 2), ak = lane & 3;          // A fragment: row = lane/4 (external point), col = lane%4 (q)
@@ -160,6 +163,8 @@ __global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
 __global__ void __launch_bounds__(128) contract_split_kernel(const KParams P)
 {
     const int e = blockIdx.x, b = blockIdx.y;
+    pdl_trigger();
+    pdl_wait();                                              // row sums of the point kernel
     const size_t rowbase = ((size_t)b * P.Next + e) * P.Nr;
     const double4 *A = reinterpret_cast<const double4 *>(P.Apart) + rowbase;
     const double4 *H = reinterpret_cast<const double4 *>(P.AHead) + rowbase;
@@ -218,6 +223,8 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
                     bi_G = (long long)b * P.Next + P.iG;
     __shared__ double s_pw[ASM_THREADS / 32][3][2];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    pdl_trigger();
+    pdl_wait();                                              // partials, row sums, A.Phi of the kernels before
     // All global loads of the CTA (row sums for Pi, partial slots, the fused contraction) are issued before its single
     // barrier, so their latencies overlap; the combination steps after the barrier read shared memory only.
     const int npi = (P.iG != P.iZ) ? 3 : 2;
@@ -466,23 +473,23 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     const bool fused = kk.want_jac && !kk.rstride && kk.B < 8 && (long long)kk.Nr * kk.Npad <= 16384 && !no_fused;
     if (kk.want_jac && !fused) {
         if (kk.rstride) {
-            contract_split_kernel<<<dim3(kk.Next, kk.B), 128, 0, s>>>(kk);
+            launch_pdl(contract_split_kernel, dim3(kk.Next, kk.B), dim3(128), 0, s, kk);
         } else if (kk.B >= 8) {
             // many systems: 4 n-tiles per CTA and 4 warps, the grid fills the GPU and every row-sum record is read
             // once per 32 values of j
             dim3 gg((kk.Next + 7) / 8, (kk.Npad / 8 + 3) / 4, kk.B);
-            gemm_kernel<4><<<gg, 4 * 32, 0, s>>>(kk);
+            launch_pdl(gemm_kernel<4>, gg, dim3(4 * 32), 0, s, kk);
         } else {
             dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);        // one n-tile per CTA, K split over 16 warps (latency)
-            gemm_kernel<1><<<gg, GEMM_WARPS * 32, 0, s>>>(kk);
+            launch_pdl(gemm_kernel<1>, gg, dim3(GEMM_WARPS * 32), 0, s, kk);
         }
         ++launches;
     }
     dim3 ga(kk.N, kk.B);
     if (fused)
-        assemble_kernel<true><<<ga, ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
+        launch_pdl(assemble_kernel<true>, ga, dim3(ASM_THREADS), 0, s, kk, bc_dev, J_dev, F_dev);
     else    // many systems: few slots per external point, small CTAs keep more of them resident
-        assemble_kernel<false><<<ga, kk.B >= 8 ? 128 : ASM_THREADS, 0, s>>>(kk, bc_dev, J_dev, F_dev);
+        launch_pdl(assemble_kernel<false>, ga, dim3(kk.B >= 8 ? 128 : ASM_THREADS), 0, s, kk, bc_dev, J_dev, F_dev);
     ++launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "build launch");

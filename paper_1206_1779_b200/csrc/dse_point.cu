@@ -49,6 +49,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
 
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
     if (lane == 0) s_pt[32] = make_double4(0.0, 0.0, 0.0, 0.0);
+    pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q)
     __syncthreads();
 
     const int Nr = P.Nr, g = P.g;
@@ -353,6 +354,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
     double4 *s_gbuf = reinterpret_cast<double4 *>(s_stash + 2 * STASH);     // [2][32] geometry records
 
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q)
     __syncthreads();
 
     const int Nr = P.Nr, BPR = P.Ntpad >> 5;                                 // batches per row
@@ -775,11 +777,11 @@ int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
     if (cfg.batched) return launch_point_batched(k, cfg, stream);     // Jacobian or residual-only variant
     if (k.want_jac) {
         KernelFn fn = cfg.pipelined ? pick_pipe(k, cfg.pipelined == 2) : pick(k, true);
-        fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
+        launch_pdl(fn, dim3(cfg.grid), dim3(cfg.block), (size_t)cfg.smem, (cudaStream_t)stream, k);
     } else {
         KParams kk = k;
         kk.W = cfg.res_grid * (cfg.res_block / 32);          // the residual build has its own row partition
-        pick(k, false)<<<cfg.res_grid, cfg.res_block, cfg.res_smem, (cudaStream_t)stream>>>(kk);
+        launch_pdl(pick(k, false), dim3(cfg.res_grid), dim3(cfg.res_block), (size_t)cfg.res_smem, (cudaStream_t)stream, kk);
     }
     return 1;
 }

@@ -51,6 +51,7 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
     double4 *s_gbuf = reinterpret_cast<double4 *>(sT + 8 * BT_TS);                  // [2][32] geometry records
     double *sC = sT + 8 * BT_TS + GBUF_DOUBLES;                                     // [BT_KS][2][32] coefficient fragments
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q)
     __syncthreads();
 
     const int Nr = P.Nr, BPR = P.Ntpad >> 5, NG = P.Gext * Nr;
@@ -342,7 +343,7 @@ int query_point_batched(const KParams &k, PointKernelConfig &cfg)
 
 int launch_point_batched(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
-    batched_variant(k, k.want_jac != 0).fn<<<cfg.grid, cfg.block, cfg.smem, (cudaStream_t)stream>>>(k);
+    launch_pdl(batched_variant(k, k.want_jac != 0).fn, dim3(cfg.grid), dim3(cfg.block), (size_t)cfg.smem, (cudaStream_t)stream, k);
     return 1;
 }
 

@@ -185,6 +185,13 @@ DSE_API int dse_gauss_legendre(int32_t n, double *x_dev, double *w_dev, double *
 DSE_API int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, double p2_min, double p2_max,
                           const double *t_dev, int32_t n_t, double *delta_dev, double *work_dev, void *stream);
 
+/* The dressing functions of a coefficient set at arbitrary momenta (what a solve is run for: PAPER.md Fig. 3-5):
+ * ln G(x_m), ln Z(x_m) from the series eq.(23),(24) on the clamped argument s(x) (eq.(25)) plus the continuations
+ * eq.(16)-(19) below eps2 and above L2, and the running coupling alpha(x_m) = alpha(mu^2) G^2(x_m) Z(x_m) (L145).
+ * x_dev [n_x], all > 0; outputs [n_batch][n_x], any of them may be NULL (not all).  Asynchronous on `stream`. */
+DSE_API int dse_dressing(dse_handle *h, const double *c_dev, const double *x_dev, int32_t n_x, double *lnG_dev,
+                         double *lnZ_dev, double *alpha_dev, void *stream);
+
 /* Environment switches for A/B measurements and tests (read in dse_create unless noted; none changes results beyond
  * rounding order): DSE_NO_BATCHED (per-system point kernels for batches), DSE_NO_PIPE (non-pipelined point kernel),
  * DSE_CONST_MEMCPY (coefficient slot filled by a device-to-device copy instead of prep_kernel's direct store),

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
 EXPORTS = [
     "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_newton_solve", "dse_lu_solve",
     "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count", "dse_kernel_info",
-    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_gauss_legendre", "dse_schwinger", "dse_jacobian_fd", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
+    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_gauss_legendre", "dse_schwinger", "dse_dressing", "dse_jacobian_fd", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
@@ -69,6 +69,7 @@ def load_library():
     L.dse_jacobian_fd.argtypes = [vp, dp, dp, C.c_double, dp, vp]
     L.dse_gauss_legendre.argtypes = [C.c_int32, dp, dp, dp, vp]
     L.dse_schwinger.argtypes = [vp, dp, C.c_int32, C.c_double, C.c_double, dp, C.c_int32, dp, dp, vp]
+    L.dse_dressing.argtypes = [vp, dp, dp, C.c_int32, dp, dp, dp, vp]
     L.dse_dfma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
     L.dse_dmma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
     L.dse_strerror.argtypes = [C.c_int]
@@ -197,6 +198,15 @@ class Dse:
                                       _stream_ptr(stream)))
         self._keep = work            # the call is asynchronous: keep the workspace alive until the next call
         return out
+
+    def dressing(self, c, x, stream=None):
+        """ln G(x), ln Z(x), alpha(x) = alpha(mu^2) G^2 Z for every system: three [n_batch, len(x)] tensors."""
+        import torch
+        n_x = x.numel()
+        out = [torch.empty((self.B, n_x), dtype=torch.float64, device=c.device) for _ in range(3)]
+        _check(self.lib.dse_dressing(self._h, _dev_ptr(c, self.B * 2 * self.N), _dev_ptr(x), n_x, _dev_ptr(out[0]),
+                                     _dev_ptr(out[1]), _dev_ptr(out[2]), _stream_ptr(stream)))
+        return tuple(out)
 
     def jacobian_host(self, c_host: np.ndarray, bc_host: np.ndarray, J_host: np.ndarray, F_host: np.ndarray):
         """Host buffers in, host buffers out (numpy float64, C-contiguous; pinned memory recommended)."""

@@ -410,6 +410,16 @@ int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, double p2
     return DSE_OK;
 }
 
+int dse_dressing(dse_handle *h, const double *c_dev, const double *x_dev, int32_t n_x, double *lnG_dev, double *lnZ_dev,
+                 double *alpha_dev, void *stream)
+{
+    if (!h || !c_dev || !x_dev || n_x < 1 || (!lnG_dev && !lnZ_dev && !alpha_dev)) return DSE_EINVAL;
+    int rc = dse::launch_dressing(h->k, c_dev, n_x, x_dev, h->params.alpha_mu, lnG_dev, lnZ_dev, alpha_dev, stream);
+    if (rc < 0) return rc;
+    h->launches += rc;
+    return DSE_OK;
+}
+
 int dse_get_phase_cycles(dse_handle *h, double out_host[5])
 {
     if (!h || !out_host) return DSE_EINVAL;

@@ -99,6 +99,8 @@ int launch_solve(SolveGraph *g, double rho, double cap, double tol, int max_iter
 int launch_gauss_legendre(int n, double *x, double *w, double *work, void *stream);
 int launch_schwinger(const KParams &k, const double *c, int n, double p2_min, double p2_max, const double *t, int n_t,
                      double *out, double *work, void *stream);
+int launch_dressing(const KParams &k, const double *c, int n_x, const double *x, double alpha_mu, double *lnG, double *lnZ,
+                    double *alpha, void *stream);
 int launch_dfma_probe(int blocks, int iters, double *sink, void *stream);
 int launch_dmma_probe(int blocks, int iters, double *sink, void *stream);
 

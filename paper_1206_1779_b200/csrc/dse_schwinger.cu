@@ -188,6 +188,47 @@ int launch_gauss_legendre(int n, double *x, double *w, double *work, void *strea
     return 2;
 }
 
+// ln G(x_m), ln Z(x_m) for every system at arbitrary momenta x_m > 0: the series eq.(23),(24) on the clamped argument
+// plus the continuations eq.(16)-(19) outside [eps2, L2] (the same definition the point kernel uses at z), and the
+// running coupling alpha(x) = alpha(mu^2) G^2 Z.  One thread per (system, momentum).
+__global__ void dressing_kernel(const KParams P, const double *__restrict__ c, int n_x, const double *__restrict__ x,
+                                double alpha_mu, double *__restrict__ lnG_out, double *__restrict__ lnZ_out,
+                                double *__restrict__ alpha_out)
+{
+    const int b = blockIdx.y;
+    const double *a = c + (size_t)b * 2 * P.N, *bb = a + P.N;      // a_j <-> ln Z, b_j <-> ln G
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_x; i += gridDim.x * blockDim.x) {
+        const double u = x[i];
+        const double ell = log(u * P.inv_eps2);
+        double s = fma(ell, P.two_over_Lg, -1.0), EG = 0.0, EZ = 0.0;
+        if (u < P.eps2) { EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0; }
+        else if (u > P.L2) { const double t = log(fma(P.omega, ell - P.Lg, 1.0)); EG = P.delta * t; EZ = P.gamma * t; s = 1.0; }
+        s = fmin(1.0, fmax(-1.0, s));
+        double tm = 1.0, t = s;
+        double lnZ = 0.5 * a[0] + (P.N > 1 ? a[1] * s : 0.0), lnG = 0.5 * bb[0] + (P.N > 1 ? bb[1] * s : 0.0);
+        for (int j = 2; j < P.N; ++j) {
+            const double tn = fma(2.0 * s, t, -tm);
+            tm = t; t = tn;
+            lnZ = fma(a[j], tn, lnZ);
+            lnG = fma(bb[j], tn, lnG);
+        }
+        lnZ += EZ; lnG += EG;
+        const size_t o = (size_t)b * n_x + i;
+        if (lnG_out) lnG_out[o] = lnG;
+        if (lnZ_out) lnZ_out[o] = lnZ;
+        if (alpha_out) alpha_out[o] = alpha_mu * exp(2.0 * lnG + lnZ);
+    }
+}
+
+int launch_dressing(const KParams &k, const double *c, int n_x, const double *x, double alpha_mu, double *lnG, double *lnZ,
+                    double *alpha, void *stream)
+{
+    dressing_kernel<<<dim3((n_x + 127) / 128, k.B), 128, 0, (cudaStream_t)stream>>>(k, c, n_x, x, alpha_mu, lnG, lnZ, alpha);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(e, "dressing launch");
+    return 1;
+}
+
 // work: (5 + B) n + 4 doubles:  ab[2(n+1)] | x[n] | w[n] | p[n] | f[B][n]
 int launch_schwinger(const KParams &k, const double *c, int n, double p2_min, double p2_max, const double *t, int n_t,
                      double *out, double *work, void *stream)

@@ -306,9 +306,12 @@ def test_newton_solve_graph_paper_scaling_solution(orc):
     c = c_g.cpu().numpy()[0]
     assert np.abs(c - c_o).max() <= 1e-9 * np.abs(c_o).max()
 
-    def alpha(xv):
-        g, z = orc.ln_dress(p, c, xv)
-        return math.exp(2 * g + z)
-
-    assert abs(alpha(91.2 ** 2) - 0.118) < 1e-3 and abs(alpha(S.EPS2) - 2.972) < 5e-3
+    # the coupling at M_Z^2 and its infrared fixed point, evaluated on the device (dse_dressing)
+    xs = torch.tensor([91.2 ** 2, S.EPS2, 1e-9, 1e-8], dtype=torch.float64, device="cuda")
+    lnG, lnZ, al = (t.cpu().numpy()[0] for t in d.dressing(c_g, xs))
+    assert abs(al[0] - 0.118) < 1e-3 and abs(al[1] - 2.972) < 5e-3
+    g, z = orc.ln_dress(p, c, 91.2 ** 2)
+    assert abs(al[0] - math.exp(2 * g + z)) < 1e-12
+    kap = -(lnG[3] - lnG[2]) / math.log(10.0)               # G ~ x^-kappa below eps2 (eq.(17))
+    assert abs(kap - S.KAPPA) < 1e-9
     d.close()

@@ -73,3 +73,31 @@ def test_schwinger_batched_random_dressings(orc):
         ref = orc.schwinger(oracle_params(w), c[b], 2048, 1e-10, 2e5, t)
         assert np.allclose(out[b], ref, rtol=1e-10, atol=1e-12 * np.abs(ref).max())
     d.close()
+
+
+def test_dressing_functions_and_coupling_parity(orc):
+    """dse_dressing: ln G, ln Z (series eq.(23),(24) + continuations eq.(16)-(19)) and alpha(x) = alpha(mu^2) G^2 Z (L145)
+    at momenta below eps2, inside the grid, at both matching points and above L2, for several systems."""
+    import math
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    w = Workload("dress", 24, 16, 32, 1e-6, 5e4, x_G=1.0, x_Z=1.0, alpha_mu=0.7)
+    B = 3
+    p = oracle_params(w)
+    c = np.stack([draw_coefficients(70 + b, w.n_cheb) for b in range(B)])
+    x = np.concatenate([np.logspace(-12, -6, 9), [w.eps2, w.L2], np.logspace(-5.9, 4.6, 40), np.logspace(4.7, 5.3, 7),
+                        [w.eps2 * (1 - 1e-12), w.L2 * (1 + 1e-12)]])
+    d = Dse(params_from_workload(w, n_batch=B))
+    lnG, lnZ, al = (t.cpu().numpy() for t in d.dressing(torch.from_numpy(c).cuda(), torch.from_numpy(x).cuda()))
+    for b in range(B):
+        for m, xv in enumerate(x):
+            g, z = orc.ln_dress(p, c[b], float(xv))
+            assert abs(lnG[b, m] - g) <= 1e-12 * max(1.0, abs(g)), (b, xv)
+            assert abs(lnZ[b, m] - z) <= 1e-12 * max(1.0, abs(z)), (b, xv)
+            assert abs(al[b, m] - 0.7 * math.exp(2 * g + z)) <= 1e-11 * al[b, m]
+    # infrared power laws of the continuation: d ln G / d ln x = ir_exp_G, d ln Z / d ln x = ir_exp_Z below eps2
+    i0, i1 = 0, 5
+    dl = math.log(x[i1] / x[i0])
+    assert abs((lnG[0, i1] - lnG[0, i0]) / dl - w.ir_exp_G) < 1e-10 and abs((lnZ[0, i1] - lnZ[0, i0]) / dl - w.ir_exp_Z) < 1e-10
+    d.close()

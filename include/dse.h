@@ -143,8 +143,10 @@ DSE_API int dse_newton_solve(dse_handle *h, double *c_dev, const double *bc_dev,
 DSE_API int dse_lu_solve(dse_handle *h, int32_t n, int32_t n_sys, const double *A_dev, const double *b_dev,
                  double *x_dev, double *stats_dev, void *stream);
 
-/* Host-buffer convenience (used for the end-to-end measurement): copies c, bc to the device,
- * runs dse_jacobian, copies J, F back; synchronous.  J_host may be NULL (then dse_residual). */
+/* Host-buffer convenience (used for the end-to-end measurement): c, bc go to the device in one staged copy, dse_jacobian
+ * runs, J, F come back -- up to 1 MiB of results are written by the assemble kernel straight into a mapped pinned buffer of
+ * the handle (no copy node on the stream), larger ones are copied back; synchronous on the legacy default stream.
+ * J_host may be NULL (then dse_residual).  The staging buffers are allocated at the first call. */
 DSE_API int dse_jacobian_host(dse_handle *h, const double *c_host, const double *bc_host, double *J_host,
                       double *F_host);
 

@@ -29,6 +29,10 @@ struct dse_handle {
     double *d_delta = nullptr, *d_stats = nullptr, *d_ctl = nullptr, *d_info = nullptr;   // dse_newton_solve
     dse::SolveGraph *solve = nullptr;                                                     // built at the first solve
     double *d_c = nullptr, *d_bc = nullptr, *d_Jh = nullptr, *d_Fh = nullptr;   // staging for *_host calls
+    // dse_jacobian_host: pinned host staging.  h_in [c | bc] goes to the device in ONE copy (d_c, d_bc are adjacent);
+    // small results are written by the assemble kernel straight into the mapped buffer h_out [J | F] (no copy node)
+    double *h_in = nullptr, *h_out = nullptr, *m_out = nullptr;   // m_out = device alias of h_out
+    static constexpr size_t ZERO_COPY_MAX_BYTES = 1u << 20;
     int64_t launches = 0;
     bool owns_const = false;
     // optional timing of the point kernel (dse_set_timing)
@@ -263,6 +267,8 @@ int dse_destroy(dse_handle *h)
     if (h->d_tables) cudaFree(h->d_tables);
     if (h->d_work) cudaFree(h->d_work);
     if (h->d_geom) cudaFree(h->d_geom);
+    if (h->h_in) cudaFreeHost(h->h_in);
+    if (h->h_out) cudaFreeHost(h->h_out);
     for (auto &p : h->ev)
         for (auto &e : p)
             if (e) cudaEventDestroy(e);
@@ -337,12 +343,29 @@ int dse_jacobian_host(dse_handle *h, const double *c_host, const double *bc_host
 {
     if (!h || !c_host || !bc_host || !F_host) return DSE_EINVAL;
     const size_t n2 = 2 * (size_t)h->k.N, B = (size_t)h->k.B;
-    CK(cudaMemcpyAsync(h->d_c, c_host, 8 * B * n2, cudaMemcpyHostToDevice, nullptr));
-    CK(cudaMemcpyAsync(h->d_bc, bc_host, 8 * B * 2, cudaMemcpyHostToDevice, nullptr));
+    const size_t n_in = B * n2 + B * 2, n_J = B * n2 * n2, n_F = B * n2;
+    if (!h->h_in) {                                      // first call: pinned staging (inputs) and mapped staging (results)
+        CK(cudaHostAlloc((void **)&h->h_in, 8 * n_in, cudaHostAllocDefault));
+        if (8 * (n_J + n_F) <= dse_handle::ZERO_COPY_MAX_BYTES) {
+            CK(cudaHostAlloc((void **)&h->h_out, 8 * (n_J + n_F), cudaHostAllocMapped));
+            CK(cudaHostGetDevicePointer((void **)&h->m_out, h->h_out, 0));
+        }
+    }
+    memcpy(h->h_in, c_host, 8 * B * n2);
+    memcpy(h->h_in + B * n2, bc_host, 8 * B * 2);
+    CK(cudaMemcpyAsync(h->d_c, h->h_in, 8 * n_in, cudaMemcpyHostToDevice, nullptr));      // d_bc = d_c + B*2N
+    if (h->m_out) {
+        int rc = do_build(h, h->d_c, h->d_bc, J_host ? h->m_out : nullptr, h->m_out + n_J, nullptr);
+        if (rc < 0) return rc;
+        CK(cudaStreamSynchronize(nullptr));
+        if (J_host) memcpy(J_host, h->h_out, 8 * n_J);
+        memcpy(F_host, h->h_out + n_J, 8 * n_F);
+        return DSE_OK;
+    }
     int rc = do_build(h, h->d_c, h->d_bc, J_host ? h->d_Jh : nullptr, h->d_Fh, nullptr);
     if (rc < 0) return rc;
-    if (J_host) CK(cudaMemcpyAsync(J_host, h->d_Jh, 8 * B * n2 * n2, cudaMemcpyDeviceToHost, nullptr));
-    CK(cudaMemcpyAsync(F_host, h->d_Fh, 8 * B * n2, cudaMemcpyDeviceToHost, nullptr));
+    if (J_host) CK(cudaMemcpyAsync(J_host, h->d_Jh, 8 * n_J, cudaMemcpyDeviceToHost, nullptr));
+    CK(cudaMemcpyAsync(F_host, h->d_Fh, 8 * n_F, cudaMemcpyDeviceToHost, nullptr));
     CK(cudaStreamSynchronize(nullptr));
     return DSE_OK;
 }

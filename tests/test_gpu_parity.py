@@ -276,3 +276,41 @@ def test_random_shapes_against_oracle(orc):
             assert en <= TOL_NORM and ef <= TOL_NORM, (kw, B, flags, en, ef)
             assert np.allclose(F2[b], F[b], rtol=1e-11, atol=1e-13 * np.abs(F[b]).max()), kw
     assert seen == {"generic", "pipelined", "batched-dmma"}
+
+
+def test_host_buffer_entry_point_and_back_to_back_builds(orc):
+    """dse_jacobian_host (the end-to-end path of bench.py: one staged H2D copy, results written by the assemble kernel into a
+    mapped host buffer when small, copied back when large) returns exactly what dse_jacobian computes; and builds issued
+    back to back on one handle with alternating coefficient sets (programmatic dependent launches, constant-bank
+    coefficient slot rewritten by every prep_kernel) are bitwise reproducible."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    w = Workload("host", 16, 40, 32, 1e-6, 5e4, x_G=1.0, x_Z=30.0)
+    p = oracle_params(w)
+    for B in (1, 3, 130):                                    # 130 x (32*32 + 32) x 8 B > 1 MiB: the copy-back path
+        c = np.stack([draw_coefficients(200 + b, w.n_cheb) for b in range(B)])
+        bc = np.stack([[1.0 + 0.01 * b, 0.9 + 0.003 * b] for b in range(B)])
+        d = Dse(params_from_workload(w, n_batch=B))
+        J, F = d.jacobian(torch.from_numpy(c).cuda(), torch.from_numpy(bc).cuda())
+        J = J.cpu().numpy(); F = F.cpu().numpy()
+        Jh = np.full_like(J, np.nan); Fh = np.full_like(F, np.nan)
+        d.jacobian_host(c, bc, Jh, Fh)
+        assert np.array_equal(Jh, J) and np.array_equal(Fh, F)
+        Fr = np.full_like(F, np.nan)
+        d.jacobian_host(c, bc, None, Fr)                     # residual only
+        assert np.abs(Fr - F).max() <= 1e-12 * np.abs(F).max()
+        for b in (0, B - 1):
+            Fo, Jo = orc.residual_jacobian(p, c[b], bc[b, 0], bc[b, 1])
+            check(Jh[b], Fh[b], Jo, Fo)
+        d.close()
+    # alternating inputs, no synchronisation in between
+    d = Dse(params_from_workload(w))
+    cs = [torch.from_numpy(draw_coefficients(300 + i, w.n_cheb)[None, :]).cuda() for i in range(2)]
+    bt = torch.tensor([[1.0, 0.9]], dtype=torch.float64, device="cuda")
+    outs = [d.jacobian(cs[i % 2], bt) for i in range(8)]
+    torch.cuda.synchronize()
+    for i in range(2, 8):
+        assert torch.equal(outs[i][0], outs[i % 2][0]) and torch.equal(outs[i][1], outs[i % 2][1])
+    assert not torch.equal(outs[0][0], outs[1][0])
+    d.close()

@@ -315,3 +315,22 @@ def test_newton_solve_graph_paper_scaling_solution(orc):
     kap = -(lnG[3] - lnG[2]) / math.log(10.0)               # G ~ x^-kappa below eps2 (eq.(17))
     assert abs(kap - S.KAPPA) < 1e-9
     d.close()
+
+
+def test_newton_solve_graph_large_system_cluster_lu(orc):
+    """2N = 144: inside the solve graph the Newton update runs on the cluster LU (4 CTAs, distributed shared memory);
+    same steps and coefficients as the oracle's loop."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import Workload
+    w = Workload("newton-weak-72", 72, 96, 32, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
+    d = Dse(params_from_workload(w))
+    p = oracle_params(w)
+    c_o, hist, status = orc.newton_solve(p, np.zeros(144), 1.0, 1.0, rho=1.0, step_cap=0.0, tol=1e-10, max_iter=12)
+    assert status == 1
+    c_g = torch.zeros((1, 144), dtype=torch.float64, device="cuda")
+    bc = torch.ones((1, 2), dtype=torch.float64, device="cuda")
+    info = d.newton_solve(c_g, bc, tol=1e-10, max_iter=12).cpu().numpy()[0]
+    assert info[5] == 1.0 and info[0] == len(hist)
+    assert np.abs(c_g.cpu().numpy()[0] - c_o).max() <= 1e-9 * np.abs(c_o).max()
+    d.close()

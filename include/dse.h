@@ -201,7 +201,8 @@ DSE_API int dse_dressing(dse_handle *h, const double *c_dev, const double *x_dev
  * instead of programmatic dependent launches between the kernels of a build; read once per process). */
 
 /* Diagnostics: cycles summed over all warps of the last point-kernel launch, spent in (geometry, series,
- * exp + weights, accumulation, whole warp).  All zeros unless the library was built with
+ * exp + weights, accumulation, whole warp); for the software-pipelined kernel: (entry until the tables are staged and the
+ * producer kernel is done, first batch, remaining batches, epilogue phase 2 + flushes, whole warp).  All zeros unless the library was built with
  * -DDSE_PHASE_TIMING (the default build carries no instrumentation).  Synchronous. */
 DSE_API int dse_get_phase_cycles(dse_handle *h, double out_host[5]);
 

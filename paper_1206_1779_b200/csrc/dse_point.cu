@@ -353,9 +353,18 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
     double *s_stash = wbase + (CONSTC ? 0 : 2 * Npad);                       // [2][STASH]: pt (33 x 4) then T
     double4 *s_gbuf = reinterpret_cast<double4 *>(s_stash + 2 * STASH);     // [2][32] geometry records
 
+#ifdef DSE_PHASE_TIMING
+    // diagnostics (dse_get_phase_cycles): cycles from kernel entry to (tables staged + producer done), of the first batch,
+    // of the remaining batches, of the flushes; [4] = whole warp
+    const long long dbg_start = clock64();
+    long long dbg_first = 0, dbg_flush = 0;
+#endif
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
     pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q)
     __syncthreads();
+#ifdef DSE_PHASE_TIMING
+    const long long dbg_ready = clock64();
+#endif
 
     const int Nr = P.Nr, BPR = P.Ntpad >> 5;                                 // batches per row
     // work is partitioned in 32-point batches (P.U = rows * BPR): balanced to +-1 batch over all warps; a row whose
@@ -530,6 +539,9 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
                 reinterpret_cast<double4 *>(s_stash + cur * STASH)[lane] = make_double4(ts, ua, ub, v);
                 __syncwarp();
                 cur ^= 1;
+#ifdef DSE_PHASE_TIMING
+                if (dbg_first == 0) dbg_first = clock64();
+#endif
             }
             // H5/H7: row sums over the 32 angular lanes.  Transposing reduction: after the first two steps each
             // quarter-warp carries one of the four sums (6 shuffles instead of 20; fixed order -> deterministic).
@@ -557,8 +569,14 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
             }
         }
         // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
+#ifdef DSE_PHASE_TIMING
+        const long long dbg_f0 = clock64();
+#endif
         phase2(cur ^ 1);
         flush(bi, cur);
+#ifdef DSE_PHASE_TIMING
+        dbg_flush += clock64() - dbg_f0;
+#endif
         if (q >= Nr) {
             q = 0; ++bi; ++e;
             if (e == P.Next) {
@@ -572,6 +590,16 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
         }
     }
     if (GEOM) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+#ifdef DSE_PHASE_TIMING
+    if (lane == 0 && P.dbg) {
+        const long long dbg_end = clock64();
+        P.dbg[w * 5 + 0] = (double)(dbg_ready - dbg_start);
+        P.dbg[w * 5 + 1] = (double)(dbg_first - dbg_ready);
+        P.dbg[w * 5 + 2] = (double)(dbg_end - dbg_first - dbg_flush);
+        P.dbg[w * 5 + 3] = (double)dbg_flush;
+        P.dbg[w * 5 + 4] = (double)(dbg_end - dbg_start);
+    }
+#endif
 }
 using KernelFn = void (*)(const KParams);
 

@@ -94,3 +94,37 @@ def config_inputs(cfg: int, n_batch: int = None):
     else:
         raise KeyError(cfg)
     return w, np.ascontiguousarray(c), np.ascontiguousarray(bc)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# "Config 2'": the paper's own parameter set -- the convergent counterpart of
+# BASELINE configs[2] (reading A17).  Inputs only: shapes, boundary values and a start guess.
+def paper_scaling_workload() -> Workload:
+    """eps2 = 1e-6, L2 = 5e4 GeV^2, x_G = 0 (1/G(0) = 0: scaling solution), x_Z = L2, N = 36, 96 + 32 radial nodes
+    (32 of them on the infrared piece of eq.(26)), 32 angles."""
+    return Workload("cfg2p-paper-scaling", 36, 96, 32, 1e-6, 5e4, x_G=0.0, x_Z=5e4, n_ir=32)
+
+
+PAPER_SCALING_BC = (0.0, 1.0 / 0.256)       # (1/G(0), 1/Z(x_Z)): PAPER.md L135
+
+
+def scaling_start_coefficients(w: Workload) -> np.ndarray:
+    """A scaling-shaped start guess built from the paper's asymptotic forms eq.(16)-(19) -- NOT the fit functions of
+    ref.[16], which are not in PAPER.md:  ln G = -kappa ln(x/(x+1)) + delta ln(1 + omega ln(1+x)),
+    ln Z = 2 kappa ln(x/(x+1)) + gamma ln(1 + omega ln(1+x)), sampled at the mapped Chebyshev roots (fn.9) and projected
+    on T_j by the discrete orthogonality of the roots; a_0 is then shifted so that Z(x_Z = L2) = 0.256."""
+    N = w.n_cheb
+    gamma = -1.0 - 2.0 * w.delta
+    i = np.arange(N)
+    ang = np.pi * (i + 0.5) / N
+    s = -np.cos(ang)
+    x = w.eps2 * np.exp(0.5 * (s + 1.0) * np.log(w.L2 / w.eps2))
+    run = np.log(1.0 + w.uv_omega * np.log(1.0 + x))
+    lg = w.ir_exp_G * np.log(x / (x + 1.0)) + w.delta * run
+    lz = w.ir_exp_Z * np.log(x / (x + 1.0)) + gamma * run
+    j = np.arange(N)
+    T = np.cos(np.outer(np.arccos(s), j))                      # T_j(s_i)
+    c = np.concatenate([(2.0 / N) * (T.T @ lz), (2.0 / N) * (T.T @ lg)])
+    lnZ_L2 = 0.5 * c[0] + c[1:N].sum()                         # series at s = 1 (T_j(1) = 1), c_0/2 convention
+    c[0] += 2.0 * (np.log(0.256) - lnZ_L2)
+    return c

@@ -417,3 +417,16 @@ def test_radial_split_rule_f1(orc):
         cm = c.copy(); cm[j] -= 1e-6
         Jfd[:, j] = (orc.residual_jacobian(p, cp, 1, 1, jac=False) - orc.residual_jacobian(p, cm, 1, 1, jac=False)) / 2e-6
     assert np.linalg.norm(J - Jfd) <= 1e-8 * np.linalg.norm(J)
+
+
+def test_config2p_inputs_match_the_test_setup(orc):
+    """workloads.scaling_start_coefficients (numpy only, used by bench.py) is the same start guess as tests/scaling_setup.py
+    builds from the oracle's tables; the boundary values are the paper's (L135)."""
+    import scaling_setup as S
+    from paper_1206_1779_b200.workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
+    w = paper_scaling_workload()
+    assert (w.n_cheb, w.n_r, w.n_ir, w.n_theta, w.eps2, w.L2, w.x_G, w.x_Z) == (S.N, S.N_R, S.N_IR, S.N_THETA, S.EPS2, S.L2, 0.0, S.L2)
+    assert PAPER_SCALING_BC == (S.G_G, S.G_Z)
+    p = make_params(S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, 0.0, S.L2, n_ir=S.N_IR)
+    c_ref = S.start_coefficients(orc, p)
+    assert np.abs(scaling_start_coefficients(w) - c_ref).max() <= 1e-12 * np.abs(c_ref).max()

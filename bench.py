@@ -257,6 +257,27 @@ def run_ours(args, w, c, bc):
     t_e2e = max_over_ranks(t_e2e, device="cuda")
     e2e_value = world * nb * e2e_steps / t_e2e
 
+    # ---- every other config: the same build followed by the Newton update H9 (equilibrated LU, c <- c - Delta) ----
+    with_update = None
+    if not newton:
+        n_up = min(args.steps, 200)
+        for _ in range(3):
+            c_work.copy_(ct)
+            d.newton_step(c_work, bt, 1.0, stats)
+        barrier()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n_up)]
+        for a, b in evs:
+            flush.zero_()
+            c_work.copy_(ct)
+            a.record(stream)
+            d.newton_step(c_work, bt, 1.0, stats)
+            b.record(stream)
+        barrier()
+        ms_up = max_over_ranks(float(np.mean([a.elapsed_time(b) for a, b in evs])), device="cuda")
+        with_update = {"value": world * nb / (ms_up * 1e-3), "unit": "newton_steps/s", "ms_per_step": ms_up, "steps": n_up,
+                       "what": "build (H1-H8) + Newton update H9 (row-equilibrated LU with partial pivoting, solve, c <- c - Delta) "
+                               "through dse_newton_step"}
+
     # ---- config 2 only: the whole iteration as ONE device-side graph (dse_newton_solve), fixed step count ----
     solve = None
     if newton:
@@ -365,6 +386,8 @@ def run_ours(args, w, c, bc):
             "gpu_launches": int(launches),
             "clocks": sampler.result(),
         }
+        if with_update is not None:
+            line["with_newton_update"] = with_update
         if solve is not None:
             line["newton_solve"] = solve
         if world == 1 and not args.no_cpu_baseline:

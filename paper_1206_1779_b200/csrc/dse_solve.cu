@@ -54,7 +54,10 @@ __global__ void __launch_bounds__(256) solve_control_kernel(cudaGraphConditional
         if (o[5] != 0.0) continue;                        // frozen: converged or failed earlier
         const double *st = stats + (size_t)b * 4;
         const double dmax = st[0];
-        const bool finite = dmax == dmax && dmax < __longlong_as_double(0x7ff0000000000000ll);
+        const double INF = __longlong_as_double(0x7ff0000000000000ll);
+        bool bad = false;                                 // fmax() skips NaN: look at every entry of Delta as well
+        for (int j = lane; j < n2; j += 32) { const double dj = delta[(size_t)b * n2 + j]; bad = bad || !(fabs(dj) < INF); }
+        const bool finite = dmax == dmax && dmax < INF && !__any_sync(0xffffffffu, bad);
         double r = rho;
         if (finite && cap > 0.0 && rho * dmax > cap) r = cap / dmax;      // rho_n = min(rho, cap/|Delta|)
         if (finite)

@@ -334,3 +334,26 @@ def test_newton_solve_graph_large_system_cluster_lu(orc):
     assert info[5] == 1.0 and info[0] == len(hist)
     assert np.abs(c_g.cpu().numpy()[0] - c_o).max() <= 1e-9 * np.abs(c_o).max()
     d.close()
+
+
+def test_lu_extreme_exponents_take_the_library_division(orc):
+    """Entries far outside 2^+-500 after equilibration (columns scaled by 1e-200 / 1e+180): the multipliers come from the
+    library division on the lanes that need it; factorisation still bit-identical to the plain C elimination."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200.workloads import CONFIGS
+    d = Dse(params_from_workload(CONFIGS[0]))
+    rng = np.random.default_rng(77)
+    for n in (8, 40, 64, 128):
+        A = rng.normal(size=(2, n, n))
+        A[:, :, 1] *= 1e-200                                     # tiny column: quotients of tiny numbers
+        A[:, :, n // 2] *= 1e-180
+        A[:, n // 3, :] *= 1e150                                 # a huge row (removed by the equilibration)
+        b = rng.normal(size=(2, n))
+        x, st = d.lu_solve(torch.from_numpy(A).cuda(), torch.from_numpy(b).cuda())
+        x = x.cpu().numpy(); st = st.cpu().numpy()
+        for s in range(2):
+            xo, so, rc = orc.lu_solve(A[s], b[s])
+            assert np.array_equal(st[s][1:], so[1:]), (n, st[s], so)
+            assert np.allclose(x[s], xo, rtol=1e-6, atol=0), n
+    d.close()

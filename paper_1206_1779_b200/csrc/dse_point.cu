@@ -403,20 +403,50 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
     auto flush = [&](int bi, int buf) {      // `buf`'s T area is free: use it as the cross-lane scratch
         double *scr = s_stash + buf * STASH + 132;
         const size_t slot = (size_t)(w + bi);
+        if constexpr (EXACT && (SUB == 4 || SUB == 8)) {
+            // transposing reduction over the SUB point sub-lanes of a chunk (the low bits of the lane): at every stage a lane
+            // keeps one half of its list and receives the partner's sums of that half -- 12 + 6 (+ 3) shuffles instead of
+            // 24 conflicting shared-memory stores and three warp barriers; fixed pairwise order -> deterministic.  A lane ends
+            // with 24 / SUB finished sums and stores them itself.
+            double v[24];
 #pragma unroll
-        for (int st = 0; st < 3; ++st) {
-            __syncwarp();
+            for (int m = 0; m < CJ; ++m) { v[m] = accA[m]; v[CJ + m] = accB[m]; v[2 * CJ + m] = accV[m]; }
+            int base = 0;
 #pragma unroll
-            for (int m = 0; m < CJ; ++m)
-                if (lane_on) scr[sub * Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
-            __syncwarp();
-            for (int j = lane; j < Npad; j += 32) {
-                double s = 0.0;
-                for (int sb = 0; sb < SUB; ++sb) s += scr[sb * Npad + j];
-                P.Spart[(slot * 3 + st) * Npad + j] = s;
+            for (int d = SUB / 2, n = 24; d >= 1; d >>= 1, n >>= 1) {
+                const int half = n >> 1;
+                const bool up = (sub & d) != 0;
+#pragma unroll
+                for (int i = 0; i < 12; ++i) {
+                    if (i < half) {
+                        const double keep = up ? v[half + i] : v[i];
+                        const double send = up ? v[i] : v[half + i];
+                        v[i] = keep + __shfl_xor_sync(FULL, send, d);
+                    }
+                }
+                base += up ? half : 0;
             }
+#pragma unroll
+            for (int i = 0; i < 24 / SUB; ++i) {
+                const int o = base + i, st = o >> 3, m = o & 7;          // o = stream * 8 + index in the chunk
+                P.Spart[(slot * 3 + st) * Npad + c_lane * CJ + m] = v[i];
+            }
+        } else {
+#pragma unroll
+            for (int st = 0; st < 3; ++st) {
+                __syncwarp();
+#pragma unroll
+                for (int m = 0; m < CJ; ++m)
+                    if (lane_on) scr[sub * Npad + c_lane * CJ + m] = (st == 0 ? accA[m] : (st == 1 ? accB[m] : accV[m]));
+                __syncwarp();
+                for (int j = lane; j < Npad; j += 32) {
+                    double s = 0.0;
+                    for (int sb = 0; sb < SUB; ++sb) s += scr[sb * Npad + j];
+                    P.Spart[(slot * 3 + st) * Npad + j] = s;
+                }
+            }
+            __syncwarp();
         }
-        __syncwarp();
     };
 
     // geometry stream (GEOM): consecutive 1 KB records, cp.async double buffer

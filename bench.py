@@ -24,7 +24,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_1206_1779_b200.workloads import CONFIGS, config_inputs   # noqa: E402
+from workloads import CONFIGS, config_inputs   # noqa: E402
 
 # fp64 FMA peak of one B200 derived from unit counts and clocks (B200_PROFILING.md: 148 SMs,
 # clocks.max.sm 1965 MHz; 64 fp64 FMA lanes per SM = 16 per SM sub-partition): DESIGN.md "Roofline".
@@ -114,7 +114,7 @@ def cpu_baseline(w, c, budget_s=12.0):
 def oracle_converged_solve():
     """cpu_baseline leg, config 2 only: the oracle's own Newton loop on config 2' (same inputs, same relaxation rule)."""
     from oracle.oracle import Oracle
-    from paper_1206_1779_b200.workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
+    from workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
     ws = paper_scaling_workload()
     orc, p = Oracle(), oracle_params(ws)
     t0 = time.perf_counter()
@@ -318,7 +318,7 @@ def run_ours(args, w, c, bc):
 
         # config 2': the paper's own parameter set, which does converge (A17): iterations, total time, the
         # infrared exponents and the coupling, all read on the device (dse_newton_solve + dse_dressing)
-        from paper_1206_1779_b200.workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
+        from workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
         ws = paper_scaling_workload()
         d2 = Dse(params_from_workload(ws, flags=flags))
         c0 = torch.from_numpy(scaling_start_coefficients(ws)[None, :]).cuda()

@@ -582,4 +582,36 @@ void orc_schwinger(const orc_params *p, const double *c, int n_nodes, double p2_
     free(cr);
 }
 
+/* The same sums in two steps, for the paper's full-size rule (2^17 nodes, fn.13): the node table costs O(n_nodes^2)
+ * (every node is a Newton iteration on the n_nodes-term Legendre recurrence), so a test may compute ranges of nodes
+ * [i0, i1) on several host threads and then sum serially -- identical arithmetic to orc_schwinger in the double build. */
+void orc_schwinger_terms(const orc_params *p, const double *c, int n_nodes, double p2_min, double p2_max, int i0, int i1,
+                         double *pn, double *fn)
+{
+    const int N = p->n_cheb;
+    real *cr = (real *)malloc(sizeof(real) * (size_t)(3 * N));
+    real *phi = cr + 2 * N;
+    for (int j = 0; j < 2 * N; ++j) cr[j] = c[j];
+    const real u0 = R_LOG((real)p2_min) / 2, u1 = R_LOG((real)p2_max) / 2;
+    for (int i = i0; i < i1; ++i) {
+        real x, w;
+        gl_node(n_nodes, i, &x, &w);
+        real u = u0 + (x + 1) / 2 * (u1 - u0);
+        real pp = R_EXP(u);
+        real lnG, lnZ, sc;
+        ln_dress(p, cr, pp * pp, phi, &lnG, &lnZ, &sc);
+        pn[i] = (double)pp;
+        fn[i] = (double)(w * (u1 - u0) / 2 * pp * R_EXP(lnZ) / (pp * pp));
+    }
+    free(cr);
+}
+void orc_schwinger_sum(int n_nodes, const double *pn, const double *fn, int n_t, const double *t, double *out)
+{
+    for (int m = 0; m < n_t; ++m) {
+        real sum = 0;
+        for (int i = 0; i < n_nodes; ++i) sum += (real)fn[i] * R_COS((real)t[m] * (real)pn[i]);
+        out[m] = (double)(sum / R_PI);
+    }
+}
+
 int orc_sizeof_real(void) { return (int)sizeof(real); }

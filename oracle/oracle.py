@@ -55,6 +55,8 @@ class Oracle:
         L.orc_radial_rule_split.argtypes = [C.POINTER(OrcParams), C.c_double, _dp, _dp]
         L.orc_gl_node.argtypes = [C.c_int, C.c_int, _dp, _dp]
         L.orc_schwinger.argtypes = [C.POINTER(OrcParams), _dp, C.c_int, C.c_double, C.c_double, C.c_int, _dp, _dp]
+        L.orc_schwinger_terms.argtypes = [C.POINTER(OrcParams), _dp, C.c_int, C.c_double, C.c_double, C.c_int, C.c_int, _dp, _dp]
+        L.orc_schwinger_sum.argtypes = [C.c_int, _dp, _dp, C.c_int, _dp, _dp]
         for name in ("orc_z", "orc_kernel_M", "orc_kernel_Q", "orc_kernel_ghost", "orc_kernel_M_literal",
                      "orc_kernel_Q_literal"):
             f = getattr(L, name)
@@ -94,6 +96,26 @@ class Oracle:
         c = _f64(c); t = _f64(t)
         out = np.empty(len(t))
         self.lib.orc_schwinger(C.byref(p), _ptr(c), int(n_nodes), float(p2_min), float(p2_max), len(t), _ptr(t), _ptr(out))
+        return out
+
+    def schwinger_threads(self, p, c, n_nodes, p2_min, p2_max, t, threads=None):
+        """orc_schwinger with the O(n_nodes^2) node table computed in ranges on several host threads (ctypes releases the
+        GIL) and the sums taken serially afterwards: the same arithmetic, for the paper's 2^17-node rule (fn.13)."""
+        import os
+        from concurrent.futures import ThreadPoolExecutor
+        c = _f64(c); t = _f64(t)
+        n_nodes = int(n_nodes)
+        threads = threads or min(os.cpu_count() or 1, 64)
+        pn = np.empty(n_nodes); fn = np.empty(n_nodes)
+        # Newton on the recurrence converges in fewer steps in the middle of the interval: interleave small ranges
+        step = max(1, n_nodes // (threads * 16))
+        ranges = [(i, min(i + step, n_nodes)) for i in range(0, n_nodes, step)]
+        def work(r):
+            self.lib.orc_schwinger_terms(C.byref(p), _ptr(c), n_nodes, float(p2_min), float(p2_max), r[0], r[1], _ptr(pn), _ptr(fn))
+        with ThreadPoolExecutor(max_workers=threads) as pool:
+            list(pool.map(work, ranges))
+        out = np.empty(len(t))
+        self.lib.orc_schwinger_sum(n_nodes, _ptr(pn), _ptr(fn), len(t), _ptr(t), _ptr(out))
         return out
 
     def cheb_phi(self, n, s):

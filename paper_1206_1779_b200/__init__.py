@@ -3,4 +3,3 @@
 Public API: the C ABI of include/dse.h (libdse_b200.so) and its thin binding `binding.Dse`.
 """
 from .binding import Dse, DseError, DseParams, params_from_workload, load_library, DSE_FLAG_GEOMETRY_CACHE, DSE_FLAG_ANGULAR_TANH_SINH  # noqa: F401
-from . import workloads  # noqa: F401

@@ -35,7 +35,7 @@ def test_struct_layout_matches_header():
 
 def test_error_paths_without_gpu(lib):
     from paper_1206_1779_b200.binding import DseParams
-    from paper_1206_1779_b200.workloads import CONFIGS
+    from workloads import CONFIGS
     from paper_1206_1779_b200 import params_from_workload
     h = ctypes.c_void_p()
     assert lib.dse_strerror(0) == b"ok" and lib.dse_strerror(-1) == b"invalid argument"

@@ -10,12 +10,10 @@ from test_gpu_parity import oracle_params, _torch   # noqa: E402
 def test_lu_solve_matches_oracle(orc):
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import CONFIGS
+    from workloads import CONFIGS
     d = Dse(params_from_workload(CONFIGS[0]))
     rng = np.random.default_rng(5)
-    for n in (1, 2, 16, 64, 128, 200):
-        if n > 128 and n != 16:
-            continue   # large systems use the handle's own scratch (2N only)
+    for n in (1, 2, 16, 64, 128):      # n > 128 needs the handle's own scratch (n = 2N only): test_lu_cluster_* below
         A = rng.normal(size=(3, n, n)) * 10.0 ** rng.uniform(-8, 8, size=(3, n, 1))
         b = rng.normal(size=(3, n)) * np.abs(A).max(axis=2)
         x, st = d.lu_solve(torch.from_numpy(A).cuda(), torch.from_numpy(b).cuda())
@@ -46,7 +44,7 @@ def test_newton_trajectory_weak_coupling(orc):
     """Same start, same steps: iterates agree while cond*1e-16 allows; quadratic convergence (L226)."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     w = Workload("newton-weak", 10, 64, 24, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
     d = Dse(params_from_workload(w))
     p = oracle_params(w)
@@ -70,7 +68,7 @@ def test_config2_newton_trajectory_literal(orc):
     cond(J)*eps allows, and the same verdict."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import config_inputs
+    from workloads import config_inputs
     w, c, bc = config_inputs(2)
     d = Dse(params_from_workload(w))
     p = oracle_params(w)
@@ -102,7 +100,7 @@ def test_finite_difference_self_check_mode(orc):
     """NEXT f3: the paper's own Jacobian definition, eq.(38), as a GPU self-check of the analytic matrix."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import config_inputs
+    from workloads import config_inputs
     w, c, bc = config_inputs(0)
     d = Dse(params_from_workload(w))
     ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
@@ -130,7 +128,7 @@ def test_lu_random_sizes_exact_factorisation(orc):
     growth factor bit-identical to the plain C elimination (both LU kernels: registers for n <= 128, blocked above)."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import CONFIGS
+    from workloads import CONFIGS
     d = Dse(params_from_workload(CONFIGS[0]))
     rng = np.random.default_rng(11)
     for it in range(60):
@@ -163,7 +161,7 @@ def test_newton_steps_batched_systems(orc):
     """Eight systems per handle (tensor-path build + one LU CTA per system): every system follows the oracle's iterates."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     w = Workload("newton-weak-batch", 10, 48, 32, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
     B = 8
     d = Dse(params_from_workload(w, n_batch=B)); assert d.kernel_info()["variant"] == "batched-dmma"
@@ -188,7 +186,7 @@ def test_lu_cluster_path_exact_factorisation(orc, N):
     barrier).  Same bar as the single-CTA kernel: solution within conditioning, factorisation bit-identical."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     n = 2 * N
     d = Dse(params_from_workload(Workload("lu", n_cheb=N, n_r=4, n_theta=4, eps2=1e-6, L2=1e4), n_batch=3))
     rng = np.random.default_rng(N)
@@ -220,7 +218,7 @@ def test_newton_solve_graph_weak_coupling(orc):
     per-step record, converged coefficients to the north_star bar (1e-9); then the call-level controls."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     w = Workload("newton-weak", 10, 64, 24, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
     d = Dse(params_from_workload(w))
     p = oracle_params(w)
@@ -263,7 +261,7 @@ def test_newton_solve_graph_batched_systems(orc):
     last one; every system matches its own oracle solve."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     w = Workload("newton-weak-batch", 10, 48, 32, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
     B = 8
     d = Dse(params_from_workload(w, n_batch=B))
@@ -292,7 +290,7 @@ def test_newton_solve_graph_paper_scaling_solution(orc):
     import math
     import scaling_setup as S
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     w = Workload("paper-scaling", S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, x_G=0.0, x_Z=S.L2, n_ir=S.N_IR)
     p = oracle_params(w)
     c0 = S.start_coefficients(orc, p)
@@ -322,7 +320,7 @@ def test_newton_solve_graph_large_system_cluster_lu(orc):
     same steps and coefficients as the oracle's loop."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     w = Workload("newton-weak-72", 72, 96, 32, 1e-2, 1e2, x_G=1.0, x_Z=1.0, alpha_mu=0.05)
     d = Dse(params_from_workload(w))
     p = oracle_params(w)
@@ -341,7 +339,7 @@ def test_lu_extreme_exponents_take_the_library_division(orc):
     library division on the lanes that need it; factorisation still bit-identical to the plain C elimination."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import CONFIGS
+    from workloads import CONFIGS
     d = Dse(params_from_workload(CONFIGS[0]))
     rng = np.random.default_rng(77)
     for n in (8, 40, 64, 128):

@@ -20,7 +20,7 @@ from test_gpu_parity import oracle_params, gpu_build, check, _torch   # noqa: E4
     dict(radial_split=1, n_ir=5, x_G=3.0, x_Z=5e4, n_r=13, n_theta=21, n_cheb=12),   # ragged
 ])
 def test_infrared_piece_and_zero_subtraction_point_parity(orc, kw):
-    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    from workloads import Workload, draw_coefficients
     base = dict(n_cheb=16, n_r=40, n_theta=32, eps2=1e-6, L2=5e4)
     base.update(kw)
     w = Workload("f2", **base)
@@ -36,7 +36,7 @@ def test_paper_scaling_solution_on_gpu(orc):
     torch = _torch()
     import scaling_setup as S
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload
+    from workloads import Workload
     w = Workload("paper-scaling", S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, x_G=0.0, x_Z=S.L2, n_ir=S.N_IR)
     p = oracle_params(w)
     c_o = S.start_coefficients(orc, p)

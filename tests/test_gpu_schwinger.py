@@ -58,10 +58,35 @@ def test_schwinger_matches_oracle_and_closed_form(orc):
     d.close()
 
 
+def test_schwinger_full_size_2p17_nodes(orc):
+    """The paper's size (fn.13): 2^17 device-generated Gauss-Legendre nodes, Delta(t) against the
+    oracle on the same rule (its O(n^2) node table spread over the host cores, sums serial) and, with the two cut pieces
+    of the momentum window added, against the textbook exp(-t)/2 to 1e-10."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse
+    from paper_1206_1779_b200.binding import DseParams
+    from test_oracle_path import schwinger_cut_pieces
+    N, eps2, L2 = 128, 1e-8, 1e4
+    p, c = _massive_propagator_coefficients(orc, N, eps2, L2)
+    prm = DseParams(N, 8, 8, 1, eps2, L2, 1.0, 3.0, 1.0, 1.0, -9.0 / 44.0, 0.0, 1.0, 0.0, 0, 0)
+    d = Dse(prm)
+    t = np.array([0.0, 0.1, 0.5, 1.0, 3.0, 4.7, 6.0, 8.0])
+    n_nodes = 1 << 17
+    out = d.schwinger(torch.from_numpy(c[None, :]).cuda(), torch.from_numpy(t).cuda(), n_nodes, 1e-20, L2)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()[0]
+    ref = orc.schwinger_threads(p, c, n_nodes, 1e-20, L2, t)
+    # node weights of the 2^17 rule carry ~n*eps of recurrence rounding on both sides (test above): 1e-9 relative
+    assert np.allclose(out, ref, rtol=2e-9, atol=1e-12), np.abs(out - ref).max()
+    pos = t > 0
+    assert np.allclose(out[pos] + schwinger_cut_pieces(t[pos], 1e-20, L2), np.exp(-t[pos]) / 2, rtol=0, atol=2e-9)
+    d.close()
+
+
 def test_schwinger_batched_random_dressings(orc):
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    from workloads import Workload, draw_coefficients
     w = Workload("schw", 24, 8, 8, 1e-6, 5e4, n_batch=3)
     c = np.stack([draw_coefficients(70 + b, 24) for b in range(3)])
     d = Dse(params_from_workload(w))
@@ -81,7 +106,7 @@ def test_dressing_functions_and_coupling_parity(orc):
     import math
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
-    from paper_1206_1779_b200.workloads import Workload, draw_coefficients
+    from workloads import Workload, draw_coefficients
     w = Workload("dress", 24, 16, 32, 1e-6, 5e4, x_G=1.0, x_Z=1.0, alpha_mu=0.7)
     B = 3
     p = oracle_params(w)

@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from oracle.oracle import make_params
-from paper_1206_1779_b200.workloads import config_inputs, draw_coefficients, KAPPA, DELTA
+from workloads import config_inputs, draw_coefficients, KAPPA, DELTA
 
 PI = math.pi
 
@@ -180,7 +180,11 @@ def test_invariances(orc):
     # boundary values only shift F (reading A13)
     F3, J3 = orc.residual_jacobian(p, c, 0.4, 1.0)
     assert np.array_equal(J3, J)
-    assert np.allclose(F3[:N] - F[:N], 0.2, atol=1e-12 * np.abs(F[:N]).max()) or True
+    # gluon rows: F_z -> F_z + (1.2 - 1.0), on every row to the rounding of F_z itself (|F_z| spans 1e7 ... 1e19 here), and
+    # resolved to 1e-8 on the rows where 0.2 is resolvable (the brute-force test covers gZ != 1 on O(1) rows)
+    dz = F3[:N] - F[:N]
+    assert np.all(np.abs(dz - 0.2) <= 8 * np.spacing(np.abs(F[:N])))          # (F is itself a sum of a few rounded terms)
+    assert np.sum(np.abs(dz - 0.2) < 1e-8) >= N // 2
     assert np.allclose(F3[N:] - F[N:], 0.5, atol=1e-12)
     # (ii)+(iii) j = 0 column identities at a single external point (phi_0 = 1/2 at every argument)
     tab = orc.tables(p)
@@ -220,7 +224,20 @@ def test_lu_solve_against_numpy(orc):
         assert rc == 0
         assert np.allclose(x, xr, rtol=1e-9, atol=1e-12 * np.abs(xr).max())
         assert stats[0] == pytest.approx(np.abs(x).max()) and stats[1] == pytest.approx(np.abs(b * r).max())
-        assert stats[2] > 0 and stats[3] >= 1 - 1e-12
+        # stats[2] = smallest |pivot|, stats[3] = growth max|U|/max|A_scaled|: against LAPACK's factorisation of the
+        # row-scaled matrix (same partial pivoting; random entries have no ties, so P, L, U are unique up to rounding)
+        import scipy.linalg
+        As = A * r[:, None]
+        _, _, U = scipy.linalg.lu(As)
+        assert stats[2] == pytest.approx(np.abs(np.diag(U)).min(), rel=1e-9)
+        assert stats[3] == pytest.approx(np.abs(np.triu(U)).max() / np.abs(As).max(), rel=1e-9)
+    # hand-worked 3x3 (exact in binary): rows scaled by 1/4, 1/8, 1/2; pivots 1, 3/4, -2/3 (worked below)
+    #   A = [[2,4,2],[8,2,4],[1,2,0]], scaled: [[.5,1,.5],[1,.25,.5],[.5,1,0]]; step 0 pivot row 1 (|1|);
+    #   rows 0,2 become [0,.875,.25], [0,.875,-.25]; step 1 pivot .875 (first of the tie wins: row 0), row 2 -> [0,0,-.5]
+    A3 = np.array([[2.0, 4.0, 2.0], [8.0, 2.0, 4.0], [1.0, 2.0, 0.0]])
+    x, stats, rc = orc.lu_solve(A3, np.array([4.0, 8.0, 2.0]))
+    assert rc == 0 and stats[1] == 1.0 and stats[2] == 0.5 and stats[3] == 1.0          # min |pivot| = |-1/2|, max|U| = 1
+    assert np.allclose(A3 @ x, [4.0, 8.0, 2.0], atol=1e-15)
     # pivoting is needed: zero on the diagonal
     x, stats, rc = orc.lu_solve(np.array([[0.0, 1.0], [1.0, 0.0]]), np.array([2.0, 3.0]))
     assert rc == 0 and np.allclose(x, [3.0, 2.0])
@@ -286,16 +303,31 @@ def _massive_propagator_coefficients(orc, N, eps2, L2):
     return p, np.concatenate([a, np.zeros(N)])
 
 
+def schwinger_cut_pieces(t, p2_min, p2_max):
+    """What the finite momentum window [p_min, p_max] of eq.(20) leaves out for sigma = 1/(p^2 + 1), independent of the
+    oracle: the tail (1/pi) int_{p_max}^inf dp cos(tp)/(p^2+1) by QUADPACK's Fourier-integral routine (scipy, QAWF) and
+    the head (1/pi) int_0^{p_min} dp cos(tp)/(p^2+1) = p_min/pi up to O(p_min^3)."""
+    import scipy.integrate as si
+    P = math.sqrt(p2_max)
+    tail = np.array([si.quad(lambda q: 1.0 / (q * q + 1.0), P, np.inf, weight="cos", wvar=float(tt))[0] for tt in t]) / PI
+    return tail + math.sqrt(p2_min) / PI
+
+
 def test_schwinger_function_closed_form(orc):
     """eq.(20): Delta(t) = (1/pi) int_0^inf dp cos(tp) sigma(p^2).  For sigma = 1/(p^2+m^2) the textbook value is
-    exp(-m t)/(2m); the cutoff at p_max = 100 leaves a tail of order sin(t p_max)/(pi t p_max^2) ~ 1e-5."""
-    p, c = _massive_propagator_coefficients(orc, 64, 1e-6, 1e4)
+    exp(-m t)/(2m).  The oracle integrates over [p_min, p_max]; with the two cut pieces added (closed form / library
+    routine, above) the textbook value is reached to 1e-10 -- a dropped 1/pi, a wrong measure d|p| = |p| du, a wrong
+    continuation below eps2 or a mis-mapped node all fail this by many orders."""
+    p, c = _massive_propagator_coefficients(orc, 128, 1e-8, 1e4)
     t = np.array([0.5, 1.0, 3.0, 6.0])
-    d = orc.schwinger(p, c, 2048, 1e-16, 1e4, t)
-    assert np.allclose(d, np.exp(-t) / 2, rtol=0, atol=5e-5)
+    d = orc.schwinger(p, c, 4096, 1e-20, 1e4, t)
     assert np.all(d > 0)                                    # a physical (positive-norm) particle: no zero crossing
-    d2 = orc.schwinger(p, c, 4096, 1e-16, 1e4, t)
-    assert np.allclose(d, d2, rtol=0, atol=1e-9)            # converged in the number of nodes
+    assert np.allclose(d + schwinger_cut_pieces(t, 1e-20, 1e4), np.exp(-t) / 2, rtol=0, atol=1e-10)
+    assert np.abs(d - np.exp(-t) / 2).max() > 1e-6          # (the cut pieces matter: the bare window is off by ~2e-5)
+    d2 = orc.schwinger(p, c, 8192, 1e-20, 1e4, t)
+    assert np.allclose(d, d2, rtol=0, atol=1e-12)           # converged in the number of nodes
+    # the threaded two-step form used for the paper's 2^17-node rule on the GPU box is the same arithmetic
+    assert np.array_equal(orc.schwinger_threads(p, c, 4096, 1e-20, 1e4, t, threads=3), d)
 
 
 def test_gl_single_node_matches_full_rule(orc):
@@ -423,7 +455,7 @@ def test_config2p_inputs_match_the_test_setup(orc):
     """workloads.scaling_start_coefficients (numpy only, used by bench.py) is the same start guess as tests/scaling_setup.py
     builds from the oracle's tables; the boundary values are the paper's (L135)."""
     import scaling_setup as S
-    from paper_1206_1779_b200.workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
+    from workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
     w = paper_scaling_workload()
     assert (w.n_cheb, w.n_r, w.n_ir, w.n_theta, w.eps2, w.L2, w.x_G, w.x_Z) == (S.N, S.N_R, S.N_IR, S.N_THETA, S.EPS2, S.L2, 0.0, S.L2)
     assert PAPER_SCALING_BC == (S.G_G, S.G_Z)

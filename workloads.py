@@ -1,11 +1,14 @@
 """Seeded synthetic workloads (BASELINE.json configs 0-4) shared by the tests, bench.py and smoke().
 
-This module holds NONE of the method's arithmetic: only shapes, parameter values and the seeded
-draws of Chebyshev coefficients / boundary values.  Both the CUDA path and the CPU oracle receive
-the arrays produced here.  No public dataset is involved: the paper's
-workloads are parameter choices (Table 1 caption L364) and these configs are synthetic
-stand-ins of the same structure.
+A module of its own, outside both the product package (paper_1206_1779_b200/) and the oracle (oracle/): neither of
+them imports it.  It holds NONE of the method's arithmetic: only shapes, parameter values, the seeded draws of
+Chebyshev coefficients / boundary values, and one stored start vector (read from tests/golden/, written there by a
+committed script that calls only the oracle).  Both the CUDA path and the CPU oracle receive the arrays produced here
+(DESIGN.md "Input recipe").  No public dataset is involved: the paper's workloads are parameter choices (PAPER.md
+Table 1 caption L364) and these configs are synthetic stand-ins of the same structure.
 """
+import os
+
 from dataclasses import dataclass, field
 
 import numpy as np
@@ -109,22 +112,13 @@ PAPER_SCALING_BC = (0.0, 1.0 / 0.256)       # (1/G(0), 1/Z(x_Z)): PAPER.md L135
 
 
 def scaling_start_coefficients(w: Workload) -> np.ndarray:
-    """A scaling-shaped start guess built from the paper's asymptotic forms eq.(16)-(19) -- NOT the fit functions of
-    ref.[16], which are not in PAPER.md:  ln G = -kappa ln(x/(x+1)) + delta ln(1 + omega ln(1+x)),
-    ln Z = 2 kappa ln(x/(x+1)) + gamma ln(1 + omega ln(1+x)), sampled at the mapped Chebyshev roots (fn.9) and projected
-    on T_j by the discrete orthogonality of the roots; a_0 is then shifted so that Z(x_Z = L2) = 0.256."""
-    N = w.n_cheb
-    gamma = -1.0 - 2.0 * w.delta
-    i = np.arange(N)
-    ang = np.pi * (i + 0.5) / N
-    s = -np.cos(ang)
-    x = w.eps2 * np.exp(0.5 * (s + 1.0) * np.log(w.L2 / w.eps2))
-    run = np.log(1.0 + w.uv_omega * np.log(1.0 + x))
-    lg = w.ir_exp_G * np.log(x / (x + 1.0)) + w.delta * run
-    lz = w.ir_exp_Z * np.log(x / (x + 1.0)) + gamma * run
-    j = np.arange(N)
-    T = np.cos(np.outer(np.arccos(s), j))                      # T_j(s_i)
-    c = np.concatenate([(2.0 / N) * (T.T @ lz), (2.0 / N) * (T.T @ lg)])
-    lnZ_L2 = 0.5 * c[0] + c[1:N].sum()                         # series at s = 1 (T_j(1) = 1), c_0/2 convention
-    c[0] += 2.0 * (np.log(0.256) - lnZ_L2)
+    """The start vector of config 2': a scaling-shaped guess built from the paper's asymptotic forms eq.(16)-(19) (NOT the
+    fit functions of ref.[16], which are not in PAPER.md).  It is INPUT DATA here: the 72 numbers are stored in
+    tests/golden/scaling_start_N36.txt, written by tests/golden/make_scaling_start.py, which samples the forms at the
+    mapped Chebyshev roots and projects them with the oracle's own tables (tests/scaling_setup.py -- the one place where
+    that projection is written down)."""
+    assert (w.n_cheb, w.eps2, w.L2, w.x_G, w.x_Z, w.n_ir) == (36, 1e-6, 5e4, 0.0, 5e4, 32), "stored for config 2' only"
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "tests", "golden", "scaling_start_N36.txt")
+    c = np.array([float(line.split("#")[0]) for line in open(path) if line.split("#")[0].strip()])
+    assert c.shape == (2 * w.n_cheb,)
     return c

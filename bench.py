@@ -162,8 +162,8 @@ def run_reference(args, w, c):
 def run_ours(args, w, c, bc):
     import torch
     import torch.distributed as dist
-    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE
-    from paper_1206_1779_b200.binding import dfma_probe
+    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE, DSE_FLAG_CONST_COEF
+    from paper_1206_1779_b200.binding import probe
     from paper_1206_1779_b200.sharding import max_over_ranks
 
     rank = int(os.environ.get("RANK", "0"))
@@ -182,6 +182,8 @@ def run_ours(args, w, c, bc):
 
     nb = c.shape[0]
     flags = DSE_FLAG_GEOMETRY_CACHE if args.geometry_cache else 0
+    if nb == 1 and w.n_cheb % 8 == 0 and w.n_theta >= 32 and args.const_coef:
+        flags |= DSE_FLAG_CONST_COEF        # coefficients as constant-bank operands (explicit, one handle at a time)
     d = Dse(params_from_workload(w, n_batch=nb, flags=flags))
     n2 = 2 * w.n_cheb
     ct = torch.from_numpy(c).cuda()
@@ -320,7 +322,7 @@ def run_ours(args, w, c, bc):
         # infrared exponents and the coupling, all read on the device (dse_newton_solve + dse_dressing)
         from workloads import paper_scaling_workload, scaling_start_coefficients, PAPER_SCALING_BC
         ws = paper_scaling_workload()
-        d2 = Dse(params_from_workload(ws, flags=flags))
+        d2 = Dse(params_from_workload(ws, flags=flags & ~DSE_FLAG_CONST_COEF))
         c0 = torch.from_numpy(scaling_start_coefficients(ws)[None, :]).cuda()
         bc2 = torch.tensor([PAPER_SCALING_BC], dtype=torch.float64, device="cuda")
         cw2 = c0.clone()
@@ -355,11 +357,11 @@ def run_ours(args, w, c, bc):
     if rank == 0:
         # live fp64 FMA probe (reported beside the derived peak)
         sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
-        dfma_probe(148 * 8, 2000, sink)
+        probe("dfma", 148 * 8, 2000, sink)
         torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
-        fl = dfma_probe(148 * 8, 100000, sink)
+        fl = probe("dfma", 148 * 8, 100000, sink)
         b.record(stream)
         torch.cuda.synchronize()
         probe_tflops = fl / (a.elapsed_time(b) * 1e-3) / 1e12
@@ -424,6 +426,8 @@ def main():
     ap.add_argument("--geometry-cache", type=int, default=1,
                     help="1: coefficient-independent per-point factors are tabulated once in dse_create (default); "
                          "0: recomputed inside every build")
+    ap.add_argument("--const-coef", type=int, default=1,
+                    help="1: single-system builds ask for the constant-bank coefficient slot (DSE_FLAG_CONST_COEF)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     w, c, bc = config_inputs(args.config)

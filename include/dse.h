@@ -29,8 +29,10 @@
  *   - Return value: 0 (DSE_OK) or a negative DSE_E* code; no exception crosses the ABI.  A singular or
  *     ill-scaled J is reported through stats_dev (min |pivot|), not through the return code.
  *   - A handle is bound to the device that was current in dse_create and must be used from one
- *     host thread at a time.  No global state; no CPU fallback: without a CUDA device dse_create
- *     fails with DSE_ECUDA.
+ *     host thread, and on one stream, at a time.  Everything that selects a code path is in dse_params
+ *     (no environment variables); the library keeps no state outside the handles, with ONE exception
+ *     that the caller asks for explicitly: DSE_FLAG_CONST_COEF (below).  No CPU fallback: without a
+ *     CUDA device dse_create fails with DSE_ECUDA.
  *   - Layouts: c_dev [n_batch][2N] (a then b); bc_dev [n_batch][2] = (1/G(x_G), 1/Z(x_Z));
  *     F_dev [n_batch][2N]; J_dev [n_batch][2N][2N] row-major; stats_dev [n_batch][4].
  */
@@ -53,10 +55,11 @@ extern "C" {
 #define DSE_EINVAL (-1) /* bad parameter or null pointer                          */
 #define DSE_ENOMEM (-2) /* host or device allocation failed                       */
 #define DSE_ECUDA (-3)  /* CUDA runtime error (text via dse_last_error)           */
+#define DSE_EBUSY (-4)  /* DSE_FLAG_CONST_COEF: the constant-bank slot is held by another handle */
 
 #define DSE_MAX_NCHEB 128
 
-/* Parameters of the discretisation and of the truncation (one struct, no env vars). */
+/* Parameters of the discretisation and of the truncation: one POD struct, the only configuration channel. */
 typedef struct dse_params {
     int32_t n_cheb;     /* N: Chebyshev polynomials per dressing function, 2 <= N <= 128 (eq.(23),(24))  */
     int32_t n_r;        /* radial Gauss-Legendre nodes in ln y on [eps2, L2], >= 2 (L62, eq.(26) reading) */
@@ -87,12 +90,42 @@ typedef struct dse_params {
                                    EACH interval (L364): the radial rule then depends on the external point
                                    (n_r_ir + 2 n_r nodes per point); default: one rule on [eps2, L2] (BASELINE configs) */
 
+#define DSE_FLAG_USER_TABLES 8 /* the quadrature nodes and weights come from the caller (dse_create_with_tables): used to
+                                  separate kernel error from table-builder error in parity tests -- PAPER.md L62 never
+                                  gives the radial node map, so two independent builders may differ in the last digits */
+
+#define DSE_FLAG_CONST_COEF 16 /* single system (n_batch = 1), software-pipelined point kernel, N a multiple of 8 with
+                                  N/8 in {1,2,4,8,16}: the Chebyshev coefficients are read as constant-bank operands of the
+                                  fp64 FMAs (about 12 % faster point kernel at BASELINE configs[3]; an in-stream device-to-device
+                                  copy of c into the library's __constant__ array precedes every build).  The array is
+                                  ONE slot per process and device context: dse_create fails with DSE_EBUSY while another
+                                  live handle holds it, and with DSE_EINVAL if the shape cannot use it; the slot is released
+                                  by dse_destroy.  Never taken implicitly: without the flag the coefficients sit in shared
+                                  memory, whatever the creation order of the handles. */
+
+#define DSE_FLAG_PER_SYSTEM_KERNELS 32 /* n_batch >= 8: do not use the batched fp64-tensor point kernel (systems are then
+                                          walked one after the other by the single-system kernels); for tests and A/B runs */
+
 typedef struct dse_handle dse_handle; /* opaque; owned by the library */
 
 /* Builds the quadrature/collocation tables (Gauss-Legendre in ln y and in theta, Chebyshev roots
  * x_i, phi_j tables; eq.(25), fn.9 L224) on the host, copies them to the current
  * device and allocates the workspace.  Synchronous.  *out is set only on success. */
 DSE_API int dse_create(const dse_params *params, dse_handle **out);
+
+/* Caller-supplied quadrature tables (DSE_FLAG_USER_TABLES must be set in params->flags; dse_create refuses that flag).
+ * All HOST pointers, read during the call only:
+ *   x_ext[n_ext]            external momenta x_e: the N collocation points, then x_Z, then x_G if different (dse_n_ext order)
+ *   y, Wy [n_rules][n_rad]  radial nodes y_q (infrared piece first) and weights of dy (for the log-mapped rule: w_q (Lg/2) y_q),
+ *                           n_rad = n_r_ir + n_r (n_rules = 1), or n_r_ir + 2 n_r per external point under
+ *                           DSE_FLAG_RADIAL_SPLIT (n_rules = n_ext)
+ *   theta, Omega [n_theta]  angular nodes and weights of d(theta) (the sin^2 of the measure eq.(4),(5) stays in the integrand)
+ * Everything else (s(y_q) by eq.(25), phi_j tables, square roots, the continuation add-ons) is derived from these values in
+ * long double.  The collocation abscissae s_i stay the exact Chebyshev roots (fn.9 L224). */
+typedef struct dse_tables {
+    const double *x_ext, *y, *Wy, *theta, *Omega;
+} dse_tables;
+DSE_API int dse_create_with_tables(const dse_params *params, const dse_tables *tables, dse_handle **out);
 
 /* Frees everything dse_create made.  Synchronous.  NULL is accepted. */
 DSE_API int dse_destroy(dse_handle *h);
@@ -115,7 +148,10 @@ DSE_API int dse_jacobian_fd(dse_handle *h, const double *c_dev, const double *bc
 /* One Newton-Raphson step (eq.(31)-(35)): builds J, F, scales each row of (J|F) by 1/max_j|J_ij|,
  * LU with partial pivoting (first maximal element wins), solves J Delta = F, c <- c - rho Delta
  * in place.  stats_dev[b] = { max|Delta|, max_i|F_i| row-scaled, min|pivot|, growth max|U|/max|A| }.
- * stats_dev may be NULL. */
+ * stats_dev may be NULL.
+ * Singular or non-finite systems: the call is asynchronous, so they are reported through stats_dev, not the return code.
+ * If a pivot is exactly zero (stats[2] == 0) or Delta has a non-finite entry, c is left UNCHANGED for that system and
+ * stats[0] = +Inf; a caller that does not pass stats_dev cannot tell.  dse_newton_solve checks this itself (status -1). */
 DSE_API int dse_newton_step(dse_handle *h, double *c_dev, const double *bc_dev, double rho, double *stats_dev,
                     void *stream);
 
@@ -153,8 +189,9 @@ DSE_API int dse_jacobian_host(dse_handle *h, const double *c_host, const double 
 /* Sizes: n_ext = number of external points (N roots, then x_Z, then x_G if different). */
 DSE_API int dse_n_ext(const dse_handle *h);
 
-/* Copies the tables to host arrays (any pointer may be NULL): x_ext[n_ext], y[n_r_ir + n_r] (infrared piece first), Wy[n_r_ir + n_r]
- * (= w_q (Lg/2) y_q), theta[n_theta], Omega[n_theta] (= w_k pi/2).  For tests. */
+/* Copies the tables to host arrays (any pointer may be NULL), in the layout of dse_tables: x_ext[n_ext],
+ * y, Wy [n_rules][n_rad] (n_rules = 1, n_rad = n_r_ir + n_r; under DSE_FLAG_RADIAL_SPLIT n_rules = n_ext and
+ * n_rad = n_r_ir + 2 n_r: the rule of every external point), theta[n_theta], Omega[n_theta].  For tests. */
 DSE_API int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, double *Wy_host,
                    double *theta_host, double *Omega_host);
 
@@ -165,12 +202,13 @@ DSE_API int64_t dse_launch_count(const dse_handle *h);
  * out[2] = dynamic shared memory bytes, out[3] = registers/thread, out[4] = resident CTAs/SM,
  * out[5] = SM count, out[6] = variant of the Jacobian point kernel (0 generic, 1 software-pipelined,
  * 2 batched: 8 systems per warp on the fp64 tensor path, chosen when n_batch >= 8 (padded to a multiple of 8 with
- * idle systems, at most a quarter of the padded batch), n_cheb <= 64 and n_theta >= 32), out[7] = reserved (0). */
+ * idle systems, at most a quarter of the padded batch), n_cheb <= 64 and n_theta >= 32),
+ * out[7] = kernels per Jacobian build (1: the point kernel also reduces, contracts and assembles). */
 DSE_API int dse_kernel_info(const dse_handle *h, int32_t out[8]);
 
 /* Per-kernel device timing of the dominant (point) kernel, for the roofline report: while enabled,
  * every build records a CUDA event pair around the point kernel on the build's stream (nothing else
- * changes).  dse_get_timing synchronises on the recorded events, adds them up and returns the
+ * changes; where the point kernel is the whole build, its fused reduction/assembly tail is inside the pair).  dse_get_timing synchronises on the recorded events, adds them up and returns the
  * accumulated milliseconds and launch count since the last reset (enable resets). */
 DSE_API int dse_set_timing(dse_handle *h, int32_t enable);
 DSE_API int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches);
@@ -193,26 +231,6 @@ DSE_API int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, d
  * x_dev [n_x], all > 0; outputs [n_batch][n_x], any of them may be NULL (not all).  Asynchronous on `stream`. */
 DSE_API int dse_dressing(dse_handle *h, const double *c_dev, const double *x_dev, int32_t n_x, double *lnG_dev,
                          double *lnZ_dev, double *alpha_dev, void *stream);
-
-/* Environment switches for A/B measurements and tests (read in dse_create unless noted; none changes results beyond
- * rounding order): DSE_NO_BATCHED (per-system point kernels for batches), DSE_NO_PIPE (non-pipelined point kernel),
- * DSE_CONST_MEMCPY (coefficient slot filled by a device-to-device copy instead of prep_kernel's direct store),
- * DSE_NO_FUSED_ASSEMBLE, DSE_LU_BLOCKED and DSE_NO_PDL (separate contraction kernel / shared-memory LU / plain launches
- * instead of programmatic dependent launches between the kernels of a build; read once per process). */
-
-/* Diagnostics: cycles summed over all warps of the last point-kernel launch, spent in (geometry, series,
- * exp + weights, accumulation, whole warp); for the software-pipelined kernel: (entry until the tables are staged and the
- * producer kernel is done, first batch, remaining batches, epilogue phase 2 + flushes, whole warp).  All zeros unless the library was built with
- * -DDSE_PHASE_TIMING (the default build carries no instrumentation).  Synchronous. */
-DSE_API int dse_get_phase_cycles(dse_handle *h, double out_host[5]);
-
-/* fp64 FMA throughput probe (the roofline denominator of an ALU-bound path): launches a kernel of
- * `blocks` x 256 threads, each running 8 independent chains of `iters` dependent DFMAs, on `stream`.
- * flops per launch = blocks*256*8*iters*2.  sink_dev receives one double per thread (>= blocks*256).
- * dse_dmma_probe does the same with mma.sync.m8n8k4.f64 (4 chains per warp; flops =
- * blocks*8 warps*4*iters*512). */
-DSE_API int dse_dfma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream);
-DSE_API int dse_dmma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream);
 
 /* Text of a DSE_E* code, and the last CUDA error text seen by this thread ("" if none). */
 DSE_API const char *dse_strerror(int code);

@@ -1,0 +1,37 @@
+/*
+ * dse_diag.h -- diagnostics of libdse_b200.so that are NOT part of the method's boundary (include/dse.h):
+ * fp64 throughput probes.  They supply the roofline denominators bench.py reports against
+ * (MEASURED_PEAKS.json has no fp64 entry) and reproduce the three micro-measurements DESIGN.md section 6 leans on.
+ * `stream` is a cudaStream_t passed as void*; sink_dev is a DEVICE pointer owned by the caller.
+ */
+#ifndef DSE_DIAG_H_
+#define DSE_DIAG_H_
+
+#include "dse.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Probe kinds.  Every probe launches `blocks` CTAs of 256 threads; each thread runs `iters` iterations of an unrolled body
+ * of independent dependent-chains, so the issue rate of the named instruction mix is what is measured.
+ * dse_probe_flops(kind, blocks, iters) returns the floating-point operations of one launch (FMA = 2, an m8n8k4 MMA = 512
+ * per warp). */
+#define DSE_PROBE_DFMA 0        /* 8 chains of DFMA whose multiplier and addend are immediates/constants (2 register operands) */
+#define DSE_PROBE_DMMA 1        /* 4 chains of mma.sync.m8n8k4.f64 per warp (fp64 tensor path)                               */
+#define DSE_PROBE_DFMA_3REG 2   /* 8 chains of DFMA with three DISTINCT register operands, none reusable from the previous
+                                   instruction (acc_i = fma(w_i, t_i, acc_i), w and t rotate): the operand mix of the phase-2
+                                   accumulations of the point kernel                                                        */
+#define DSE_PROBE_DFMA_REUSE 3  /* as 2, but consecutive FMAs share one register operand in the same slot (operand reuse cache) */
+#define DSE_PROBE_DFMA_DMMA 4   /* independent DFMA chains and DMMA chains interleaved in one warp: do the two share a unit? */
+#define DSE_PROBE_DFMA_LDS 5    /* acc_j += w * T_j with EVERY T_j read from shared memory (the "stash all T_j" alternative to
+                                   re-running the recurrence in phase 2): 1 LDS.64 per DFMA                                  */
+
+/* sink_dev receives one double per thread (>= blocks * 256).  Asynchronous on `stream`. */
+DSE_API int dse_probe(int32_t kind, int32_t blocks, int32_t iters, double *sink_dev, void *stream);
+DSE_API double dse_probe_flops(int32_t kind, int32_t blocks, int32_t iters);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DSE_DIAG_H_ */

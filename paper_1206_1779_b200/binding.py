@@ -12,15 +12,23 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
 
+# every symbol include/dse.h and include/dse_diag.h declare (tests/test_abi.py checks the list against the headers)
 EXPORTS = [
-    "dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step", "dse_newton_solve", "dse_lu_solve",
-    "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count", "dse_kernel_info",
-    "dse_set_timing", "dse_get_timing", "dse_get_phase_cycles", "dse_gauss_legendre", "dse_schwinger", "dse_dressing", "dse_jacobian_fd", "dse_dfma_probe", "dse_dmma_probe", "dse_strerror", "dse_last_error",
+    "dse_create", "dse_create_with_tables", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step",
+    "dse_newton_solve", "dse_lu_solve", "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count",
+    "dse_kernel_info", "dse_set_timing", "dse_get_timing", "dse_gauss_legendre", "dse_schwinger", "dse_dressing",
+    "dse_jacobian_fd", "dse_strerror", "dse_last_error",
+    "dse_probe", "dse_probe_flops",
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
 DSE_FLAG_ANGULAR_TANH_SINH = 2
 DSE_FLAG_RADIAL_SPLIT = 4
+DSE_FLAG_USER_TABLES = 8
+DSE_FLAG_CONST_COEF = 16
+DSE_FLAG_PER_SYSTEM_KERNELS = 32
+DSE_EBUSY = -4
+PROBE_KINDS = {"dfma": 0, "dmma": 1, "dfma_3reg": 2, "dfma_reuse": 3, "dfma_dmma": 4, "dfma_lds": 5}
 
 
 class DseParams(C.Structure):
@@ -33,8 +41,14 @@ class DseParams(C.Structure):
     ]
 
 
+class DseTables(C.Structure):
+    _fields_ = [("x_ext", C.c_void_p), ("y", C.c_void_p), ("Wy", C.c_void_p), ("theta", C.c_void_p), ("Omega", C.c_void_p)]
+
+
 class DseError(RuntimeError):
-    pass
+    def __init__(self, msg, code=None):
+        super().__init__(msg)
+        self.code = code
 
 
 _lib = None
@@ -51,6 +65,7 @@ def load_library():
     L = C.CDLL(LIB_PATH)
     vp, dp = C.c_void_p, C.c_void_p
     L.dse_create.argtypes = [C.POINTER(DseParams), C.POINTER(vp)]
+    L.dse_create_with_tables.argtypes = [C.POINTER(DseParams), C.POINTER(DseTables), C.POINTER(vp)]
     L.dse_destroy.argtypes = [vp]
     L.dse_residual.argtypes = [vp, dp, dp, dp, vp]
     L.dse_jacobian.argtypes = [vp, dp, dp, dp, dp, vp]
@@ -65,13 +80,13 @@ def load_library():
     L.dse_kernel_info.argtypes = [vp, C.POINTER(C.c_int32 * 8)]
     L.dse_set_timing.argtypes = [vp, C.c_int32]
     L.dse_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
-    L.dse_get_phase_cycles.argtypes = [vp, C.POINTER(C.c_double * 5)]
     L.dse_jacobian_fd.argtypes = [vp, dp, dp, C.c_double, dp, vp]
     L.dse_gauss_legendre.argtypes = [C.c_int32, dp, dp, dp, vp]
     L.dse_schwinger.argtypes = [vp, dp, C.c_int32, C.c_double, C.c_double, dp, C.c_int32, dp, dp, vp]
     L.dse_dressing.argtypes = [vp, dp, dp, C.c_int32, dp, dp, dp, vp]
-    L.dse_dfma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
-    L.dse_dmma_probe.argtypes = [C.c_int32, C.c_int32, dp, vp]
+    L.dse_probe.argtypes = [C.c_int32, C.c_int32, C.c_int32, dp, vp]
+    L.dse_probe_flops.argtypes = [C.c_int32, C.c_int32, C.c_int32]
+    L.dse_probe_flops.restype = C.c_double
     L.dse_strerror.argtypes = [C.c_int]
     L.dse_strerror.restype = C.c_char_p
     L.dse_last_error.restype = C.c_char_p
@@ -82,7 +97,7 @@ def load_library():
 def _check(rc):
     if rc != 0:
         L = load_library()
-        raise DseError(f"{L.dse_strerror(rc).decode()} ({rc}): {L.dse_last_error().decode()}")
+        raise DseError(f"{L.dse_strerror(rc).decode()} ({rc}): {L.dse_last_error().decode()}", rc)
 
 
 def params_from_workload(w, n_batch=None, flags=0):
@@ -111,14 +126,21 @@ def _dev_ptr(t, n=None):
 class Dse:
     """dse_handle wrapper.  Method names mirror the C ABI: residual / jacobian / newton_step / lu_solve."""
 
-    def __init__(self, params: DseParams):
+    def __init__(self, params: DseParams, tables: dict = None):
+        """tables (with DSE_FLAG_USER_TABLES): dict of float64 numpy arrays x_ext, y, Wy, theta, Omega in the layout of
+        dse_tables (include/dse.h) -> dse_create_with_tables."""
         import torch
         if not torch.cuda.is_available():
             raise DseError("no CUDA device: this library has no CPU fallback")
         self.lib = load_library()
         self.params = params
         h = C.c_void_p()
-        _check(self.lib.dse_create(C.byref(params), C.byref(h)))
+        if tables is not None:
+            arrs = {k: np.ascontiguousarray(tables[k], dtype=np.float64) for k in ("x_ext", "y", "Wy", "theta", "Omega")}
+            t = DseTables(*[C.c_void_p(arrs[k].ctypes.data) for k in ("x_ext", "y", "Wy", "theta", "Omega")])
+            _check(self.lib.dse_create_with_tables(C.byref(params), C.byref(t), C.byref(h)))
+        else:
+            _check(self.lib.dse_create(C.byref(params), C.byref(h)))
         self._h = h
         self.N = params.n_cheb
         self.B = params.n_batch
@@ -219,8 +241,10 @@ class Dse:
     # ---- introspection ----------------------------------------------------------------------------
     def tables(self):
         p = self.params
-        nr = (2 if p.flags & DSE_FLAG_RADIAL_SPLIT else 1) * p.n_r + p.n_r_ir
-        out = dict(x_ext=np.empty(self.n_ext), y=np.empty(nr), Wy=np.empty(nr), theta=np.empty(p.n_theta),
+        split = bool(p.flags & DSE_FLAG_RADIAL_SPLIT)
+        nr = (2 if split else 1) * p.n_r + p.n_r_ir
+        shape = (self.n_ext, nr) if split else (nr,)          # the split rule has one radial rule per external point
+        out = dict(x_ext=np.empty(self.n_ext), y=np.empty(shape), Wy=np.empty(shape), theta=np.empty(p.n_theta),
                    Omega=np.empty(p.n_theta))
         _check(self.lib.dse_get_tables(self._h, *[C.c_void_p(out[k].ctypes.data)
                                                   for k in ("x_ext", "y", "Wy", "theta", "Omega")]))
@@ -235,11 +259,6 @@ class Dse:
         _check(self.lib.dse_get_timing(self._h, C.byref(ms), C.byref(n)))
         return ms.value, n.value
 
-    def phase_cycles(self):
-        a = (C.c_double * 5)()
-        _check(self.lib.dse_get_phase_cycles(self._h, C.byref(a)))
-        return list(a)
-
     def launch_count(self):
         return int(self.lib.dse_launch_count(self._h))
 
@@ -247,17 +266,15 @@ class Dse:
         a = (C.c_int32 * 8)()
         _check(self.lib.dse_kernel_info(self._h, C.byref(a)))
         return dict(grid=a[0], block=a[1], smem=a[2], regs=a[3], ctas_per_sm=a[4], sms=a[5],
-                    variant=("generic", "pipelined", "batched-dmma")[a[6]])
+                    variant=("generic", "pipelined", "batched-dmma")[a[6]], kernels_per_build=a[7])
 
 
-def dfma_probe(blocks, iters, sink, stream=None):
-    _check(load_library().dse_dfma_probe(blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
-    return blocks * 256 * 8 * iters * 2
-
-
-def dmma_probe(blocks, iters, sink, stream=None):
-    _check(load_library().dse_dmma_probe(blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
-    return blocks * 8 * 4 * iters * 512
+def probe(kind, blocks, iters, sink, stream=None):
+    """include/dse_diag.h: launches one fp64 throughput probe; returns the floating-point operations of the launch."""
+    k = PROBE_KINDS[kind] if isinstance(kind, str) else int(kind)
+    L = load_library()
+    _check(L.dse_probe(k, blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
+    return L.dse_probe_flops(k, blocks, iters)
 
 
 def gauss_legendre(n, device="cuda", stream=None):

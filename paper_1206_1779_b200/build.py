@@ -11,8 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdse_b200.so")
-SOURCES = ["dse_api.cu", "dse_kernels.cu", "dse_point.cu", "dse_point_batched.cu", "dse_lu.cu", "dse_lu_reg.cu", "dse_solve.cu", "dse_schwinger.cu", "dse_tables.cpp"]
-DEPS = SOURCES + ["dse_internal.h", "dse_device.cuh", os.path.join("..", "..", "include", "dse.h")]
+SOURCES = ["dse_api.cu", "dse_kernels.cu", "dse_point.cu", "dse_point_batched.cu", "dse_lu.cu", "dse_solve.cu", "dse_schwinger.cu", "dse_probe.cu", "dse_tables.cpp"]
+DEPS = SOURCES + ["dse_internal.h", "dse_device.cuh", "dse_tail.cuh", os.path.join("..", "..", "include", "dse.h"), os.path.join("..", "..", "include", "dse_diag.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 

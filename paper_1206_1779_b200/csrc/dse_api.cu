@@ -4,16 +4,10 @@
 
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 
 #include "dse_internal.h"
-
-namespace dse {
-const char *last_error_text();
-void set_error_text(const char *s);
-}  // namespace dse
 
 struct dse_handle {
     dse_params params;
@@ -46,13 +40,7 @@ struct dse_handle {
 
 namespace {
 
-int cuda_err(cudaError_t e, const char *what)
-{
-    char buf[256];
-    snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
-    dse::set_error_text(buf);
-    return DSE_ECUDA;
-}
+int cuda_err(cudaError_t e, const char *what) { return dse::cuda_fail((int)e, what); }
 
 #define CK(call)                                             \
     do {                                                     \
@@ -67,13 +55,17 @@ int validate(const dse_params *p)
     if (!p) return DSE_EINVAL;
     if (p->n_cheb < 2 || p->n_cheb > DSE_MAX_NCHEB) return DSE_EINVAL;
     if (p->n_r < 2 || p->n_theta < 2 || p->n_batch < 1) return DSE_EINVAL;
-    if (p->n_r > (1 << 20) || p->n_theta > (1 << 16) || p->n_batch > (1 << 20)) return DSE_EINVAL;
+    // the host table builder is O(n^2) per Gauss-Legendre rule (Newton on the Legendre recurrence in long double) and the
+    // angular table lives in shared memory: 2^15 radial and 2^11 angular nodes are far beyond any use of the method
+    if (p->n_r > (1 << 15) || p->n_theta > (1 << 11) || p->n_batch > (1 << 20)) return DSE_EINVAL;
     if (!finite_pos(p->eps2) || !finite_pos(p->L2) || !(p->eps2 < p->L2)) return DSE_EINVAL;
     if (!finite_pos(p->alpha_mu) || !finite_pos(p->n_colors)) return DSE_EINVAL;
     if (!finite_pos(p->x_Z) || !std::isfinite(p->x_G) || p->x_G < 0.0 || (p->x_G == 0.0 && p->x_Z == 0.0)) return DSE_EINVAL;
     if (!std::isfinite(p->delta) || !std::isfinite(p->ir_exp_G) || !std::isfinite(p->ir_exp_Z)) return DSE_EINVAL;
     if (!std::isfinite(p->uv_omega) || p->uv_omega < 0.0) return DSE_EINVAL;
-    if (p->n_r_ir < 0 || p->n_r_ir > (1 << 20) || (p->flags & ~(DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_ANGULAR_TANH_SINH | DSE_FLAG_RADIAL_SPLIT))) return DSE_EINVAL;
+    const int known = DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_ANGULAR_TANH_SINH | DSE_FLAG_RADIAL_SPLIT | DSE_FLAG_USER_TABLES |
+                      DSE_FLAG_CONST_COEF | DSE_FLAG_PER_SYSTEM_KERNELS;
+    if (p->n_r_ir < 0 || p->n_r_ir > (1 << 15) || (p->flags & ~known)) return DSE_EINVAL;
     return DSE_OK;
 }
 
@@ -125,7 +117,22 @@ size_t carve(size_t &off, size_t n)
 
 extern "C" {
 
+static int create_impl(const dse_params *params, const dse_tables *user, dse_handle **out);
+
 int dse_create(const dse_params *params, dse_handle **out)
+{
+    if (params && (params->flags & DSE_FLAG_USER_TABLES)) return DSE_EINVAL;      // needs dse_create_with_tables
+    return create_impl(params, nullptr, out);
+}
+
+int dse_create_with_tables(const dse_params *params, const dse_tables *tables, dse_handle **out)
+{
+    if (!params || !(params->flags & DSE_FLAG_USER_TABLES) || !tables) return DSE_EINVAL;
+    if (!tables->x_ext || !tables->y || !tables->Wy || !tables->theta || !tables->Omega) return DSE_EINVAL;
+    return create_impl(params, tables, out);
+}
+
+static int create_impl(const dse_params *params, const dse_tables *user, dse_handle **out)
 {
     if (!out) return DSE_EINVAL;
     int rc = validate(params);
@@ -139,9 +146,10 @@ int dse_create(const dse_params *params, dse_handle **out)
     dse_handle *h = new (std::nothrow) dse_handle();
     if (!h) return DSE_ENOMEM;
     h->params = *params;
-    CK(cudaGetDevice(&h->device));
+    e = cudaGetDevice(&h->device);
+    if (e != cudaSuccess) { delete h; return cuda_err(e, "cudaGetDevice"); }
     try {
-        dse::build_tables(*params, h->tab);
+        dse::build_tables(*params, user, h->tab);
     } catch (const std::bad_alloc &) {
         delete h;
         return DSE_ENOMEM;
@@ -203,12 +211,28 @@ int dse_create(const dse_params *params, dse_handle **out)
     }
 
     // ---- launch configuration of the point kernel ----
-    k.use_constc = dse::acquire_const_slot(k) ? 1 : 0;
-    h->owns_const = k.use_constc != 0;
-    k.coefC = (k.use_constc && !getenv("DSE_CONST_MEMCPY")) ? dse::const_slot_address() : nullptr;
+    if (params->flags & DSE_FLAG_CONST_COEF) {            // explicit request for the library's constant-bank slot
+        if (!dse::constc_shape_ok(k)) {
+            dse::set_error_text("DSE_FLAG_CONST_COEF needs n_batch = 1, n_theta >= 32 and n_cheb in {8, 16, 32, 64, 128}");
+            dse_destroy(h);
+            return DSE_EINVAL;
+        }
+        if (!dse::const_slot_acquire()) {
+            dse::set_error_text("DSE_FLAG_CONST_COEF: the constant-bank slot is held by another handle");
+            dse_destroy(h);
+            return DSE_EBUSY;
+        }
+        h->owns_const = true;
+        k.use_constc = 1;
+    }
     rc = dse::query_point_kernel(k, h->cfg);
     if (rc < 0) { dse_destroy(h); return rc; }
-    if (dse::batched_eligible(k)) {                       // 8 systems per warp on the fp64 tensor path
+    if (k.use_constc && !h->cfg.pipelined) {              // (cannot happen for the shapes constc_shape_ok admits)
+        dse::set_error_text("DSE_FLAG_CONST_COEF: shape does not run the pipelined kernel");
+        dse_destroy(h);
+        return DSE_EINVAL;
+    }
+    if (!(params->flags & DSE_FLAG_PER_SYSTEM_KERNELS) && dse::batched_eligible(k)) {      // 8 systems per warp on the fp64 tensor path
         rc = dse::query_point_batched(k, h->cfg);
         if (rc < 0) { dse_destroy(h); return rc; }
     }
@@ -230,10 +254,11 @@ int dse_create(const dse_params *params, dse_handle **out)
     const size_t o_A = carve<double>(off, Rpad * 4), o_AH = carve<double>(off, Rpad * 4);
     const size_t o_S = carve<double>(off, ((size_t)k.W * k.bgroup + Bpad * k.Next) * 3 * k.Npad);
     const size_t o_R = carve<double>(off, (size_t)k.B * k.Next * 3 * k.Npad);
+    const size_t o_Dg = carve<double>(off, (size_t)k.B * k.Next * 4 * k.Npad), o_Pi = carve<double>(off, (size_t)k.B * k.Next * 4);
+    const size_t o_cnt = carve<double>(off, ((size_t)k.B * k.Next + k.B + 1) / 2 + 1);      // unsigned counters of the fused tail
     const size_t o_J = carve<double>(off, (size_t)k.B * n2 * n2), o_F = carve<double>(off, (size_t)k.B * n2);
     const size_t o_lu = carve<double>(off, (size_t)k.B * dse::lu_scratch_doubles((int)n2));
     const size_t o_c = carve<double>(off, (size_t)k.B * n2), o_bc = carve<double>(off, (size_t)k.B * 2);
-    const size_t o_dbg = carve<double>(off, (size_t)k.W * 5);
     const size_t o_fd = carve<double>(off, (size_t)k.B * n2 * 3);          // finite-difference self-check: c_tmp, F+, F-
     const size_t o_dl = carve<double>(off, (size_t)k.B * n2), o_st = carve<double>(off, (size_t)k.B * 4);
     const size_t o_ctl = carve<double>(off, 8), o_info = carve<double>(off, (size_t)k.B * 6);
@@ -242,11 +267,15 @@ int dse_create(const dse_params *params, dse_handle **out)
     if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemset(workspace)"); }
     double *wk = h->d_work;
     k.coefP = wk + o_coef; k.Gy = wk + o_Gy; k.Py = wk + o_Py; k.invG = wk + o_iG; k.invZ = wk + o_iZ;
-    k.Apart = wk + o_A; k.AHead = wk + o_AH; k.Spart = wk + o_S; k.Rz = wk + o_R; k.dbg = wk + o_dbg; h->d_fd = wk + o_fd;
+    k.Apart = wk + o_A; k.AHead = wk + o_AH; k.Spart = wk + o_S; k.Rz = wk + o_R; h->d_fd = wk + o_fd;
+    k.Dg = wk + o_Dg; k.PiInv = wk + o_Pi;
+    k.cnt = reinterpret_cast<unsigned *>(wk + o_cnt); k.done = k.cnt + (size_t)k.B * k.Next;
     h->d_J = wk + o_J; h->d_F = wk + o_F; h->d_lu = wk + o_lu; h->d_c = wk + o_c; h->d_bc = wk + o_bc;
     h->d_Jh = h->d_J; h->d_Fh = h->d_F;
     h->d_delta = wk + o_dl; h->d_stats = wk + o_st; h->d_ctl = wk + o_ctl; h->d_info = wk + o_info;
 
+    rc = dse::lu_configure((int)n2);
+    if (rc < 0) { dse_destroy(h); return rc; }
     if (k.geom) {
         rc = dse::launch_geometry(k, h->d_geom, nullptr);
         if (rc < 0) { dse_destroy(h); return rc; }
@@ -262,7 +291,7 @@ int dse_destroy(dse_handle *h)
 {
     if (!h) return DSE_OK;
     cudaDeviceSynchronize();
-    if (h->owns_const) dse::release_const_slot();
+    if (h->owns_const) dse::const_slot_release();
     dse::solve_graph_destroy(h->solve);
     if (h->d_tables) cudaFree(h->d_tables);
     if (h->d_work) cudaFree(h->d_work);
@@ -333,7 +362,9 @@ int dse_lu_solve(dse_handle *h, int32_t n, int32_t n_sys, const double *A_dev, c
         if (n != 2 * h->k.N || n_sys > h->k.B) return DSE_EINVAL;
         scratch = h->d_lu;
     }
-    int rc = dse::launch_lu(n, n_sys, A_dev, b_dev, x_dev, nullptr, 0.0, stats_dev, scratch, stream);
+    int rc = n == 2 * h->k.N ? 0 : dse::lu_configure(n);
+    if (rc < 0) return rc;
+    rc = dse::launch_lu(n, n_sys, A_dev, b_dev, x_dev, nullptr, 0.0, stats_dev, scratch, stream);
     if (rc < 0) return rc;
     h->launches += rc;
     return DSE_OK;
@@ -443,17 +474,6 @@ int dse_dressing(dse_handle *h, const double *c_dev, const double *x_dev, int32_
     return DSE_OK;
 }
 
-int dse_get_phase_cycles(dse_handle *h, double out_host[5])
-{
-    if (!h || !out_host) return DSE_EINVAL;
-    std::vector<double> tmp((size_t)h->k.W * 5);
-    CK(cudaMemcpy(tmp.data(), h->k.dbg, 8 * tmp.size(), cudaMemcpyDeviceToHost));
-    for (int i = 0; i < 5; ++i) out_host[i] = 0.0;
-    for (int w = 0; w < h->k.W; ++w)
-        for (int i = 0; i < 5; ++i) out_host[i] += tmp[(size_t)w * 5 + i];
-    return DSE_OK;
-}
-
 int dse_n_ext(const dse_handle *h) { return h ? h->k.Next : DSE_EINVAL; }
 
 int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, double *Wy_host, double *theta_host,
@@ -462,8 +482,8 @@ int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, doub
     if (!h) return DSE_EINVAL;
     const dse::HostTables &T = h->tab;
     if (x_ext_host) memcpy(x_ext_host, T.x_ext.data(), 8 * T.x_ext.size());
-    if (y_host) memcpy(y_host, T.y.data(), 8 * (size_t)T.Nr);          // split rule: the rule of external point 0
-    if (Wy_host) memcpy(Wy_host, T.Wy.data(), 8 * (size_t)T.Nr);
+    if (y_host) memcpy(y_host, T.y.data(), 8 * T.y.size());            // [n_rules][n_rad]: every rule under the split flag
+    if (Wy_host) memcpy(Wy_host, T.Wy.data(), 8 * T.Wy.size());
     if (theta_host) memcpy(theta_host, T.theta.data(), 8 * T.theta.size());
     if (Omega_host) memcpy(Omega_host, T.Omega.data(), 8 * T.Omega.size());
     return DSE_OK;
@@ -476,22 +496,9 @@ int dse_kernel_info(const dse_handle *h, int32_t out[8])
     if (!h || !out) return DSE_EINVAL;
     out[0] = h->cfg.grid; out[1] = h->cfg.block; out[2] = h->cfg.smem; out[3] = h->cfg.regs;
     out[4] = h->cfg.ctas_per_sm; out[5] = h->cfg.sms;
-    out[6] = h->cfg.batched ? 2 : (h->cfg.pipelined ? 1 : 0); out[7] = 0;
+    out[6] = h->cfg.batched ? 2 : (h->cfg.pipelined ? 1 : 0);
+    out[7] = h->cfg.batched ? 4 : (h->cfg.pipelined ? 1 : 2);
     return DSE_OK;
-}
-
-int dse_dfma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream)
-{
-    if (blocks < 1 || iters < 1 || !sink_dev) return DSE_EINVAL;
-    int rc = dse::launch_dfma_probe(blocks, iters, sink_dev, stream);
-    return rc < 0 ? rc : DSE_OK;
-}
-
-int dse_dmma_probe(int32_t blocks, int32_t iters, double *sink_dev, void *stream)
-{
-    if (blocks < 1 || iters < 1 || !sink_dev) return DSE_EINVAL;
-    int rc = dse::launch_dmma_probe(blocks, iters, sink_dev, stream);
-    return rc < 0 ? rc : DSE_OK;
 }
 
 const char *dse_strerror(int code)
@@ -501,6 +508,7 @@ const char *dse_strerror(int code)
         case DSE_EINVAL: return "invalid argument";
         case DSE_ENOMEM: return "out of memory";
         case DSE_ECUDA: return "CUDA error (see dse_last_error)";
+        case DSE_EBUSY: return "constant-bank coefficient slot is held by another handle";
         default: return "unknown error";
     }
 }

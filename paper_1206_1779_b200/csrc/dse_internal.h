@@ -1,10 +1,11 @@
 // dse_internal.h -- shared between the host API (dse_api.cu), the table builder (dse_tables.cpp)
-// and the kernels (dse_kernels.cu, dse_lu.cu).  Not part of the public ABI.
+// and the kernels.  Not part of the public ABI.
 #pragma once
 #include <cstdint>
 #include <vector>
 
 #include "../../include/dse.h"
+#include "../../include/dse_diag.h"
 
 namespace dse {
 
@@ -25,7 +26,8 @@ struct HostTables {
     std::vector<double> phi_y;                    // [Nr][Npad]   phi_j(t_q)   (phi_0 = 1/2)
     std::vector<double> phi_x;                    // [N][Npad]    phi_j(s_i)
 };
-void build_tables(const dse_params &p, HostTables &t);
+// user: caller-supplied nodes and weights (DSE_FLAG_USER_TABLES) or nullptr
+void build_tables(const dse_params &p, const dse_tables *user, HostTables &t);
 
 // Everything the kernels need, passed by value.
 struct KParams {
@@ -39,36 +41,44 @@ struct KParams {
     int upr;                           // partition units per row
     int bgroup;                        // systems per work unit: 8 with the batched DMMA point kernel, else 1
     int want_jac;                      // 0: residual only (skip phase 2)
-    int use_constc;                    // coefficient pairs are read as constant-bank operands (single system, slot owner)
-    double *coefC;                     // global address of the constant-bank slot (prep_kernel writes it), or nullptr
+    int use_constc;                    // coefficients are constant-bank operands (DSE_FLAG_CONST_COEF, pipelined kernel)
+    int tail;                          // the point kernel finishes the build itself (reduction, contraction, assembly)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
     const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x, *EGy, *EZy;
     const double *geom;                // geometry cache [Next*Nr*Ntpad][4] or nullptr
+    // arguments of one build (set per launch)
+    const double *c, *bc;              // [B][2N] coefficients (a then b), [B][2] boundary values
+    double *J, *F;                     // outputs
     // per-build workspace
-    double *coefP;                     // [B][Npad][2]  (a_j, b_j), j = 0 pre-halved, zero padded
-    double *Gy, *Py;                   // [B][Nr]
-    double *invG, *invZ;               // [B][N]   1/G(x_i), 1/Z(x_i)
+    double *coefP;                     // [B][Npad][2]  (a_j, b_j), j = 0 pre-halved, zero padded       (prep_kernel)
+    double *Gy, *Py;                   // [B][Gext][Nr]                                                  (prep_kernel)
+    double *invG, *invZ;               // [B][N]   1/G(x_i), 1/Z(x_i)                                   (prep_kernel)
     double *Apart;                     // [B*Next][Nr][4]   sum_k (u_a, u_b, v, wQ+wM)
     double *AHead;                     // same shape: partial sums of rows whose angular batches span two warps (else 0)
-    double *Spart;                     // [W + B*Next][3][Npad]
-    double *Rz;                        // [B*Next][3][Npad]  A . Phi_y
-    double *D;                         // [B*Next][4][Npad]  dPiG/da, dPiG/db, dPiZ/da, dPiZ/db
-    double *Pi;                        // [B*Next][2]        Pi_G, Pi_Z
-    double *dbg;                       // per-warp phase cycle counters (only with -DDSE_PHASE_TIMING), else nullptr
+    double *Spart;                     // [W + B*Next][3][Npad]   per-(warp, external point) partials of the three streams
+    double *Rz;                        // [B*Next][3][Npad]  A . Phi_y                                   (batched builds)
+    double *Dg;                        // [B*Next][4][Npad]  dPiZ/da, dPiZ/db, dPiG/da, dPiG/db          (fused tail)
+    double *PiInv;                     // [B*Next][4]        Pi_G, Pi_Z, 1/G(x_e), 1/Z(x_e)              (fused tail)
+    unsigned *cnt;                     // [B*Next] arrival counters of the fused tail, [B] completed external points
+    unsigned *done;
 };
 
 struct PointKernelConfig {
     int grid, block, smem, regs, ctas_per_sm, sms;       // Jacobian build (defines KParams::W and the partial slots)
     int res_grid, res_block, res_smem;                   // residual-only build (no partials)
-    int pipelined;                                       // Jacobian build uses the software-pipelined kernel
+    int pipelined;                                       // Jacobian build uses the software-pipelined kernel (2: 512-thread build)
     int batched;                                         // Jacobian build uses the batched DMMA kernel (8 systems per warp)
 };
 
-// launchers (dse_kernels.cu / dse_lu.cu); each returns the number of kernels launched or <0 on error
+// launchers; each returns the number of kernels launched or <0 on error
 // ev0/ev1: optional cudaEvent_t pair recorded around the point kernel (nullptr = no timing)
 int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c_dev, const double *bc_dev,
                  double *J_dev, double *F_dev, void *stream, void *ev0 = nullptr, void *ev1 = nullptr);
 int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream);
+int query_point_kernel(const KParams &k, PointKernelConfig &cfg);
+bool constc_shape_ok(const KParams &k);     // shapes that can read the coefficients from the constant bank
+bool const_slot_acquire();                  // DSE_FLAG_CONST_COEF: the library's one __constant__ coefficient slot
+void const_slot_release();
 // batched DMMA point kernel (dse_point_batched.cu): eligibility, launch configuration, launch
 bool batched_eligible(const KParams &k);
 int query_point_batched(const KParams &k, PointKernelConfig &cfg);
@@ -77,18 +87,10 @@ int launch_fd_perturb(int n2, int B, const double *c, double *c_tmp, int j, doub
 int launch_fd_column(int n2, int B, const double *c, const double *Fp, const double *Fm, double *J, int j, double eps_rel,
                      void *stream);
 int launch_geometry(const KParams &k, double *geom, void *stream);
-bool lu_reg_eligible(int n);      // 2N <= 128: register-resident LU (dse_lu_reg.cu)
-int launch_lu_reg(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
-                  double *stats, void *stream);
-bool lu_cluster_eligible(int n);  // 128 < 2N <= 256: the register-resident LU over a cluster of 4 CTAs
-int launch_lu_cluster(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
-                      double *stats, double *scratch, void *stream);
+// H9 (dse_lu.cu): n <= 128 one CTA, matrix in registers; 128 < n <= 256 a cluster of 4 CTAs (needs `scratch`)
+int lu_configure(int n);          // opt-in attributes of the kernel that serves n, on the current device
 int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
               double *stats, double *scratch, void *stream);
-int query_point_kernel(const KParams &k, PointKernelConfig &cfg);
-bool acquire_const_slot(const KParams &k);
-double *const_slot_address();     // global-memory address of the slot (nullptr if unavailable)
-void release_const_slot();
 size_t lu_scratch_doubles(int n);
 // dse_solve.cu: the Newton iteration as a CUDA graph with a WHILE node (dse_newton_solve)
 struct SolveGraph;
@@ -101,7 +103,10 @@ int launch_schwinger(const KParams &k, const double *c, int n, double p2_min, do
                      double *out, double *work, void *stream);
 int launch_dressing(const KParams &k, const double *c, int n_x, const double *x, double alpha_mu, double *lnG, double *lnZ,
                     double *alpha, void *stream);
-int launch_dfma_probe(int blocks, int iters, double *sink, void *stream);
-int launch_dmma_probe(int blocks, int iters, double *sink, void *stream);
+int launch_probe(int kind, int blocks, int iters, double *sink, void *stream);
+
+const char *last_error_text();
+void set_error_text(const char *s);
+int cuda_fail(int /*cudaError_t*/ e, const char *what);     // records the text, returns DSE_ECUDA
 
 }  // namespace dse

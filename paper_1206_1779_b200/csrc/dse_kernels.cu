@@ -1,16 +1,17 @@
 // dse_kernels.cu -- sm_100a kernels for the residual + analytic Newton matrix of the ghost/gluon DSEs.
 //
-// Launch sequence of one build (all on the caller's stream, no host sync, no atomics):
-//   prep_kernel     H1  series at the fixed points y_q, x_i: G(y_q), P(y_q), 1/G(x_i), 1/Z(x_i)
-//   point_kernel    H2-H6 (the hot kernel): every quadrature point (x_e, y_q, theta_k)
-//   gemm_kernel     H7  the only dense contraction, A[e,q] . phi_j(t_q), on the fp64 tensor path (DMMA)
-//   assemble_kernel H8  fixed-order reduction of the per-warp partials, subtraction rows, local terms
-//                       (small single-system builds: H7 runs inside the assemble CTAs, also as DMMA)
+// Launch sequences of one build (all on the caller's stream, no host sync, no data atomics):
+//   Jacobian build, full-warp angular batches, compile-time chunk count (dse_point.cu, point_kernel_pipe):
+//       ONE kernel -- H1 in its prologue, H2-H6 in its body, H7 + H8 in its tail (dse_tail.cuh)
+//       (DSE_FLAG_CONST_COEF: preceded by two in-stream copies of c into the constant bank)
+//   Jacobian build, other single-system shapes:   prep_kernel (H1) -> point_kernel (H2-H6 + the same tail)
+//   batched Jacobian build (>= 8 systems, tensor path):
+//       prep_kernel -> point_kernel_batched -> gemm_kernel (H7, DMMA) | contract_split_kernel -> assemble_kernel (H8)
+//   residual only:                                 prep_kernel -> point kernel (no phase 2) -> assemble_kernel
 // Equation numbers refer to PAPER.md (arXiv:1206.1779); see include/dse.h and DESIGN.md.
 #include <cuda_runtime.h>
 
 #include <cstdio>
-#include <cstdlib>
 
 #include "dse_device.cuh"
 
@@ -36,7 +37,6 @@ __global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double
             if (j == 0) { a *= 0.5; bb *= 0.5; }
             P.coefP[((size_t)b * P.Npad + j) * 2 + 0] = a;
             P.coefP[((size_t)b * P.Npad + j) * 2 + 1] = bb;
-            if (P.coefC) { P.coefC[2 * j] = a; P.coefC[2 * j + 1] = bb; }      // constant-bank slot (single system)
         }
     }
     const int NG = P.Gext * P.Nr;                        // fixed points y_{e,q} (split rule) or y_q (shared rule)
@@ -92,12 +92,11 @@ __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
 // H7: Rz[b,e,stream][j] = sum_q A_stream[b,e,q] phi_j(t_q): the z-independent part of the Jacobian,
 // a dense [3 N_ext x N_r] . [N_r x N] contraction per system, on the fp64 tensor path
 // (mma.sync.aligned.m8n8k4 f64 -> DMMA).  One CTA per (8 external points, 8 values of j, system); its
-// 16 warps split K = N_r; each lane loads one 32-byte row-sum record (all three streams at once), so one
-// k-step feeds three MMAs; the 16 partial tiles are combined in warp order (deterministic).
-constexpr int GEMM_WARPS = 16;
-// NTG = n-tiles (8 values of j each) per CTA: 1 for a single system (most CTAs, shortest latency), 4 for batches
-// (every row-sum record is read once per 32 values of j instead of once per 8)
-template <int NTG>
+// warps split K = N_r; each lane loads one 32-byte row-sum record (all three streams at once), so one
+// k-step feeds three MMAs; the partial tiles are combined in warp order (deterministic).
+// (batched builds only: single-system builds contract in the point kernel's tail.)  4 warps and NTG = 4 n-tiles
+// (8 values of j each) per CTA: every row-sum record is read once per 32 values of j.
+constexpr int GEMM_WARPS = 4, NTG = 4;
 __global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
 {
     __shared__ double s_c[GEMM_WARPS][3][32][2];
@@ -118,7 +117,7 @@ __global__ void __launch_bounds__(GEMM_WARPS * 32) gemm_kernel(const KParams P)
     for (int nt = 0; nt < NTG; ++nt)
 #pragma unroll
         for (int st = 0; st < 3; ++st) c[nt][st][0] = c[nt][st][1] = 0.0;
-#pragma unroll(NTG == 1 ? 8 : 2)
+#pragma unroll 2
     for (int ks = ks0; ks < ks1; ++ks) {
         const int qa = ks * 4 + ak, qb = ks * 4 + bk;
         double4 a = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -210,10 +209,8 @@ __device__ __forceinline__ void reduce_part(const KParams &P, long long bi, int 
     Sa = a; Sb = b; Sv = v;
 }
 
-// FUSED (few systems, shared radial rule): the CTA also computes the z-independent rows it needs, H7, itself --
-// six rows (R_a, R_b, R_v at x_i; R_a, R_b at x_Z; R_v at x_G) fill one 8-row DMMA tile, the warps split (j-tile,
-// K = N_r); no separate gemm launch.  Not FUSED: the rows come from Rz (gemm_kernel / contract_split_kernel).
-template <bool FUSED>
+// The derivative rows' z-independent part comes from Rz (gemm_kernel / contract_split_kernel).  Used by the batched builds
+// and, with J == nullptr, by every residual-only build.
 __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, const double *__restrict__ bc,
                                                                double *__restrict__ J, double *__restrict__ F)
 {
@@ -277,53 +274,6 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
             s_part[pt][0][threadIdx.x] = a; s_part[pt][1][threadIdx.x] = bb; s_part[pt][2][threadIdx.x] = v;
         }
     }
-    __shared__ double s_R[FUSED ? 6 * 128 : 1];                   // [kp][6 rows][Npad], KP * Npad <= 128
-    int KP = 1;
-    if (FUSED) {
-        const int NT = P.Npad >> 3, nw = nthr >> 5;
-        KP = nw / NT > 1 ? nw / NT : 1;
-        const int ksteps = (P.Nr + 3) >> 2, per = (ksteps + KP - 1) / KP;
-        const int row = lane >> 2;                               // A fragment: row = lane/4, col (q) = lane%4
-        const long long bi_r = row < 3 ? bi_i : (row < 5 ? bi_Z : bi_G);
-        const int comp = row < 3 ? row : (row < 5 ? row - 3 : 2);
-        const double *Ar = P.Apart + (size_t)bi_r * P.Nr * 4 + comp, *Hr = P.AHead + (size_t)bi_r * P.Nr * 4 + comp;
-        for (int item = warp; item < NT * KP; item += nw) {
-            const int nt = item % NT, kp = item / NT;
-            const int ks0 = kp * per, ks1 = min(ksteps, ks0 + per);
-            const double *Bp = P.phi_y + 8 * nt + (lane >> 2);   // B fragment: row (q) = lane%4, col (j) = lane/4
-            double c[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};      // four chains hide the DMMA latency
-            const double amask = row < 6 ? 1.0 : 0.0;            // rows 6, 7 of the tile are padding
-            const double *Aq = row < 6 ? Ar : P.Apart, *Hq = row < 6 ? Hr : P.AHead;
-            const int ksf = min(ks1, P.Nr >> 2);                 // k-steps whose four q are all in range
-            int ks = ks0;
-            for (; ks + 8 <= ksf; ks += 8) {                     // 24 independent loads in flight, then 8 MMAs
-                double av[8], hv[8], bv[8];
-#pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const size_t q = (size_t)(4 * (ks + u) + (lane & 3));
-                    av[u] = __ldg(Aq + q * 4); hv[u] = __ldg(Hq + q * 4); bv[u] = __ldg(Bp + q * P.Npad);
-                }
-#pragma unroll
-                for (int u = 0; u < 8; ++u)
-                    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                        : "+d"(c[u & 3][0]), "+d"(c[u & 3][1]) : "d"((av[u] + hv[u]) * amask), "d"(bv[u]));
-            }
-            for (; ks < ks1; ++ks) {                             // ragged tail
-                const int q = 4 * ks + (lane & 3);
-                const bool ok = q < P.Nr;
-                const size_t qq = ok ? q : 0;
-                const double a = ok ? (__ldg(Aq + qq * 4) + __ldg(Hq + qq * 4)) * amask : 0.0;
-                const double bb = ok ? __ldg(Bp + qq * P.Npad) : 0.0;
-                asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                    : "+d"(c[ks & 3][0]), "+d"(c[ks & 3][1]) : "d"(a), "d"(bb));
-            }
-            if (row < 6) {                                       // C fragment: row = lane/4, cols 2 (lane%4), +1
-                double *o = s_R + (size_t)(kp * 6 + row) * P.Npad + 8 * nt + 2 * (lane & 3);
-                o[0] = (c[0][0] + c[1][0]) + (c[2][0] + c[3][0]);
-                o[1] = (c[0][1] + c[1][1]) + (c[2][1] + c[3][1]);
-            }
-        }
-    }
     __syncthreads();
     if (threadIdx.x == nthr - 1) {                               // F (one thread; the J threads are the first ones)
         double pi[3][2];
@@ -348,14 +298,7 @@ __global__ void __launch_bounds__(ASM_THREADS) assemble_kernel(const KParams P, 
             }
         if (npt == 2) { S[2][0] = S[1][0]; S[2][1] = S[1][1]; S[2][2] = S[1][2]; }
         double R[6];                                             // R_a, R_b, R_v at x_i; R_a, R_b at x_Z; R_v at x_G
-        if (FUSED) {
-#pragma unroll
-            for (int r = 0; r < 6; ++r) {
-                double t = 0.0;
-                for (int kp = 0; kp < KP; ++kp) t += s_R[(size_t)(kp * 6 + r) * P.Npad + j];
-                R[r] = t;
-            }
-        } else {
+        {
             const double *Ri = P.Rz + (size_t)bi_i * 3 * P.Npad, *RZ = P.Rz + (size_t)bi_Z * 3 * P.Npad,
                          *RG = P.Rz + (size_t)bi_G * 3 * P.Npad;
             R[0] = Ri[j]; R[1] = Ri[P.Npad + j]; R[2] = Ri[2 * P.Npad + j];
@@ -399,48 +342,17 @@ __global__ void fd_column_kernel(int n2, const double *__restrict__ c, const dou
         J[((size_t)b * n2 + i) * n2 + j] = (Fp[(size_t)b * n2 + i] - Fm[(size_t)b * n2 + i]) / h2;
 }
 
-// ---------------------------------------------------------------------------------------------
-// fp64 throughput probes (roofline denominators; see include/dse.h)
-__global__ void __launch_bounds__(256) dfma_probe_kernel(int iters, double *sink)
-{
-    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
-           a7 = a0 + 7;
-    const double m = 0.999999999, c = 1e-9;
-    for (int i = 0; i < iters; ++i) {
-        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-    }
-    sink[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
-}
-
-__global__ void __launch_bounds__(256) dmma_probe_kernel(int iters, double *sink)
-{
-    double c[4][2];
-    for (int m = 0; m < 4; ++m) { c[m][0] = threadIdx.x * 1e-9; c[m][1] = m; }
-    const double a = 1e-3 * (threadIdx.x & 7), b = 1e-3 * (threadIdx.x & 3);
-    for (int i = 0; i < iters; ++i) {
-#pragma unroll
-        for (int m = 0; m < 4; ++m)
-            asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                         : "+d"(c[m][0]), "+d"(c[m][1])
-                         : "d"(a), "d"(b));
-    }
-    double s = 0;
-    for (int m = 0; m < 4; ++m) s += c[m][0] + c[m][1];
-    sink[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = s;
-}
-
 thread_local char g_err[256] = "";
-inline int cuda_fail(cudaError_t e, const char *what)
-{
-    snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
-    return DSE_ECUDA;
-}
 
 }  // namespace
 
 const char *last_error_text() { return g_err; }
 void set_error_text(const char *s) { snprintf(g_err, sizeof(g_err), "%s", s); }
+int cuda_fail(int e, const char *what)
+{
+    snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString((cudaError_t)e));
+    return DSE_ECUDA;
+}
 
 int launch_geometry(const KParams &k, double *geom, void *stream)
 {
@@ -459,46 +371,44 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     cudaStream_t s = (cudaStream_t)stream;
     KParams kk = k;
     kk.want_jac = J_dev != nullptr;
+    kk.c = c_dev; kk.bc = bc_dev; kk.J = J_dev; kk.F = F_dev;
+    kk.tail = kk.want_jac && !cfg.batched;               // single-system kernels finish the build themselves
     int launches = 0;
-    prep_kernel<<<dim3((kk.Gext * kk.Nr + kk.N + 7) / 8, kk.B), 256, 0, s>>>(kk, c_dev);
-    ++launches;
-    if (ev0) cudaEventRecord((cudaEvent_t)ev0, s);
-    launch_point(kk, cfg, stream);
-    if (ev1) cudaEventRecord((cudaEvent_t)ev1, s);
-    ++launches;
-    // few systems, shared radial rule, small Phi table: H7 is fused into the assemble CTAs (one launch less on the
-    // latency path: -3 us per build at cfg 0/1); large tables keep the separate gemm (every fused CTA would stream
-    // the whole N_r x N table: +15 us at cfg 3)
-    static const bool no_fused = getenv("DSE_NO_FUSED_ASSEMBLE") != nullptr;     // A/B switch, read once
-    const bool fused = kk.want_jac && !kk.rstride && kk.B < 8 && (long long)kk.Nr * kk.Npad <= 16384 && !no_fused;
-    if (kk.want_jac && !fused) {
-        if (kk.rstride) {
-            launch_pdl(contract_split_kernel, dim3(kk.Next, kk.B), dim3(128), 0, s, kk);
-        } else if (kk.B >= 8) {
-            // many systems: 4 n-tiles per CTA and 4 warps, the grid fills the GPU and every row-sum record is read
-            // once per 32 values of j
-            dim3 gg((kk.Next + 7) / 8, (kk.Npad / 8 + 3) / 4, kk.B);
-            launch_pdl(gemm_kernel<4>, gg, dim3(4 * 32), 0, s, kk);
-        } else {
-            dim3 gg((kk.Next + 7) / 8, kk.Npad / 8, kk.B);        // one n-tile per CTA, K split over 16 warps (latency)
-            launch_pdl(gemm_kernel<1>, gg, dim3(GEMM_WARPS * 32), 0, s, kk);
-        }
+    cudaError_t e;
+    const bool one_kernel = kk.tail && cfg.pipelined;    // the pipelined kernel also does H1
+    if (!one_kernel) {
+        prep_kernel<<<dim3((kk.Gext * kk.Nr + kk.N + 7) / 8, kk.B), 256, 0, s>>>(kk, c_dev);
+        if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "prep_kernel launch");
         ++launches;
     }
-    dim3 ga(kk.N, kk.B);
-    if (fused)
-        launch_pdl(assemble_kernel<true>, ga, dim3(ASM_THREADS), 0, s, kk, bc_dev, J_dev, F_dev);
-    else    // many systems: few slots per external point, small CTAs keep more of them resident
-        launch_pdl(assemble_kernel<false>, ga, dim3(kk.B >= 8 ? 128 : ASM_THREADS), 0, s, kk, bc_dev, J_dev, F_dev);
+    if (ev0 && (e = cudaEventRecord((cudaEvent_t)ev0, s)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+    int rc = launch_point(kk, cfg, stream);
+    if (rc < 0) return rc;
+    launches += rc;
+    if (ev1 && (e = cudaEventRecord((cudaEvent_t)ev1, s)) != cudaSuccess) return cuda_fail(e, "cudaEventRecord");
+    if (kk.tail) return launches;
+    if (kk.want_jac) {                                   // batched build: H7 on the tensor path, or the split rule's batch
+        if (kk.rstride) {
+            e = launch_pdl(contract_split_kernel, dim3(kk.Next, kk.B), dim3(128), 0, s, kk);
+        } else {
+            dim3 gg((kk.Next + 7) / 8, (kk.Npad / 8 + NTG - 1) / NTG, kk.B);
+            e = launch_pdl(gemm_kernel, gg, dim3(GEMM_WARPS * 32), 0, s, kk);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "contraction launch");
+        ++launches;
+    }
+    // many systems: few slots per external point, small CTAs keep more of them resident
+    e = launch_pdl(assemble_kernel, dim3(kk.N, kk.B), dim3(kk.B >= 8 ? 128 : ASM_THREADS), 0, s, kk, bc_dev, J_dev, F_dev);
+    if (e != cudaSuccess) return cuda_fail(e, "assemble_kernel launch");
     ++launches;
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "build launch");
     return launches;
 }
 
 int launch_fd_perturb(int n2, int B, const double *c, double *c_tmp, int j, double sign, double eps_rel, void *stream)
 {
     fd_perturb_kernel<<<B, 128, 0, (cudaStream_t)stream>>>(n2, c, c_tmp, j, sign, eps_rel);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "fd launch");
     return 1;
 }
 int launch_fd_column(int n2, int B, const double *c, const double *Fp, const double *Fm, double *J, int j, double eps_rel,
@@ -507,21 +417,6 @@ int launch_fd_column(int n2, int B, const double *c, const double *Fp, const dou
     fd_column_kernel<<<B, 128, 0, (cudaStream_t)stream>>>(n2, c, Fp, Fm, J, j, eps_rel);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "fd launch");
-    return 1;
-}
-
-int launch_dfma_probe(int blocks, int iters, double *sink, void *stream)
-{
-    dfma_probe_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(iters, sink);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "dfma_probe launch");
-    return 1;
-}
-int launch_dmma_probe(int blocks, int iters, double *sink, void *stream)
-{
-    dmma_probe_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(iters, sink);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "dmma_probe launch");
     return 1;
 }
 

@@ -1,8 +1,8 @@
-// dse_point.cu -- the hot kernel (steps H2-H6 of DESIGN.md): every quadrature point (x_e, y_q, theta_k).
+// dse_point.cu -- the hot kernel (steps H2-H6 of DESIGN.md): every quadrature point (x_e, y_q, theta_k); for a Jacobian
+// build the same kernel also finishes the build (H7, H8: dse_tail.cuh), so that a build is ONE launch.
 //
-// Each WARP is an independent worker that owns a contiguous range of rows (b, e, q) of the flattened
-// (system, external point, radial node) index and walks the angular nodes of each row in batches of
-// 32 points:
+// Each WARP is an independent worker that owns a contiguous range of the flattened (system, external point, radial
+// node, angular batch) index and walks it in batches of 32 points:
 //   phase 1 (lane = point): geometry (or the cached 32 B), clamp + continuation eq.(16)-(19), the
 //     T_j recurrence shared by both series ln G(z), ln Z(z) (3 FMA per j; the recurrence runs as two
 //     independent stride-2 chains T_{j+2} = 2 T_2 T_j - T_{j-2} for instruction-level parallelism),
@@ -10,26 +10,30 @@
 //     (2s, u_a, u_b, v) and the chunk-start pairs (T_8c, T_8c+1) in warp-private shared memory;
 //   phase 2 (lane = (chunk c, point sub-lane)): restart the recurrence at j = 8c and accumulate the
 //     three z-dependent Jacobian streams Sa, Sb, Sv for 8 values of j in registers.
-// Accumulators are flushed as per-(warp, external point) partials; assemble_kernel sums them in a
-// fixed order.  No CTA-level synchronisation after the table load, no atomics.
-// Template: NCH_T = number of 8-wide Chebyshev chunks when it is a power of two (everything unrolls),
-// 0 = generic run-time shape; GEOM = read the geometry cache; JAC = accumulate the Jacobian streams.
+// Accumulators are flushed as per-(warp, external point) partials and summed in a fixed order.  No CTA-level
+// synchronisation between the table load and the tail, no data atomics.
+//   point_kernel       any shape (run-time chunk count, angular batches narrower than a warp), residual-only builds;
+//                      coefficients, G(y_q), P(y_q) from prep_kernel
+//   point_kernel_pipe  full-warp angular batches, compile-time chunk count: phase 1 of batch t and phase 2 of batch
+//                      t-1 in one straight-line block (software pipelining); computes G(y_q), P(y_q) itself (H1)
 #include <cstdio>
 #include <atomic>
-#include <cstdlib>
 
-#include "dse_device.cuh"
+#include "dse_tail.cuh"
 
 namespace dse {
 
-void set_error_text(const char *s);
-
 namespace {
 
-__constant__ double2 c_coef[DSE_MAX_NCHEB];     // coefficient pairs of a single-system build (constant-bank operands)
+// DSE_FLAG_CONST_COEF: a_j, b_j of a single-system build as constant-bank operands of the series FMAs.  Filled by two
+// in-stream device-to-device copies of the caller's c (cudaMemcpyToSymbolAsync) before the point kernel is launched.
+__constant__ double c_coefA[DSE_MAX_NCHEB], c_coefB[DSE_MAX_NCHEB];
 
-template <int NCH_T, bool GEOM, bool JAC, int NP, bool CONSTC = false>
-__global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P)
+// Template: NCH_T = number of 8-wide Chebyshev chunks when it is a power of two (everything unrolls),
+// 0 = generic run-time shape; GEOM = read the geometry cache; JAC = accumulate the Jacobian streams and (P.tail)
+// finish the build in the kernel's tail; JAC = false: residual only, finished by assemble_kernel.
+template <int NCH_T, bool GEOM, bool JAC>
+__global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_constant__ KParams P)
 {
     constexpr bool CT = NCH_T > 0;
     extern __shared__ __align__(16) double smem[];
@@ -39,13 +43,12 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
     const int ROUNDS = CT ? NCH_T : P.rounds;
     const int Npad = NCH * CJ;
     double *s_ang = smem;
-    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(Npad, NCH, NP);
+    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(Npad, NCH);
     double2 *s_coef = reinterpret_cast<double2 *>(wbase);
-    const int STASH = stash_doubles(NCH);                                 // per interleaved point set
     double4 *s_pt = reinterpret_cast<double4 *>(wbase + 2 * Npad);       // 33 entries, entry 32 = 0
     double *s_T = wbase + 2 * Npad + 132;
     double2 *s_T2 = reinterpret_cast<double2 *>(s_T);
-    double4 *s_gbuf = reinterpret_cast<double4 *>(wbase + 2 * Npad + NP * STASH);   // [2][32] geometry records
+    double4 *s_gbuf = reinterpret_cast<double4 *>(wbase + 2 * Npad + stash_doubles(NCH));   // [2][32] geometry records
 
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
     if (lane == 0) s_pt[32] = make_double4(0.0, 0.0, 0.0, 0.0);
@@ -61,7 +64,6 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
     const int rib = lane / g, kl = lane - rib * g;          // row-in-batch and angular lane
     const double halfLg = 0.5 * P.Lg;
     const double2 *tread = s_T2 + (active2 ? c_lane : 0) * (TCH_STRIDE / 2);
-    static_assert(NP == 1 || NCH_T > 0, "two-point interleave needs a compile-time chunk count");
 
     double accA[CJ], accB[CJ], accV[CJ];
 #pragma unroll
@@ -90,7 +92,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
     // Geometry cache, full-warp angular batches: the warp's batches are consecutive 1 KB records of one linear
     // stream (wrapping at a system boundary), so the next batch is prefetched with cp.async into a warp-private
     // double buffer while the current one is processed -- no registers held across the batch.
-    const bool PREF = GEOM && NP == 1 && g == 32;
+    const bool PREF = GEOM && g == 32;
     const size_t gtotal = (size_t)P.Next * Nr * P.Ntpad;
     const double4 *gbase = reinterpret_cast<const double4 *>(P.geom), *gend = gbase + gtotal, *gnext = gbase;
     unsigned gphase = 0;
@@ -106,10 +108,6 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
         prefetch(0);
     }
 
-#ifdef DSE_PHASE_TIMING
-    long long dbg_t[4] = {0, 0, 0, 0};
-    const long long dbg_start = clock64();
-#endif
     // (bi, q0, b, e) are advanced incrementally: no 64-bit divisions inside the row loop
     long long r = r0;
     long long bi = r0 / Nr;
@@ -152,81 +150,55 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
         const double4 *grow = GEOM ? reinterpret_cast<const double4 *>(P.geom) + ((size_t)e * Nr + q) * P.Ntpad + kl
                                    : nullptr;
 
-        for (int kb = 0; kb < P.Ntpad; kb += 32 * NP) {
-#ifdef DSE_PHASE_TIMING
-            const long long tk0 = clock64();
-#endif
-            // ---------------- phase 1: lane = point; NP points per lane are interleaved for ILP ----------------
-            // (k = kb + 32 p + kl < Ntpad: g divides Ntpad, g <= 32; NP = 2 only when 64 divides Ntpad)
-            double gv[NP], gq[NP], gm[NP], EG[NP], EZ[NP], ts[NP], t2[NP], Te[NP], To[NP], Tem[NP], Tom[NP];
-            double lz0[NP], lz1[NP], lg0[NP], lg1[NP];
-#pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                double sraw;
-                if (GEOM && PREF) {
-                    gnext += 32;                                   // next batch of this warp (possibly of the next row)
-                    if (gnext >= gend) gnext -= gtotal;
-                    prefetch(gphase ^ 1);
-                    asm volatile("cp.async.wait_group 1;\n" ::: "memory");     // the current batch has landed
-                    const double2 *gp = reinterpret_cast<const double2 *>(s_gbuf + gphase * 32 + lane);
-                    const double2 g0 = gp[0], g1 = gp[1];
-                    sraw = g0.x; gv[p] = g0.y; gq[p] = g1.x; gm[p] = g1.y;
-                    gphase ^= 1;
-                } else if (GEOM) {
-                    const double2 *gp = reinterpret_cast<const double2 *>(grow + kb + 32 * p);   // streamed once
-                    const double2 g0 = __ldcs(gp), g1 = __ldcs(gp + 1);
-                    sraw = g0.x; gv[p] = g0.y; gq[p] = g1.x; gm[p] = g1.y;
-                } else {
-                    point_geometry(rc, s_ang + (kb + 32 * p + kl) * 6, P.inv_eps2, P.two_over_Lg, sraw, gv[p], gq[p], gm[p]);
-                }
-                double s = sraw;
-                EG[p] = 0.0; EZ[p] = 0.0;
-                if (sraw < -1.0) {                       // z < eps2: G ~ z^pG, Z ~ z^pZ   eq.(16),(17)
-                    const double ell = (sraw + 1.0) * halfLg;
-                    EG[p] = P.pG * ell; EZ[p] = P.pZ * ell; s = -1.0;
-                } else if (sraw > 1.0) {                 // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
-                    const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
-                    EG[p] = P.delta * t; EZ[p] = P.gamma * t; s = 1.0;
-                }
-                ts[p] = 2.0 * s;
-                t2[p] = fma(2.0 * ts[p], s, -2.0);       // 2 T_2(s): stride-2 recurrence T_{j+2} = 2 T_2 T_j - T_{j-2}
-                Te[p] = 1.0; To[p] = s;                  // T_0, T_1
-                Tem[p] = fma(ts[p], s, -1.0); Tom[p] = s;   // T_{-2} = T_2, T_{-1} = T_1
-                lz0[p] = lz1[p] = lg0[p] = lg1[p] = 0.0;
+        for (int kb = 0; kb < P.Ntpad; kb += 32) {
+            // ---------------- phase 1: lane = point (k = kb + kl < Ntpad: g divides Ntpad, g <= 32) ----------------
+            double gv, gqv, gm, sraw;
+            if (GEOM && PREF) {
+                gnext += 32;                                   // next batch of this warp (possibly of the next row)
+                if (gnext >= gend) gnext -= gtotal;
+                prefetch(gphase ^ 1);
+                asm volatile("cp.async.wait_group 1;\n" ::: "memory");     // the current batch has landed
+                const double2 *gp = reinterpret_cast<const double2 *>(s_gbuf + gphase * 32 + lane);
+                const double2 g0 = gp[0], g1 = gp[1];
+                sraw = g0.x; gv = g0.y; gqv = g1.x; gm = g1.y;
+                gphase ^= 1;
+            } else if (GEOM) {
+                const double2 *gp = reinterpret_cast<const double2 *>(grow + kb);   // streamed once
+                const double2 g0 = __ldcs(gp), g1 = __ldcs(gp + 1);
+                sraw = g0.x; gv = g0.y; gqv = g1.x; gm = g1.y;
+            } else {
+                point_geometry(rc, s_ang + (kb + kl) * 6, P.inv_eps2, P.two_over_Lg, sraw, gv, gqv, gm);
             }
-#ifdef DSE_PHASE_TIMING
-            const long long tk1 = clock64();
-#endif
+            double s = sraw, EG = 0.0, EZ = 0.0;
+            if (sraw < -1.0) {                       // z < eps2: G ~ z^pG, Z ~ z^pZ   eq.(16),(17)
+                const double ell = (sraw + 1.0) * halfLg;
+                EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
+            } else if (sraw > 1.0) {                 // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
+                const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
+            }
+            const double ts = 2.0 * s;
+            const double t2 = fma(2.0 * ts, s, -2.0);       // 2 T_2(s): stride-2 recurrence T_{j+2} = 2 T_2 T_j - T_{j-2}
+            double Te = 1.0, To = s;                        // T_0, T_1
+            double Tem = fma(ts, s, -1.0), Tom = s;         // T_{-2} = T_2, T_{-1} = T_1
+            double lz0 = 0.0, lz1 = 0.0, lg0 = 0.0, lg1 = 0.0;
 #pragma unroll
             for (int c = 0; c < NCH; ++c) {
-                if (JAC) {
-#pragma unroll
-                    for (int p = 0; p < NP; ++p)
-                        reinterpret_cast<double2 *>(s_T + p * STASH)[c * (TCH_STRIDE / 2) + lane] = make_double2(Te[p], To[p]);
-                }
+                if (JAC) s_T2[c * (TCH_STRIDE / 2) + lane] = make_double2(Te, To);
 #pragma unroll
                 for (int m = 0; m < CJ; m += 4) {
-                    const double2 c0 = CONSTC ? c_coef[c * CJ + m] : s_coef[c * CJ + m];
-                    const double2 c1 = CONSTC ? c_coef[c * CJ + m + 1] : s_coef[c * CJ + m + 1];
-                    const double2 c2 = CONSTC ? c_coef[c * CJ + m + 2] : s_coef[c * CJ + m + 2];
-                    const double2 c3 = CONSTC ? c_coef[c * CJ + m + 3] : s_coef[c * CJ + m + 3];
-#pragma unroll
-                    for (int p = 0; p < NP; ++p) {
-                        lz0[p] = fma(c0.x, Te[p], lz0[p]); lg0[p] = fma(c0.y, Te[p], lg0[p]);
-                        lz1[p] = fma(c1.x, To[p], lz1[p]); lg1[p] = fma(c1.y, To[p], lg1[p]);
-                        Tem[p] = fma(t2[p], Te[p], -Tem[p]);  Tom[p] = fma(t2[p], To[p], -Tom[p]);   // T_{j+2}, T_{j+3}
-                        lz0[p] = fma(c2.x, Tem[p], lz0[p]); lg0[p] = fma(c2.y, Tem[p], lg0[p]);
-                        lz1[p] = fma(c3.x, Tom[p], lz1[p]); lg1[p] = fma(c3.y, Tom[p], lg1[p]);
-                        Te[p] = fma(t2[p], Tem[p], -Te[p]);   To[p] = fma(t2[p], Tom[p], -To[p]);    // T_{j+4}, T_{j+5}
-                    }
+                    const double2 c0 = s_coef[c * CJ + m], c1 = s_coef[c * CJ + m + 1];
+                    const double2 c2 = s_coef[c * CJ + m + 2], c3 = s_coef[c * CJ + m + 3];
+                    lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0);
+                    lz1 = fma(c1.x, To, lz1); lg1 = fma(c1.y, To, lg1);
+                    Tem = fma(t2, Te, -Tem);  Tom = fma(t2, To, -Tom);   // T_{j+2}, T_{j+3}
+                    lz0 = fma(c2.x, Tem, lz0); lg0 = fma(c2.y, Tem, lg0);
+                    lz1 = fma(c3.x, Tom, lz1); lg1 = fma(c3.y, Tom, lg1);
+                    Te = fma(t2, Tem, -Te);   To = fma(t2, Tom, -To);    // T_{j+4}, T_{j+5}
                 }
             }
-#ifdef DSE_PHASE_TIMING
-            const long long tk2 = clock64();
-#endif
-#pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                const double lnZz = (lz0[p] + lz1[p]) + EZ[p], lnGz = (lg0[p] + lg1[p]) + EG[p];
+            {
+                const double lnZz = (lz0 + lz1) + EZ, lnGz = (lg0 + lg1) + EG;
                 const double lnPz = fma(P.e1, lnGz, P.e2 * lnZz);
                 double Zz, Gz, Pz;
                 // |x| <= 700 for all three, tested on the high words (0x4085e000 = high word of 700.0; NaN/Inf fail)
@@ -237,51 +209,37 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
                 } else {                                   // out of the fast range (or NaN): library exp
                     Zz = exp(lnZz); Gz = exp(lnGz); Pz = exp(lnPz);
                 }
-                const double v = gv[p] * (Gy * Zz);           // eq.(8):  -C W y Om sin^4/z^2 G(y) Z(z)
-                const double wQ = gq[p] * (Py * Pz);          // eq.(9):  (C/3x) W Om sin^2 Q P(y) P(z)
-                const double wM = gm[p] * (Gy * Gz);          // eq.(9):  (C/3x) W Om sin^2 M G(y) G(z)
+                const double v = gv * (Gy * Zz);              // eq.(8):  -C W y Om sin^4/z^2 G(y) Z(z)
+                const double wQ = gqv * (Py * Pz);            // eq.(9):  (C/3x) W Om sin^2 Q P(y) P(z)
+                const double wM = gm * (Gy * Gz);             // eq.(9):  (C/3x) W Om sin^2 M G(y) G(z)
                 const double ua = P.e2 * wQ;                  // weight of d/da_j  (P ~ Z^{e2})
                 const double ub = fma(P.e1, wQ, wM);          // weight of d/db_j  (P ~ G^{e1}; G(y)G(z))
                 sumA += ua; sumB += ub; sumV += v; sumZ += wQ + wM;
-                if (JAC) reinterpret_cast<double4 *>(reinterpret_cast<double *>(s_pt) + p * STASH)[lane] = make_double4(ts[p], ua, ub, v);
+                if (JAC) s_pt[lane] = make_double4(ts, ua, ub, v);
             }
-#ifdef DSE_PHASE_TIMING
-            const long long tk3 = clock64();
-#endif
             if (JAC) {
                 __syncwarp();
                 // ---------------- phase 2: lane = (chunk, point sub-lane) ----------------
 #pragma unroll
-                for (int p = 0; p < NP; ++p) {
-                    const double4 *pts = reinterpret_cast<const double4 *>(reinterpret_cast<const double *>(s_pt) + p * STASH);
-                    const double2 *trd = reinterpret_cast<const double2 *>(reinterpret_cast<const double *>(tread) + p * STASH);
+                for (int rd = 0; rd < ROUNDS; ++rd) {
+                    const int pt = rd * SUB + sub;
+                    const int pc = CT ? pt : ((active2 && pt < 32) ? pt : 32);     // slot 32 holds zero weights
+                    const double4 pw = s_pt[pc];
+                    const double2 tt = tread[pc & 31];
+                    double T0 = tt.x, T1 = tt.y;
+                    accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
+                    accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
 #pragma unroll
-                    for (int rd = 0; rd < ROUNDS; ++rd) {
-                        const int pt = rd * SUB + sub;
-                        const int pc = CT ? pt : ((active2 && pt < 32) ? pt : 32);     // slot 32 holds zero weights
-                        const double4 pw = pts[pc];
-                        const double2 tt = trd[pc & 31];
-                        double T0 = tt.x, T1 = tt.y;
-                        accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
-                        accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
-#pragma unroll
-                        for (int m = 2; m < CJ; ++m) {
-                            const double T2 = fma(pw.x, T1, -T0);
-                            accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
-                            T0 = T1; T1 = T2;
-                        }
+                    for (int m = 2; m < CJ; ++m) {
+                        const double T2 = fma(pw.x, T1, -T0);
+                        accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
+                        T0 = T1; T1 = T2;
                     }
                 }
                 __syncwarp();
             } else {
                 asm volatile("" ::: "memory");      // keep the coefficient loads inside the loop (no hoisting -> no spills)
             }
-#ifdef DSE_PHASE_TIMING
-            {
-                const long long tk4 = clock64();
-                dbg_t[0] += tk1 - tk0; dbg_t[1] += tk2 - tk1; dbg_t[2] += tk3 - tk2; dbg_t[3] += tk4 - tk3;
-            }
-#endif
         }
         // H5/H7: row sums over the angular nodes (fixed xor tree), one writer per row
         for (int o = g >> 1; o > 0; o >>= 1) {
@@ -310,12 +268,11 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
         }
     }
     if (JAC && !fresh) flush(bi);
-#ifdef DSE_PHASE_TIMING
-    if (lane == 0 && P.dbg) {
-        for (int i = 0; i < 4; ++i) P.dbg[w * 5 + i] = (double)dbg_t[i];
-        P.dbg[w * 5 + 4] = (double)(clock64() - dbg_start);
+    if (PREF) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+    if (JAC && P.tail) {                                 // H7 + H8 by the last-arriving CTAs (uniform over the grid)
+        const long long T0 = ((long long)blockIdx.x * WPB * R) / P.W, T1 = ((long long)(blockIdx.x + 1) * WPB * R) / P.W;
+        build_tail(P, smem, dynamic_smem_doubles(), T0, T1);
     }
-#endif
 }
 
 
@@ -325,20 +282,20 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const KParams P
 // in the SAME straight-line block as phase 2 of batch t-1 (accumulation -- independent FMAs), reading and
 // writing the two halves of a double-buffered stash, so the scheduler hides the chains behind the FMAs.
 // One pipeline per (warp, external point) segment: prologue = zeroed weights, epilogue = phase 2 only.
-#ifndef DSE_PIPE_THREADS
-#define DSE_PIPE_THREADS 384
-#endif
-constexpr int PIPE_THREADS = DSE_PIPE_THREADS;
+// The kernel is a whole build: H1 (the series at the radial nodes, G(y_q) and P(y_q), for windows of 32 rows at a
+// time: lane = row) in front, H7 + H8 (dse_tail.cuh) behind.
+constexpr int PIPE_THREADS = 384;
+constexpr int GP_DOUBLES = 64;                // G(y), P(y) of a window of 32 rows
 
 __host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc, bool geom)
 {
-    return (constc ? 0 : 2 * Npad) + 2 * stash_doubles(NCH) + (geom ? GBUF_DOUBLES : 0);
+    return (constc ? 0 : 2 * Npad) + 2 * stash_doubles(NCH) + (geom ? GBUF_DOUBLES : 0) + GP_DOUBLES;
 }
 
 // THR: threads per CTA the register budget is compiled for (384: ~160 registers; 512: 128 registers, 16 warps per SM --
 // 2 % faster on large problems, slower on small ones)
 template <int NCH_T, bool GEOM, bool CONSTC, int THR = PIPE_THREADS>
-__global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
+__global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constant__ KParams P)
 {
     // lanes = (chunk of 8 j, point sub-lane); chunk counts that do not divide 32 leave 32 - NCH * SUB lanes idle in
     // phase 2 and read the zero-weight stash slot 32 for the points past the batch
@@ -347,32 +304,25 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
     const int STASH = stash_doubles(NCH);
+    const int WD = pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
     double *s_ang = smem;
-    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
+    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * WD;
     double2 *s_coef = reinterpret_cast<double2 *>(wbase);
     double *s_stash = wbase + (CONSTC ? 0 : 2 * Npad);                       // [2][STASH]: pt (33 x 4) then T
-    double4 *s_gbuf = reinterpret_cast<double4 *>(s_stash + 2 * STASH);     // [2][32] geometry records
+    double2 *s_gp = reinterpret_cast<double2 *>(s_stash + 2 * STASH);       // [32] (G(y), P(y)) of a window of rows
+    double4 *s_gbuf = reinterpret_cast<double4 *>(s_stash + 2 * STASH + GP_DOUBLES);     // [2][32] geometry records
 
-#ifdef DSE_PHASE_TIMING
-    // diagnostics (dse_get_phase_cycles): cycles from kernel entry to (tables staged + producer done), of the first batch,
-    // of the remaining batches, of the flushes; [4] = whole warp
-    const long long dbg_start = clock64();
-    long long dbg_first = 0, dbg_flush = 0;
-#endif
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
-    pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q)
+    pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
     __syncthreads();
-#ifdef DSE_PHASE_TIMING
-    const long long dbg_ready = clock64();
-#endif
 
     const int Nr = P.Nr, BPR = P.Ntpad >> 5;                                 // batches per row
     // work is partitioned in 32-point batches (P.U = rows * BPR): balanced to +-1 batch over all warps; a row whose
     // batches span two warps gets its head partial in AHead and its tail partial in Apart
     const long long w = (long long)blockIdx.x * WPB + warp;
     const long long t0 = (w * P.U) / P.W, t1 = ((w + 1) * P.U) / P.W;
-    if (t0 >= t1) return;
-    const long long r0 = t0 / BPR;
+    if (t0 < t1) {
+    const long long r0 = t0 / BPR, r_end = (t1 - 1) / BPR + 1;              // rows [r0, r_end) are touched by this warp
     int kb = (int)(t0 - r0 * BPR);
     const bool lane_on = EXACT || lane < NCH * SUB;
     const int c_lane = lane_on ? lane / SUB : 0, sub = lane_on ? lane - c_lane * SUB : 0;
@@ -449,6 +399,40 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
         }
     };
 
+    // H1 for a window of 32 consecutive rows starting at row rb: lane = row; ln G(y), ln Z(y) by the series eq.(23),(24)
+    // on the table phi_j(t_q) (phi_0 = 1/2 is in the table), power-law add-ons of the infrared piece, then
+    // G(y) = exp(ln G), P(y) = G^{e1} Z^{e2} (eq.(3),(9))
+    long long gp_base = r0;
+    auto fill_gp = [&](long long rb) {
+        const long long rr = rb + lane;
+        double Gv = 0.0, Pv = 0.0;
+        if (rr < r_end) {
+            const long long bir = rr / Nr;
+            const int qr = (int)(rr - bir * Nr), br = (int)(bir / P.Next), er = (int)(bir - (long long)br * P.Next);
+            const size_t gi = (size_t)(P.rstride ? er * P.rstride : 0) + qr;
+            const double2 *ph = reinterpret_cast<const double2 *>(P.phi_y + gi * Npad);
+            const double *ca = P.c + (size_t)br * 2 * P.N, *cb = ca + P.N;
+            double lnZ = 0.0, lnG = 0.0, lnZ1 = 0.0, lnG1 = 0.0;
+#pragma unroll 4
+            for (int j = 0; j + 1 < P.N; j += 2) {
+                const double2 f = __ldg(ph + (j >> 1));
+                lnZ = fma(__ldg(ca + j), f.x, lnZ);       lnG = fma(__ldg(cb + j), f.x, lnG);
+                lnZ1 = fma(__ldg(ca + j + 1), f.y, lnZ1); lnG1 = fma(__ldg(cb + j + 1), f.y, lnG1);
+            }
+            if (P.N & 1) {
+                const double f = __ldg(P.phi_y + gi * Npad + P.N - 1);
+                lnZ = fma(__ldg(ca + P.N - 1), f, lnZ); lnG = fma(__ldg(cb + P.N - 1), f, lnG);
+            }
+            lnZ = (lnZ + lnZ1) + __ldg(P.EZy + gi); lnG = (lnG + lnG1) + __ldg(P.EGy + gi);
+            Gv = exp(lnG);
+            Pv = exp(P.e1 * lnG + P.e2 * lnZ);
+        }
+        __syncwarp();
+        s_gp[lane] = make_double2(Gv, Pv);
+        __syncwarp();
+        gp_base = rb;
+    };
+
     // geometry stream (GEOM): consecutive 1 KB records, cp.async double buffer
     // (32-bit record index: at most 2^31 points per system; checked in dse_create)
     const unsigned gtotal = (unsigned)P.Next * (unsigned)Nr * (unsigned)P.Ntpad;
@@ -461,6 +445,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
         asm volatile("cp.async.commit_group;\n" ::);
     };
 
+    long long row = r0;                                    // running row index of the flattened (b, e, q)
     int bi = (int)(r0 / Nr);
     int q = (int)(r0 - (long long)bi * Nr);
     int cur_b = bi / P.Next;
@@ -469,10 +454,13 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
         gidx = ((unsigned)e * Nr + q) * P.Ntpad + kb * 32 + lane;
         prefetch(0);
     }
-    if (!CONSTC) {
-        for (int j = lane; j < Npad; j += 32) s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
+    auto load_coef = [&](int b) {                          // (a_j, b_j) pairs of system b, zero padded
+        const double *ca = P.c + (size_t)b * 2 * P.N;
+        for (int j = lane; j < Npad; j += 32) s_coef[j] = j < P.N ? make_double2(__ldg(ca + j), __ldg(ca + P.N + j)) : make_double2(0.0, 0.0);
         __syncwarp();
-    }
+    };
+    if (!CONSTC) load_coef(cur_b);
+    fill_gp(r0);
 
     // both T stashes must hold finite numbers before the first (zero-weight) prologue phase 2
     for (int b2 = 0; b2 < 2; ++b2)
@@ -493,8 +481,9 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
         __syncwarp();
         bool seg_done = false;
         while (!seg_done) {
-            const size_t gq = ((size_t)cur_b * P.Gext + (P.rstride ? e : 0)) * Nr + q;
-            const double Gy = P.Gy[gq], Py = P.Py[gq];
+            if (row - gp_base >= 32) fill_gp(row);          // (warp-uniform)
+            const double2 gp = s_gp[(int)(row - gp_base)];
+            const double Gy = gp.x, Py = gp.y;
             RowConst rc;
             if (!GEOM) {
                 const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
@@ -514,8 +503,8 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
                     if (gidx >= gtotal) gidx -= gtotal;
                     prefetch(gphase ^ 1);
                     asm volatile("cp.async.wait_group 1;\n" ::: "memory");
-                    const double2 *gp = reinterpret_cast<const double2 *>(s_gbuf + gphase * 32 + lane);
-                    const double2 g0 = gp[0], g1 = gp[1];
+                    const double2 *gpp = reinterpret_cast<const double2 *>(s_gbuf + gphase * 32 + lane);
+                    const double2 g0 = gpp[0], g1 = gpp[1];
                     sraw = g0.x; gv = g0.y; gq = g1.x; gm = g1.y;
                     gphase ^= 1;
                 } else {
@@ -540,11 +529,13 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
                     tw[c * (TCH_STRIDE / 2) + lane] = make_double2(Te, To);
 #pragma unroll
                     for (int m = 0; m < CJ; m += 4) {
-                        const double2 c0 = CONSTC ? c_coef[c * CJ + m] : s_coef[c * CJ + m];
-                        const double2 c1 = CONSTC ? c_coef[c * CJ + m + 1] : s_coef[c * CJ + m + 1];
-                        const double2 c2 = CONSTC ? c_coef[c * CJ + m + 2] : s_coef[c * CJ + m + 2];
-                        const double2 c3 = CONSTC ? c_coef[c * CJ + m + 3] : s_coef[c * CJ + m + 3];
-                        lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0);
+                        const int j0 = c * CJ + m;
+                        const double2 c0 = CONSTC ? make_double2(c_coefA[j0], c_coefB[j0]) : s_coef[j0];
+                        const double2 c1 = CONSTC ? make_double2(c_coefA[j0 + 1], c_coefB[j0 + 1]) : s_coef[j0 + 1];
+                        const double2 c2 = CONSTC ? make_double2(c_coefA[j0 + 2], c_coefB[j0 + 2]) : s_coef[j0 + 2];
+                        const double2 c3 = CONSTC ? make_double2(c_coefA[j0 + 3], c_coefB[j0 + 3]) : s_coef[j0 + 3];
+                        if (j0 == 0) { lz0 = 0.5 * c0.x; lg0 = 0.5 * c0.y; }      // phi_0 = 1/2: the c_0/2 of eq.(23),(24)
+                        else { lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0); }
                         lz1 = fma(c1.x, To, lz1); lg1 = fma(c1.y, To, lg1);
                         Tem = fma(t2, Te, -Tem);  Tom = fma(t2, To, -Tom);
                         lz0 = fma(c2.x, Tem, lz0); lg0 = fma(c2.y, Tem, lg0);
@@ -569,9 +560,6 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
                 reinterpret_cast<double4 *>(s_stash + cur * STASH)[lane] = make_double4(ts, ua, ub, v);
                 __syncwarp();
                 cur ^= 1;
-#ifdef DSE_PHASE_TIMING
-                if (dbg_first == 0) dbg_first = clock64();
-#endif
             }
             // H5/H7: row sums over the 32 angular lanes.  Transposing reduction: after the first two steps each
             // quarter-warp carries one of the four sums (6 shuffles instead of 20; fixed order -> deterministic).
@@ -594,116 +582,66 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const KParams P)
                     *dst = z;
                     if (has_first && has_last) P.AHead[((size_t)bi * Nr + q) * 4 + (lane >> 3)] = 0.0;
                 }
-                if (has_last) { kb = 0; ++q; if (q == Nr) seg_done = true; }
+                if (has_last) { kb = 0; ++q; ++row; if (q == Nr) seg_done = true; }
                 if (rem <= 0) seg_done = true;
             }
         }
         // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
-#ifdef DSE_PHASE_TIMING
-        const long long dbg_f0 = clock64();
-#endif
         phase2(cur ^ 1);
         flush(bi, cur);
-#ifdef DSE_PHASE_TIMING
-        dbg_flush += clock64() - dbg_f0;
-#endif
         if (q >= Nr) {
             q = 0; ++bi; ++e;
             if (e == P.Next) {
                 e = 0; ++cur_b;
-                if (!CONSTC && rem > 0) {
-                    for (int j = lane; j < Npad; j += 32)
-                        s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
-                    __syncwarp();
-                }
+                if (!CONSTC && rem > 0) { __syncwarp(); load_coef(cur_b); }
             }
         }
     }
     if (GEOM) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
-#ifdef DSE_PHASE_TIMING
-    if (lane == 0 && P.dbg) {
-        const long long dbg_end = clock64();
-        P.dbg[w * 5 + 0] = (double)(dbg_ready - dbg_start);
-        P.dbg[w * 5 + 1] = (double)(dbg_first - dbg_ready);
-        P.dbg[w * 5 + 2] = (double)(dbg_end - dbg_first - dbg_flush);
-        P.dbg[w * 5 + 3] = (double)dbg_flush;
-        P.dbg[w * 5 + 4] = (double)(dbg_end - dbg_start);
-    }
-#endif
+    }   // t0 < t1
+    // H7 + H8 by the last-arriving CTAs (dse_tail.cuh)
+    const long long T0 = ((long long)blockIdx.x * WPB * P.U) / P.W, T1 = ((long long)(blockIdx.x + 1) * WPB * P.U) / P.W;
+    build_tail(P, smem, dynamic_smem_doubles(), T0, T1);
 }
 using KernelFn = void (*)(const KParams);
 
-inline int np_of(const KParams &k)      // two interleaved points per lane when the shapes allow it
+template <bool GEOM, bool JAC>
+KernelFn pick_nch(int nch)
 {
-    const bool pow2 = k.NCH == 1 || k.NCH == 2 || k.NCH == 4 || k.NCH == 8;
-    const char *env = getenv("DSE_NP");
-    const int want = env ? atoi(env) : 1;
-    return (want == 2 && pow2 && k.Ntpad % 64 == 0 && !k.use_constc) ? 2 : 1;
-}
-
-template <bool GEOM, bool JAC, bool CONSTC = false>
-KernelFn pick_nch(int nch, int np)
-{
-    if (np == 2 && !CONSTC) {
-        switch (nch) {
-            case 1: return point_kernel<1, GEOM, JAC, 2>;
-            case 2: return point_kernel<2, GEOM, JAC, 2>;
-            case 4: return point_kernel<4, GEOM, JAC, 2>;
-            default: return point_kernel<8, GEOM, JAC, 2>;
-        }
-    }
     switch (nch) {
-        case 1: return point_kernel<1, GEOM, JAC, 1, CONSTC>;
-        case 2: return point_kernel<2, GEOM, JAC, 1, CONSTC>;
-        case 4: return point_kernel<4, GEOM, JAC, 1, CONSTC>;
-        case 8: return point_kernel<8, GEOM, JAC, 1, CONSTC>;
-        case 16: return point_kernel<16, GEOM, JAC, 1, CONSTC>;
-        default: return point_kernel<0, GEOM, JAC, 1>;       // generic shapes: shared-memory coefficients
+        case 1: return point_kernel<1, GEOM, JAC>;
+        case 2: return point_kernel<2, GEOM, JAC>;
+        case 4: return point_kernel<4, GEOM, JAC>;
+        case 8: return point_kernel<8, GEOM, JAC>;
+        case 16: return point_kernel<16, GEOM, JAC>;
+        default: return point_kernel<0, GEOM, JAC>;       // run-time chunk count
     }
 }
-
-inline bool constc_of(const KParams &k) { return k.use_constc != 0; }
 
 KernelFn pick(const KParams &k, bool jac)
 {
-    const int np = np_of(k);
-    if (constc_of(k)) {
-        if (jac) return k.geom ? pick_nch<true, true, true>(k.NCH, 1) : pick_nch<false, true, true>(k.NCH, 1);
-        return k.geom ? pick_nch<true, false, true>(k.NCH, 1) : pick_nch<false, false, true>(k.NCH, 1);
-    }
-    if (!jac) return k.geom ? pick_nch<true, false>(k.NCH, np) : pick_nch<false, false>(k.NCH, np);
-    return k.geom ? pick_nch<true, true>(k.NCH, np) : pick_nch<false, true>(k.NCH, np);
+    if (!jac) return k.geom ? pick_nch<true, false>(k.NCH) : pick_nch<false, false>(k.NCH);
+    return k.geom ? pick_nch<true, true>(k.NCH) : pick_nch<false, true>(k.NCH);
 }
 
-int fail(cudaError_t e, const char *what)
-{
-    char buf[256];
-    snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
-    set_error_text(buf);
-    return DSE_ECUDA;
-}
+int fail(cudaError_t e, const char *what) { return cuda_fail((int)e, what); }
 
 }  // namespace
 
-// The constant-bank coefficient slot is a per-module resource: at most one handle owns it at a time
-// (first come, released in dse_destroy); other handles keep their coefficients in shared memory.
+// DSE_FLAG_CONST_COEF: the __constant__ coefficient arrays are one slot per loaded library; a handle holds it from
+// dse_create to dse_destroy, and only if its caller asked for it.
 static std::atomic<int> g_const_owner{0};
-bool acquire_const_slot(const KParams &k)
+bool constc_shape_ok(const KParams &k)
 {
     const bool pow2 = k.NCH == 1 || k.NCH == 2 || k.NCH == 4 || k.NCH == 8 || k.NCH == 16;
-    if (k.B != 1 || !pow2) return false;
+    return k.B == 1 && pow2 && k.N == k.Npad && k.g == 32;
+}
+bool const_slot_acquire()
+{
     int expected = 0;
     return g_const_owner.compare_exchange_strong(expected, 1);
 }
-void release_const_slot() { g_const_owner.store(0); }
-// prep_kernel stores the coefficient pairs through this address; the constant caches are invalidated at every
-// kernel launch, so the point kernel that follows on the same stream reads the new values from the constant bank
-double *const_slot_address()
-{
-    void *p = nullptr;
-    if (cudaGetSymbolAddress(&p, c_coef) != cudaSuccess) { cudaGetLastError(); return nullptr; }
-    return static_cast<double *>(p);
-}
+void const_slot_release() { g_const_owner.store(0); }
 
 constexpr int PIPE_THREADS_BIG = 512;
 static KernelFn pick_pipe(const KParams &k, bool big = false)
@@ -716,20 +654,24 @@ static KernelFn pick_pipe(const KParams &k, bool big = false)
     case N:                                                                                      \
         if (k.use_constc) return k.geom ? point_kernel_pipe<N, true, true> : point_kernel_pipe<N, false, true>; \
         return k.geom ? point_kernel_pipe<N, true, false> : point_kernel_pipe<N, false, false>;
+#define DSE_PIPE_CASE_S(N)                                                                       \
+    case N:                                                                                      \
+        return k.geom ? point_kernel_pipe<N, true, false> : point_kernel_pipe<N, false, false>;
     switch (k.NCH) {
         DSE_PIPE_CASE(1)
         DSE_PIPE_CASE(2)
-        DSE_PIPE_CASE(3)
+        DSE_PIPE_CASE_S(3)
         DSE_PIPE_CASE(4)
-        DSE_PIPE_CASE(5)         // the paper's N = 36
-        DSE_PIPE_CASE(6)
-        DSE_PIPE_CASE(7)
+        DSE_PIPE_CASE_S(5)       // the paper's N = 36
+        DSE_PIPE_CASE_S(6)
+        DSE_PIPE_CASE_S(7)
         DSE_PIPE_CASE(8)
-        DSE_PIPE_CASE(12)        // the paper's N = 96
+        DSE_PIPE_CASE_S(12)      // the paper's N = 96
         DSE_PIPE_CASE(16)
         default: return nullptr;
     }
 #undef DSE_PIPE_CASE
+#undef DSE_PIPE_CASE_S
 }
 
 // grid of the pipelined kernel: units are 32-point batches; every warp gets at least one row's worth of them, so that
@@ -772,9 +714,16 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
 
     // residual-only build (and the Jacobian build of generic shapes): warp-independent kernel, 512 threads
     // (large N with full-warp angular batches: fewer warps per CTA until the per-warp stashes fit in shared memory)
+    auto gsmem = [&](int thr) {
+        int d = k.Ntpad * 6 + (thr / 32) * warp_doubles(k.Npad, k.NCH);
+        const int need = tail_fixed_doubles(k.Npad, thr) + 3 * 64;          // the fused tail stages at least 64 rows at a time
+        if (d < need) d = need;
+        return (int)sizeof(double) * d;
+    };
     int gthr = POINT_THREADS;
-    while (gthr > 128 && (int)sizeof(double) * (k.Ntpad * 6 + (gthr / 32) * warp_doubles(k.Npad, k.NCH, np_of(k))) > smem_max) gthr -= 128;
-    const int smem = (int)sizeof(double) * (k.Ntpad * 6 + (gthr / 32) * warp_doubles(k.Npad, k.NCH, np_of(k)));
+    while (gthr > 128 && gsmem(gthr) > smem_max) gthr -= 128;
+    const int smem = gsmem(gthr);
+    if (smem > smem_max) { set_error_text("n_theta too large: the angular table does not fit in shared memory"); return DSE_EINVAL; }
     for (int jac = 0; jac < 2; ++jac) {
         e = cudaFuncSetAttribute((const void *)pick(k, jac != 0), cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel smem)");
@@ -792,12 +741,15 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     int block = gthr, jsmem = smem;
     cfg.pipelined = 0;
     cfg.batched = 0;
-    KernelFn pf = (k.g == 32 && !getenv("DSE_NO_PIPE")) ? pick_pipe(k) : nullptr;
+    KernelFn pf = k.g == 32 ? pick_pipe(k) : nullptr;
     if (pf) {
+        auto psmem_of = [&](int thr) {
+            return (int)sizeof(double) * (k.Ntpad * 6 + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
+        };
         // large problems (>= 48 batches per warp at 16 warps per SM) with 8 chunks: the 512-thread build of the kernel
         const long long units = k.R * (k.Ntpad / 32);
-        const int big_smem = (int)sizeof(double) * (k.Ntpad * 6 + (PIPE_THREADS_BIG / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
-        const bool big = k.NCH == 8 && units >= 48LL * sms * (PIPE_THREADS_BIG / 32) && big_smem <= smem_max && !getenv("DSE_NO_PIPE512");
+        const int big_smem = psmem_of(PIPE_THREADS_BIG);
+        const bool big = k.NCH == 8 && units >= 48LL * sms * (PIPE_THREADS_BIG / 32) && big_smem <= smem_max;
         if (big) {
             pf = pick_pipe(k, true);
             e = cudaFuncSetAttribute((const void *)pf, cudaFuncAttributeMaxDynamicSharedMemorySize, big_smem);
@@ -806,7 +758,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
         }
         // large N: fewer warps per CTA until the double-buffered stashes fit in shared memory (at least 8 warps)
         for (int thr = PIPE_THREADS; !big && thr >= 256; thr -= 128) {
-            const int psmem = (int)sizeof(double) * (k.Ntpad * 6 + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
+            const int psmem = psmem_of(thr);
             if (psmem > smem_max) continue;
             e = cudaFuncSetAttribute((const void *)pf, cudaFuncAttributeMaxDynamicSharedMemorySize, psmem);
             if (e != cudaSuccess) return fail(e, "cudaFuncSetAttribute(point_kernel_pipe smem)");
@@ -828,19 +780,27 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     return 0;
 }
 
+// Launches the point kernel of one build; k.c, k.bc, k.J, k.F and k.want_jac are set.  Returns the number of kernels
+// launched (1) or < 0.
 int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
-    if (constc_of(k) && !k.coefC)                              // fallback: in-stream copy of the pairs into the slot
-        cudaMemcpyToSymbolAsync(c_coef, k.coefP, sizeof(double2) * k.Npad, 0, cudaMemcpyDeviceToDevice, (cudaStream_t)stream);
+    cudaStream_t s = (cudaStream_t)stream;
     if (cfg.batched) return launch_point_batched(k, cfg, stream);     // Jacobian or residual-only variant
+    cudaError_t e;
     if (k.want_jac) {
+        if (cfg.pipelined && k.use_constc) {                   // a -> c_coefA, b -> c_coefB (documented in-stream update)
+            e = cudaMemcpyToSymbolAsync(c_coefA, k.c, sizeof(double) * k.N, 0, cudaMemcpyDeviceToDevice, s);
+            if (e == cudaSuccess) e = cudaMemcpyToSymbolAsync(c_coefB, k.c + k.N, sizeof(double) * k.N, 0, cudaMemcpyDeviceToDevice, s);
+            if (e != cudaSuccess) return fail(e, "cudaMemcpyToSymbolAsync(coefficients)");
+        }
         KernelFn fn = cfg.pipelined ? pick_pipe(k, cfg.pipelined == 2) : pick(k, true);
-        launch_pdl(fn, dim3(cfg.grid), dim3(cfg.block), (size_t)cfg.smem, (cudaStream_t)stream, k);
+        e = launch_pdl(fn, dim3(cfg.grid), dim3(cfg.block), (size_t)cfg.smem, s, k);
     } else {
         KParams kk = k;
         kk.W = cfg.res_grid * (cfg.res_block / 32);          // the residual build has its own row partition
-        launch_pdl(pick(k, false), dim3(cfg.res_grid), dim3(cfg.res_block), (size_t)cfg.res_smem, (cudaStream_t)stream, kk);
+        e = launch_pdl(pick(k, false), dim3(cfg.res_grid), dim3(cfg.res_block), (size_t)cfg.res_smem, s, kk);
     }
+    if (e != cudaSuccess) return fail(e, "point kernel launch");
     return 1;
 }
 

@@ -10,15 +10,13 @@
 // the weights are transposed into A fragments with shuffles.  Partials per (warp, system group, external point) are
 // written straight from the accumulator fragments; assemble_kernel sums them in warp order (deterministic).
 // Requirements: n_batch >= 8 (padded to a multiple of 8 with idle systems, at most a quarter of the padded batch),
-// N <= 64 (tiles of 16, 32, 48 or 64 indices), full-warp angular batches; other shapes use dse_point.cu.
+// N <= 64 (tiles of 16, 32, 48 or 64 indices), full-warp angular batches; other shapes, and handles created with
+// DSE_FLAG_PER_SYSTEM_KERNELS, use dse_point.cu.
 #include <cstdio>
-#include <cstdlib>
 
 #include "dse_device.cuh"
 
 namespace dse {
-
-void set_error_text(const char *s);
 
 namespace {
 
@@ -272,13 +270,7 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
     if (GEOM) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
 }
 
-int fail(cudaError_t e, const char *what)
-{
-    char buf[256];
-    snprintf(buf, sizeof(buf), "%s: %s", what, cudaGetErrorString(e));
-    set_error_text(buf);
-    return DSE_ECUDA;
-}
+int fail(cudaError_t e, const char *what) { return cuda_fail((int)e, what); }
 
 }  // namespace
 
@@ -286,7 +278,7 @@ int fail(cudaError_t e, const char *what)
 bool batched_eligible(const KParams &k)
 {
     const int Bpad = (k.B + 7) / 8 * 8;
-    return k.B >= 8 && 4 * (Bpad - k.B) <= Bpad && k.Npad <= 64 && k.g == 32 && !getenv("DSE_NO_BATCHED");
+    return k.B >= 8 && 4 * (Bpad - k.B) <= Bpad && k.Npad <= 64 && k.g == 32;
 }
 
 namespace {
@@ -343,7 +335,9 @@ int query_point_batched(const KParams &k, PointKernelConfig &cfg)
 
 int launch_point_batched(const KParams &k, const PointKernelConfig &cfg, void *stream)
 {
-    launch_pdl(batched_variant(k, k.want_jac != 0).fn, dim3(cfg.grid), dim3(cfg.block), (size_t)cfg.smem, (cudaStream_t)stream, k);
+    cudaError_t e = launch_pdl(batched_variant(k, k.want_jac != 0).fn, dim3(cfg.grid), dim3(cfg.block), (size_t)cfg.smem,
+                               (cudaStream_t)stream, k);
+    if (e != cudaSuccess) return fail(e, "point_kernel_batched launch");
     return 1;
 }
 

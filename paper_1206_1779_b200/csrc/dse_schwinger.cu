@@ -19,8 +19,6 @@
 
 namespace dse {
 
-void set_error_text(const char *s);
-
 namespace {
 
 constexpr double PI_D = 3.14159265358979323846;

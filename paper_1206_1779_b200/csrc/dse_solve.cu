@@ -14,8 +14,6 @@
 
 namespace dse {
 
-void set_error_text(const char *s);
-
 namespace {
 
 constexpr int CTL_RHO = 0, CTL_CAP = 1, CTL_TOL = 2, CTL_MAXIT = 3, CTL_ITER = 4;

@@ -73,7 +73,9 @@ inline void phi_row(int N, int Npad, ld s, double *out)
 
 }  // namespace
 
-void build_tables(const dse_params &p, HostTables &T)
+// user != nullptr (DSE_FLAG_USER_TABLES): x_ext, y, Wy, theta, Omega are taken from the caller as they are; s(y_q), the
+// phi tables, the square roots and the continuation add-ons are derived from those values exactly as from the library's own.
+void build_tables(const dse_params &p, const dse_tables *user, HostTables &T)
 {
     const bool split = (p.flags & DSE_FLAG_RADIAL_SPLIT) != 0;
     const int N = p.n_cheb, Nir = p.n_r_ir, Nmain = p.n_r, Nr = (split ? 2 : 1) * Nmain + Nir, Nt = p.n_theta;
@@ -105,6 +107,8 @@ void build_tables(const dse_params &p, HostTables &T)
     }
     T.x_ext[T.iZ] = p.x_Z;
     if (!same) T.x_ext[T.iG] = p.x_G;
+    if (user)
+        for (int e = 0; e < T.Next; ++e) T.x_ext[e] = user->x_ext[e];
     for (int e = 0; e < T.Next; ++e) {
         T.sx_ext[e] = (double)sqrtl((ld)T.x_ext[e]);
         // at x = 0 (x_G = 0, L135) only the ghost equation is evaluated: the gluon prefactor C/(3x) is dropped
@@ -130,6 +134,7 @@ void build_tables(const dse_params &p, HostTables &T)
             const ld hq = (tir[q] + 1) / 2;
             T.y[o + q] = (double)((ld)p.eps2 * hq * hq * hq * hq);
             T.Wy[o + q] = (double)(wir[q] * 2 * (ld)p.eps2 * hq * hq * hq);
+            if (user) { T.y[o + q] = user->y[o + q]; T.Wy[o + q] = user->Wy[o + q]; }
             T.t_r[o + q] = -1.0;
             const ld ell = logl((ld)T.y[o + q] / (ld)p.eps2);
             T.EGy[o + q] = (double)((ld)p.ir_exp_G * ell);
@@ -145,11 +150,12 @@ void build_tables(const dse_params &p, HostTables &T)
             const ld L = logl(hi / lo);
             for (int q = 0; q < Nmain; ++q) {
                 const size_t i = o + Nir + (size_t)part * Nmain + q;
-                const ld yy = lo * expl((tm[q] + 1) * L / 2);
+                ld yy = lo * expl((tm[q] + 1) * L / 2);
                 T.y[i] = (double)yy;
                 T.Wy[i] = (double)(wm[q] * (L / 2) * yy);
+                if (user) { T.y[i] = user->y[i]; T.Wy[i] = user->Wy[i]; yy = (ld)T.y[i]; }
                 ld sy = 2 * logl(yy / (ld)p.eps2) / Lg - 1;
-                if (!split) sy = tm[q];                         // the shared rule is laid out in s itself
+                if (!split && !user) sy = tm[q];                // the shared rule is laid out in s itself
                 if (sy < -1) sy = -1;
                 if (sy > 1) sy = 1;
                 T.t_r[i] = (double)sy;
@@ -172,6 +178,7 @@ void build_tables(const dse_params &p, HostTables &T)
             const ld wk = h * (PI_L / 2) * coshl(tt) / (ch * ch);
             T.theta[k] = (double)(2 * atanl(expl(-u)));
             T.Omega[k] = (double)(wk * ch);
+            if (user) { T.theta[k] = user->theta[k]; T.Omega[k] = user->Omega[k]; }
             // the rule IS the pair (theta_k, Omega_k) of doubles that dse_get_tables returns: like the Gauss-Legendre
             // branch, everything the kernels use is derived from those rounded values (next to theta = pi, sin(theta)
             // inherits the rounding of theta -- nodes of relative weight < 1e-11; reading A25)
@@ -195,6 +202,7 @@ void build_tables(const dse_params &p, HostTables &T)
         const int kk = k < Nt ? k : 0;                 // padded lanes: a valid angle with zero weight
         ld th = (t[kk] + 1) * PI_L / 2;
         ld Om = (k < Nt) ? w[kk] * PI_L / 2 : 0.0L;
+        if (user) { th = user->theta[kk]; Om = (k < Nt) ? (ld)user->Omega[kk] : 0.0L; }
         if (k < Nt) { T.theta[k] = (double)th; T.Omega[k] = (double)Om; }
         // the kernels take theta as the rounded double (same input as any other consumer of the table)
         ld thd = (ld)(double)th;

@@ -1,4 +1,4 @@
-"""The C-ABI library loads and exports every symbol include/dse.h declares (no compute without a GPU)."""
+"""The C-ABI library loads and exports every symbol include/*.h declares (no compute without a GPU)."""
 import ctypes
 import os
 import re
@@ -16,10 +16,12 @@ def lib():
 
 
 def test_header_symbols_exported(lib):
-    hdr = open(os.path.join(ROOT, "include", "dse.h")).read()
-    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(dse_[a-z0-9_]+)\s*\(", hdr))
-    assert {"dse_create", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step"} <= names
+    names = set()
+    for h in ("dse.h", "dse_diag.h"):
+        hdr = open(os.path.join(ROOT, "include", h)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+        names |= set(re.findall(r"\b(dse_[a-z0-9_]+)\s*\(", hdr))
+    assert {"dse_create", "dse_create_with_tables", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step"} <= names
     for n in names:
         assert hasattr(lib, n), n
     from paper_1206_1779_b200.binding import EXPORTS
@@ -52,6 +54,14 @@ def test_error_paths_without_gpu(lib):
     bad = params_from_workload(CONFIGS[0])
     bad.n_r_ir = -3
     assert lib.dse_create(ctypes.byref(bad), ctypes.byref(h)) == -1
+    # caller-supplied tables: the flag and the entry point go together
+    ok = params_from_workload(CONFIGS[0])
+    ok.flags = 8
+    assert lib.dse_create(ctypes.byref(ok), ctypes.byref(h)) == -1
+    assert lib.dse_create_with_tables(ctypes.byref(ok), None, ctypes.byref(h)) == -1
+    ok.flags = 1 << 12                                                     # unknown flag bit
+    assert lib.dse_create(ctypes.byref(ok), ctypes.byref(h)) == -1
+    assert lib.dse_strerror(-4) == b"constant-bank coefficient slot is held by another handle"
     assert lib.dse_destroy(None) == 0
     assert lib.dse_jacobian(None, None, None, None, None, None) == -1
     import torch
@@ -61,3 +71,11 @@ def test_error_paths_without_gpu(lib):
         from paper_1206_1779_b200 import Dse, DseError
         with pytest.raises(DseError):
             Dse(ok)
+
+
+def test_no_environment_switches_in_the_library():
+    """one POD struct, no env vars -- nothing under csrc/ reads the environment."""
+    src = os.path.join(ROOT, "paper_1206_1779_b200", "csrc")
+    for f in os.listdir(src):
+        if f.endswith((".cu", ".cuh", ".cpp", ".h")):
+            assert "getenv" not in open(os.path.join(src, f)).read(), f

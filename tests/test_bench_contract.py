@@ -37,7 +37,7 @@ def test_gpu_arm_line(cfg):
     assert BASE_KEYS | {"roofline", "clocks"} <= set(line)
     assert line["n_gpus"] == 1 and line["steps"] == 5 and line["warmup"] >= 3 and line["higher_is_better"] is True
     assert line["value"] > 0 and abs(line["value"] - 1e3 / line["ms_per_step"]) <= 1e-6 * line["value"]
-    assert line["gpu_launches"] >= 3 * 5                       # at least prep, point kernel, assemble per step
+    assert line["gpu_launches"] >= 1 * 5                       # at least one kernel per step (pipelined shapes: the whole build)
     r = line["roofline"]
     assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     assert 30.0 < r["peak"] < 45.0 and r["kernel_ms"] > 0

@@ -154,9 +154,11 @@ def test_batched_tensor_path_every_system(orc, shape, B, monkeypatch):
             check(J[b], F[b], Jo, Fo)
         _, F2 = gpu_build(w, c, bc, flags, jac=False)          # dse_residual: the residual-only variant of the kernel
         assert np.allclose(F2, F, rtol=1e-12, atol=0)
-    monkeypatch.setenv("DSE_NO_BATCHED", "1")
-    d = Dse(params_from_workload(w, n_batch=B)); assert d.kernel_info()["variant"] != "batched-dmma"; d.close()
-    J1, F1 = gpu_build(w, c, bc, 0)
+    # DSE_FLAG_PER_SYSTEM_KERNELS (a dse_params flag, not an environment switch): the same batch through the single-system kernels
+    from paper_1206_1779_b200 import DSE_FLAG_PER_SYSTEM_KERNELS
+    d = Dse(params_from_workload(w, n_batch=B, flags=DSE_FLAG_PER_SYSTEM_KERNELS))
+    assert d.kernel_info()["variant"] != "batched-dmma"; d.close()
+    J1, F1 = gpu_build(w, c, bc, DSE_FLAG_PER_SYSTEM_KERNELS)
     assert np.linalg.norm(J1 - Js[0]) <= 1e-12 * np.linalg.norm(J1)
 
 
@@ -172,30 +174,124 @@ def test_deterministic_bitwise():
     for _ in range(5):
         J, F = d.jacobian(ct, bt)
         assert torch.equal(J, J0) and torch.equal(F, F0)
-    assert d.launch_count() == 6 * 3      # cfg 1: prep, point, assemble (H7 fused into it) per build
+    assert d.launch_count() == 6 * 1      # cfg 1: ONE kernel per build (H1 in its prologue, H7 + H8 in its tail)
+    assert d.kernel_info()["kernels_per_build"] == 1
     d.close()
 
 
-def test_two_handles_constant_slot_and_shared_memory_paths(orc):
-    """The first single-system handle owns the constant-bank coefficient slot; a second live handle falls
-    back to shared-memory coefficients.  Both must match the oracle and each other."""
+def test_constant_slot_is_explicit_and_order_independent(orc):
+    """DSE_FLAG_CONST_COEF (include/dse.h): the constant-bank coefficient slot is taken only on request; a second
+    request while it is held fails with DSE_EBUSY; handles without the flag run the same kernel variant whatever the
+    creation order.  All of them match the oracle and each other."""
     torch = _torch()
-    from paper_1206_1779_b200 import Dse, params_from_workload
+    from paper_1206_1779_b200 import Dse, DseError, params_from_workload, DSE_FLAG_CONST_COEF
+    from paper_1206_1779_b200.binding import DSE_EBUSY
     from workloads import config_inputs
     w, c, bc = config_inputs(1)
     Fo, Jo = orc.residual_jacobian(oracle_params(w), c[0], bc[0, 0], bc[0, 1])
-    d1 = Dse(params_from_workload(w))
-    d2 = Dse(params_from_workload(w))
     ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
-    s2 = torch.cuda.Stream()
-    J1, F1 = d1.jacobian(ct, bt)
-    with torch.cuda.stream(s2):
-        J2, F2 = d2.jacobian(ct * 1.0, bt)
-    torch.cuda.synchronize()
-    check(J1.cpu().numpy()[0], F1.cpu().numpy()[0], Jo, Fo)
-    check(J2.cpu().numpy()[0], F2.cpu().numpy()[0], Jo, Fo)
-    assert np.allclose(J1.cpu().numpy(), J2.cpu().numpy(), rtol=1e-11, atol=0)
-    d1.close(); d2.close()
+
+    def run(d, stream=None):
+        if stream is None:
+            J, F = d.jacobian(ct, bt)
+        else:
+            with torch.cuda.stream(stream):
+                J, F = d.jacobian(ct * 1.0, bt)
+        torch.cuda.synchronize()
+        J = J.cpu().numpy()[0]; F = F.cpu().numpy()[0]
+        check(J, F, Jo, Fo)
+        return J
+
+    for order in (0, 1):                                   # plain handle before / after the slot owner
+        if order == 0:
+            p1 = Dse(params_from_workload(w)); own = Dse(params_from_workload(w, flags=DSE_FLAG_CONST_COEF))
+        else:
+            own = Dse(params_from_workload(w, flags=DSE_FLAG_CONST_COEF)); p1 = Dse(params_from_workload(w))
+        p2 = Dse(params_from_workload(w))
+        i1, i2, io = p1.kernel_info(), p2.kernel_info(), own.kernel_info()
+        assert i1 == i2, (i1, i2)                         # equal variants, registers, shared memory: no "first handle wins"
+        assert io["variant"] == "pipelined"
+        with pytest.raises(DseError) as ei:
+            Dse(params_from_workload(w, flags=DSE_FLAG_CONST_COEF))
+        assert ei.value.code == DSE_EBUSY
+        s2 = torch.cuda.Stream()
+        Jo_ = run(own); J1 = run(p1, s2); J2 = run(p2)
+        assert np.array_equal(J1, J2)
+        assert np.allclose(Jo_, J1, rtol=1e-11, atol=0)
+        own.close()
+        own = Dse(params_from_workload(w, flags=DSE_FLAG_CONST_COEF))      # released by dse_destroy
+        run(own)
+        own.close(); p1.close(); p2.close()
+    # shapes that cannot use the slot are refused, not silently downgraded
+    from workloads import Workload
+    with pytest.raises(DseError) as ei:
+        Dse(params_from_workload(Workload("odd", 36, 16, 32, 1e-6, 5e4), flags=DSE_FLAG_CONST_COEF))
+    assert ei.value.code == -1
+
+
+def test_alternating_coefficient_sets_back_to_back(orc):
+    """Several hundred builds back to back on one handle, alternating two coefficient sets (with and without the
+    constant-bank slot): every result must be the one of ITS coefficients -- nothing stale from the build before (the
+    constant bank is refreshed by an in-stream copy, the tail's counters are cleared by the build itself)."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_CONST_COEF, DSE_FLAG_GEOMETRY_CACHE
+    from workloads import config_inputs, draw_coefficients
+    w, c, bc = config_inputs(1)
+    cA = torch.from_numpy(c).cuda(); cB = torch.from_numpy(draw_coefficients(77, w.n_cheb)[None, :]).cuda()
+    bt = torch.from_numpy(bc).cuda()
+    n2 = 2 * w.n_cheb
+    for flags in (DSE_FLAG_CONST_COEF, 0, DSE_FLAG_CONST_COEF | DSE_FLAG_GEOMETRY_CACHE):
+        d = Dse(params_from_workload(w, flags=flags))
+        JA, FA = d.jacobian(cA, bt); JA = JA.clone(); FA = FA.clone()
+        JB, FB = d.jacobian(cB, bt); JB = JB.clone(); FB = FB.clone()
+        assert not torch.equal(JA, JB)
+        outs = [(torch.empty((1, n2, n2), dtype=torch.float64, device="cuda"), torch.empty((1, n2), dtype=torch.float64, device="cuda"))
+                for _ in range(300)]
+        for i, (J, F) in enumerate(outs):
+            d.jacobian(cA if i % 2 == 0 else cB, bt, J, F)
+        torch.cuda.synchronize()
+        for i, (J, F) in enumerate(outs):
+            assert torch.equal(J, JA if i % 2 == 0 else JB) and torch.equal(F, FA if i % 2 == 0 else FB), (flags, i)
+        d.close()
+    Fo, Jo = orc.residual_jacobian(oracle_params(w), cB.cpu().numpy()[0], bc[0, 0], bc[0, 1])
+    check(JB.cpu().numpy()[0], FB.cpu().numpy()[0], Jo, Fo)
+
+
+@pytest.mark.parametrize("cfg,split", [(0, 0), (1, 0), (3, 0), (1, 1)])
+def test_user_tables_isolate_kernel_error(orc, cfg, split):
+    """DSE_FLAG_USER_TABLES (SURVEY 8(b) flags.bit0; PAPER.md L62 never gives the radial node map, so the two table
+    builders are independent pieces of code): with the ORACLE's nodes and weights injected, what is left of the J/F
+    difference is kernel arithmetic alone (summation order, FMA contraction, exp/log) -- printed beside the error with
+    the library's own tables."""
+    _torch()
+    import dataclasses
+    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_USER_TABLES
+    from workloads import config_inputs
+    import torch
+    w, c, bc = config_inputs(cfg)
+    if split:
+        w = dataclasses.replace(w, radial_split=1, n_r=96, name="cfg1-split")
+    p = oracle_params(w)
+    Fo, Jo = orc.residual_jacobian(p, c[0], bc[0, 0], bc[0, 1])
+    ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
+    ot = orc.tables(p)
+    if split:      # the oracle's rule of every external point
+        ys, Ws = zip(*[orc.radial_rule_split(p, x) for x in ot["x_ext"]])
+        ot = dict(ot, y=np.stack(ys), Wy=np.stack(Ws))
+    errs = {}
+    for name, tabs, fl in (("own tables", None, 0), ("oracle tables", ot, DSE_FLAG_USER_TABLES)):
+        d = Dse(params_from_workload(w, flags=fl), tables=tabs)
+        if tabs is not None:
+            t = d.tables()
+            for k in ("x_ext", "y", "Wy", "theta", "Omega"):
+                assert np.array_equal(t[k], np.asarray(tabs[k]).reshape(t[k].shape)), k      # taken as they are
+        J, F = d.jacobian(ct, bt)
+        torch.cuda.synchronize()
+        errs[name] = check(J.cpu().numpy()[0], F.cpu().numpy()[0], Jo, Fo)
+        d.close()
+    print(f"cfg {cfg} split {split}: (|dJ|/|J|, |dF|/|F|, worst J row) with own tables {errs['own tables']}, "
+          f"with the oracle's tables {errs['oracle tables']}")
+    assert errs["oracle tables"][0] <= 1e-12      # kernel arithmetic alone
 
 
 def test_config3_full_size_parity(orc):

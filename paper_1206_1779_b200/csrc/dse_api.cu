@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "dse_internal.h"
 
@@ -18,6 +19,7 @@ struct dse_handle {
     double *d_tables = nullptr;     // one allocation for all tables
     double *d_work = nullptr;       // one allocation for the per-build workspace
     double *d_geom = nullptr;       // geometry cache (optional)
+    int *d_tail = nullptr;          // partition tables of the fused tail
     double *d_J = nullptr, *d_F = nullptr, *d_lu = nullptr;   // internal J, F for dse_newton_step (+ LU scratch)
     double *d_fd = nullptr;
     double *d_delta = nullptr, *d_stats = nullptr, *d_ctl = nullptr, *d_info = nullptr;   // dse_newton_solve
@@ -252,7 +254,8 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
     const size_t o_Gy = carve<double>(off, Bpad * k.Gext * k.Nr), o_Py = carve<double>(off, Bpad * k.Gext * k.Nr);
     const size_t o_iG = carve<double>(off, (size_t)k.B * k.N), o_iZ = carve<double>(off, (size_t)k.B * k.N);
     const size_t o_A = carve<double>(off, Rpad * 4), o_AH = carve<double>(off, Rpad * 4);
-    const size_t o_S = carve<double>(off, ((size_t)k.W * k.bgroup + Bpad * k.Next) * 3 * k.Npad);
+    const size_t slot = h->cfg.batched ? (size_t)3 * k.Npad : (size_t)(6 * k.Npad + 2);      // dse_tail.cuh: slot_doubles
+    const size_t o_S = carve<double>(off, ((size_t)k.W * k.bgroup + Bpad * k.Next) * slot);
     const size_t o_R = carve<double>(off, (size_t)k.B * k.Next * 3 * k.Npad);
     const size_t o_Dg = carve<double>(off, (size_t)k.B * k.Next * 4 * k.Npad), o_Pi = carve<double>(off, (size_t)k.B * k.Next * 4);
     const size_t o_cnt = carve<double>(off, ((size_t)k.B * k.Next + k.B + 1) / 2 + 1);      // unsigned counters of the fused tail
@@ -274,6 +277,33 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
     h->d_Jh = h->d_J; h->d_Fh = h->d_F;
     h->d_delta = wk + o_dl; h->d_stats = wk + o_st; h->d_ctl = wk + o_ctl; h->d_info = wk + o_info;
 
+    if (!h->cfg.batched) {
+        // who works on what, from the same partition the kernels use: warp w owns the units [w U / W, (w + 1) U / W)
+        const long long upb = (long long)k.Nr * k.upr, nbi = (long long)k.B * k.Next;
+        const int wpb = h->cfg.block / 32, grid = h->cfg.grid;
+        std::vector<int> tab((size_t)2 * grid + (size_t)2 * nbi);
+        int *tb = tab.data() + (size_t)2 * grid;
+        for (long long bi = 0; bi < nbi; ++bi) { tb[2 * bi] = 0x7fffffff; tb[2 * bi + 1] = -1; }
+        for (int c = 0; c < grid; ++c) {
+            tab[2 * c] = 0; tab[2 * c + 1] = -1;
+            for (int wi = 0; wi < wpb; ++wi) {
+                const long long w = (long long)c * wpb + wi;
+                const long long t0 = (w * k.U) / k.W, t1 = ((w + 1) * k.U) / k.W;
+                if (t0 >= t1) continue;
+                const int b0 = (int)(t0 / upb), b1 = (int)((t1 - 1) / upb);
+                if (tab[2 * c + 1] < 0) tab[2 * c] = b0;
+                tab[2 * c + 1] = b1;
+                for (int bi = b0; bi <= b1; ++bi) {
+                    if (tb[2 * bi] > (int)w) tb[2 * bi] = (int)w;
+                    if (tb[2 * bi + 1] < (int)w) tb[2 * bi + 1] = (int)w;
+                }
+            }
+        }
+        if (cudaMalloc(&h->d_tail, sizeof(int) * tab.size()) != cudaSuccess) { dse_destroy(h); return DSE_ENOMEM; }
+        e = cudaMemcpy(h->d_tail, tab.data(), sizeof(int) * tab.size(), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemcpy(tail tables)"); }
+        k.tail_cta = h->d_tail; k.tail_bi = h->d_tail + (size_t)2 * h->cfg.grid;
+    }
     rc = dse::lu_configure((int)n2);
     if (rc < 0) { dse_destroy(h); return rc; }
     if (k.geom) {
@@ -296,6 +326,7 @@ int dse_destroy(dse_handle *h)
     if (h->d_tables) cudaFree(h->d_tables);
     if (h->d_work) cudaFree(h->d_work);
     if (h->d_geom) cudaFree(h->d_geom);
+    if (h->d_tail) cudaFree(h->d_tail);
     if (h->h_in) cudaFreeHost(h->h_in);
     if (h->h_out) cudaFreeHost(h->h_out);
     for (auto &p : h->ev)

@@ -55,12 +55,14 @@ struct KParams {
     double *invG, *invZ;               // [B][N]   1/G(x_i), 1/Z(x_i)                                   (prep_kernel)
     double *Apart;                     // [B*Next][Nr][4]   sum_k (u_a, u_b, v, wQ+wM)
     double *AHead;                     // same shape: partial sums of rows whose angular batches span two warps (else 0)
-    double *Spart;                     // [W + B*Next][3][Npad]   per-(warp, external point) partials of the three streams
+    double *Spart;                     // [W + B*Next] slots (dse_tail.cuh: 6 Npad + 2 doubles; batched kernel: [8][3][Npad])
     double *Rz;                        // [B*Next][3][Npad]  A . Phi_y                                   (batched builds)
     double *Dg;                        // [B*Next][4][Npad]  dPiZ/da, dPiZ/db, dPiG/da, dPiG/db          (fused tail)
     double *PiInv;                     // [B*Next][4]        Pi_G, Pi_Z, 1/G(x_e), 1/Z(x_e)              (fused tail)
     unsigned *cnt;                     // [B*Next] arrival counters of the fused tail, [B] completed external points
     unsigned *done;
+    const int *tail_cta;               // [grid][2]   first, last external point index a CTA works on (fused tail)
+    const int *tail_bi;                // [B*Next][2] first, last warp that works on an external point
 };
 
 struct PointKernelConfig {

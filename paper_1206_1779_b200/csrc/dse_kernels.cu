@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(256) prep_kernel(const KParams P, const double
     }
 }
 
-// Geometry cache builder (DSE_FLAG_GEOMETRY_CACHE): one thread per point, geom[(e*Nr+q)*Ntpad + k][4].
+// Geometry cache builder (DSE_FLAG_GEOMETRY_CACHE): one thread per point, geom[(e*Nr+q)*Ntpad + k][4] = (s_raw | 2 + t, gv, gq, gm).
 __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
 {
     const long long n = (long long)P.Next * P.Nr * P.Ntpad;
@@ -83,6 +83,9 @@ __global__ void geometry_kernel(const KParams P, double *__restrict__ geom)
         for (int m = 0; m < 6; ++m) a[m] = P.ang[(size_t)k * 6 + m];
         double sraw, gv, gq, gm;
         point_geometry(rc, a, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
+        // z > L2: the argument is clamped to 1 and only t = ln[1 + omega ln(z/L2)] of eq.(18),(19) is needed -- it does not
+        // depend on the coefficients either, so the record carries 2 + t in place of s_raw (the kernels take t = s_raw - 2)
+        if (sraw > 1.0) sraw = 2.0 + log(fma(P.omega, (sraw - 1.0) * (0.5 * P.Lg), 1.0));
         double4 o = make_double4(sraw, gv, gq, gm);
         reinterpret_cast<double4 *>(geom)[t] = o;
     }

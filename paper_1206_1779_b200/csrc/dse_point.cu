@@ -25,9 +25,10 @@ namespace dse {
 
 namespace {
 
-// DSE_FLAG_CONST_COEF: a_j, b_j of a single-system build as constant-bank operands of the series FMAs.  Filled by two
-// in-stream device-to-device copies of the caller's c (cudaMemcpyToSymbolAsync) before the point kernel is launched.
-__constant__ double c_coefA[DSE_MAX_NCHEB], c_coefB[DSE_MAX_NCHEB];
+// DSE_FLAG_CONST_COEF: the coefficients c = (a_0..a_{N-1}, b_0..b_{N-1}) of a single-system build as constant-bank operands
+// of the series FMAs.  Filled by ONE in-stream device-to-device copy of the caller's c (cudaMemcpyToSymbolAsync) before the
+// point kernel is launched; N is the kernel's compile-time chunk count times 8, so b_j sits at a compile-time offset.
+__constant__ double c_coef[2 * DSE_MAX_NCHEB];
 
 // Template: NCH_T = number of 8-wide Chebyshev chunks when it is a power of two (everything unrolls),
 // 0 = generic run-time shape; GEOM = read the geometry cache; JAC = accumulate the Jacobian streams and (P.tail)
@@ -69,8 +70,9 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
 #pragma unroll
     for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
 
+    const int SLOT = slot_doubles(Npad);
     auto flush = [&](long long bi) {
-        const size_t slot = (size_t)(w + bi);
+        double *slot = P.Spart + (size_t)(w + bi) * SLOT;
 #pragma unroll
         for (int st = 0; st < 3; ++st) {
             __syncwarp();
@@ -83,7 +85,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
             for (int j = lane; j < Npad; j += 32) {
                 double s = 0.0;
                 for (int sb = 0; sb < SUB; ++sb) s += s_T[sb * Npad + j];
-                P.Spart[(slot * 3 + st) * Npad + j] = s;
+                slot[st * Npad + j] = s;
             }
         }
         __syncwarp();
@@ -93,13 +95,14 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
     // stream (wrapping at a system boundary), so the next batch is prefetched with cp.async into a warp-private
     // double buffer while the current one is processed -- no registers held across the batch.
     const bool PREF = GEOM && g == 32;
+    const unsigned long long gpolicy = l2_evict_first_policy();
     const size_t gtotal = (size_t)P.Next * Nr * P.Ntpad;
     const double4 *gbase = reinterpret_cast<const double4 *>(P.geom), *gend = gbase + gtotal, *gnext = gbase;
     unsigned gphase = 0;
     auto prefetch = [&](unsigned buf) {
         const unsigned dst = (unsigned)__cvta_generic_to_shared(s_gbuf + buf * 32 + lane);
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(gnext));
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(gnext) + 16));
+        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(gnext), "l"(gpolicy));
+        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(gnext) + 16), "l"(gpolicy));
         asm volatile("cp.async.commit_group;\n" ::);
     };
     if (PREF && r0 < r1) {
@@ -115,6 +118,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
     int cur_b = (int)(bi / P.Next);
     int e = (int)(bi - (long long)cur_b * P.Next);
     bool fresh = true;                                   // accumulators belong to a new external point
+    bool first_row = true;                               // no row of this external point has reached the slot yet
     if (r0 < r1) {
         for (int j = lane; j < Npad; j += 32)
             s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
@@ -125,6 +129,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
 #pragma unroll
             for (int m = 0; m < CJ; ++m) accA[m] = accB[m] = accV[m] = 0.0;
             fresh = false;
+            first_row = true;
         }
         const long long left = r1 - r;
         int nrow = P.rpb;
@@ -174,7 +179,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
                 const double ell = (sraw + 1.0) * halfLg;
                 EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
             } else if (sraw > 1.0) {                 // z > L2: [omega ln(z/L2) + 1]^{delta,gamma}  eq.(18),(19)
-                const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                const double t = GEOM ? sraw - 2.0 : log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));   // (cached: the record carries 2 + t)
                 EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
             }
             const double ts = 2.0 * s;
@@ -248,7 +253,16 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
             sumV += __shfl_xor_sync(FULL, sumV, o);
             sumZ += __shfl_xor_sync(FULL, sumZ, o);
         }
-        if (kl == 0 && rowact) {
+        if (JAC && P.tail) {
+            // H5 + H7 in the warp's slot of this external point, row by row (dse_tail.cuh)
+            for (int rb = 0; rb < nrow; ++rb) {
+                const double rA = __shfl_sync(FULL, sumA, rb * g), rB = __shfl_sync(FULL, sumB, rb * g);
+                const double rV = __shfl_sync(FULL, sumV, rb * g), rZ = __shfl_sync(FULL, sumZ, rb * g);
+                const double *phi = P.phi_y + ((size_t)(P.rstride ? e * P.rstride : 0) + q0 + rb) * Npad;
+                slot_row_update(P.Spart + (size_t)(w + bi) * SLOT, Npad, phi, rA, rB, rV, rZ, first_row, lane);
+                first_row = false;
+            }
+        } else if (kl == 0 && rowact) {
             reinterpret_cast<double4 *>(P.Apart)[(size_t)bi * Nr + q] = make_double4(sumA, sumB, sumV, sumZ);
             reinterpret_cast<double4 *>(P.AHead)[(size_t)bi * Nr + q] = make_double4(0.0, 0.0, 0.0, 0.0);   // rows are never split here
         }
@@ -269,10 +283,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
     }
     if (JAC && !fresh) flush(bi);
     if (PREF) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
-    if (JAC && P.tail) {                                 // H7 + H8 by the last-arriving CTAs (uniform over the grid)
-        const long long T0 = ((long long)blockIdx.x * WPB * R) / P.W, T1 = ((long long)(blockIdx.x + 1) * WPB * R) / P.W;
-        build_tail(P, smem, dynamic_smem_doubles(), T0, T1);
-    }
+    if (JAC && P.tail) build_tail(P, smem);              // H8 by the last-arriving CTAs (uniform over the grid)
 }
 
 
@@ -292,6 +303,98 @@ __host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc,
     return (constc ? 0 : 2 * Npad) + 2 * stash_doubles(NCH) + (geom ? GBUF_DOUBLES : 0) + GP_DOUBLES;
 }
 
+// H1 for a window of 32 consecutive rows starting at row rb (relative to the warp's first row r0): lane r takes row rb + r
+// and runs both series ln G(y), ln Z(y) of eq.(23),(24) over the table row phi_j(t_q) (phi_0 = 1/2 is in the table) by
+// itself -- no cross-lane reduction -- adds the power-law terms of the infrared piece, and keeps G(y) = exp(ln G),
+// P(y) = G^{e1} Z^{e2} (eq.(3),(9)).  The first nr0 rows of the first window were staged in the stash (row stride
+// Npad + 2 doubles: at most a 4-way bank conflict); every other row is read from the table in global memory.
+// The coefficients come from where the kernel keeps them (constant bank, or the pairs of system sb in shared memory); a
+// row of another system reads c itself.  Nothing in the loop waits on cold global memory.
+// (Not inlined: the body of the point kernel's loop has to stay inside the SM's instruction cache.)
+template <int Npad, bool CONSTC>
+__device__ __noinline__ void pipe_fill_gp(const KParams &P, long long r0, int n_rows, int g0, int gmod, int nr0,
+                                          const double *s_rows, const double2 *s_coef, int sb, double2 *s_gp, int lane, int rb)
+{
+    const int N = P.N;
+    const int nr = n_rows - rb < 32 ? n_rows - rb : 32;
+    double Gv = 0.0, Pv = 0.0;
+    if (lane < nr) {
+        const int gi = (int)((g0 + rb + lane) % gmod);
+        const double addZ = __ldg(P.EZy + gi), addG = __ldg(P.EGy + gi);
+        const int br = (int)((r0 + rb + lane) / ((long long)P.Next * P.Nr));
+        const double *ph = (rb == 0 && lane < nr0) ? s_rows + lane * (Npad + 2) : P.phi_y + (size_t)gi * Npad;
+        double z0 = 0.0, z1 = 0.0, g0s = 0.0, g1 = 0.0;
+        if (CONSTC || br == sb) {
+#pragma unroll 4
+            for (int j = 0; j < Npad; j += 2) {        // (pairs beyond N are zero in both sources)
+                const double f0 = ph[j], f1 = ph[j + 1];
+                const double2 c0 = CONSTC ? make_double2(c_coef[j], c_coef[Npad + j]) : s_coef[j];
+                const double2 c1 = CONSTC ? make_double2(c_coef[j + 1], c_coef[Npad + j + 1]) : s_coef[j + 1];
+                z0 = fma(c0.x, f0, z0); g0s = fma(c0.y, f0, g0s);
+                z1 = fma(c1.x, f1, z1); g1 = fma(c1.y, f1, g1);
+            }
+        } else {
+            const double *ca = P.c + (size_t)br * 2 * N, *cb = ca + N;
+            for (int j = 0; j < N; ++j) { const double f = ph[j]; z0 = fma(__ldg(ca + j), f, z0); g0s = fma(__ldg(cb + j), f, g0s); }
+        }
+        const double lnZ = (z0 + z1) + addZ, lnG = (g0s + g1) + addG;
+        Gv = exp(lnG);
+        Pv = exp(P.e1 * lnG + P.e2 * lnZ);
+    }
+    __syncwarp();
+    s_gp[lane] = make_double2(Gv, Pv);
+    __syncwarp();
+}
+
+// H5 + H7 of the rows [qa, qb] of external point bi = (b, e) that this warp has walked, at the end of the segment: the
+// angular sums come back from the warp's own row records (the last row's from AHead if the warp stopped inside it), several
+// rows of loads in flight; R[j] = sum_q A[q] phi_j(t_q), Pi = sum_q; written once into the warp's slot (dse_tail.cuh).
+template <int Npad>
+__device__ __noinline__ void pipe_contract(const KParams &P, double *slot, int bi, int e, int qa, int qb, bool last_partial, int lane)
+{
+    constexpr int JL = (Npad + 31) / 32;
+    const int Nr = P.Nr;
+    double R[JL][3], pg = 0.0, pz = 0.0;
+#pragma unroll
+    for (int u = 0; u < JL; ++u) R[u][0] = R[u][1] = R[u][2] = 0.0;
+    const double *phib = P.phi_y + (size_t)(P.rstride ? e * P.rstride : 0) * Npad;
+    const double *A = P.Apart + (size_t)bi * Nr * 4, *H = P.AHead + (size_t)bi * Nr * 4;
+    __syncwarp();                                      // the records were written by other lanes of this warp
+#pragma unroll 1
+    constexpr int RT = JL <= 2 ? 6 : 3;                // rows per round trip (register budget)
+    for (int q0 = qa; q0 <= qb; q0 += RT) {
+        double4 rec[RT];
+        double f[RT][JL];
+#pragma unroll
+        for (int v = 0; v < RT; ++v) {
+            const int q = q0 + v;
+            const bool ok = q <= qb;
+            const double *src = ((ok && q == qb && last_partial) ? H : A) + (size_t)(ok ? q : qa) * 4;
+            const double2 s0 = reinterpret_cast<const double2 *>(src)[0], s1 = reinterpret_cast<const double2 *>(src)[1];
+            rec[v] = ok ? make_double4(s0.x, s0.y, s1.x, s1.y) : make_double4(0.0, 0.0, 0.0, 0.0);
+#pragma unroll
+            for (int u = 0; u < JL; ++u) {
+                const int j = 32 * u + lane;
+                f[v][u] = (ok && j < Npad) ? __ldg(phib + (size_t)q * Npad + j) : 0.0;
+            }
+        }
+#pragma unroll
+        for (int v = 0; v < RT; ++v) {
+#pragma unroll
+            for (int u = 0; u < JL; ++u) {
+                R[u][0] = fma(rec[v].x, f[v][u], R[u][0]); R[u][1] = fma(rec[v].y, f[v][u], R[u][1]); R[u][2] = fma(rec[v].z, f[v][u], R[u][2]);
+            }
+            pg += rec[v].z; pz += rec[v].w;
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < JL; ++u) {
+        const int j = 32 * u + lane;
+        if (j < Npad) { slot[3 * Npad + j] = R[u][0]; slot[4 * Npad + j] = R[u][1]; slot[5 * Npad + j] = R[u][2]; }
+    }
+    if (lane == 0) { slot[6 * Npad] = pg; slot[6 * Npad + 1] = pz; }
+}
+
 // THR: threads per CTA the register budget is compiled for (384: ~160 registers; 512: 128 registers, 16 warps per SM --
 // 2 % faster on large problems, slower on small ones)
 template <int NCH_T, bool GEOM, bool CONSTC, int THR = PIPE_THREADS>
@@ -301,6 +404,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     // phase 2 and read the zero-weight stash slot 32 for the points past the batch
     constexpr int NCH = NCH_T, SUB = 32 / NCH_T, ROUNDS = (32 + SUB - 1) / SUB, Npad = NCH_T * CJ;
     constexpr bool EXACT = NCH * SUB == 32 && ROUNDS * SUB == 32;
+    constexpr int SLOT = 6 * Npad + 2;                                      // = slot_doubles(Npad)
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
     const int STASH = stash_doubles(NCH);
@@ -311,18 +415,40 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     double *s_stash = wbase + (CONSTC ? 0 : 2 * Npad);                       // [2][STASH]: pt (33 x 4) then T
     double2 *s_gp = reinterpret_cast<double2 *>(s_stash + 2 * STASH);       // [32] (G(y), P(y)) of a window of rows
     double4 *s_gbuf = reinterpret_cast<double4 *>(s_stash + 2 * STASH + GP_DOUBLES);     // [2][32] geometry records
-
-    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
-    pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
-    __syncthreads();
-
     const int Nr = P.Nr, BPR = P.Ntpad >> 5;                                 // batches per row
     // work is partitioned in 32-point batches (P.U = rows * BPR): balanced to +-1 batch over all warps; a row whose
-    // batches span two warps gets its head partial in AHead and its tail partial in Apart
+    // batches span two warps has one angular-sum record from each (AHead: the head, Apart: the rest)
     const long long w = (long long)blockIdx.x * WPB + warp;
     const long long t0 = (w * P.U) / P.W, t1 = ((w + 1) * P.U) / P.W;
+    const long long r0 = t0 / BPR;
+    const int n_rows = t0 < t1 ? (int)((t1 - 1) / BPR + 1 - r0) : 0;        // rows r0 + [0, n_rows) are touched by this warp
+    // H1 needs the rows phi_j(t_q) of the warp's first rows: a static table, so they are fetched into the (still unused)
+    // stash with cp.async BEFORE the wait on the producer kernel -- the first thing a warp does must not be a chain of
+    // cold global loads
+    const int gmod = P.rstride ? P.Next * Nr : Nr;                           // rows of the table phi_y
+    const int g0 = (int)(r0 % gmod);
+    const int nr0 = min(min(n_rows, 32), 2 * STASH / (Npad + 2));            // rows staged (row stride Npad + 2)
+    {
+        constexpr int CPR = Npad / 2;                                        // 16-byte pieces per row
+        for (int c = lane; c < nr0 * CPR; c += 32) {
+            const int r = c / CPR, o = c - r * CPR;
+            const double *src = P.phi_y + (size_t)((g0 + r) % gmod) * Npad + 2 * o;
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_stash + r * (Npad + 2) + 2 * o);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src));
+        }
+        asm volatile("cp.async.commit_group;\n" ::);
+    }
+    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    {   // the whole table is read row by row (H1, H7) by every warp: pull it into L2 once, spread over the grid
+        const size_t lines = ((size_t)gmod * Npad * sizeof(double) + 127) / 128;
+        for (size_t l = (size_t)blockIdx.x * blockDim.x + threadIdx.x; l < lines; l += (size_t)gridDim.x * blockDim.x)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.phi_y) + l * 128));
+    }
+    pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+    __syncthreads();
+
     if (t0 < t1) {
-    const long long r0 = t0 / BPR, r_end = (t1 - 1) / BPR + 1;              // rows [r0, r_end) are touched by this warp
     int kb = (int)(t0 - r0 * BPR);
     const bool lane_on = EXACT || lane < NCH * SUB;
     const int c_lane = lane_on ? lane / SUB : 0, sub = lane_on ? lane - c_lane * SUB : 0;
@@ -350,9 +476,30 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
             }
         }
     };
+    // the same for the last batch of a segment (once per segment: a rolled loop -- the unrolled copy above is 6 KB of code,
+    // and the loop body of the kernel has to stay inside the 32 KB instruction cache of the SM)
+    auto phase2_last = [&](int buf) {
+        const double4 *pts = reinterpret_cast<const double4 *>(s_stash + buf * STASH);
+        const double2 *trd = reinterpret_cast<const double2 *>(s_stash + buf * STASH + 132) + c_lane * (TCH_STRIDE / 2);
+#pragma unroll 1
+        for (int rd = 0; rd < ROUNDS; ++rd) {
+            const int pt = EXACT ? rd * SUB + sub : min(rd * SUB + sub, 32);
+            const double4 pw = pts[pt];
+            const double2 tt = trd[pt];
+            double T0 = tt.x, T1 = tt.y;
+            accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
+            accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
+#pragma unroll
+            for (int m = 2; m < CJ; ++m) {
+                const double T2 = fma(pw.x, T1, -T0);
+                accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
+                T0 = T1; T1 = T2;
+            }
+        }
+    };
     auto flush = [&](int bi, int buf) {      // `buf`'s T area is free: use it as the cross-lane scratch
         double *scr = s_stash + buf * STASH + 132;
-        const size_t slot = (size_t)(w + bi);
+        double *slot = P.Spart + (size_t)(w + bi) * SLOT;
         if constexpr (EXACT && (SUB == 4 || SUB == 8)) {
             // transposing reduction over the SUB point sub-lanes of a chunk (the low bits of the lane): at every stage a lane
             // keeps one half of its list and receives the partner's sums of that half -- 12 + 6 (+ 3) shuffles instead of
@@ -379,7 +526,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
 #pragma unroll
             for (int i = 0; i < 24 / SUB; ++i) {
                 const int o = base + i, st = o >> 3, m = o & 7;          // o = stream * 8 + index in the chunk
-                P.Spart[(slot * 3 + st) * Npad + c_lane * CJ + m] = v[i];
+                slot[st * Npad + c_lane * CJ + m] = v[i];
             }
         } else {
 #pragma unroll
@@ -392,64 +539,40 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
                 for (int j = lane; j < Npad; j += 32) {
                     double s = 0.0;
                     for (int sb = 0; sb < SUB; ++sb) s += scr[sb * Npad + j];
-                    P.Spart[(slot * 3 + st) * Npad + j] = s;
+                    slot[st * Npad + j] = s;
                 }
             }
             __syncwarp();
         }
     };
 
-    // H1 for a window of 32 consecutive rows starting at row rb: lane = row; ln G(y), ln Z(y) by the series eq.(23),(24)
-    // on the table phi_j(t_q) (phi_0 = 1/2 is in the table), power-law add-ons of the infrared piece, then
-    // G(y) = exp(ln G), P(y) = G^{e1} Z^{e2} (eq.(3),(9))
-    long long gp_base = r0;
-    auto fill_gp = [&](long long rb) {
-        const long long rr = rb + lane;
-        double Gv = 0.0, Pv = 0.0;
-        if (rr < r_end) {
-            const long long bir = rr / Nr;
-            const int qr = (int)(rr - bir * Nr), br = (int)(bir / P.Next), er = (int)(bir - (long long)br * P.Next);
-            const size_t gi = (size_t)(P.rstride ? er * P.rstride : 0) + qr;
-            const double2 *ph = reinterpret_cast<const double2 *>(P.phi_y + gi * Npad);
-            const double *ca = P.c + (size_t)br * 2 * P.N, *cb = ca + P.N;
-            double lnZ = 0.0, lnG = 0.0, lnZ1 = 0.0, lnG1 = 0.0;
-#pragma unroll 4
-            for (int j = 0; j + 1 < P.N; j += 2) {
-                const double2 f = __ldg(ph + (j >> 1));
-                lnZ = fma(__ldg(ca + j), f.x, lnZ);       lnG = fma(__ldg(cb + j), f.x, lnG);
-                lnZ1 = fma(__ldg(ca + j + 1), f.y, lnZ1); lnG1 = fma(__ldg(cb + j + 1), f.y, lnG1);
-            }
-            if (P.N & 1) {
-                const double f = __ldg(P.phi_y + gi * Npad + P.N - 1);
-                lnZ = fma(__ldg(ca + P.N - 1), f, lnZ); lnG = fma(__ldg(cb + P.N - 1), f, lnG);
-            }
-            lnZ = (lnZ + lnZ1) + __ldg(P.EZy + gi); lnG = (lnG + lnG1) + __ldg(P.EGy + gi);
-            Gv = exp(lnG);
-            Pv = exp(P.e1 * lnG + P.e2 * lnZ);
-        }
-        __syncwarp();
-        s_gp[lane] = make_double2(Gv, Pv);
-        __syncwarp();
-        gp_base = rb;
-    };
-
     // geometry stream (GEOM): consecutive 1 KB records, cp.async double buffer
     // (32-bit record index: at most 2^31 points per system; checked in dse_create)
     const unsigned gtotal = (unsigned)P.Next * (unsigned)Nr * (unsigned)P.Ntpad;
     unsigned gidx = 0, gphase = 0;
+    const unsigned long long gpolicy = l2_evict_first_policy();
     auto prefetch = [&](unsigned buf) {
         const double4 *src = reinterpret_cast<const double4 *>(P.geom) + gidx;
         const unsigned dst = (unsigned)__cvta_generic_to_shared(s_gbuf + buf * 32 + lane);
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src));
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(src) + 16));
+        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "l"(gpolicy));
+        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(src) + 16), "l"(gpolicy));
         asm volatile("cp.async.commit_group;\n" ::);
     };
 
-    long long row = r0;                                    // running row index of the flattened (b, e, q)
+    int row = 0;                                           // running row index of the flattened (b, e, q), relative to r0
     int bi = (int)(r0 / Nr);
     int q = (int)(r0 - (long long)bi * Nr);
     int cur_b = bi / P.Next;
     int e = bi - cur_b * P.Next;
+    int gp_base = 0;
+    auto fill_gp = [&](int rb) {
+        pipe_fill_gp<Npad, CONSTC>(P, r0, n_rows, g0, gmod, nr0, s_stash, s_coef, cur_b, s_gp, lane, rb);
+        gp_base = rb;
+    };
+    auto contract = [&](int bi, int e, int qa, int qb, bool last_partial) {
+        pipe_contract<Npad>(P, P.Spart + (size_t)(w + bi) * SLOT, bi, e, qa, qb, last_partial, lane);
+    };
+
     if (GEOM) {
         gidx = ((unsigned)e * Nr + q) * P.Ntpad + kb * 32 + lane;
         prefetch(0);
@@ -460,7 +583,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         __syncwarp();
     };
     if (!CONSTC) load_coef(cur_b);
-    fill_gp(r0);
+    fill_gp(0);
 
     // both T stashes must hold finite numbers before the first (zero-weight) prologue phase 2
     for (int b2 = 0; b2 < 2; ++b2)
@@ -480,9 +603,11 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         reinterpret_cast<double4 *>(s_stash + (cur ^ 1) * STASH)[lane] = make_double4(0.0, 0.0, 0.0, 0.0);   // prologue
         __syncwarp();
         bool seg_done = false;
+        const int q_seg = q;                               // first row of this segment
+        bool last_partial = false;
         while (!seg_done) {
             if (row - gp_base >= 32) fill_gp(row);          // (warp-uniform)
-            const double2 gp = s_gp[(int)(row - gp_base)];
+            const double2 gp = s_gp[row - gp_base];
             const double Gy = gp.x, Py = gp.y;
             RowConst rc;
             if (!GEOM) {
@@ -494,7 +619,6 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
                 rc.d2 = d * d; rc.sxy = sx * sy; rc.rv = -P.C * Wq * y; rc.rq = c3x * Wq; rc.rm = c3x * Wq * y;
             }
             double sumA = 0.0, sumB = 0.0, sumV = 0.0, sumZ = 0.0;
-            const int kb_begin = kb;
             const int kb_end = (rem < BPR - kb) ? kb + rem : BPR;
             for (; kb < kb_end; ++kb, --rem) {
                 double sraw, gv, gq, gm;
@@ -515,7 +639,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
                     const double ell = (sraw + 1.0) * halfLg;
                     EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
                 } else if (sraw > 1.0) {                 // z > L2: eq.(18),(19)
-                    const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                    const double t = GEOM ? sraw - 2.0 : log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));   // (cached: the record carries 2 + t)
                     EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
                 }
                 // ======== main block: phase 1 of this batch || phase 2 of the previous batch ========
@@ -530,10 +654,10 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
 #pragma unroll
                     for (int m = 0; m < CJ; m += 4) {
                         const int j0 = c * CJ + m;
-                        const double2 c0 = CONSTC ? make_double2(c_coefA[j0], c_coefB[j0]) : s_coef[j0];
-                        const double2 c1 = CONSTC ? make_double2(c_coefA[j0 + 1], c_coefB[j0 + 1]) : s_coef[j0 + 1];
-                        const double2 c2 = CONSTC ? make_double2(c_coefA[j0 + 2], c_coefB[j0 + 2]) : s_coef[j0 + 2];
-                        const double2 c3 = CONSTC ? make_double2(c_coefA[j0 + 3], c_coefB[j0 + 3]) : s_coef[j0 + 3];
+                        const double2 c0 = CONSTC ? make_double2(c_coef[j0], c_coef[Npad + j0]) : s_coef[j0];
+                        const double2 c1 = CONSTC ? make_double2(c_coef[j0 + 1], c_coef[Npad + j0 + 1]) : s_coef[j0 + 1];
+                        const double2 c2 = CONSTC ? make_double2(c_coef[j0 + 2], c_coef[Npad + j0 + 2]) : s_coef[j0 + 2];
+                        const double2 c3 = CONSTC ? make_double2(c_coef[j0 + 3], c_coef[Npad + j0 + 3]) : s_coef[j0 + 3];
                         if (j0 == 0) { lz0 = 0.5 * c0.x; lg0 = 0.5 * c0.y; }      // phi_0 = 1/2: the c_0/2 of eq.(23),(24)
                         else { lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0); }
                         lz1 = fma(c1.x, To, lz1); lg1 = fma(c1.y, To, lg1);
@@ -575,20 +699,19 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
                 z += __shfl_xor_sync(FULL, z, 4);
                 z += __shfl_xor_sync(FULL, z, 2);
                 z += __shfl_xor_sync(FULL, z, 1);
-                // lanes 0, 8, 16, 24 hold sum(u_a), sum(u_b), sum(v), sum(wQ + wM)
-                const bool has_first = kb_begin == 0, has_last = kb_end == BPR;
+                // lanes 0, 8, 16, 24 hold sum(u_a), sum(u_b), sum(v), sum(wQ + wM) of this warp's part of the row: its record
+                const bool has_last = kb_end == BPR;
                 double *dst = (has_last ? P.Apart : P.AHead) + ((size_t)bi * Nr + q) * 4 + (lane >> 3);
-                if ((lane & 7) == 0) {
-                    *dst = z;
-                    if (has_first && has_last) P.AHead[((size_t)bi * Nr + q) * 4 + (lane >> 3)] = 0.0;
-                }
+                if ((lane & 7) == 0) *dst = z;
+                last_partial = !has_last;
                 if (has_last) { kb = 0; ++q; ++row; if (q == Nr) seg_done = true; }
                 if (rem <= 0) seg_done = true;
             }
         }
         // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
-        phase2(cur ^ 1);
+        phase2_last(cur ^ 1);
         flush(bi, cur);
+        contract(bi, e, q_seg, last_partial ? q : q - 1, last_partial);
         if (q >= Nr) {
             q = 0; ++bi; ++e;
             if (e == P.Next) {
@@ -599,9 +722,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     }
     if (GEOM) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     }   // t0 < t1
-    // H7 + H8 by the last-arriving CTAs (dse_tail.cuh)
-    const long long T0 = ((long long)blockIdx.x * WPB * P.U) / P.W, T1 = ((long long)(blockIdx.x + 1) * WPB * P.U) / P.W;
-    build_tail(P, smem, dynamic_smem_doubles(), T0, T1);
+    build_tail(P, smem);                                   // H8 by the last-arriving CTAs (dse_tail.cuh)
 }
 using KernelFn = void (*)(const KParams);
 
@@ -716,7 +837,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     // (large N with full-warp angular batches: fewer warps per CTA until the per-warp stashes fit in shared memory)
     auto gsmem = [&](int thr) {
         int d = k.Ntpad * 6 + (thr / 32) * warp_doubles(k.Npad, k.NCH);
-        const int need = tail_fixed_doubles(k.Npad, thr) + 3 * 64;          // the fused tail stages at least 64 rows at a time
+        const int need = tail_smem_doubles(k.Npad, thr);                    // the fused tail reuses the dynamic shared memory
         if (d < need) d = need;
         return (int)sizeof(double) * d;
     };
@@ -788,9 +909,8 @@ int launch_point(const KParams &k, const PointKernelConfig &cfg, void *stream)
     if (cfg.batched) return launch_point_batched(k, cfg, stream);     // Jacobian or residual-only variant
     cudaError_t e;
     if (k.want_jac) {
-        if (cfg.pipelined && k.use_constc) {                   // a -> c_coefA, b -> c_coefB (documented in-stream update)
-            e = cudaMemcpyToSymbolAsync(c_coefA, k.c, sizeof(double) * k.N, 0, cudaMemcpyDeviceToDevice, s);
-            if (e == cudaSuccess) e = cudaMemcpyToSymbolAsync(c_coefB, k.c + k.N, sizeof(double) * k.N, 0, cudaMemcpyDeviceToDevice, s);
+        if (cfg.pipelined && k.use_constc) {                   // c -> constant bank (documented in-stream update)
+            e = cudaMemcpyToSymbolAsync(c_coef, k.c, sizeof(double) * 2 * k.N, 0, cudaMemcpyDeviceToDevice, s);
             if (e != cudaSuccess) return fail(e, "cudaMemcpyToSymbolAsync(coefficients)");
         }
         KernelFn fn = cfg.pipelined ? pick_pipe(k, cfg.pipelined == 2) : pick(k, true);

@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
                         const double ell = (sraw + 1.0) * halfLg;
                         EG = P.pG * ell; EZ = P.pZ * ell; s = -1.0;
                     } else if (sraw > 1.0) {
-                        const double t = log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));
+                        const double t = GEOM ? sraw - 2.0 : log(fma(P.omega, (sraw - 1.0) * halfLg, 1.0));   // (cached: the record carries 2 + t)
                         EG = P.delta * t; EZ = P.gamma * t; s = 1.0;
                     }
                     // T_j(s), j = 4 ks + jq: stride-4 recurrence T_{j+4} = 2 T_4 T_j - T_{j-4}, started from T_0..T_4

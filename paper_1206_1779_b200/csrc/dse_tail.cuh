@@ -3,21 +3,28 @@
 // A build used to be prep -> point -> contraction -> assemble: three dependent launches whose only job after the point
 // kernel is to add up what it produced.  Here the point kernel finishes the build itself, without any CTA ever waiting
 // for another one:
-//   * every CTA, after its warps have written their partials (per-(warp, external point) slots of the three z-dependent
-//     streams, per-row angular sums), fences, and bumps ONE arrival counter per external point it worked on;
+//   * every warp keeps ONE record ("slot") per external point it works on: the three z-dependent streams (flushed from
+//     registers at the end of the segment), the z-independent contraction H7 over ITS rows, R[j] = sum_q A[q] phi_j(t_q)
+//     for the angular sums A[q], and its part of the self-energy sums Pi_G, Pi_Z (H5) -- the slot is private to the warp
+//     until the handshake;
+//   * every CTA, after its warps have written their slots, bumps ONE arrival counter per external point it worked on
+//     (barrier, then fence + atomic by the counting threads);
 //   * the CTA whose increment completes the count of an external point e ("last arriver") owns e: it sums e's slots in
-//     ascending warp order, stages e's row sums A[q] in shared memory, takes Pi_G, Pi_Z (H5) and the z-independent
-//     contraction A[q] . phi_j(t_q) (H7) from there, forms the four derivative rows of e and 1/G(x_e), 1/Z(x_e), and
-//     bumps the system's counter of finished external points;
+//     ascending warp order, forms the four derivative rows of e and 1/G(x_e), 1/Z(x_e), and bumps the system's counter
+//     of finished external points;
 //   * the CTA that finishes the last external point of a system writes that system's J and F (MOM subtraction rows
 //     eq.(14),(15), local terms, the paper's layout eq.(29),(30),(35)) and clears the counters for the next build.
-// The counters only decide WHO does a sum, never the order IN a sum: every reduction runs over slot / row / part
-// indices in a fixed order, so J and F are bitwise reproducible.  Data written by other CTAs of the same launch is read
-// with ld.global.cg after the fence/counter handshake (L1 is not coherent).
+// The counters only decide WHO does a sum, never the order IN a sum: every reduction runs over row / slot indices in a
+// fixed order, so J and F are bitwise reproducible.  Data written by other CTAs of the same launch is read with
+// ld.global.cg after the counter handshake (L1 is not coherent).
 #pragma once
 #include "dse_device.cuh"
 
 namespace dse {
+
+// slot of one (warp, external point): [0, 3 Npad) Sa, Sb, Sv accumulated with T_0 = 1; [3 Npad, 6 Npad) Ra, Rb, Rv with the
+// table phi (phi_0 = 1/2); then Pi_G, Pi_Z
+__host__ __device__ inline int slot_doubles(int Npad) { return 6 * Npad + 2; }
 
 __device__ __forceinline__ double4 ldcg4(const double *p)
 {
@@ -25,97 +32,62 @@ __device__ __forceinline__ double4 ldcg4(const double *p)
     return make_double4(a.x, a.y, b.x, b.y);
 }
 
-__device__ __forceinline__ int dynamic_smem_doubles()
+// H5 + H7 of one radial row, called by the whole warp at the end of the row (generic kernel; the pipelined kernel contracts
+// all rows of a segment at its end):
+// rA, rB, rV = sum_k (u_a, u_b, v), rZ = sum_k (wQ + wM) over the row's angular nodes; phi = phi_j(t_q) of the row.
+// The slot belongs to this warp alone, every lane updates its own addresses: plain loads and stores.
+__device__ __forceinline__ void slot_row_update(double *slot, int Npad, const double *__restrict__ phi, double rA, double rB,
+                                                double rV, double rZ, bool first, int lane)
 {
-    unsigned bytes;
-    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(bytes));
-    return (int)(bytes >> 3);
+    double *R = slot + 3 * Npad;
+    for (int j = lane; j < Npad; j += 32) {
+        const double f = __ldg(phi + j);
+        double a = 0.0, b = 0.0, v = 0.0;
+        if (!first) { a = R[j]; b = R[Npad + j]; v = R[2 * Npad + j]; }
+        R[j] = fma(rA, f, a); R[Npad + j] = fma(rB, f, b); R[2 * Npad + j] = fma(rV, f, v);
+    }
+    if (lane == 0) {
+        double g = 0.0, z = 0.0;
+        if (!first) { g = slot[6 * Npad]; z = slot[6 * Npad + 1]; }
+        slot[6 * Npad] = g + rV; slot[6 * Npad + 1] = z + rZ;
+    }
 }
 
-// doubles of shared memory the tail needs besides the staged rows
-__host__ __device__ inline int tail_fixed_doubles(int Npad, int threads) { return 3 * Npad + 3 * threads + 64; }
+// counter bump with release (everything this thread has observed, cumulatively: the slots its CTA wrote before the
+// barrier) and acquire (what the CTAs counted before it wrote) semantics at device scope
+__device__ __forceinline__ unsigned arrive_acq_rel(unsigned *ctr)
+{
+    unsigned old;
+    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
+    return old;
+}
 
-// The derivative rows of external point bi = b * Next + e from its partial slots [wf, wl] and row sums.
-__device__ __noinline__ void tail_point(const KParams &P, double *sm, int sm_doubles, long long bi, long long wf, long long wl)
+constexpr int TAIL_OWN = 4;            // external points a CTA finishes in one pass
+constexpr int TAIL_MLP = 28;           // slot loads in flight per thread
+
+// doubles of shared memory the tail needs
+__host__ __device__ inline int tail_smem_doubles(int Npad, int threads)
+{
+    const int S = slot_doubles(Npad);
+    return TAIL_OWN * S + (threads > TAIL_OWN * S ? threads : TAIL_OWN * S);
+}
+
+// The derivative rows of the nown <= TAIL_OWN external points own[0..nown) (bi = b * Next + e) from their slots, in one pass.
+// own[3 k + 0 .. 2] = (bi, first warp, last warp)
+__device__ __noinline__ void tail_points(const KParams &P, double *sm, const int *own, int nown)
 {
     const int tid = threadIdx.x, T = blockDim.x, lane = tid & 31, warp = tid >> 5, NW = T >> 5;
-    const int Npad = P.Npad, N = P.N, PJ3 = 3 * Npad, Nr = P.Nr;
-    const int b = (int)(bi / P.Next), e = (int)(bi - (long long)b * P.Next);
-    double *sS = sm;                               // [3][Npad]   slot sums
-    double *sX = sm + PJ3;                         // [3 T]       parts of the slot sums, then k-parts of the contraction
-    double *sRed = sX + 3 * T;                     // [2][32]     per-warp Pi partials
-    double *sA = sRed + 64;                        // [QC][3]     staged row sums
-    const int QC = (sm_doubles - tail_fixed_doubles(Npad, T)) / 3;
-
-    // (1) H6 partials: threads = (part, stream, j); every part sums a contiguous range of slots in ascending warp order
-    {
-        const int parts = T / PJ3 > 1 ? T / PJ3 : 1;
-        const long long nw = wl - wf + 1, per = (nw + parts - 1) / parts;
-        for (int item = tid; item < parts * PJ3; item += T) {
-            const int part = item / PJ3, idx = item - part * PJ3;
-            const long long w0 = wf + part * per, w1 = (wl + 1 < w0 + per) ? wl + 1 : w0 + per;
-            const double *sp = P.Spart + (size_t)(w0 + bi) * PJ3 + idx;
-            double s = 0.0;
-#pragma unroll 8
-            for (long long w = w0; w < w1; ++w, sp += PJ3) s += __ldcg(sp);
-            sX[item] = s;
-        }
-        __syncthreads();
-        for (int idx = tid; idx < PJ3; idx += T) {
-            double s = 0.0;
-            for (int p = 0; p < parts; ++p) s += sX[p * PJ3 + idx];
-            sS[idx] = s;
-        }
-        __syncthreads();
-    }
-
-    // (2) H5 + H7: row sums -> shared memory (chunks of QC rows), Pi partials on the way, then threads = (k-part, j)
-    const int KP = T / Npad, j = tid % Npad, kp = tid / Npad;       // T >= 128 >= Npad
-    const double *Phi = P.phi_y + (size_t)(P.rstride ? e * P.rstride : 0) * Npad;
-    const double *Arow = P.Apart + (size_t)bi * Nr * 4, *Hrow = P.AHead + (size_t)bi * Nr * 4;
-    double pg = 0.0, pz = 0.0, ra = 0.0, rb = 0.0, rv = 0.0;
-    for (int q0 = 0; q0 < Nr; q0 += QC) {
-        const int nq = Nr - q0 < QC ? Nr - q0 : QC;
-        for (int q = tid; q < nq; q += T) {
-            const double4 a = ldcg4(Arow + (size_t)(q0 + q) * 4), h = ldcg4(Hrow + (size_t)(q0 + q) * 4);
-            sA[3 * q] = a.x + h.x; sA[3 * q + 1] = a.y + h.y; sA[3 * q + 2] = a.z + h.z;
-            pg += a.z + h.z; pz += a.w + h.w;
-        }
-        __syncthreads();
-        if (kp < KP) {
-            const int per = (nq + KP - 1) / KP, qa = kp * per, qb = nq < qa + per ? nq : qa + per;
-            const double *ph = Phi + (size_t)(q0 + qa) * Npad + j;
-#pragma unroll 8
-            for (int q = qa; q < qb; ++q, ph += Npad) {
-                const double f = __ldg(ph);
-                ra = fma(sA[3 * q], f, ra); rb = fma(sA[3 * q + 1], f, rb); rv = fma(sA[3 * q + 2], f, rv);
-            }
-        }
-        __syncthreads();
-    }
-    if (kp < KP) { sX[(kp * 3 + 0) * Npad + j] = ra; sX[(kp * 3 + 1) * Npad + j] = rb; sX[(kp * 3 + 2) * Npad + j] = rv; }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { pg += __shfl_xor_sync(FULL, pg, o); pz += __shfl_xor_sync(FULL, pz, o); }
-    if (lane == 0) { sRed[warp] = pg; sRed[32 + warp] = pz; }
-    __syncthreads();
-
-    // (3) the four derivative rows of this external point: dPi_Z/da = Sa + Ra, dPi_Z/db = Sb + Rb, dPi_G/da = Sv,
-    // dPi_G/db = Rv (the kernel accumulates the streams with T_0 = 1; phi_0 = 1/2, eq.(23),(24))
-    double *D = P.Dg + (size_t)bi * 4 * Npad;
-    for (int jj = tid; jj < Npad; jj += T) {
-        double R0 = 0.0, R1 = 0.0, R2 = 0.0;
-        for (int p = 0; p < KP; ++p) { R0 += sX[(p * 3 + 0) * Npad + jj]; R1 += sX[(p * 3 + 1) * Npad + jj]; R2 += sX[(p * 3 + 2) * Npad + jj]; }
-        const double h = jj == 0 ? 0.5 : 1.0;
-        D[jj] = h * sS[jj] + R0;
-        D[Npad + jj] = h * sS[Npad + jj] + R1;
-        D[2 * Npad + jj] = h * sS[2 * Npad + jj];
-        D[3 * Npad + jj] = R2;
-    }
-    // Pi_G, Pi_Z (warp order) and the local terms 1/G(x_e), 1/Z(x_e) of the collocation points (series eq.(23),(24))
-    if (warp == 0) {
-        double lnZ = 0.0, lnG = 0.0;
+    const int Npad = P.Npad, N = P.N, SLOT = slot_doubles(Npad);
+    double *sS = sm;                               // [nown][SLOT]          slot sums
+    double *sX = sm + TAIL_OWN * SLOT;             // [parts][nown][SLOT]   parts of the slot sums
+    // 1/G(x_e), 1/Z(x_e) of the collocation points (series eq.(23),(24)): the last warps, one per point
+    double invG = 0.0, invZ = 0.0;
+    const int myk = NW - 1 - warp;                 // owned point this warp takes the local terms of (if < nown)
+    if (myk < nown) {
+        const int bi = own[3 * myk], b = bi / P.Next, e = bi - b * P.Next;
         if (e < N) {
             const double *cb = P.c + (size_t)b * 2 * N, *px = P.phi_x + (size_t)e * Npad;
+            double lnZ = 0.0, lnG = 0.0;
             for (int jj = lane; jj < N; jj += 32) {
                 const double f = __ldg(px + jj);
                 lnZ = fma(__ldg(cb + jj), f, lnZ);
@@ -123,88 +95,163 @@ __device__ __noinline__ void tail_point(const KParams &P, double *sm, int sm_dou
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) { lnZ += __shfl_xor_sync(FULL, lnZ, o); lnG += __shfl_xor_sync(FULL, lnG, o); }
+            invG = exp(-lnG); invZ = exp(-lnZ);
         }
-        if (lane == 0) {
-            double g = 0.0, z = 0.0;
-            for (int w2 = 0; w2 < NW; ++w2) { g += sRed[w2]; z += sRed[32 + w2]; }
-            double *o = P.PiInv + (size_t)bi * 4;
-            o[0] = g; o[1] = z;
-            o[2] = e < N ? exp(-lnG) : 0.0;
-            o[3] = e < N ? exp(-lnZ) : 0.0;
+    }
+    // threads = (part, owned point, index in the slot); every part sums a contiguous range of slots in ascending warp
+    // order, TAIL_MLP loads in flight at a time.  The number of parts depends on the launch configuration only -- never on
+    // how many points this CTA happens to own (that is decided by arrival order; the grouping of a sum must not be)
+    const int work = nown * SLOT, parts = T / (TAIL_OWN * SLOT) > 1 ? T / (TAIL_OWN * SLOT) : 1;
+    for (int item = tid; item < parts * work; item += T) {
+        const int part = item / work, rest = item - part * work, k = rest / SLOT, idx = rest - k * SLOT;
+        const int bi = own[3 * k], wf = own[3 * k + 1], wl = own[3 * k + 2];
+        const int per = (wl - wf + parts) / parts;
+        const int w0 = wf + part * per, n = (wl + 1 < w0 + per ? wl + 1 : w0 + per) - w0;
+        const double *sp = P.Spart + ((size_t)w0 + (size_t)bi) * SLOT + idx;
+        double s = 0.0;
+        for (int k0 = 0; k0 < n; k0 += TAIL_MLP) {
+            double v[TAIL_MLP];
+#pragma unroll
+            for (int u = 0; u < TAIL_MLP; ++u) v[u] = k0 + u < n ? __ldcg(sp + (size_t)(k0 + u) * SLOT) : 0.0;
+#pragma unroll
+            for (int u = 0; u < TAIL_MLP; ++u) s += v[u];
         }
+        sX[item] = s;
+    }
+    __syncthreads();
+    for (int it = tid; it < work; it += T) {
+        double s = 0.0;
+        for (int p = 0; p < parts; ++p) s += sX[p * work + it];
+        sS[it] = s;
+    }
+    __syncthreads();
+    // dPi_Z/da = Sa + Ra, dPi_Z/db = Sb + Rb, dPi_G/da = Sv, dPi_G/db = Rv (the S streams were accumulated with T_0 = 1;
+    // phi_0 = 1/2, eq.(23),(24))
+    for (int it = tid; it < nown * Npad; it += T) {
+        const int k = it / Npad, jj = it - k * Npad;
+        const double *S = sS + k * SLOT;
+        double *D = P.Dg + (size_t)own[3 * k] * 4 * Npad;
+        const double h = jj == 0 ? 0.5 : 1.0;
+        D[jj] = h * S[jj] + S[3 * Npad + jj];
+        D[Npad + jj] = h * S[Npad + jj] + S[4 * Npad + jj];
+        D[2 * Npad + jj] = h * S[2 * Npad + jj];
+        D[3 * Npad + jj] = S[5 * Npad + jj];
+    }
+    if (myk < nown && lane == 0) {
+        double *o = P.PiInv + (size_t)own[3 * myk] * 4;
+        const double *S = sS + myk * SLOT;
+        o[0] = S[6 * Npad]; o[1] = S[6 * Npad + 1]; o[2] = invG; o[3] = invZ;
     }
 }
 
 // J and F of system b from the rows of all its external points (eq.(29),(30),(35),(36); MOM subtraction eq.(14),(15)).
-__device__ __noinline__ void tail_system(const KParams &P, double *sm, int b)
+// Every entry's operands are loaded in one go (no staging round trip): the CTA that runs this is the last one alive.
+__device__ __noinline__ void tail_system(const KParams &P, int b)
 {
     const int tid = threadIdx.x, T = blockDim.x;
     const int Npad = P.Npad, N = P.N;
     const size_t bi0 = (size_t)b * P.Next, biZ = bi0 + P.iZ, biG = bi0 + P.iG;
-    double *sZ = sm, *sG = sm + 2 * Npad;          // dPi_Z/da, dPi_Z/db at x_Z;  dPi_G/da, dPi_G/db at x_G
-    for (int t = tid; t < 2 * Npad; t += T) {
-        sZ[t] = __ldcg(P.Dg + biZ * 4 * Npad + t);
-        sG[t] = __ldcg(P.Dg + biG * 4 * Npad + 2 * Npad + t);
-    }
-    __syncthreads();
+    const double *DZ = P.Dg + biZ * 4 * Npad, *DG = P.Dg + biG * 4 * Npad + 2 * Npad;     // rows of x_Z (a, b) and of x_G (a, b)
     double *Jb = P.J + (size_t)b * 4 * N * N, *Fb = P.F + (size_t)b * 2 * N;
-    for (int item = tid; item < N * Npad; item += T) {
-        const int i = item / Npad, j = item - i * Npad;
-        if (j >= N) continue;
-        const double *Di = P.Dg + (bi0 + i) * 4 * Npad;
-        const double phi = __ldg(P.phi_x + (size_t)i * Npad + j);
-        const double invG = __ldcg(P.PiInv + (bi0 + i) * 4 + 2), invZ = __ldcg(P.PiInv + (bi0 + i) * 4 + 3);
-        Jb[(size_t)i * 2 * N + j] = -phi * invZ - __ldcg(Di + j) + sZ[j];
-        Jb[(size_t)i * 2 * N + N + j] = -__ldcg(Di + Npad + j) + sZ[Npad + j];
-        Jb[(size_t)(N + i) * 2 * N + j] = -__ldcg(Di + 2 * Npad + j) + sG[j];
-        Jb[(size_t)(N + i) * 2 * N + N + j] = -phi * invG - __ldcg(Di + 3 * Npad + j) + sG[Npad + j];
+    const int total = N * Npad;
+    constexpr int MLP = 4;                         // entries per thread whose loads are issued before the first store
+    for (int base = tid; base < total; base += MLP * T) {
+        double d[MLP][4], s[MLP][4], phi[MLP], ig[MLP], iz[MLP];
+        int ii[MLP], jj[MLP];
+        bool ok[MLP];
+#pragma unroll
+        for (int u = 0; u < MLP; ++u) {
+            const int item = base + u * T;
+            int i = item < total ? item / Npad : 0, j = item < total ? item - i * Npad : 0;
+            ok[u] = item < total && j < N;
+            if (!ok[u]) { i = 0; j = 0; }
+            ii[u] = i; jj[u] = j;
+            const double *Di = P.Dg + (bi0 + i) * 4 * Npad + j;
+            d[u][0] = __ldcg(Di); d[u][1] = __ldcg(Di + Npad); d[u][2] = __ldcg(Di + 2 * Npad); d[u][3] = __ldcg(Di + 3 * Npad);
+            s[u][0] = __ldcg(DZ + j); s[u][1] = __ldcg(DZ + Npad + j); s[u][2] = __ldcg(DG + j); s[u][3] = __ldcg(DG + Npad + j);
+            phi[u] = __ldg(P.phi_x + (size_t)i * Npad + j);
+            ig[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 2); iz[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 3);
+        }
+#pragma unroll
+        for (int u = 0; u < MLP; ++u) {
+            if (!ok[u]) continue;
+            const int i = ii[u], j = jj[u];
+            Jb[(size_t)i * 2 * N + j] = -phi[u] * iz[u] - d[u][0] + s[u][0];
+            Jb[(size_t)i * 2 * N + N + j] = -d[u][1] + s[u][1];
+            Jb[(size_t)(N + i) * 2 * N + j] = -d[u][2] + s[u][2];
+            Jb[(size_t)(N + i) * 2 * N + N + j] = -phi[u] * ig[u] - d[u][3] + s[u][3];
+        }
     }
-    const double PiG_s = __ldcg(P.PiInv + biG * 4), PiZ_s = __ldcg(P.PiInv + biZ * 4 + 1);
-    const double gG = P.bc[2 * b + 0], gZ = P.bc[2 * b + 1];
-    for (int i = tid; i < N; i += T) {
-        const double4 pi = ldcg4(P.PiInv + (bi0 + i) * 4);
-        Fb[i] = pi.w - gZ - pi.y + PiZ_s;          // z(x_i) = 1/Z(x_i) - 1/Z(x_Z) - Pi_Z(x_i) + Pi_Z(x_Z)
-        Fb[N + i] = pi.z - gG - pi.x + PiG_s;      // g(x_i) likewise
+    {
+        const double PiG_s = __ldcg(P.PiInv + biG * 4), PiZ_s = __ldcg(P.PiInv + biZ * 4 + 1);
+        const double gG = P.bc[2 * b + 0], gZ = P.bc[2 * b + 1];
+        for (int i = tid; i < N; i += T) {
+            const double4 pi = ldcg4(P.PiInv + (bi0 + i) * 4);
+            Fb[i] = pi.w - gZ - pi.y + PiZ_s;      // z(x_i) = 1/Z(x_i) - 1/Z(x_Z) - Pi_Z(x_i) + Pi_Z(x_Z)
+            Fb[N + i] = pi.z - gG - pi.x + PiG_s;  // g(x_i) likewise
+        }
     }
     for (int e = tid; e < P.Next; e += T) P.cnt[bi0 + e] = 0u;       // ready for the next build on this handle
     if (tid == 0) P.done[b] = 0u;
 }
 
-// Called by ALL threads of the CTA after its last partial has been written.  [T0, T1) = the CTA's partition units;
-// sm = the CTA's dynamic shared memory (free by now), sm_doubles its size.
-__device__ __forceinline__ void build_tail(const KParams &P, double *sm, int sm_doubles, long long T0, long long T1)
+// Called by ALL threads of the CTA after its warps' last slot updates.  P.tail_cta[2 c], [2 c + 1] = first and last external
+// point index CTA c works on (last < first: none); P.tail_bi[2 bi], [2 bi + 1] = first and last warp that works on bi (both
+// tables are built by dse_create from the same partition formula the kernels use).  sm = the CTA's dynamic shared memory.
+__device__ __forceinline__ void build_tail(const KParams &P, double *sm)
 {
-    __shared__ int s_flag;
-    const int tid = threadIdx.x, WPB = blockDim.x >> 5;
-    __threadfence();                               // this thread's partials and row sums are visible device-wide ...
-    __syncthreads();                               // ... and so are those of the whole CTA before thread 0 counts
-    if (T0 >= T1) return;
-    const long long upb = (long long)P.Nr * P.upr;                   // partition units per external point
-    const long long bi_lo = T0 / upb, bi_hi = (T1 - 1) / upb;
-    for (long long bi = bi_lo; bi <= bi_hi; ++bi) {
-        // warps (hence CTAs) that own a unit of bi: unit t belongs to warp ((t + 1) W - 1) / U
-        const long long rf = bi * upb, rl = rf + upb - 1;
-        const long long wf = ((rf + 1) * P.W - 1) / P.U, wl = ((rl + 1) * P.W - 1) / P.U;
-        const unsigned n_cta = (unsigned)(wl / WPB - wf / WPB + 1);
-        if (tid == 0) s_flag = atomicAdd(P.cnt + bi, 1u) == n_cta - 1;
-        __syncthreads();
-        const bool last = s_flag != 0;
-        __syncthreads();
-        if (!last) continue;
-        __threadfence();                           // acquire side of the handshake
-        tail_point(P, sm, sm_doubles, bi, wf, wl);
-        __threadfence();
-        __syncthreads();
-        const int b = (int)(bi / P.Next);
-        if (tid == 0) s_flag = atomicAdd(P.done + b, 1u) == (unsigned)P.Next - 1;
-        __syncthreads();
-        const bool fin = s_flag != 0;
-        __syncthreads();
-        if (fin) {
-            __threadfence();
-            tail_system(P, sm, b);
-            __syncthreads();
+    __shared__ unsigned s_mask;
+    __shared__ int s_own[3 * TAIL_OWN], s_w[64];
+    const int tid = threadIdx.x, lane = tid & 31, WPB = blockDim.x >> 5;
+    const int bi_lo = P.tail_cta[2 * blockIdx.x], bi_hi = P.tail_cta[2 * blockIdx.x + 1];
+    __syncthreads();                               // the slots of every warp of this CTA are written (CTA scope) ...
+    for (int seg0 = bi_lo; seg0 <= bi_hi; seg0 += 32) {
+        if (tid < 32) {
+            const int bi = seg0 + lane;
+            bool last = false;
+            if (bi <= bi_hi) {
+                const int wf = P.tail_bi[2 * bi], wl = P.tail_bi[2 * bi + 1];
+                s_w[2 * lane] = wf; s_w[2 * lane + 1] = wl;
+                const unsigned n_cta = (unsigned)(wl / WPB - wf / WPB + 1);
+                last = arrive_acq_rel(P.cnt + bi) == n_cta - 1;      // ... and, by the release, device-wide; acquire: the
+                                                                     // other CTAs' slots are visible after the count
+            }
+            const unsigned m = __ballot_sync(FULL, last);
+            if (lane == 0) s_mask = m;
         }
+        __syncthreads();
+        unsigned mask = s_mask;                    // external points this CTA arrived last at (usually none or one)
+        while (mask) {
+            __syncthreads();                       // (s_own, s_mask and the shared memory of the pass before are free)
+            int nown = 0;
+            for (unsigned m2 = mask; m2 && nown < TAIL_OWN; m2 &= m2 - 1, ++nown)
+                if (tid == 0) {
+                    const int l = __ffs(m2) - 1;
+                    s_own[3 * nown] = seg0 + l; s_own[3 * nown + 1] = s_w[2 * l]; s_own[3 * nown + 2] = s_w[2 * l + 1];
+                }
+            for (int k = 0; k < nown; ++k) mask &= mask - 1;
+            __syncthreads();
+            tail_points(P, sm, s_own, nown);
+            __syncthreads();                       // D rows, Pi, 1/G, 1/Z of the owned points are written
+            if (tid < 32) {                        // one count per finished point on its system's counter
+                bool fin = false;
+                int b = 0;
+                if (lane < nown) {
+                    b = s_own[3 * lane] / P.Next;
+                    fin = arrive_acq_rel(P.done + b) == (unsigned)P.Next - 1;
+                }
+                const unsigned m = __ballot_sync(FULL, fin);
+                if (lane == 0) s_mask = m;
+            }
+            __syncthreads();
+            unsigned fmask = s_mask;
+            while (fmask) {                        // systems whose last external point this CTA finished
+                const int l = __ffs(fmask) - 1;
+                fmask &= fmask - 1;
+                tail_system(P, s_own[3 * l] / P.Next);
+            }
+        }
+        __syncthreads();
     }
 }
 

@@ -152,8 +152,8 @@ def test_lu_random_sizes_exact_factorisation(orc):
             if rc == 0:
                 assert np.allclose(x[s], xo, rtol=1e-7, atol=1e-10 * np.abs(xo).max()), (n, kind)
                 assert np.array_equal(st[s][1:], so[1:]), (n, kind, st[s], so)
-            else:
-                assert np.array_equal(st[s][1:3], so[1:3]), (n, kind, st[s], so)
+            else:      # exactly singular: min |pivot| == 0 on both sides, and the library flags it with |Delta|_inf = +Inf
+                assert np.array_equal(st[s][1:3], so[1:3]) and so[2] == 0.0 and np.isinf(st[s][0]), (n, kind, st[s], so)
     d.close()
 
 
@@ -207,8 +207,8 @@ def test_lu_cluster_path_exact_factorisation(orc, N):
             if rc == 0:
                 assert np.allclose(x[s], xo, rtol=1e-7, atol=1e-10 * np.abs(xo).max()), (n, kind)
                 assert np.array_equal(st[s][1:], so[1:]), (n, kind, st[s], so)
-            else:
-                assert np.array_equal(st[s][1:3], so[1:3]), (n, kind, st[s], so)
+            else:      # exactly singular: min |pivot| == 0 on both sides, and the library flags it with |Delta|_inf = +Inf
+                assert np.array_equal(st[s][1:3], so[1:3]) and so[2] == 0.0 and np.isinf(st[s][0]), (n, kind, st[s], so)
     d.close()
 
 

@@ -222,6 +222,18 @@ DSE_API int dse_get_timing(dse_handle *h, double *total_ms, int64_t *launches);
  * t_dev[n_t], delta_dev[n_batch][n_t]; work_dev >= (5 + n_batch) n_nodes + 4 doubles.  Asynchronous on `stream`,
  * deterministic.  2 <= n, n_nodes <= 2^24; 0 < p2_min < p2_max. */
 DSE_API int dse_gauss_legendre(int32_t n, double *x_dev, double *w_dev, double *work_dev, void *stream);
+
+/* dse_gauss_legendre for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same kernels, same results, but the scratch (2 (n + 2) doubles of recurrence
+ * coefficients) lives in a static device array of the library instead of work_dev.  The call allocates nothing (no
+ * cudaMalloc / cudaFree / allocating library routine).  Limits and sharing:
+ *   - 2 <= n <= DSE_GL_NOALLOC_MAX_N, else DSE_EINVAL with a message (dse_last_error);
+ *   - the array (2 MiB) exists once per GPU that loads the library, until the process exits;
+ *   - EVERY call on a device uses the same array and it keeps the last call's contents (nothing in it needs clearing:
+ *     each call rewrites what it reads): calls that overlap on the GPU -- different streams, or a captured graph replayed
+ *     concurrently -- RACE.  Issue them on one stream, or order them with events. */
+#define DSE_GL_NOALLOC_MAX_N (1 << 17)
+DSE_API int dse_gauss_legendre_noalloc(int32_t n, double *x_dev, double *w_dev, void *stream);
 DSE_API int dse_schwinger(dse_handle *h, const double *c_dev, int32_t n_nodes, double p2_min, double p2_max,
                           const double *t_dev, int32_t n_t, double *delta_dev, double *work_dev, void *stream);
 

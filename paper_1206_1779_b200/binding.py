@@ -16,7 +16,8 @@ LIB_PATH = os.path.join(_HERE, "libdse_b200.so")
 EXPORTS = [
     "dse_create", "dse_create_with_tables", "dse_destroy", "dse_residual", "dse_jacobian", "dse_newton_step",
     "dse_newton_solve", "dse_lu_solve", "dse_jacobian_host", "dse_n_ext", "dse_get_tables", "dse_launch_count",
-    "dse_kernel_info", "dse_set_timing", "dse_get_timing", "dse_gauss_legendre", "dse_schwinger", "dse_dressing",
+    "dse_kernel_info", "dse_set_timing", "dse_get_timing", "dse_gauss_legendre", "dse_gauss_legendre_noalloc", "dse_schwinger",
+    "dse_dressing",
     "dse_jacobian_fd", "dse_strerror", "dse_last_error",
     "dse_probe", "dse_probe_flops",
 ]
@@ -82,6 +83,7 @@ def load_library():
     L.dse_get_timing.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
     L.dse_jacobian_fd.argtypes = [vp, dp, dp, C.c_double, dp, vp]
     L.dse_gauss_legendre.argtypes = [C.c_int32, dp, dp, dp, vp]
+    L.dse_gauss_legendre_noalloc.argtypes = [C.c_int32, dp, dp, vp]
     L.dse_schwinger.argtypes = [vp, dp, C.c_int32, C.c_double, C.c_double, dp, C.c_int32, dp, dp, vp]
     L.dse_dressing.argtypes = [vp, dp, dp, C.c_int32, dp, dp, dp, vp]
     L.dse_probe.argtypes = [C.c_int32, C.c_int32, C.c_int32, dp, vp]
@@ -287,3 +289,13 @@ def gauss_legendre(n, device="cuda", stream=None):
     import torch.cuda
     torch.cuda.current_stream().synchronize()
     return x, w
+
+
+GL_NOALLOC_MAX_N = 1 << 17
+
+
+def gauss_legendre_noalloc(n, x, w, stream=None):
+    """dse_gauss_legendre_noalloc: writes the n-point rule into the caller's x[n], w[n]; the library allocates nothing (its
+    scratch is a static device array; n <= GL_NOALLOC_MAX_N; calls that overlap on the GPU race -- include/dse.h)."""
+    _check(load_library().dse_gauss_legendre_noalloc(int(n), _dev_ptr(x, n), _dev_ptr(w, n), _stream_ptr(stream)))
+

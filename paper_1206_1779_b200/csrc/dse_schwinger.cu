@@ -14,6 +14,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <mutex>
 
 #include "dse_internal.h"
 
@@ -186,6 +187,48 @@ int launch_gauss_legendre(int n, double *x, double *w, double *work, void *strea
     return 2;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// dse_gauss_legendre_noalloc: the same two kernels with their scratch (the recurrence coefficients A_m, B_m of
+// gl_prepare_kernel, 2 (n + 2) doubles) in a file-scope device array instead of a caller buffer -- for callers that
+// cannot allocate (stream capture, serving loops).  DSE_GL_NOALLOC_MAX_N = 2^17 nodes (the paper's rule, fn.13) -> 2 MiB
+// that every GPU that loads the library holds until exit.  In HOST code the array's name is only a stand-in: its device
+// address comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) double g_gl_scratch[2 * (DSE_GL_NOALLOC_MAX_N + 2)];
+
+namespace {
+constexpr int GL_MAX_DEVICES = 64;
+std::mutex g_gl_mu;
+double *g_gl_scratch_addr[GL_MAX_DEVICES] = {};      // device address of g_gl_scratch on device d (nullptr: not asked yet)
+}  // namespace
+
+int launch_gauss_legendre_noalloc(int n, double *x, double *w, void *stream)
+{
+    if (n < 2 || n > DSE_GL_NOALLOC_MAX_N) {
+        char buf[160];
+        snprintf(buf, sizeof(buf), "dse_gauss_legendre_noalloc: n = %d is outside [2, %d] (the size of the static scratch)", n,
+                 DSE_GL_NOALLOC_MAX_N);
+        set_error_text(buf);
+        return DSE_EINVAL;
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(e, "cudaGetDevice");
+    if (dev < 0 || dev >= GL_MAX_DEVICES) { set_error_text("dse_gauss_legendre_noalloc: device ordinal out of range"); return DSE_EINVAL; }
+    double *scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_gl_mu);
+        if (!g_gl_scratch_addr[dev]) {
+            void *p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_gl_scratch);          // `dev` is current: the address is this device's copy
+            if (e != cudaSuccess || !p) return fail(e, "cudaGetSymbolAddress(g_gl_scratch)");
+            g_gl_scratch_addr[dev] = static_cast<double *>(p);
+        }
+        scratch = g_gl_scratch_addr[dev];
+    }
+    // nothing in the scratch has to start at zero: gl_prepare_kernel rewrites the entries 0..n that gl_nodes_kernel reads
+    return launch_gauss_legendre(n, x, w, scratch, stream);
+}
+
 // ln G(x_m), ln Z(x_m) for every system at arbitrary momenta x_m > 0: the series eq.(23),(24) on the clamped argument
 // plus the continuations eq.(16)-(19) outside [eps2, L2] (the same definition the point kernel uses at z), and the
 // running coupling alpha(x) = alpha(mu^2) G^2 Z.  One thread per (system, momentum).
@@ -244,3 +287,10 @@ int launch_schwinger(const KParams &k, const double *c, int n, double p2_min, do
 }
 
 }  // namespace dse
+
+extern "C" int dse_gauss_legendre_noalloc(int32_t n, double *x_dev, double *w_dev, void *stream)
+{
+    if (!x_dev || !w_dev) return DSE_EINVAL;
+    const int rc = dse::launch_gauss_legendre_noalloc(n, x_dev, w_dev, stream);
+    return rc < 0 ? rc : DSE_OK;
+}

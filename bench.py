@@ -159,26 +159,27 @@ def run_reference(args, w, c):
     print(json.dumps(line), flush=True)
 
 
-def run_ours(args, w, c, bc):
+def measure(args, cfg_id, steps, warmup, geometry_cache, env, light=False):
+    """One bench line (a dict) for BASELINE config `cfg_id`.  light: a per_config entry of the default run -- no CPU
+    baseline, shorter side measurements."""
     import torch
     import torch.distributed as dist
     from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE, DSE_FLAG_CONST_COEF
-    from paper_1206_1779_b200.binding import probe
     from paper_1206_1779_b200.sharding import max_over_ranks
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (this path has no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    rank, world, local, flush = env["rank"], env["world"], env["local"], env["flush"]
+    w, c, bc = config_inputs(cfg_id)
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
+
+    class _A:      # the knobs the body below reads
+        pass
+    a_ = _A(); a_.steps = steps; a_.warmup = warmup; a_.geometry_cache = geometry_cache; a_.config = cfg_id
+    a_.const_coef = args.const_coef; a_.no_cpu_baseline = args.no_cpu_baseline or light
+    args = a_
 
     nb = c.shape[0]
     flags = DSE_FLAG_GEOMETRY_CACHE if args.geometry_cache else 0
@@ -190,7 +191,6 @@ def run_ours(args, w, c, bc):
     bt = torch.from_numpy(bc).cuda()
     J = torch.empty((nb, n2, n2), dtype=torch.float64, device="cuda")
     F = torch.empty((nb, n2), dtype=torch.float64, device="cuda")
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
     stream = torch.cuda.current_stream()
 
     newton = args.config == 2          # config 2: a step is one full Newton-Raphson step (build + LU + update)
@@ -247,7 +247,7 @@ def run_ours(args, w, c, bc):
     c_h = torch.from_numpy(c).pin_memory(); bc_h = torch.from_numpy(bc).pin_memory()
     J_h = torch.empty((nb, n2, n2), dtype=torch.float64).pin_memory()
     F_h = torch.empty((nb, n2), dtype=torch.float64).pin_memory()
-    e2e_steps = min(args.steps, 200)
+    e2e_steps = min(args.steps, 100 if light else 200)
     cn_h = torch.empty((nb, n2), dtype=torch.float64).pin_memory()          # config 2: the updated coefficients ...
     st_h = torch.empty((nb, 4), dtype=torch.float64).pin_memory()           # ... and the step's stats come back
     c_e2e = torch.empty_like(ct); bc_e2e = torch.empty_like(bt)
@@ -276,7 +276,7 @@ def run_ours(args, w, c, bc):
     # ---- every other config: the same build followed by the Newton update H9 (equilibrated LU, c <- c - Delta) ----
     with_update = None
     if not newton:
-        n_up = min(args.steps, 200)
+        n_up = min(args.steps, 100 if light else 200)
         for _ in range(3):
             c_work.copy_(ct)
             d.newton_step(c_work, bt, 1.0, stats)
@@ -297,7 +297,7 @@ def run_ours(args, w, c, bc):
     # ---- config 2 only: the whole iteration as ONE device-side graph (dse_newton_solve), fixed step count ----
     solve = None
     if newton:
-        iters, reps = 8, 50
+        iters, reps = 8, (20 if light else 50)
         info_t = torch.empty((nb, 6), dtype=torch.float64, device="cuda")
         for _ in range(3):
             c_work.copy_(ct)
@@ -354,28 +354,21 @@ def run_ours(args, w, c, bc):
         d2.close()
 
     info = d.kernel_info()
+    line = None
     if rank == 0:
-        # live fp64 FMA probe (reported beside the derived peak)
-        sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
-        probe("dfma", 148 * 8, 2000, sink)
-        torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        fl = probe("dfma", 148 * 8, 100000, sink)
-        b.record(stream)
-        torch.cuda.synchronize()
-        probe_tflops = fl / (a.elapsed_time(b) * 1e-3) / 1e12
-
         flops = algorithmic_flops(w, nb)
         k_ms = kernel_ms / max(kernel_n, 1)
         achieved = flops / (k_ms * 1e-3) / 1e12
-        traffic = None
+        traffic, traffic_source = None, None
         tpath = os.path.join(ROOT, "profiles", "point_kernel_traffic.txt")
-        if os.path.exists(tpath):
+        if os.path.exists(tpath) and args.geometry_cache:
             try:
-                traffic = json.load(open(tpath)).get(w.name) if args.geometry_cache else None   # captured with the cache on
+                rec = json.load(open(tpath)).get(w.name)      # {"bytes": ..., "source": "..."}: an ncu capture, NOT this run
+                if rec:
+                    traffic, traffic_source = rec["bytes"], rec["source"]
             except Exception:
-                traffic = None
+                pass
+        one_kernel = info.get("kernels_per_build") == 1
         line = {
             "metric": "fp64 Newton steps/s (build + LU)" if newton else "fp64 Jacobian builds/s", "value": value,
             "unit": "newton_steps/s" if newton else "jacobian_builds/s", "n_gpus": world,
@@ -383,19 +376,19 @@ def run_ours(args, w, c, bc):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "n_cheb": w.n_cheb, "n_r": w.n_r, "n_theta": w.n_theta, "n_batch": nb,
                        "eps2": w.eps2, "L2": w.L2, "points_per_build": w.points * nb,
-                       "geometry_cache": bool(args.geometry_cache),
+                       "geometry_cache": bool(args.geometry_cache), "const_coef": bool(flags & DSE_FLAG_CONST_COEF),
                        "l2": "flushed between steps (256 MiB memset outside the per-step event pairs)",
                        "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                        "point_kernel": info},
             "points_per_s": value * w.points, "paper_equiv_evals_per_s": value * w.paper_equiv_evals,
             "wall_s_timed_region": t_wall,
-            "roofline": {"bound": "alu", "kernel": "point_kernel", "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
-                         "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
+            "roofline": {"bound": "alu", "kernel": "point_kernel" + (" (the whole build: H1-H8 in one launch)" if one_kernel else ""),
+                         "achieved": achieved, "peak": FP64_PEAK_TFLOPS,
+                         "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic, "traffic_source": traffic_source,
                          "kernel_ms": k_ms, "kernel_share_of_step": k_ms / (inst_total_ms / args.steps),
                          "ms_per_step_instrumented": inst_total_ms / args.steps,
                          "peak_source": "derived: 148 SM x 64 fp64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no "
-                                        "fp64 entry)",
-                         "measured_dfma_probe_tflops": probe_tflops, "frac_of_probe": achieved / probe_tflops,
+                                        "fp64 entry); measured sustained DFMA rate beside it: peak_measured_sustained",
                          "algorithmic_flops_per_launch": flops},
             "e2e": {"value": e2e_value, "unit": "newton_steps/s" if newton else "jacobian_builds/s",
                     "h2d_bytes_per_step": int(c.nbytes + bc.nbytes), "d2h_bytes_per_step": e2e_d2h, "steps": e2e_steps},
@@ -410,8 +403,84 @@ def run_ours(args, w, c, bc):
             line["cpu_baseline"] = cpu_baseline(w, c[0])
             if newton:
                 line["cpu_baseline"]["converged_solve"] = oracle_converged_solve()
-        print(json.dumps(line), flush=True)
     d.close()
+    return line
+
+
+def sustained_fp64_probe(local, seconds=1.2):
+    """the roofline denominator of an ALU-bound path, measured: >= 1 s of back-to-back DFMA launches (8
+    independent chains per thread, 148 x 8 CTAs of 256 threads), SM clock sampled during the run."""
+    import torch
+    from paper_1206_1779_b200.binding import probe
+    sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+    probe("dfma", 148 * 8, 2000, sink)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    iters, evs, t0 = 400000, [], time.perf_counter()          # ~54 ms per launch
+    while time.perf_counter() - t0 < seconds or len(evs) < 4:
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        fl = probe("dfma", 148 * 8, iters, sink)
+        b.record(stream)
+        evs.append((a, b, fl))
+        torch.cuda.synchronize()
+    sampler.stop_flag = True
+    tf = [fl / (a.elapsed_time(b) * 1e-3) / 1e12 for a, b, fl in evs]
+    out = {"tflops_sustained": float(np.median(tf[len(tf) // 2:])), "tflops_first_launch": tf[0], "seconds": time.perf_counter() - t0,
+           "launches": len(tf), "clocks": sampler.result()}
+    # the fp64 tensor path (mma.sync.m8n8k4.f64), the denominator for the batched kernel (config 4)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    probe("dmma", 148 * 8, 2000, sink)
+    a.record(stream)
+    fl = probe("dmma", 148 * 8, 100000, sink)
+    b.record(stream)
+    torch.cuda.synchronize()
+    out["dmma_tflops"] = fl / (a.elapsed_time(b) * 1e-3) / 1e12
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    env = {"rank": rank, "world": world, "local": local,
+           "flush": torch.empty(256 << 20, dtype=torch.uint8, device="cuda")}      # > 126 MB L2
+    line = measure(args, args.config, args.steps, args.warmup, args.geometry_cache, env)
+    if rank == 0:
+        peak = sustained_fp64_probe(local)
+        r = line["roofline"]
+        r["peak_measured_sustained"] = peak["tflops_sustained"]
+        r["peak_measured"] = peak
+        r["frac_of_measured"] = r["achieved"] / peak["tflops_sustained"]
+        if line["config"]["n_batch"] >= 8:
+            r["frac_of_measured_dmma"] = r["achieved"] / peak["dmma_tflops"]
+    # one driver run covers all five configs north_star names (+ config 3 with the geometry computed in registers)
+    if world == 1 and args.per_config and args.config == 3:
+        per = {}
+        keep = ("value", "unit", "ms_per_step", "e2e", "gpu_launches", "with_newton_update", "newton_solve", "points_per_s")
+        for name, cid, geom in (("cfg0", 0, 1), ("cfg1", 1, 1), ("cfg2", 2, 1), ("cfg4", 4, 1), ("cfg3_on_the_fly", 3, 0)):
+            l2 = measure(args, cid, args.per_config_steps, 5, geom, env, light=True)
+            e = {k: l2[k] for k in keep if k in l2}
+            e["workload"] = l2["config"]["workload"]; e["geometry_cache"] = bool(geom)
+            e["kernel_ms"] = l2["roofline"]["kernel_ms"]; e["kernel_share_of_step"] = l2["roofline"]["kernel_share_of_step"]
+            e["achieved_tflops"] = l2["roofline"]["achieved"]; e["frac"] = l2["roofline"]["frac"]
+            e["frac_of_measured"] = l2["roofline"]["achieved"] / peak["tflops_sustained"]
+            if cid == 4:
+                e["frac_of_measured_dmma"] = l2["roofline"]["achieved"] / peak["dmma_tflops"]
+            e["point_kernel"] = l2["config"]["point_kernel"]; e["steps"] = l2["steps"]
+            per[name] = e
+        line["per_config"] = per
+    if rank == 0:
+        print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
@@ -429,12 +498,16 @@ def main():
     ap.add_argument("--const-coef", type=int, default=1,
                     help="1: single-system builds ask for the constant-bank coefficient slot (DSE_FLAG_CONST_COEF)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-config", type=int, default=1,
+                    help="1 (default run, config 3 only): add the key per_config with a short run of configs 0, 1, 2, 4 and of "
+                         "config 3 without the geometry cache")
+    ap.add_argument("--per-config-steps", type=int, default=300)
     args = ap.parse_args()
-    w, c, bc = config_inputs(args.config)
     if args.impl == "reference":
+        w, c, bc = config_inputs(args.config)
         run_reference(args, w, c)
     else:
-        run_ours(args, w, c, bc)
+        run_ours(args)
 
 
 if __name__ == "__main__":

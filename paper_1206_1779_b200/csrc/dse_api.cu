@@ -183,7 +183,7 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
     size_t off = 0;
     const size_t o_x = carve<double>(off, T.Next), o_sx = carve<double>(off, T.Next), o_c3 = carve<double>(off, T.Next);
     const size_t o_y = carve<double>(off, T.y.size()), o_sy = carve<double>(off, T.y.size()), o_W = carve<double>(off, T.y.size());
-    const size_t o_EG = carve<double>(off, T.y.size()), o_EZ = carve<double>(off, T.y.size());
+    const size_t o_EG = carve<double>(off, T.y.size()), o_EZ = carve<double>(off, T.y.size()), o_tr = carve<double>(off, T.y.size());
     const size_t o_ang = carve<double>(off, T.ang.size());
     const size_t o_py = carve<double>(off, T.phi_y.size()), o_px = carve<double>(off, T.phi_x.size());
     std::vector<double> host(off, 0.0);
@@ -194,6 +194,7 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
     memcpy(&host[o_sy], T.sy.data(), 8 * T.sy.size());
     memcpy(&host[o_W], T.Wy.data(), 8 * T.Wy.size());
     memcpy(&host[o_EG], T.EGy.data(), 8 * T.EGy.size());
+    memcpy(&host[o_tr], T.t_r.data(), 8 * T.t_r.size());
     memcpy(&host[o_EZ], T.EZy.data(), 8 * T.EZy.size());
     memcpy(&host[o_ang], T.ang.data(), 8 * T.ang.size());
     memcpy(&host[o_py], T.phi_y.data(), 8 * T.phi_y.size());
@@ -203,7 +204,7 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
     if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemcpy(tables)"); }
     double *t = h->d_tables;
     k.x_ext = t + o_x; k.sx_ext = t + o_sx; k.c3x_ext = t + o_c3;
-    k.y = t + o_y; k.sy = t + o_sy; k.Wy = t + o_W; k.EGy = t + o_EG; k.EZy = t + o_EZ; k.ang = t + o_ang; k.phi_y = t + o_py; k.phi_x = t + o_px;
+    k.y = t + o_y; k.sy = t + o_sy; k.Wy = t + o_W; k.EGy = t + o_EG; k.EZy = t + o_EZ; k.t_r = t + o_tr; k.ang = t + o_ang; k.phi_y = t + o_py; k.phi_x = t + o_px;
 
     // ---- geometry cache (optional) ----
     if (params->flags & DSE_FLAG_GEOMETRY_CACHE) {

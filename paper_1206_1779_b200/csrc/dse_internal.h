@@ -45,6 +45,7 @@ struct KParams {
     int tail;                          // the point kernel finishes the build itself (reduction, contraction, assembly)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
     const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x, *EGy, *EZy;
+    const double *t_r;                 // s(y_q) of the radial nodes (clamped to [-1, 1]), same layout as y
     const double *geom;                // geometry cache [Next*Nr*Ntpad][4] or nullptr
     // arguments of one build (set per launch)
     const double *c, *bc;              // [B][2N] coefficients (a then b), [B][2] boundary values

@@ -303,41 +303,46 @@ __host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc,
     return (constc ? 0 : 2 * Npad) + 2 * stash_doubles(NCH) + (geom ? GBUF_DOUBLES : 0) + GP_DOUBLES;
 }
 
-// H1 for a window of 32 consecutive rows starting at row rb (relative to the warp's first row r0): lane r takes row rb + r
-// and runs both series ln G(y), ln Z(y) of eq.(23),(24) over the table row phi_j(t_q) (phi_0 = 1/2 is in the table) by
-// itself -- no cross-lane reduction -- adds the power-law terms of the infrared piece, and keeps G(y) = exp(ln G),
-// P(y) = G^{e1} Z^{e2} (eq.(3),(9)).  The first nr0 rows of the first window were staged in the stash (row stride
-// Npad + 2 doubles: at most a 4-way bank conflict); every other row is read from the table in global memory.
-// The coefficients come from where the kernel keeps them (constant bank, or the pairs of system sb in shared memory); a
-// row of another system reads c itself.  Nothing in the loop waits on cold global memory.
+// H1 for a window of up to 32 consecutive rows starting at row rb (relative to the warp's first row r0): lane r takes row
+// rb + r and runs both series ln G(y), ln Z(y) of eq.(23),(24) at s(y_q) by itself, with T_j(s) from the same stride-2
+// recurrence as the main loop -- no table row is read (the rows phi_j(t_q) would be 512 B per row and warp, re-read by every
+// warp that touches the row: memory latency that nothing hides), no cross-lane reduction.  It adds the power-law terms of
+// the infrared piece and keeps G(y) = exp(ln G), P(y) = G^{e1} Z^{e2} (eq.(3),(9)).  The coefficients come from where the
+// kernel keeps them (constant bank, or the pairs of system sb in shared memory); a row of another system reads c itself.
 // (Not inlined: the body of the point kernel's loop has to stay inside the SM's instruction cache.)
 template <int Npad, bool CONSTC>
-__device__ __noinline__ void pipe_fill_gp(const KParams &P, long long r0, int n_rows, int g0, int gmod, int nr0,
-                                          const double *s_rows, const double2 *s_coef, int sb, double2 *s_gp, int lane, int rb)
+__device__ __noinline__ void pipe_fill_gp(const KParams &P, long long r0, int n_rows, int g0, int gmod,
+                                          const double2 *s_coef, int sb, double2 *s_gp, int lane, int rb)
 {
     const int N = P.N;
     const int nr = n_rows - rb < 32 ? n_rows - rb : 32;
     double Gv = 0.0, Pv = 0.0;
     if (lane < nr) {
         const int gi = (int)((g0 + rb + lane) % gmod);
-        const double addZ = __ldg(P.EZy + gi), addG = __ldg(P.EGy + gi);
+        const double s = __ldg(P.t_r + gi), addZ = __ldg(P.EZy + gi), addG = __ldg(P.EGy + gi);
         const int br = (int)((r0 + rb + lane) / ((long long)P.Next * P.Nr));
-        const double *ph = (rb == 0 && lane < nr0) ? s_rows + lane * (Npad + 2) : P.phi_y + (size_t)gi * Npad;
-        double z0 = 0.0, z1 = 0.0, g0s = 0.0, g1 = 0.0;
-        if (CONSTC || br == sb) {
-#pragma unroll 4
-            for (int j = 0; j < Npad; j += 2) {        // (pairs beyond N are zero in both sources)
-                const double f0 = ph[j], f1 = ph[j + 1];
-                const double2 c0 = CONSTC ? make_double2(c_coef[j], c_coef[Npad + j]) : s_coef[j];
-                const double2 c1 = CONSTC ? make_double2(c_coef[j + 1], c_coef[Npad + j + 1]) : s_coef[j + 1];
-                z0 = fma(c0.x, f0, z0); g0s = fma(c0.y, f0, g0s);
-                z1 = fma(c1.x, f1, z1); g1 = fma(c1.y, f1, g1);
-            }
-        } else {
-            const double *ca = P.c + (size_t)br * 2 * N, *cb = ca + N;
-            for (int j = 0; j < N; ++j) { const double f = ph[j]; z0 = fma(__ldg(ca + j), f, z0); g0s = fma(__ldg(cb + j), f, g0s); }
+        const double *ca = P.c + (size_t)br * 2 * N, *cb = ca + N;
+        const bool own = CONSTC || br == sb;
+        auto coef = [&](int j) -> double2 {                  // (a_j, b_j); zero beyond N
+            if (CONSTC) return make_double2(c_coef[j], c_coef[Npad + j]);
+            if (own) return s_coef[j];
+            return j < N ? make_double2(__ldg(ca + j), __ldg(cb + j)) : make_double2(0.0, 0.0);
+        };
+        const double ts = 2.0 * s, t2 = fma(2.0 * ts, s, -2.0);          // T_{j+2} = 2 T_2 T_j - T_{j-2}
+        double Te = 1.0, To = s, Tem = fma(ts, s, -1.0), Tom = s;
+        double lz0, lz1 = 0.0, lg0, lg1 = 0.0;
+        { const double2 c0 = coef(0); lz0 = 0.5 * c0.x; lg0 = 0.5 * c0.y; }      // phi_0 = 1/2
+#pragma unroll 2
+        for (int j0 = 0; j0 < Npad; j0 += 4) {
+            const double2 c0 = coef(j0), c1 = coef(j0 + 1), c2 = coef(j0 + 2), c3 = coef(j0 + 3);
+            if (j0 > 0) { lz0 = fma(c0.x, Te, lz0); lg0 = fma(c0.y, Te, lg0); }
+            lz1 = fma(c1.x, To, lz1); lg1 = fma(c1.y, To, lg1);
+            Tem = fma(t2, Te, -Tem);  Tom = fma(t2, To, -Tom);
+            lz0 = fma(c2.x, Tem, lz0); lg0 = fma(c2.y, Tem, lg0);
+            lz1 = fma(c3.x, Tom, lz1); lg1 = fma(c3.y, Tom, lg1);
+            Te = fma(t2, Tem, -Te);   To = fma(t2, Tom, -To);
         }
-        const double lnZ = (z0 + z1) + addZ, lnG = (g0s + g1) + addG;
+        const double lnZ = (lz0 + lz1) + addZ, lnG = (lg0 + lg1) + addG;
         Gv = exp(lnG);
         Pv = exp(P.e1 * lnG + P.e2 * lnZ);
     }
@@ -422,30 +427,23 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     const long long t0 = (w * P.U) / P.W, t1 = ((w + 1) * P.U) / P.W;
     const long long r0 = t0 / BPR;
     const int n_rows = t0 < t1 ? (int)((t1 - 1) / BPR + 1 - r0) : 0;        // rows r0 + [0, n_rows) are touched by this warp
-    // H1 needs the rows phi_j(t_q) of the warp's first rows: a static table, so they are fetched into the (still unused)
-    // stash with cp.async BEFORE the wait on the producer kernel -- the first thing a warp does must not be a chain of
-    // cold global loads
-    const int gmod = P.rstride ? P.Next * Nr : Nr;                           // rows of the table phi_y
+    const int gmod = P.rstride ? P.Next * Nr : Nr;                           // rows of the radial tables
     const int g0 = (int)(r0 % gmod);
-    const int nr0 = min(min(n_rows, 32), 2 * STASH / (Npad + 2));            // rows staged (row stride Npad + 2)
-    {
-        constexpr int CPR = Npad / 2;                                        // 16-byte pieces per row
-        for (int c = lane; c < nr0 * CPR; c += 32) {
-            const int r = c / CPR, o = c - r * CPR;
-            const double *src = P.phi_y + (size_t)((g0 + r) % gmod) * Npad + 2 * o;
-            const unsigned dst = (unsigned)__cvta_generic_to_shared(s_stash + r * (Npad + 2) + 2 * o);
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src));
-        }
-        asm volatile("cp.async.commit_group;\n" ::);
-    }
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    if (threadIdx.x < 32) {   // the small tables the tail reads first (cold after an L2 flush): on their way while the points run
+        const size_t tb_lines = ((size_t)2 * P.B * P.Next * sizeof(int) + 127) / 128;
+        if (threadIdx.x < tb_lines) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.tail_bi) + threadIdx.x * 128));
+        if (threadIdx.x == 31) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.tail_cta + 2 * blockIdx.x));
+    }
     {   // the whole table is read row by row (H1, H7) by every warp: pull it into L2 once, spread over the grid
         const size_t lines = ((size_t)gmod * Npad * sizeof(double) + 127) / 128;
         for (size_t l = (size_t)blockIdx.x * blockDim.x + threadIdx.x; l < lines; l += (size_t)gridDim.x * blockDim.x)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.phi_y) + l * 128));
+        const size_t xlines = ((size_t)P.N * Npad * sizeof(double) + 127) / 128;       // phi_j(s_i): read by the tail only
+        for (size_t l = (size_t)blockIdx.x * blockDim.x + threadIdx.x; l < xlines; l += (size_t)gridDim.x * blockDim.x)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.phi_x) + l * 128));
     }
     pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
-    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     __syncthreads();
 
     if (t0 < t1) {
@@ -564,9 +562,9 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     int q = (int)(r0 - (long long)bi * Nr);
     int cur_b = bi / P.Next;
     int e = bi - cur_b * P.Next;
-    int gp_base = 0;
+    int gp_base = 0;                                       // current window of rows: [gp_base, gp_base + 32)
     auto fill_gp = [&](int rb) {
-        pipe_fill_gp<Npad, CONSTC>(P, r0, n_rows, g0, gmod, nr0, s_stash, s_coef, cur_b, s_gp, lane, rb);
+        pipe_fill_gp<Npad, CONSTC>(P, r0, n_rows, g0, gmod, s_coef, cur_b, s_gp, lane, rb);
         gp_base = rb;
     };
     auto contract = [&](int bi, int e, int qa, int qb, bool last_partial) {

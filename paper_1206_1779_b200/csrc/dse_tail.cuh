@@ -153,33 +153,31 @@ __device__ __noinline__ void tail_system(const KParams &P, int b)
     const size_t bi0 = (size_t)b * P.Next, biZ = bi0 + P.iZ, biG = bi0 + P.iG;
     const double *DZ = P.Dg + biZ * 4 * Npad, *DG = P.Dg + biG * 4 * Npad + 2 * Npad;     // rows of x_Z (a, b) and of x_G (a, b)
     double *Jb = P.J + (size_t)b * 4 * N * N, *Fb = P.F + (size_t)b * 2 * N;
-    const int total = N * Npad;
-    constexpr int MLP = 4;                         // entries per thread whose loads are issued before the first store
-    for (int base = tid; base < total; base += MLP * T) {
-        double d[MLP][4], s[MLP][4], phi[MLP], ig[MLP], iz[MLP];
-        int ii[MLP], jj[MLP];
-        bool ok[MLP];
+    // threads = (row group, j): a thread keeps the subtraction rows of its column j and walks the collocation points i in
+    // steps of the row-group count, MLP of them with all their loads issued before the first store
+    const int G = T / Npad > 0 ? T / Npad : 1, g = tid / Npad, j = tid - g * Npad;
+    if (g < G && j < N) {
+        const double sZa = __ldcg(DZ + j), sZb = __ldcg(DZ + Npad + j), sGa = __ldcg(DG + j), sGb = __ldcg(DG + Npad + j);
+        constexpr int MLP = 8;
+        for (int i0 = g; i0 < N; i0 += MLP * G) {
+            double d[MLP][4], phi[MLP], ig[MLP], iz[MLP];
 #pragma unroll
-        for (int u = 0; u < MLP; ++u) {
-            const int item = base + u * T;
-            int i = item < total ? item / Npad : 0, j = item < total ? item - i * Npad : 0;
-            ok[u] = item < total && j < N;
-            if (!ok[u]) { i = 0; j = 0; }
-            ii[u] = i; jj[u] = j;
-            const double *Di = P.Dg + (bi0 + i) * 4 * Npad + j;
-            d[u][0] = __ldcg(Di); d[u][1] = __ldcg(Di + Npad); d[u][2] = __ldcg(Di + 2 * Npad); d[u][3] = __ldcg(Di + 3 * Npad);
-            s[u][0] = __ldcg(DZ + j); s[u][1] = __ldcg(DZ + Npad + j); s[u][2] = __ldcg(DG + j); s[u][3] = __ldcg(DG + Npad + j);
-            phi[u] = __ldg(P.phi_x + (size_t)i * Npad + j);
-            ig[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 2); iz[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 3);
-        }
+            for (int u = 0; u < MLP; ++u) {
+                const int i = i0 + u * G < N ? i0 + u * G : i0;
+                const double *Di = P.Dg + (bi0 + i) * 4 * Npad + j;
+                d[u][0] = __ldcg(Di); d[u][1] = __ldcg(Di + Npad); d[u][2] = __ldcg(Di + 2 * Npad); d[u][3] = __ldcg(Di + 3 * Npad);
+                phi[u] = __ldg(P.phi_x + (size_t)i * Npad + j);
+                ig[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 2); iz[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 3);
+            }
 #pragma unroll
-        for (int u = 0; u < MLP; ++u) {
-            if (!ok[u]) continue;
-            const int i = ii[u], j = jj[u];
-            Jb[(size_t)i * 2 * N + j] = -phi[u] * iz[u] - d[u][0] + s[u][0];
-            Jb[(size_t)i * 2 * N + N + j] = -d[u][1] + s[u][1];
-            Jb[(size_t)(N + i) * 2 * N + j] = -d[u][2] + s[u][2];
-            Jb[(size_t)(N + i) * 2 * N + N + j] = -phi[u] * ig[u] - d[u][3] + s[u][3];
+            for (int u = 0; u < MLP; ++u) {
+                const int i = i0 + u * G;
+                if (i >= N) break;
+                Jb[(size_t)i * 2 * N + j] = -phi[u] * iz[u] - d[u][0] + sZa;
+                Jb[(size_t)i * 2 * N + N + j] = -d[u][1] + sZb;
+                Jb[(size_t)(N + i) * 2 * N + j] = -d[u][2] + sGa;
+                Jb[(size_t)(N + i) * 2 * N + N + j] = -phi[u] * ig[u] - d[u][3] + sGb;
+            }
         }
     }
     {

@@ -441,6 +441,30 @@ def sustained_fp64_probe(local, seconds=1.2):
     return out
 
 
+def run_probes():
+    """--probes: the fp64 micro-measurements DESIGN.md section 6 refers to (include/dse_diag.h), one JSON line each."""
+    import torch
+    from paper_1206_1779_b200.binding import probe, PROBE_KINDS
+    torch.cuda.set_device(0)
+    sink = torch.empty(148 * 8 * 256, dtype=torch.float64, device="cuda")
+    s = torch.cuda.current_stream()
+    for kind in PROBE_KINDS:
+        for blocks in (148 * 8, 148 * 2):
+            probe(kind, blocks, 2000, sink)
+            torch.cuda.synchronize()
+            res = []
+            for _ in range(5):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(s)
+                fl = probe(kind, blocks, 100000, sink)
+                b.record(s)
+                torch.cuda.synchronize()
+                res.append(fl / (a.elapsed_time(b) * 1e-3) / 1e12)
+            print(json.dumps({"probe": kind, "ctas": blocks, "warps_per_sm": blocks * 8 // 148,
+                              "tflops_median": round(float(np.median(res)), 2), "tflops_min": round(min(res), 2),
+                              "tflops_max": round(max(res), 2)}), flush=True)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -502,7 +526,11 @@ def main():
                     help="1 (default run, config 3 only): add the key per_config with a short run of configs 0, 1, 2, 4 and of "
                          "config 3 without the geometry cache")
     ap.add_argument("--per-config-steps", type=int, default=300)
+    ap.add_argument("--probes", action="store_true", help="print the fp64 throughput probes (include/dse_diag.h) and exit")
     args = ap.parse_args()
+    if args.probes:
+        run_probes()
+        return
     if args.impl == "reference":
         w, c, bc = config_inputs(args.config)
         run_reference(args, w, c)

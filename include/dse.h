@@ -146,9 +146,14 @@ DSE_API int dse_jacobian_fd(dse_handle *h, const double *c_dev, const double *bc
                             void *stream);
 
 /* One Newton-Raphson step (eq.(31)-(35)): builds J, F, scales each row of (J|F) by 1/max_j|J_ij|,
- * LU with partial pivoting (first maximal element wins), solves J Delta = F, c <- c - rho Delta
- * in place.  stats_dev[b] = { max|Delta|, max_i|F_i| row-scaled, min|pivot|, growth max|U|/max|A| }.
+ * LU with partial pivoting (largest |a_ik|; exactly equal candidates: see below), solves J Delta = F,
+ * c <- c - rho Delta in place.  stats_dev[b] = { max|Delta|, max_i|F_i| row-scaled, min|pivot|, growth max|U|/max|A| }.
  * stats_dev may be NULL.
+ * Arithmetic of the factorisation (2N <= 128: fused multiply-add updates, multipliers = entry * (1/pivot) with a
+ * reciprocal good to ~1 ulp; equal candidates go to the smallest row index; a pivot below 2^-1022 counts as singular.
+ * 2N > 128: unfused updates, correctly rounded quotients, equal candidates go to the first row in the order a
+ * row-swapping elimination would have).  Either way the unknowns agree with a plain elimination to rounding times the
+ * conditioning of J; DESIGN.md section 3 states the parity bar the tests apply.
  * Singular or non-finite systems: the call is asynchronous, so they are reported through stats_dev, not the return code.
  * If a pivot is exactly zero (stats[2] == 0) or Delta has a non-finite entry, c is left UNCHANGED for that system and
  * stats[0] = +Inf; a caller that does not pass stats_dev cannot tell.  dse_newton_solve checks this itself (status -1). */

@@ -7,6 +7,21 @@ pytestmark = pytest.mark.gpu
 from test_gpu_parity import oracle_params, _torch   # noqa: E402
 
 
+def check_lu_stats(st, so, ties=False, ctx=None):
+    """Parity bar of the one-CTA LU (2N <= 128): it fuses its updates and multiplies by a reciprocal, so it
+    is NOT bit-identical to the plain C elimination.  The equilibration is the same arithmetic: max|F| scaled agrees
+    exactly.  Without ties in the pivot search the pivot sequence is the oracle's, hence the smallest pivot and the growth
+    factor agree to rounding: |d pmin| <= 1e-9 pmin + 1e-12 max|U| (scaled units: max|A| = 1, so max|U| = growth) and
+    growth to 1e-11 relative.  With exact ties in the search (small-integer matrices) rounding may order two equal
+    candidates differently on the two sides: then only sanity is asserted here and the unknowns carry the parity."""
+    assert st[1] == so[1], (ctx, st, so)
+    if ties:
+        assert st[2] > 0.0 and st[3] >= 1.0 - 1e-12, (ctx, st, so)
+        return
+    assert abs(st[2] - so[2]) <= 1e-9 * so[2] + 1e-12 * so[3], (ctx, st, so)
+    assert abs(st[3] - so[3]) <= 1e-11 * so[3], (ctx, st, so)
+
+
 def test_lu_solve_matches_oracle(orc):
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
@@ -22,11 +37,9 @@ def test_lu_solve_matches_oracle(orc):
             xo, so, rc = orc.lu_solve(A[s], b[s])
             assert rc == 0
             assert np.allclose(x[s], xo, rtol=1e-9, atol=1e-13 * np.abs(xo).max())
-            assert np.allclose(st[s], so, rtol=1e-9)
-            # the factorisation itself (scaling, pivot choice, multipliers, unfused updates) is bit-identical to the
-            # plain C elimination: max|F| scaled, smallest pivot and growth factor agree exactly
-            assert np.array_equal(st[s][1:], so[1:]), (n, st[s], so)
-    # frequent ties in the pivot search (small integer entries): the first maximal element must win, as in the plain loop
+            assert abs(st[s][0] - so[0]) <= 1e-9 * so[0]
+            check_lu_stats(st[s], so, ctx=n)
+    # frequent ties in the pivot search (small integer entries): any maximal element is a valid pivot
     for n in (24, 64, 100):
         A = rng.integers(-3, 4, size=(2, n, n)).astype(np.float64) + 7.0 * np.eye(n)
         b = rng.integers(-5, 6, size=(2, n)).astype(np.float64)
@@ -36,7 +49,7 @@ def test_lu_solve_matches_oracle(orc):
             xo, so, rc = orc.lu_solve(A[s], b[s])
             assert rc == 0
             assert np.allclose(x[s], xo, rtol=1e-9, atol=1e-13 * np.abs(xo).max())
-            assert np.array_equal(st[s][1:], so[1:]), (n, st[s], so)
+            check_lu_stats(st[s], so, ties=True, ctx=n)
     d.close()
 
 
@@ -123,9 +136,9 @@ def test_finite_difference_self_check_mode(orc):
     d.close()
 
 
-def test_lu_random_sizes_exact_factorisation(orc):
-    """Random sizes, scalings, tie-rich and singular matrices: solution within conditioning, scaling / smallest pivot /
-    growth factor bit-identical to the plain C elimination (both LU kernels: registers for n <= 128, blocked above)."""
+def test_lu_random_sizes(orc):
+    """Random sizes, scalings, tie-rich and singular matrices through the one-CTA panel LU (every padded size 32, 64, 96,
+    128, ragged last panels): solution within conditioning, statistics at the bar of check_lu_stats."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
     from workloads import CONFIGS
@@ -151,7 +164,7 @@ def test_lu_random_sizes_exact_factorisation(orc):
             xo, so, rc = orc.lu_solve(A[s], b[s])
             if rc == 0:
                 assert np.allclose(x[s], xo, rtol=1e-7, atol=1e-10 * np.abs(xo).max()), (n, kind)
-                assert np.array_equal(st[s][1:], so[1:]), (n, kind, st[s], so)
+                check_lu_stats(st[s], so, ties=kind == 2, ctx=(n, kind))
             else:      # exactly singular: min |pivot| == 0 on both sides, and the library flags it with |Delta|_inf = +Inf
                 assert np.array_equal(st[s][1:3], so[1:3]) and so[2] == 0.0 and np.isinf(st[s][0]), (n, kind, st[s], so)
     d.close()
@@ -183,7 +196,8 @@ def test_newton_steps_batched_systems(orc):
 @pytest.mark.parametrize("N", [65, 80, 96, 128])
 def test_lu_cluster_path_exact_factorisation(orc, N):
     """128 < 2N <= 256: the register-resident LU over a cluster of 4 CTAs (distributed shared memory, split cluster
-    barrier).  Same bar as the single-CTA kernel: solution within conditioning, factorisation bit-identical."""
+    barrier).  This kernel keeps unfused updates and correctly rounded quotients: solution within conditioning,
+    factorisation bit-identical to the plain C elimination (also with ties: it tracks the textbook row positions)."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
     from workloads import Workload
@@ -334,9 +348,10 @@ def test_newton_solve_graph_large_system_cluster_lu(orc):
     d.close()
 
 
-def test_lu_extreme_exponents_take_the_library_division(orc):
-    """Entries far outside 2^+-500 after equilibration (columns scaled by 1e-200 / 1e+180): the multipliers come from the
-    library division on the lanes that need it; factorisation still bit-identical to the plain C elimination."""
+def test_lu_extreme_exponents(orc):
+    """Entries far outside 2^+-500 after equilibration (columns scaled by 1e-200 / 1e-180, a 1e150 row): the reciprocal of
+    the pivot stays in range (normal pivots down to 2^-1022) and the factorisation stays at the bar of check_lu_stats
+    (the smallest pivot, ~1e-200, to 1e-9 RELATIVE)."""
     torch = _torch()
     from paper_1206_1779_b200 import Dse, params_from_workload
     from workloads import CONFIGS
@@ -352,6 +367,6 @@ def test_lu_extreme_exponents_take_the_library_division(orc):
         x = x.cpu().numpy(); st = st.cpu().numpy()
         for s in range(2):
             xo, so, rc = orc.lu_solve(A[s], b[s])
-            assert np.array_equal(st[s][1:], so[1:]), (n, st[s], so)
+            assert st[s][1] == so[1] and abs(st[s][2] - so[2]) <= 1e-9 * so[2] and abs(st[s][3] - so[3]) <= 1e-11 * so[3], (n, st[s], so)
             assert np.allclose(x[s], xo, rtol=1e-6, atol=0), n
     d.close()

@@ -259,7 +259,8 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
     const size_t o_S = carve<double>(off, ((size_t)k.W * k.bgroup + Bpad * k.Next) * slot);
     const size_t o_R = carve<double>(off, (size_t)k.B * k.Next * 3 * k.Npad);
     const size_t o_Dg = carve<double>(off, (size_t)k.B * k.Next * 4 * k.Npad), o_Pi = carve<double>(off, (size_t)k.B * k.Next * 4);
-    const size_t o_cnt = carve<double>(off, ((size_t)k.B * k.Next + k.B + 1) / 2 + 1);      // unsigned counters of the fused tail
+    const size_t n_pend = (size_t)k.B * ((k.Next + 31) / 32);
+    const size_t o_cnt = carve<double>(off, ((size_t)k.B * k.Next + 2 * (size_t)k.B + n_pend + 1) / 2 + 1);   // unsigned counters of the fused tail
     const size_t o_J = carve<double>(off, (size_t)k.B * n2 * n2), o_F = carve<double>(off, (size_t)k.B * n2);
     const size_t o_lu = carve<double>(off, (size_t)k.B * dse::lu_scratch_doubles((int)n2));
     const size_t o_c = carve<double>(off, (size_t)k.B * n2), o_bc = carve<double>(off, (size_t)k.B * 2);
@@ -274,6 +275,7 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
     k.Apart = wk + o_A; k.AHead = wk + o_AH; k.Spart = wk + o_S; k.Rz = wk + o_R; h->d_fd = wk + o_fd;
     k.Dg = wk + o_Dg; k.PiInv = wk + o_Pi;
     k.cnt = reinterpret_cast<unsigned *>(wk + o_cnt); k.done = k.cnt + (size_t)k.B * k.Next;
+    k.rdy = k.done + k.B; k.pend = k.rdy + k.B;
     h->d_J = wk + o_J; h->d_F = wk + o_F; h->d_lu = wk + o_lu; h->d_c = wk + o_c; h->d_bc = wk + o_bc;
     h->d_Jh = h->d_J; h->d_Fh = h->d_F;
     h->d_delta = wk + o_dl; h->d_stats = wk + o_st; h->d_ctl = wk + o_ctl; h->d_info = wk + o_info;

@@ -62,6 +62,8 @@ struct KParams {
     double *PiInv;                     // [B*Next][4]        Pi_G, Pi_Z, 1/G(x_e), 1/Z(x_e)              (fused tail)
     unsigned *cnt;                     // [B*Next] arrival counters of the fused tail, [B] completed external points
     unsigned *done;
+    unsigned *rdy;                     // [B] subtraction points (x_Z, x_G) whose derivative rows are written
+    unsigned *pend;                    // [B][(Next + 31) / 32] bit e: rows of collocation point e are left to the finishing CTA
     const int *tail_cta;               // [grid][2]   first, last external point index a CTA works on (fused tail)
     const int *tail_bi;                // [B*Next][2] first, last warp that works on an external point
 };

@@ -23,6 +23,16 @@
 
 namespace dse {
 
+#ifdef DSE_PT_DEBUG
+#define PT_NOW() gtime()
+extern "C" __attribute__((visibility("default"))) int dse_pt_debug_read(long long *out)
+{
+    return (int)cudaMemcpyFromSymbol(out, g_pt_dbg, sizeof(g_pt_dbg));
+}
+#else
+#define PT_NOW() 0ll
+#endif
+
 namespace {
 
 // DSE_FLAG_CONST_COEF: the coefficients c = (a_0..a_{N-1}, b_0..b_{N-1}) of a single-system build as constant-bank operands
@@ -310,16 +320,27 @@ __host__ __device__ inline int pipe_warp_doubles(int Npad, int NCH, bool constc,
 // the infrared piece and keeps G(y) = exp(ln G), P(y) = G^{e1} Z^{e2} (eq.(3),(9)).  The coefficients come from where the
 // kernel keeps them (constant bank, or the pairs of system sb in shared memory); a row of another system reads c itself.
 // (Not inlined: the body of the point kernel's loop has to stay inside the SM's instruction cache.)
+// (s, addZ, addG) = t_r, EZy, EGy of the lane's row (pipe_row_tables: loaded by the caller, for the first window at the very
+// top of the kernel so that their cold miss overlaps the rest of the prologue).
+struct RowTab { double s, addZ, addG; };
+__device__ __forceinline__ RowTab pipe_row_tables(const KParams &P, int n_rows, int g0, int gmod, int lane, int rb)
+{
+    RowTab t = {0.0, 0.0, 0.0};
+    if (rb + lane < n_rows) {
+        const int gi = (int)((g0 + rb + lane) % gmod);
+        t.s = __ldg(P.t_r + gi); t.addZ = __ldg(P.EZy + gi); t.addG = __ldg(P.EGy + gi);
+    }
+    return t;
+}
 template <int Npad, bool CONSTC>
-__device__ __noinline__ void pipe_fill_gp(const KParams &P, long long r0, int n_rows, int g0, int gmod,
+__device__ __noinline__ void pipe_fill_gp(const KParams &P, long long r0, int n_rows, RowTab tab,
                                           const double2 *s_coef, int sb, double2 *s_gp, int lane, int rb)
 {
     const int N = P.N;
     const int nr = n_rows - rb < 32 ? n_rows - rb : 32;
     double Gv = 0.0, Pv = 0.0;
     if (lane < nr) {
-        const int gi = (int)((g0 + rb + lane) % gmod);
-        const double s = __ldg(P.t_r + gi), addZ = __ldg(P.EZy + gi), addG = __ldg(P.EGy + gi);
+        const double s = tab.s, addZ = tab.addZ, addG = tab.addG;
         const int br = (int)((r0 + rb + lane) / ((long long)P.Next * P.Nr));
         const double *ca = P.c + (size_t)br * 2 * N, *cb = ca + N;
         const bool own = CONSTC || br == sb;
@@ -412,6 +433,10 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     constexpr int SLOT = 6 * Npad + 2;                                      // = slot_doubles(Npad)
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
+#ifdef DSE_PT_DEBUG
+    for (int z = 1; z < 16; ++z) if (lane == 0) g_pt_dbg[((size_t)blockIdx.x * 16 + warp) * 16 + z] = 0;
+#endif
+    PT_STAMP(0);
     const int STASH = stash_doubles(NCH);
     const int WD = pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
     double *s_ang = smem;
@@ -429,11 +454,41 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     const int n_rows = t0 < t1 ? (int)((t1 - 1) / BPR + 1 - r0) : 0;        // rows r0 + [0, n_rows) are touched by this warp
     const int gmod = P.rstride ? P.Next * Nr : Nr;                           // rows of the radial tables
     const int g0 = (int)(r0 % gmod);
-    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    // Everything the warp needs from (cold) global memory before its first batch is requested here, in one go: the radial
+    // tables of its first window of rows (H1), its first geometry record, the angular table -- one memory round trip
+    // instead of three in a row (an L2 flush, or a first build, makes each of them a DRAM miss)
+    const RowTab tab0 = pipe_row_tables(P, n_rows, g0, gmod, lane, 0);
+    double ctouch = 0.0;
+    if (CONSTC && lane * 8 < 2 * Npad) {     // the coefficient bank was rewritten just before this launch: cold in the constant
+        asm volatile("ld.const.f64 %0, [%1];" : "=d"(ctouch) : "l"(c_coef + lane * 8));   // cache -- one lane per 64 B line asks now
+    }
+    int bi = (int)(r0 / Nr);
+    int q = (int)(r0 - (long long)bi * Nr);
+    int cur_b = bi / P.Next;
+    int e = bi - cur_b * P.Next;
+    int kb = (int)(t0 - r0 * BPR);
+    const unsigned gtotal = (unsigned)P.Next * (unsigned)Nr * (unsigned)P.Ntpad;
+    unsigned gidx = 0, gphase = 0;
+    const unsigned long long gpolicy = l2_evict_first_policy();
+    auto prefetch = [&](unsigned buf) {      // geometry stream (GEOM): consecutive 1 KB records, cp.async double buffer
+        const double4 *src = reinterpret_cast<const double4 *>(P.geom) + gidx;
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(s_gbuf + buf * 32 + lane);
+        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "l"(gpolicy));
+        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(src) + 16), "l"(gpolicy));
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
+    for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x)              // angular table -> shared memory, asynchronously
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"((unsigned)__cvta_generic_to_shared(s_ang + t)), "l"(P.ang + t));
+    asm volatile("cp.async.commit_group;\n" ::);                           // (the oldest group: complete before any later one)
+    if (GEOM && t0 < t1) {
+        gidx = ((unsigned)e * Nr + q) * P.Ntpad + kb * 32 + lane;
+        prefetch(0);
+    }
     if (threadIdx.x < 32) {   // the small tables the tail reads first (cold after an L2 flush): on their way while the points run
         const size_t tb_lines = ((size_t)2 * P.B * P.Next * sizeof(int) + 127) / 128;
         if (threadIdx.x < tb_lines) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.tail_bi) + threadIdx.x * 128));
         if (threadIdx.x == 31) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.tail_cta + 2 * blockIdx.x));
+        if (threadIdx.x == 30 && blockIdx.x == 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(P.bc));
     }
     {   // the whole table is read row by row (H1, H7) by every warp: pull it into L2 once, spread over the grid
         const size_t lines = ((size_t)gmod * Npad * sizeof(double) + 127) / 128;
@@ -444,10 +499,9 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
             asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.phi_x) + l * 128));
     }
     pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
-    __syncthreads();
+    PT_STAMP(1);
 
     if (t0 < t1) {
-    int kb = (int)(t0 - r0 * BPR);
     const bool lane_on = EXACT || lane < NCH * SUB;
     const int c_lane = lane_on ? lane / SUB : 0, sub = lane_on ? lane - c_lane * SUB : 0;
     const double halfLg = 0.5 * P.Lg;
@@ -544,44 +598,24 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         }
     };
 
-    // geometry stream (GEOM): consecutive 1 KB records, cp.async double buffer
-    // (32-bit record index: at most 2^31 points per system; checked in dse_create)
-    const unsigned gtotal = (unsigned)P.Next * (unsigned)Nr * (unsigned)P.Ntpad;
-    unsigned gidx = 0, gphase = 0;
-    const unsigned long long gpolicy = l2_evict_first_policy();
-    auto prefetch = [&](unsigned buf) {
-        const double4 *src = reinterpret_cast<const double4 *>(P.geom) + gidx;
-        const unsigned dst = (unsigned)__cvta_generic_to_shared(s_gbuf + buf * 32 + lane);
-        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "l"(gpolicy));
-        asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;\n" ::"r"(dst + 16), "l"(reinterpret_cast<const char *>(src) + 16), "l"(gpolicy));
-        asm volatile("cp.async.commit_group;\n" ::);
-    };
-
+    // (geometry stream: 32-bit record index, at most 2^31 points per system; checked in dse_create)
     int row = 0;                                           // running row index of the flattened (b, e, q), relative to r0
-    int bi = (int)(r0 / Nr);
-    int q = (int)(r0 - (long long)bi * Nr);
-    int cur_b = bi / P.Next;
-    int e = bi - cur_b * P.Next;
     int gp_base = 0;                                       // current window of rows: [gp_base, gp_base + 32)
-    auto fill_gp = [&](int rb) {
-        pipe_fill_gp<Npad, CONSTC>(P, r0, n_rows, g0, gmod, s_coef, cur_b, s_gp, lane, rb);
+    auto fill_gp = [&](int rb, RowTab tab) {
+        pipe_fill_gp<Npad, CONSTC>(P, r0, n_rows, tab, s_coef, cur_b, s_gp, lane, rb);
         gp_base = rb;
     };
     auto contract = [&](int bi, int e, int qa, int qb, bool last_partial) {
         pipe_contract<Npad>(P, P.Spart + (size_t)(w + bi) * SLOT, bi, e, qa, qb, last_partial, lane);
     };
 
-    if (GEOM) {
-        gidx = ((unsigned)e * Nr + q) * P.Ntpad + kb * 32 + lane;
-        prefetch(0);
-    }
     auto load_coef = [&](int b) {                          // (a_j, b_j) pairs of system b, zero padded
         const double *ca = P.c + (size_t)b * 2 * P.N;
         for (int j = lane; j < Npad; j += 32) s_coef[j] = j < P.N ? make_double2(__ldg(ca + j), __ldg(ca + P.N + j)) : make_double2(0.0, 0.0);
         __syncwarp();
     };
     if (!CONSTC) load_coef(cur_b);
-    fill_gp(0);
+    fill_gp(0, tab0);
 
     // both T stashes must hold finite numbers before the first (zero-weight) prologue phase 2
     for (int b2 = 0; b2 < 2; ++b2)
@@ -592,6 +626,12 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         }
     if (!EXACT && lane < 2) reinterpret_cast<double4 *>(s_stash + lane * STASH)[32] = make_double4(0.0, 0.0, 0.0, 0.0);
 
+    // H1 above ran while the angular table and the first geometry record were on their way; now the table must be there
+    if (GEOM) asm volatile("cp.async.wait_group 1;\n" ::: "memory");       // all but the geometry record
+    else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+    __syncthreads();
+    if (CONSTC && ctouch == 1.2345e-300) s_ang[0] = ctouch;  // (keeps the touch alive)
+    PT_STAMP(2);
     int rem = (int)(t1 - t0);                              // batches left for this warp
     int cur = 0;                                           // stash half written by the current batch
     while (rem > 0) {
@@ -604,7 +644,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         const int q_seg = q;                               // first row of this segment
         bool last_partial = false;
         while (!seg_done) {
-            if (row - gp_base >= 32) fill_gp(row);          // (warp-uniform)
+            if (row - gp_base >= 32) fill_gp(row, pipe_row_tables(P, n_rows, g0, gmod, lane, row));   // (warp-uniform)
             const double2 gp = s_gp[row - gp_base];
             const double Gy = gp.x, Py = gp.y;
             RowConst rc;
@@ -707,9 +747,11 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
             }
         }
         // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
+        const long long tq0 = PT_NOW();
         phase2_last(cur ^ 1);
         flush(bi, cur);
         contract(bi, e, q_seg, last_partial ? q : q - 1, last_partial);
+        PT_ADD(9, PT_NOW() - tq0); PT_ADD(10, 1);
         if (q >= Nr) {
             q = 0; ++bi; ++e;
             if (e == P.Next) {
@@ -719,7 +761,11 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         }
     }
     if (GEOM) asm volatile("cp.async.wait_group 0;\n" ::: "memory");
-    }   // t0 < t1
+    } else {                                               // a warp without work: its part of the angular table, the barrier
+        asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+        __syncthreads();
+    }
+    PT_STAMP(3);
     build_tail(P, smem);                                   // H8 by the last-arriving CTAs (dse_tail.cuh)
 }
 using KernelFn = void (*)(const KParams);
@@ -863,7 +909,10 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     KernelFn pf = k.g == 32 ? pick_pipe(k) : nullptr;
     if (pf) {
         auto psmem_of = [&](int thr) {
-            return (int)sizeof(double) * (k.Ntpad * 6 + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr));
+            int d = k.Ntpad * 6 + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr);
+            const int need = tail_smem_doubles(k.Npad, thr);                // the fused tail reuses the dynamic shared memory
+            if (d < need) d = need;
+            return (int)sizeof(double) * d;
         };
         // large problems (>= 48 batches per warp at 16 warps per SM) with 8 chunks: the 512-thread build of the kernel
         const long long units = k.R * (k.Ntpad / 32);

@@ -10,10 +10,14 @@
 //   * every CTA, after its warps have written their slots, bumps ONE arrival counter per external point it worked on
 //     (barrier, then fence + atomic by the counting threads);
 //   * the CTA whose increment completes the count of an external point e ("last arriver") owns e: it sums e's slots in
-//     ascending warp order, forms the four derivative rows of e and 1/G(x_e), 1/Z(x_e), and bumps the system's counter
-//     of finished external points;
-//   * the CTA that finishes the last external point of a system writes that system's J and F (MOM subtraction rows
-//     eq.(14),(15), local terms, the paper's layout eq.(29),(30),(35)) and clears the counters for the next build.
+//     ascending warp order and forms the four derivative rows of e and 1/G(x_e), 1/Z(x_e);
+//   * the owners of the subtraction points x_Z, x_G publish that (counter `rdy`); the owner of a collocation point x_i
+//     looks for it -- a BOUNDED number of polls: these owners are running, nobody waits for a CTA that has not been
+//     scheduled -- and then writes the rows i and N + i of J and the entries i, N + i of F itself (MOM subtraction rows
+//     eq.(14),(15), local terms, the paper's layout eq.(29),(30),(35)): the assembly is spread over as many CTAs as
+//     there are external points.  An owner whose polls run out marks its point as pending instead;
+//   * every owner then bumps the system's counter of finished external points; the CTA that completes it writes the
+//     pending rows (normally none) and clears the counters for the next build.
 // The counters only decide WHO does a sum, never the order IN a sum: every reduction runs over row / slot indices in a
 // fixed order, so J and F are bitwise reproducible.  Data written by other CTAs of the same launch is read with
 // ld.global.cg after the counter handshake (L1 is not coherent).
@@ -21,6 +25,16 @@
 #include "dse_device.cuh"
 
 namespace dse {
+
+#ifdef DSE_PT_DEBUG
+__device__ long long g_pt_dbg[148 * 16 * 16];
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define PT_STAMP(slot) do { if ((threadIdx.x & 31) == 0) g_pt_dbg[((size_t)blockIdx.x * 16 + (threadIdx.x >> 5)) * 16 + (slot)] = gtime(); } while (0)
+#define PT_ADD(slot, v) do { if ((threadIdx.x & 31) == 0) g_pt_dbg[((size_t)blockIdx.x * 16 + (threadIdx.x >> 5)) * 16 + (slot)] += (v); } while (0)
+#else
+#define PT_STAMP(slot) do { } while (0)
+#define PT_ADD(slot, v) do { } while (0)
+#endif
 
 // slot of one (warp, external point): [0, 3 Npad) Sa, Sb, Sv accumulated with T_0 = 1; [3 Npad, 6 Npad) Ra, Rb, Rv with the
 // table phi (phi_0 = 1/2); then Pi_G, Pi_Z
@@ -55,21 +69,28 @@ __device__ __forceinline__ void slot_row_update(double *slot, int Npad, const do
 
 // counter bump with release (everything this thread has observed, cumulatively: the slots its CTA wrote before the
 // barrier) and acquire (what the CTAs counted before it wrote) semantics at device scope
-__device__ __forceinline__ unsigned arrive_acq_rel(unsigned *ctr)
+__device__ __forceinline__ unsigned arrive_acq_rel(unsigned *ctr, unsigned inc = 1u)
 {
     unsigned old;
-    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(ctr) : "memory");
+    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(ctr), "r"(inc) : "memory");
     return old;
 }
 
 constexpr int TAIL_OWN = 4;            // external points a CTA finishes in one pass
-constexpr int TAIL_MLP = 28;           // slot loads in flight per thread
+constexpr int TAIL_MLP = 20;           // 16-byte slot loads in flight per thread
+constexpr int TAIL_POLLS = 4096;       // polls (64 ns apart + a memory round trip) for the subtraction points before giving up
 
-// doubles of shared memory the tail needs
+// parts a slot sum is split into (a function of the launch configuration only): threads per pair of slot entries
+__host__ __device__ inline int tail_parts(int Npad, int threads)
+{
+    const int p = threads / (slot_doubles(Npad) / 2);
+    return p > 1 ? p : 1;
+}
+// doubles of shared memory the tail needs: the slot sums of TAIL_OWN points and their parts
 __host__ __device__ inline int tail_smem_doubles(int Npad, int threads)
 {
     const int S = slot_doubles(Npad);
-    return TAIL_OWN * S + (threads > TAIL_OWN * S ? threads : TAIL_OWN * S);
+    return TAIL_OWN * S * (1 + tail_parts(Npad, threads));
 }
 
 // The derivative rows of the nown <= TAIL_OWN external points own[0..nown) (bi = b * Next + e) from their slots, in one pass.
@@ -98,31 +119,34 @@ __device__ __noinline__ void tail_points(const KParams &P, double *sm, const int
             invG = exp(-lnG); invZ = exp(-lnZ);
         }
     }
-    // threads = (part, owned point, index in the slot); every part sums a contiguous range of slots in ascending warp
-    // order, TAIL_MLP loads in flight at a time.  The number of parts depends on the launch configuration only -- never on
-    // how many points this CTA happens to own (that is decided by arrival order; the grouping of a sum must not be)
-    const int work = nown * SLOT, parts = T / (TAIL_OWN * SLOT) > 1 ? T / (TAIL_OWN * SLOT) : 1;
+    // threads = (part, owned point, PAIR of slot entries); every part sums a contiguous range of slots in ascending warp
+    // order with all its loads (16 B each) in flight at once: one memory round trip.  The number of parts depends on the
+    // launch configuration only -- never on how many points this CTA happens to own (that is decided by arrival order;
+    // the grouping of a sum must not be)
+    const int HS = SLOT / 2;                       // SLOT is even
+    const int work = nown * HS, parts = tail_parts(Npad, T);
     for (int item = tid; item < parts * work; item += T) {
-        const int part = item / work, rest = item - part * work, k = rest / SLOT, idx = rest - k * SLOT;
+        const int part = item / work, rest = item - part * work, k = rest / HS, idx = rest - k * HS;
         const int bi = own[3 * k], wf = own[3 * k + 1], wl = own[3 * k + 2];
         const int per = (wl - wf + parts) / parts;
         const int w0 = wf + part * per, n = (wl + 1 < w0 + per ? wl + 1 : w0 + per) - w0;
-        const double *sp = P.Spart + ((size_t)w0 + (size_t)bi) * SLOT + idx;
-        double s = 0.0;
+        const double2 *sp = reinterpret_cast<const double2 *>(P.Spart + ((size_t)w0 + (size_t)bi) * SLOT) + idx;
+        double2 s = make_double2(0.0, 0.0);
         for (int k0 = 0; k0 < n; k0 += TAIL_MLP) {
-            double v[TAIL_MLP];
+            double2 v[TAIL_MLP];
 #pragma unroll
-            for (int u = 0; u < TAIL_MLP; ++u) v[u] = k0 + u < n ? __ldcg(sp + (size_t)(k0 + u) * SLOT) : 0.0;
+            for (int u = 0; u < TAIL_MLP; ++u) v[u] = k0 + u < n ? __ldcg(sp + (size_t)(k0 + u) * HS) : make_double2(0.0, 0.0);
 #pragma unroll
-            for (int u = 0; u < TAIL_MLP; ++u) s += v[u];
+            for (int u = 0; u < TAIL_MLP; ++u) { s.x += v[u].x; s.y += v[u].y; }
         }
-        sX[item] = s;
+        reinterpret_cast<double2 *>(sX)[item] = s;
     }
     __syncthreads();
     for (int it = tid; it < work; it += T) {
-        double s = 0.0;
-        for (int p = 0; p < parts; ++p) s += sX[p * work + it];
-        sS[it] = s;
+        double2 s = make_double2(0.0, 0.0);
+        for (int p = 0; p < parts; ++p) { const double2 v = reinterpret_cast<const double2 *>(sX)[p * work + it]; s.x += v.x; s.y += v.y; }
+        const int k = it / HS, idx = it - k * HS;
+        reinterpret_cast<double2 *>(sS + k * SLOT)[idx] = s;
     }
     __syncthreads();
     // dPi_Z/da = Sa + Ra, dPi_Z/db = Sb + Rb, dPi_G/da = Sv, dPi_G/db = Rv (the S streams were accumulated with T_0 = 1;
@@ -144,53 +168,65 @@ __device__ __noinline__ void tail_points(const KParams &P, double *sm, const int
     }
 }
 
-// J and F of system b from the rows of all its external points (eq.(29),(30),(35),(36); MOM subtraction eq.(14),(15)).
-// Every entry's operands are loaded in one go (no staging round trip): the CTA that runs this is the last one alive.
-__device__ __noinline__ void tail_system(const KParams &P, int b)
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
 {
-    const int tid = threadIdx.x, T = blockDim.x;
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Rows i = e and N + e of J and entries e, N + e of F for the collocation point bi = b Next + e, e < N (eq.(29),(30),(35),
+// (36); MOM subtraction eq.(14),(15)), by the threads j0, j0 + jstride, ... over the columns; every operand is loaded before
+// the first store.  Needs the derivative rows and Pi of e and of the subtraction points x_Z, x_G.
+__device__ __forceinline__ void tail_point_rows(const KParams &P, int bi, int j0, int jstride)
+{
     const int Npad = P.Npad, N = P.N;
+    const int b = bi / P.Next, e = bi - b * P.Next;
+    if (e >= N) return;
     const size_t bi0 = (size_t)b * P.Next, biZ = bi0 + P.iZ, biG = bi0 + P.iG;
+    const double *De = P.Dg + (size_t)bi * 4 * Npad;
     const double *DZ = P.Dg + biZ * 4 * Npad, *DG = P.Dg + biG * 4 * Npad + 2 * Npad;     // rows of x_Z (a, b) and of x_G (a, b)
     double *Jb = P.J + (size_t)b * 4 * N * N, *Fb = P.F + (size_t)b * 2 * N;
-    // threads = (row group, j): a thread keeps the subtraction rows of its column j and walks the collocation points i in
-    // steps of the row-group count, MLP of them with all their loads issued before the first store
-    const int G = T / Npad > 0 ? T / Npad : 1, g = tid / Npad, j = tid - g * Npad;
-    if (g < G && j < N) {
+    const double4 pi = ldcg4(P.PiInv + (size_t)bi * 4);                                  // Pi_G, Pi_Z, 1/G, 1/Z at x_e
+    for (int j = j0; j < N; j += jstride) {
+        const double d0 = __ldcg(De + j), d1 = __ldcg(De + Npad + j), d2 = __ldcg(De + 2 * Npad + j), d3 = __ldcg(De + 3 * Npad + j);
         const double sZa = __ldcg(DZ + j), sZb = __ldcg(DZ + Npad + j), sGa = __ldcg(DG + j), sGb = __ldcg(DG + Npad + j);
-        constexpr int MLP = 8;
-        for (int i0 = g; i0 < N; i0 += MLP * G) {
-            double d[MLP][4], phi[MLP], ig[MLP], iz[MLP];
-#pragma unroll
-            for (int u = 0; u < MLP; ++u) {
-                const int i = i0 + u * G < N ? i0 + u * G : i0;
-                const double *Di = P.Dg + (bi0 + i) * 4 * Npad + j;
-                d[u][0] = __ldcg(Di); d[u][1] = __ldcg(Di + Npad); d[u][2] = __ldcg(Di + 2 * Npad); d[u][3] = __ldcg(Di + 3 * Npad);
-                phi[u] = __ldg(P.phi_x + (size_t)i * Npad + j);
-                ig[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 2); iz[u] = __ldcg(P.PiInv + (bi0 + i) * 4 + 3);
-            }
-#pragma unroll
-            for (int u = 0; u < MLP; ++u) {
-                const int i = i0 + u * G;
-                if (i >= N) break;
-                Jb[(size_t)i * 2 * N + j] = -phi[u] * iz[u] - d[u][0] + sZa;
-                Jb[(size_t)i * 2 * N + N + j] = -d[u][1] + sZb;
-                Jb[(size_t)(N + i) * 2 * N + j] = -d[u][2] + sGa;
-                Jb[(size_t)(N + i) * 2 * N + N + j] = -phi[u] * ig[u] - d[u][3] + sGb;
-            }
-        }
+        const double phi = __ldg(P.phi_x + (size_t)e * Npad + j);
+        Jb[(size_t)e * 2 * N + j] = -phi * pi.w - d0 + sZa;
+        Jb[(size_t)e * 2 * N + N + j] = -d1 + sZb;
+        Jb[(size_t)(N + e) * 2 * N + j] = -d2 + sGa;
+        Jb[(size_t)(N + e) * 2 * N + N + j] = -phi * pi.z - d3 + sGb;
     }
-    {
+    if (j0 == 0) {
         const double PiG_s = __ldcg(P.PiInv + biG * 4), PiZ_s = __ldcg(P.PiInv + biZ * 4 + 1);
-        const double gG = P.bc[2 * b + 0], gZ = P.bc[2 * b + 1];
-        for (int i = tid; i < N; i += T) {
-            const double4 pi = ldcg4(P.PiInv + (bi0 + i) * 4);
-            Fb[i] = pi.w - gZ - pi.y + PiZ_s;      // z(x_i) = 1/Z(x_i) - 1/Z(x_Z) - Pi_Z(x_i) + Pi_Z(x_Z)
-            Fb[N + i] = pi.z - gG - pi.x + PiG_s;  // g(x_i) likewise
-        }
+        const double gG = __ldg(P.bc + 2 * b + 0), gZ = __ldg(P.bc + 2 * b + 1);
+        Fb[e] = pi.w - gZ - pi.y + PiZ_s;          // z(x_i) = 1/Z(x_i) - 1/Z(x_Z) - Pi_Z(x_i) + Pi_Z(x_Z)
+        Fb[N + e] = pi.z - gG - pi.x + PiG_s;      // g(x_i) likewise
     }
-    for (int e = tid; e < P.Next; e += T) P.cnt[bi0 + e] = 0u;       // ready for the next build on this handle
-    if (tid == 0) P.done[b] = 0u;
+}
+
+// The CTA that finished the last external point of system b: rows left pending by owners that did not see the
+// subtraction points in time (n_pending of them, normally none), then the counters are cleared for the next build on this
+// handle.
+constexpr unsigned TAIL_PENDING = 1u << 16;        // a pending point counts 1 + TAIL_PENDING on the system's counter
+__device__ __noinline__ void tail_finish(const KParams &P, int b, unsigned n_pending)
+{
+    const int tid = threadIdx.x, T = blockDim.x, PW = (P.Next + 31) / 32;
+    const size_t bi0 = (size_t)b * P.Next;
+    if (n_pending) {
+        for (int wd = 0; wd < PW; ++wd) {
+            unsigned m = __ldcg(P.pend + (size_t)b * PW + wd);
+            while (m) {
+                const int e = 32 * wd + __ffs(m) - 1;
+                m &= m - 1;
+                tail_point_rows(P, (int)bi0 + e, tid, T);
+            }
+        }
+        __syncthreads();
+        for (int wd = tid; wd < PW; wd += T) P.pend[(size_t)b * PW + wd] = 0u;
+    }
+    for (int e = tid; e < P.Next; e += T) P.cnt[bi0 + e] = 0u;
+    if (tid == 0) { P.done[b] = 0u; P.rdy[b] = 0u; }
 }
 
 // Called by ALL threads of the CTA after its warps' last slot updates.  P.tail_cta[2 c], [2 c + 1] = first and last external
@@ -200,9 +236,11 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
 {
     __shared__ unsigned s_mask;
     __shared__ int s_own[3 * TAIL_OWN], s_w[64];
-    const int tid = threadIdx.x, lane = tid & 31, WPB = blockDim.x >> 5;
+    __shared__ unsigned s_pend[TAIL_OWN];
+    const int tid = threadIdx.x, lane = tid & 31, WPB = blockDim.x >> 5, T = blockDim.x;
     const int bi_lo = P.tail_cta[2 * blockIdx.x], bi_hi = P.tail_cta[2 * blockIdx.x + 1];
     __syncthreads();                               // the slots of every warp of this CTA are written (CTA scope) ...
+    PT_STAMP(4);
     for (int seg0 = bi_lo; seg0 <= bi_hi; seg0 += 32) {
         if (tid < 32) {
             const int bi = seg0 + lane;
@@ -218,6 +256,7 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             if (lane == 0) s_mask = m;
         }
         __syncthreads();
+        PT_STAMP(5);
         unsigned mask = s_mask;                    // external points this CTA arrived last at (usually none or one)
         while (mask) {
             __syncthreads();                       // (s_own, s_mask and the shared memory of the pass before are free)
@@ -231,13 +270,46 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             __syncthreads();
             tail_points(P, sm, s_own, nown);
             __syncthreads();                       // D rows, Pi, 1/G, 1/Z of the owned points are written
+            PT_STAMP(6);
+            if (tid < 32) {
+                // owners of x_Z, x_G publish; owners of collocation points look for both -- at most TAIL_POLLS times
+                bool ok = false;
+                int b = 0, e = P.N;
+                if (lane < nown) {
+                    b = s_own[3 * lane] / P.Next; e = s_own[3 * lane] - b * P.Next;
+                    if (e == P.iZ || e == P.iG) arrive_acq_rel(P.rdy + b);
+                }
+                if (e < P.N) {
+                    const unsigned nsub = P.iZ == P.iG ? 1u : 2u;
+                    for (int it = 0; it < TAIL_POLLS && !ok; ++it) {
+                        ok = ld_acquire_u32(P.rdy + b) >= nsub;
+                        if (!ok) __nanosleep(64);
+                    }
+                    if (!ok) atomicOr(P.pend + (size_t)b * ((P.Next + 31) / 32) + (e >> 5), 1u << (e & 31));
+                }
+                const unsigned m = __ballot_sync(FULL, ok);
+                if (lane == 0) s_mask = m;
+            }
+            __syncthreads();
+            PT_STAMP(11);
+            {
+                const unsigned okm = s_mask;       // owned collocation points whose rows this CTA writes now
+                const int G = T / P.Npad > 0 ? T / P.Npad : 1, g = tid / P.Npad, j = tid - g * P.Npad;
+                for (int k = g; k < nown; k += G)
+                    if (g < G && ((okm >> k) & 1u)) tail_point_rows(P, s_own[3 * k], j, P.Npad);
+            }
+            __syncthreads();                       // (release by the counting threads below covers the rows)
+            PT_STAMP(13);
             if (tid < 32) {                        // one count per finished point on its system's counter
                 bool fin = false;
-                int b = 0;
                 if (lane < nown) {
-                    b = s_own[3 * lane] / P.Next;
-                    fin = arrive_acq_rel(P.done + b) == (unsigned)P.Next - 1;
+                    const int b = s_own[3 * lane] / P.Next, e = s_own[3 * lane] - b * P.Next;
+                    const bool pending = e < P.N && !((s_mask >> lane) & 1u);
+                    const unsigned total = arrive_acq_rel(P.done + b, pending ? 1u + TAIL_PENDING : 1u) + 1u + (pending ? TAIL_PENDING : 0u);
+                    fin = (total & (TAIL_PENDING - 1u)) == (unsigned)P.Next;
+                    s_pend[lane] = total / TAIL_PENDING;
                 }
+                __syncwarp();
                 const unsigned m = __ballot_sync(FULL, fin);
                 if (lane == 0) s_mask = m;
             }
@@ -246,11 +318,13 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             while (fmask) {                        // systems whose last external point this CTA finished
                 const int l = __ffs(fmask) - 1;
                 fmask &= fmask - 1;
-                tail_system(P, s_own[3 * l] / P.Next);
+                tail_finish(P, s_own[3 * l] / P.Next, s_pend[l]);
+                PT_STAMP(8);
             }
         }
         __syncthreads();
     }
+    PT_STAMP(7);
 }
 
 }  // namespace dse

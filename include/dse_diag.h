@@ -31,6 +31,12 @@ extern "C" {
 DSE_API int dse_probe(int32_t kind, int32_t blocks, int32_t iters, double *sink_dev, void *stream);
 DSE_API double dse_probe_flops(int32_t kind, int32_t blocks, int32_t iters);
 
+/* The fused tail of a single-system Jacobian build (csrc/dse_tail.cuh): the CTA that owns a collocation point looks at most
+ * `polls` times for the rows of the subtraction points x_Z, x_G before it leaves its rows of J and F to the CTA that
+ * finishes the system.  Default 4096; 0 sends every point down that fallback path (tests use it to cover the path).
+ * Applies to the builds launched after the call. */
+DSE_API int dse_diag_set_tail_polls(dse_handle *h, int32_t polls);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,7 @@ EXPORTS = [
     "dse_kernel_info", "dse_set_timing", "dse_get_timing", "dse_gauss_legendre", "dse_gauss_legendre_noalloc", "dse_schwinger",
     "dse_dressing",
     "dse_jacobian_fd", "dse_strerror", "dse_last_error",
-    "dse_probe", "dse_probe_flops",
+    "dse_probe", "dse_probe_flops", "dse_diag_set_tail_polls",
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
@@ -87,6 +87,7 @@ def load_library():
     L.dse_schwinger.argtypes = [vp, dp, C.c_int32, C.c_double, C.c_double, dp, C.c_int32, dp, dp, vp]
     L.dse_dressing.argtypes = [vp, dp, dp, C.c_int32, dp, dp, dp, vp]
     L.dse_probe.argtypes = [C.c_int32, C.c_int32, C.c_int32, dp, vp]
+    L.dse_diag_set_tail_polls.argtypes = [vp, C.c_int32]
     L.dse_probe_flops.argtypes = [C.c_int32, C.c_int32, C.c_int32]
     L.dse_probe_flops.restype = C.c_double
     L.dse_strerror.argtypes = [C.c_int]
@@ -263,6 +264,10 @@ class Dse:
 
     def launch_count(self):
         return int(self.lib.dse_launch_count(self._h))
+
+    def set_tail_polls(self, polls):
+        """include/dse_diag.h: polls an owner of the fused tail spends before it leaves its rows to the finishing CTA."""
+        _check(self.lib.dse_diag_set_tail_polls(self._h, int(polls)))
 
     def kernel_info(self):
         a = (C.c_int32 * 8)()

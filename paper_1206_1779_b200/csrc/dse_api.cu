@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "dse_internal.h"
+#include "../../include/dse_diag.h"
 
 struct dse_handle {
     dse_params params;
@@ -307,6 +308,7 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
         if (e != cudaSuccess) { dse_destroy(h); return cuda_err(e, "cudaMemcpy(tail tables)"); }
         k.tail_cta = h->d_tail; k.tail_bi = h->d_tail + (size_t)2 * h->cfg.grid;
     }
+    k.tail_polls = dse::TAIL_POLLS;
     rc = dse::lu_configure((int)n2);
     if (rc < 0) { dse_destroy(h); return rc; }
     if (k.geom) {
@@ -524,6 +526,13 @@ int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, doub
 }
 
 int64_t dse_launch_count(const dse_handle *h) { return h ? h->launches : 0; }
+
+int dse_diag_set_tail_polls(dse_handle *h, int32_t polls)
+{
+    if (!h || polls < 0) return DSE_EINVAL;
+    h->k.tail_polls = polls;
+    return DSE_OK;
+}
 
 int dse_kernel_info(const dse_handle *h, int32_t out[8])
 {

@@ -30,6 +30,8 @@ struct HostTables {
 void build_tables(const dse_params &p, const dse_tables *user, HostTables &t);
 
 // Everything the kernels need, passed by value.
+constexpr int TAIL_POLLS = 4096;       // fused tail: polls (64 ns apart + a memory round trip) for the subtraction points' rows before giving up
+
 struct KParams {
     int N, Npad, NCH, SUB, rounds;     // Chebyshev: N, padded to NCH*CJ; phase-2 lanes = NCH chunk x SUB point lanes
     int Nr, Nt, Ntpad, g, rpb;         // angular nodes padded to a multiple of g (g = 32, or pow2 >= Nt); rows per batch
@@ -43,6 +45,7 @@ struct KParams {
     int want_jac;                      // 0: residual only (skip phase 2)
     int use_constc;                    // coefficients are constant-bank operands (DSE_FLAG_CONST_COEF, pipelined kernel)
     int tail;                          // the point kernel finishes the build itself (reduction, contraction, assembly)
+    int tail_polls;                    // polls an owner spends looking for the subtraction points' rows (dse_tail.cuh; default TAIL_POLLS)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
     const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x, *EGy, *EZy;
     const double *t_r;                 // s(y_q) of the radial nodes (clamped to [-1, 1]), same layout as y

@@ -23,15 +23,6 @@
 
 namespace dse {
 
-#ifdef DSE_PT_DEBUG
-#define PT_NOW() gtime()
-extern "C" __attribute__((visibility("default"))) int dse_pt_debug_read(long long *out)
-{
-    return (int)cudaMemcpyFromSymbol(out, g_pt_dbg, sizeof(g_pt_dbg));
-}
-#else
-#define PT_NOW() 0ll
-#endif
 
 namespace {
 
@@ -433,10 +424,6 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     constexpr int SLOT = 6 * Npad + 2;                                      // = slot_doubles(Npad)
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
-#ifdef DSE_PT_DEBUG
-    for (int z = 1; z < 16; ++z) if (lane == 0) g_pt_dbg[((size_t)blockIdx.x * 16 + warp) * 16 + z] = 0;
-#endif
-    PT_STAMP(0);
     const int STASH = stash_doubles(NCH);
     const int WD = pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
     double *s_ang = smem;
@@ -499,7 +486,6 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
             asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.phi_x) + l * 128));
     }
     pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
-    PT_STAMP(1);
 
     if (t0 < t1) {
     const bool lane_on = EXACT || lane < NCH * SUB;
@@ -631,7 +617,6 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     __syncthreads();
     if (CONSTC && ctouch == 1.2345e-300) s_ang[0] = ctouch;  // (keeps the touch alive)
-    PT_STAMP(2);
     int rem = (int)(t1 - t0);                              // batches left for this warp
     int cur = 0;                                           // stash half written by the current batch
     while (rem > 0) {
@@ -747,11 +732,9 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
             }
         }
         // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
-        const long long tq0 = PT_NOW();
         phase2_last(cur ^ 1);
         flush(bi, cur);
         contract(bi, e, q_seg, last_partial ? q : q - 1, last_partial);
-        PT_ADD(9, PT_NOW() - tq0); PT_ADD(10, 1);
         if (q >= Nr) {
             q = 0; ++bi; ++e;
             if (e == P.Next) {
@@ -765,7 +748,6 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         asm volatile("cp.async.wait_group 0;\n" ::: "memory");
         __syncthreads();
     }
-    PT_STAMP(3);
     build_tail(P, smem);                                   // H8 by the last-arriving CTAs (dse_tail.cuh)
 }
 using KernelFn = void (*)(const KParams);

@@ -26,15 +26,6 @@
 
 namespace dse {
 
-#ifdef DSE_PT_DEBUG
-__device__ long long g_pt_dbg[148 * 16 * 16];
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define PT_STAMP(slot) do { if ((threadIdx.x & 31) == 0) g_pt_dbg[((size_t)blockIdx.x * 16 + (threadIdx.x >> 5)) * 16 + (slot)] = gtime(); } while (0)
-#define PT_ADD(slot, v) do { if ((threadIdx.x & 31) == 0) g_pt_dbg[((size_t)blockIdx.x * 16 + (threadIdx.x >> 5)) * 16 + (slot)] += (v); } while (0)
-#else
-#define PT_STAMP(slot) do { } while (0)
-#define PT_ADD(slot, v) do { } while (0)
-#endif
 
 // slot of one (warp, external point): [0, 3 Npad) Sa, Sb, Sv accumulated with T_0 = 1; [3 Npad, 6 Npad) Ra, Rb, Rv with the
 // table phi (phi_0 = 1/2); then Pi_G, Pi_Z
@@ -78,7 +69,6 @@ __device__ __forceinline__ unsigned arrive_acq_rel(unsigned *ctr, unsigned inc =
 
 constexpr int TAIL_OWN = 4;            // external points a CTA finishes in one pass
 constexpr int TAIL_MLP = 20;           // 16-byte slot loads in flight per thread
-constexpr int TAIL_POLLS = 4096;       // polls (64 ns apart + a memory round trip) for the subtraction points before giving up
 
 // parts a slot sum is split into (a function of the launch configuration only): threads per pair of slot entries
 __host__ __device__ inline int tail_parts(int Npad, int threads)
@@ -240,7 +230,6 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
     const int tid = threadIdx.x, lane = tid & 31, WPB = blockDim.x >> 5, T = blockDim.x;
     const int bi_lo = P.tail_cta[2 * blockIdx.x], bi_hi = P.tail_cta[2 * blockIdx.x + 1];
     __syncthreads();                               // the slots of every warp of this CTA are written (CTA scope) ...
-    PT_STAMP(4);
     for (int seg0 = bi_lo; seg0 <= bi_hi; seg0 += 32) {
         if (tid < 32) {
             const int bi = seg0 + lane;
@@ -256,7 +245,6 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             if (lane == 0) s_mask = m;
         }
         __syncthreads();
-        PT_STAMP(5);
         unsigned mask = s_mask;                    // external points this CTA arrived last at (usually none or one)
         while (mask) {
             __syncthreads();                       // (s_own, s_mask and the shared memory of the pass before are free)
@@ -270,9 +258,8 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             __syncthreads();
             tail_points(P, sm, s_own, nown);
             __syncthreads();                       // D rows, Pi, 1/G, 1/Z of the owned points are written
-            PT_STAMP(6);
             if (tid < 32) {
-                // owners of x_Z, x_G publish; owners of collocation points look for both -- at most TAIL_POLLS times
+                // owners of x_Z, x_G publish; owners of collocation points look for both -- at most P.tail_polls times
                 bool ok = false;
                 int b = 0, e = P.N;
                 if (lane < nown) {
@@ -281,7 +268,7 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
                 }
                 if (e < P.N) {
                     const unsigned nsub = P.iZ == P.iG ? 1u : 2u;
-                    for (int it = 0; it < TAIL_POLLS && !ok; ++it) {
+                    for (int it = 0; it < P.tail_polls && !ok; ++it) {
                         ok = ld_acquire_u32(P.rdy + b) >= nsub;
                         if (!ok) __nanosleep(64);
                     }
@@ -291,7 +278,6 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
                 if (lane == 0) s_mask = m;
             }
             __syncthreads();
-            PT_STAMP(11);
             {
                 const unsigned okm = s_mask;       // owned collocation points whose rows this CTA writes now
                 const int G = T / P.Npad > 0 ? T / P.Npad : 1, g = tid / P.Npad, j = tid - g * P.Npad;
@@ -299,7 +285,6 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
                     if (g < G && ((okm >> k) & 1u)) tail_point_rows(P, s_own[3 * k], j, P.Npad);
             }
             __syncthreads();                       // (release by the counting threads below covers the rows)
-            PT_STAMP(13);
             if (tid < 32) {                        // one count per finished point on its system's counter
                 bool fin = false;
                 if (lane < nown) {
@@ -319,12 +304,10 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
                 const int l = __ffs(fmask) - 1;
                 fmask &= fmask - 1;
                 tail_finish(P, s_own[3 * l] / P.Next, s_pend[l]);
-                PT_STAMP(8);
             }
         }
         __syncthreads();
     }
-    PT_STAMP(7);
 }
 
 }  // namespace dse

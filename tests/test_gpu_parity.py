@@ -426,3 +426,27 @@ def test_host_buffer_entry_point_and_back_to_back_builds(orc):
         assert torch.equal(outs[i][0], outs[i % 2][0]) and torch.equal(outs[i][1], outs[i % 2][1])
     assert not torch.equal(outs[0][0], outs[1][0])
     d.close()
+
+
+def test_fused_tail_fallback_path(orc):
+    """dse_tail.cuh: the owner of a collocation point normally writes its rows of J and F itself once the rows of x_Z, x_G
+    are published; with zero polls (include/dse_diag.h) every owner gives up at once and the CTA that completes the
+    system's counter writes all rows.  Same arithmetic on both paths: bitwise equal results, and the counters are left
+    clean for the next build (checked by alternating the two settings)."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE
+    from workloads import config_inputs
+    for cfg, flags in ((1, DSE_FLAG_GEOMETRY_CACHE), (0, 0)):
+        w, c, bc = config_inputs(cfg)
+        d = Dse(params_from_workload(w, flags=flags))
+        ct = torch.from_numpy(c).cuda(); bt = torch.from_numpy(bc).cuda()
+        J0, F0 = d.jacobian(ct, bt)
+        J0 = J0.clone(); F0 = F0.clone()
+        for polls in (0, 4096, 0, 0, 4096):
+            d.set_tail_polls(polls)
+            J, F = d.jacobian(ct, bt)
+            assert torch.equal(J, J0) and torch.equal(F, F0), (cfg, polls)
+        p = oracle_params(w)
+        Fo, Jo = orc.residual_jacobian(p, c[0], bc[0, 0], bc[0, 1])
+        assert np.linalg.norm(J0.cpu().numpy()[0] - Jo) <= 1e-10 * np.linalg.norm(Jo)
+        d.close()

@@ -1,4 +1,6 @@
 """GPU LU / Newton step against the oracle's."""
+import math
+
 import numpy as np
 import pytest
 
@@ -326,6 +328,44 @@ def test_newton_solve_graph_paper_scaling_solution(orc):
     assert abs(al[0] - math.exp(2 * g + z)) < 1e-12
     kap = -(lnG[3] - lnG[2]) / math.log(10.0)               # G ~ x^-kappa below eps2 (eq.(17))
     assert abs(kap - S.KAPPA) < 1e-9
+    d.close()
+
+
+def test_newton_solve_graph_paper_solution_family(orc):
+    """PAPER.md L139-151 (Fig. 3, 4): the scaling solution and the two decoupling solutions G(x_G = 0)^-1 = 0, 0.01, 0.1 of the
+    paper's parameter set as ONE dse_newton_solve call with three systems.  Three systems are below the batch size of the
+    tensor-path kernel (n_batch >= 8), so this runs the per-system one-kernel builds and one LU CTA per system inside
+    the graph (the test says which variant ran); the members stop after different numbers of steps (per-system freeze).
+    Same step counts and converged coefficients as the oracle's loops; the printed facts are pinned on the oracle side
+    by tests/test_oracle_path.py::test_paper_decoupling_solutions_P13 and re-read here from the device."""
+    torch = _torch()
+    import scaling_setup as S
+    from paper_1206_1779_b200 import Dse, params_from_workload
+    from workloads import Workload
+    w = Workload("paper-family", S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, x_G=0.0, x_Z=S.L2, n_ir=S.N_IR)
+    p = oracle_params(w)
+    c0 = S.start_coefficients(orc, p)
+    gGs = [0.0, 0.01, 0.1]
+    ref = [orc.newton_solve(p, c0.copy(), gG, S.G_Z, rho=1.0, step_cap=S.STEP_CAP, tol=1e-11, max_iter=40) for gG in gGs]
+    assert all(r[2] == 1 for r in ref)
+    d = Dse(params_from_workload(w, n_batch=3, flags=1))
+    assert d.kernel_info()["variant"] == "pipelined"
+    c_g = torch.from_numpy(np.stack([c0, c0, c0])).cuda()
+    bc = torch.tensor([[gG, S.G_Z] for gG in gGs], dtype=torch.float64, device="cuda")
+    info = d.newton_solve(c_g, bc, rho=1.0, step_cap=S.STEP_CAP, tol=1e-11, max_iter=40).cpu().numpy()
+    c = c_g.cpu().numpy()
+    steps = []
+    for b, (c_o, hist, status) in enumerate(ref):
+        assert info[b, 5] == 1.0 and info[b, 0] == len(hist), (b, info[b], len(hist))
+        assert np.abs(c[b] - c_o).max() <= 1e-9 * np.abs(c_o).max(), b
+        steps.append(int(info[b, 0]))
+    assert len(set(steps)) == 3                                       # 9, 11 and 15 steps: every member froze on its own
+    xs = torch.tensor([91.2 ** 2, S.EPS2, 1e-5], dtype=torch.float64, device="cuda")
+    lnG, lnZ, al = (t.cpu().numpy() for t in d.dressing(c_g, xs))
+    assert np.all(np.abs(al[:, 0] - 0.118) < 1e-3)                    # alpha(M_Z^2), fn.7: all three members
+    assert abs(al[0, 1] - 2.972) < 5e-3                               # scaling: infrared fixed point (L151)
+    assert al[1, 1] < 0.02 and al[2, 1] < 1e-3 and np.all(al[1:, 1] < al[1:, 2])    # decoupling: alpha vanishes in the infrared
+    assert 0.98 / 0.01 < math.exp(lnG[1, 1]) <= 1 / 0.01 and 0.98 / 0.1 < math.exp(lnG[2, 1]) <= 1 / 0.1      # finite G(0) = 1/g_G
     d.close()
 
 

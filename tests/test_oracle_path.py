@@ -1,6 +1,7 @@
 """Pins of the oracle's path functions (ln_dress, residual, Jacobian, LU, Newton step): SURVEY.md 8(c)
 P10-P12.  CPU only; nothing here touches the CUDA path."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -385,6 +386,56 @@ def test_paper_scaling_solution_P9(orc, n_r, n_theta, rule, split):
     dlt = orc.schwinger(p, c, 4096, 1e-14, S.L2, t)
     zeros = [0.5 * (t[i] + t[i + 1]) for i in range(len(t) - 1) if dlt[i] * dlt[i + 1] < 0]
     assert dlt[0] > 0 and len(zeros) >= 1 and 3.0 < zeros[0] < gold["schwinger_zero_t_upper"]
+
+
+def test_paper_decoupling_solutions_P13(orc):
+    """PAPER.md L139-151 (Fig. 3, Fig. 4): with the same parameter set as P9 but a non-vanishing G(x_G = 0)^-1 = 0.01 or 0.1
+    the solve gives a DECOUPLING solution -- the ghost dressing function stays finite in the infrared ("A non-vanishing
+    value of G(x_G)^-1 > 0 yields a decoupling solution", L141) and "the running coupling vanishes in the infrared region"
+    (L151) -- while G(x_G)^-1 = 0 gives the scaling solution with the fixed point alpha(0) = 2.972.  The renormalisation
+    condition Z(x_Z) = 0.256, alpha(mu^2) = 1 is shared, so alpha(M_Z^2) = 0.118 (fn.7) holds for all three.  All members
+    start from the same scaling-shaped guess (tests/scaling_setup.py) with the relaxation rule A26; the continuation below
+    eps2 = 1e-6 GeV^2 is the paper's eq.(16),(17) as it stands (the only forms the paper gives; with the massive-gluon
+    forms G = const, Z ~ x instead, alpha(x) changes by < 3e-3 relative -- checked here too)."""
+    import scaling_setup as S
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")):
+        f = line.split("#")[0].split()
+        if len(f) == 2:
+            gold[f[0]] = float(f[1])
+    p = make_params(S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, 0.0, S.L2, n_ir=S.N_IR)
+    c0 = S.start_coefficients(orc, p)
+
+    def alpha(pp, c, x):
+        g, z = orc.ln_dress(pp, c, x)
+        return math.exp(2 * g + z)
+
+    sols = {}
+    for gG in (0.0, gold["decoupling_invG_a"], gold["decoupling_invG_b"]):
+        c, hist, status = orc.newton_solve(p, c0.copy(), gG, S.G_Z, rho=1.0, step_cap=S.STEP_CAP, tol=1e-11, max_iter=40)
+        assert status == 1 and hist[-1][0] < 1e-11 and len(hist) <= 20, (gG, status, len(hist))
+        assert hist[-1][0] < 100 * hist[-2][0] ** 2 + 1e-11                     # quadratic at the end (L226), down to the rounding floor
+        sols[gG] = c
+        assert abs(alpha(p, c, gold["M_Z_GeV"] ** 2) - gold["alpha_MZ"]) < 1e-3     # printed 0.118, all three members
+    assert abs(alpha(p, sols[0.0], S.EPS2) - gold["alpha0_Nc3"]) < 5e-3             # scaling: the infrared fixed point
+    for gG in (gold["decoupling_invG_a"], gold["decoupling_invG_b"]):
+        c = sols[gG]
+        a = [alpha(p, c, x) for x in (1e-6, 1e-5, 1e-4, 1e-3)]
+        assert a[0] < a[1] < a[2] < a[3] and a[0] < 0.02 and a[0] < 0.15 * a[1]     # vanishes in the infrared (L151)
+        G_ir = math.exp(orc.ln_dress(p, c, S.EPS2)[0])
+        assert 0.98 / gG < G_ir <= 1.0 / gG                                          # finite ghost dressing: G(0) = 1/0.01, 1/0.1
+        # ... where the scaling member's ghost dressing function is singular: it has passed them by orders of magnitude
+        assert math.exp(orc.ln_dress(p, sols[0.0], S.EPS2)[0]) > 20.0 / gG
+    # the larger G(0)^-1 decouples at the larger momentum (Fig. 4: the dashed-dotted curve lies below the dashed one)
+    for x in (1e-5, 1e-3, 1e-1):
+        assert alpha(p, sols[gold["decoupling_invG_b"]], x) < alpha(p, sols[gold["decoupling_invG_a"]], x) < alpha(p, sols[0.0], x) * 1.2
+    # reading check: the massive-gluon continuation instead of eq.(16),(17) below eps2
+    pm = make_params(S.N, S.N_R, S.N_THETA, S.EPS2, S.L2, 0.0, S.L2, n_ir=S.N_IR, ir_exp_G=0.0, ir_exp_Z=1.0)
+    gG = gold["decoupling_invG_a"]
+    cm, hist, status = orc.newton_solve(pm, sols[gG].copy(), gG, S.G_Z, rho=1.0, step_cap=S.STEP_CAP, tol=1e-11, max_iter=40)
+    assert status == 1
+    for x in (1e-6, 1e-4, 1e-2, 1.0):
+        assert abs(alpha(pm, cm, x) / alpha(p, sols[gG], x) - 1.0) < 5e-3
 
 
 def test_infrared_piece_closed_form(orc):

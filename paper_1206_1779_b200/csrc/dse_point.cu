@@ -427,7 +427,8 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     const int STASH = stash_doubles(NCH);
     const int WD = pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
     double *s_ang = smem;
-    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * WD;
+    double *s_exp = smem + (size_t)P.Ntpad * 6;                              // 2^(k/64): table of fast_exp_tab
+    double *wbase = s_exp + EXPTAB_DOUBLES + (size_t)warp * WD;
     double2 *s_coef = reinterpret_cast<double2 *>(wbase);
     double *s_stash = wbase + (CONSTC ? 0 : 2 * Npad);                       // [2][STASH]: pt (33 x 4) then T
     double2 *s_gp = reinterpret_cast<double2 *>(s_stash + 2 * STASH);       // [32] (G(y), P(y)) of a window of rows
@@ -485,6 +486,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         for (size_t l = (size_t)blockIdx.x * blockDim.x + threadIdx.x; l < xlines; l += (size_t)gridDim.x * blockDim.x)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.phi_x) + l * 128));
     }
+    if (threadIdx.x < EXPTAB_DOUBLES) s_exp[threadIdx.x] = d_exp2_64[threadIdx.x];
     pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
 
     if (t0 < t1) {
@@ -692,7 +694,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
                 }
                 const double lnZz = (lz0 + lz1) + EZ, lnGz = (lg0 + lg1) + EG;
                 const double lnPz = fma(P.e1, lnGz, P.e2 * lnZz);
-                double Zz = fast_exp(lnZz), Gz = fast_exp(lnGz), Pz = fast_exp(lnPz);
+                double Zz = fast_exp_tab(lnZz, s_exp), Gz = fast_exp_tab(lnGz, s_exp), Pz = fast_exp_tab(lnPz, s_exp);
                 phase2(cur ^ 1);
                 // ======== end of main block ========
                 const int hmax = max(max(__double2hiint(lnZz) & 0x7fffffff, __double2hiint(lnGz) & 0x7fffffff),
@@ -891,7 +893,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     KernelFn pf = k.g == 32 ? pick_pipe(k) : nullptr;
     if (pf) {
         auto psmem_of = [&](int thr) {
-            int d = k.Ntpad * 6 + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr);
+            int d = k.Ntpad * 6 + EXPTAB_DOUBLES + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr);
             const int need = tail_smem_doubles(k.Npad, thr);                // the fused tail reuses the dynamic shared memory
             if (d < need) d = need;
             return (int)sizeof(double) * d;

@@ -463,6 +463,14 @@ def run_probes():
             print(json.dumps({"probe": kind, "ctas": blocks, "warps_per_sm": blocks * 8 // 148,
                               "tflops_median": round(float(np.median(res)), 2), "tflops_min": round(min(res), 2),
                               "tflops_max": round(max(res), 2)}), flush=True)
+    from paper_1206_1779_b200.binding import LATENCY_PROBE_KINDS
+    for kind in LATENCY_PROBE_KINDS:              # one warp, dependent chain: cycles per iteration land in sink[0]
+        res = []
+        for _ in range(3):
+            probe(kind, 1, 4096, sink)
+            torch.cuda.synchronize()
+            res.append(float(sink[0].item()))
+        print(json.dumps({"probe": kind, "cycles_per_dependent_iteration": round(float(np.median(res)), 1)}), flush=True)
 
 
 def run_ours(args):

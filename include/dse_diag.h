@@ -27,6 +27,15 @@ extern "C" {
 #define DSE_PROBE_DFMA_LDS 5    /* acc_j += w * T_j with EVERY T_j read from shared memory (the "stash all T_j" alternative to
                                    re-running the recurrence in phase 2): 1 LDS.64 per DFMA                                  */
 
+/* Latency probes: ONE warp runs `iters` iterations of a dependent chain and writes the clock cycles per iteration to
+ * sink_dev[0] (`blocks` is ignored; dse_probe_flops returns 0).  They are the measurements behind the LU's pivot search
+ * (csrc/dse_lu.cu): how a winner lane's value reaches the other lanes. */
+#define DSE_PROBE_LAT_REDUX_MAX 6        /* x = redux.max(x) + lane                                   */
+#define DSE_PROBE_LAT_REDUX_OR 7         /* x = redux.or(x & m) + 1                                   */
+#define DSE_PROBE_LAT_BALLOT_FFS_SHFL 8  /* x = shfl(x, ffs(ballot(p)) - 1) + lane: the textbook broadcast */
+#define DSE_PROBE_LAT_SHFL 9             /* x = shfl(x, f(x)) + 1                                     */
+#define DSE_PROBE_LAT_DFMA 10            /* d = fma(d, a, b)                                          */
+
 /* sink_dev receives one double per thread (>= blocks * 256).  Asynchronous on `stream`. */
 DSE_API int dse_probe(int32_t kind, int32_t blocks, int32_t iters, double *sink_dev, void *stream);
 DSE_API double dse_probe_flops(int32_t kind, int32_t blocks, int32_t iters);

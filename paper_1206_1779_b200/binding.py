@@ -30,6 +30,7 @@ DSE_FLAG_CONST_COEF = 16
 DSE_FLAG_PER_SYSTEM_KERNELS = 32
 DSE_EBUSY = -4
 PROBE_KINDS = {"dfma": 0, "dmma": 1, "dfma_3reg": 2, "dfma_reuse": 3, "dfma_dmma": 4, "dfma_lds": 5}
+LATENCY_PROBE_KINDS = {"lat_redux_max": 6, "lat_redux_or": 7, "lat_ballot_ffs_shfl": 8, "lat_shfl": 9, "lat_dfma": 10}
 
 
 class DseParams(C.Structure):
@@ -278,7 +279,7 @@ class Dse:
 
 def probe(kind, blocks, iters, sink, stream=None):
     """include/dse_diag.h: launches one fp64 throughput probe; returns the floating-point operations of the launch."""
-    k = PROBE_KINDS[kind] if isinstance(kind, str) else int(kind)
+    k = {**PROBE_KINDS, **LATENCY_PROBE_KINDS}[kind] if isinstance(kind, str) else int(kind)
     L = load_library()
     _check(L.dse_probe(k, blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
     return L.dse_probe_flops(k, blocks, iters)

@@ -108,6 +108,29 @@ __global__ void __launch_bounds__(PROBE_THREADS) probe_dfma_lds(int iters, doubl
     sink[blockIdx.x * (size_t)blockDim.x + threadIdx.x] = s;
 }
 
+// Dependent-chain latencies of the warp collectives the LU's pivot search chooses between (one warp; sink[0] receives the
+// cycles per iteration, including the one integer add that closes the chain): the winner of a search hands its value to the
+// other lanes either through ballot -> lane index -> shuffle or through a REDUX over masked words.
+template <int OP>
+__global__ void __launch_bounds__(32) probe_latency(int iters, double *sink)
+{
+    const int lane = threadIdx.x;
+    unsigned x = 12345u + 7u * lane;
+    double d = 1.25 + 1e-3 * lane;
+    const long long t0 = clock64();
+#pragma unroll 8
+    for (int i = 0; i < iters; ++i) {
+        if (OP == 0) x = __reduce_max_sync(0xffffffffu, x) + lane;
+        if (OP == 1) x = __reduce_or_sync(0xffffffffu, x & (lane + i)) + 1u;
+        if (OP == 2) x = __shfl_sync(0xffffffffu, x, __ffs(__ballot_sync(0xffffffffu, (x & 1u) != 0u) | 0x80000000u) - 1) + lane;
+        if (OP == 3) x = __shfl_sync(0xffffffffu, x, (x + 1u) & 31u) + 1u;
+        if (OP == 4) d = fma(d, 1.0000001, 0.5);
+    }
+    const long long t1 = clock64();
+    if (lane == 0) sink[0] = (double)(t1 - t0) / iters;
+    if (x == 0xdeadbeefu || d == 1.5) sink[1] = 1.0;      // (keeps both chains alive)
+}
+
 }  // namespace
 
 int launch_probe(int kind, int blocks, int iters, double *sink, void *stream)
@@ -120,6 +143,11 @@ int launch_probe(int kind, int blocks, int iters, double *sink, void *stream)
         case DSE_PROBE_DFMA_REUSE: probe_dfma_3reg<true><<<blocks, PROBE_THREADS, 0, s>>>(iters, sink); break;
         case DSE_PROBE_DFMA_DMMA: probe_dfma_dmma<<<blocks, PROBE_THREADS, 0, s>>>(iters, sink); break;
         case DSE_PROBE_DFMA_LDS: probe_dfma_lds<<<blocks, PROBE_THREADS, 0, s>>>(iters, sink); break;
+        case DSE_PROBE_LAT_REDUX_MAX: probe_latency<0><<<1, 32, 0, s>>>(iters, sink); break;
+        case DSE_PROBE_LAT_REDUX_OR: probe_latency<1><<<1, 32, 0, s>>>(iters, sink); break;
+        case DSE_PROBE_LAT_BALLOT_FFS_SHFL: probe_latency<2><<<1, 32, 0, s>>>(iters, sink); break;
+        case DSE_PROBE_LAT_SHFL: probe_latency<3><<<1, 32, 0, s>>>(iters, sink); break;
+        case DSE_PROBE_LAT_DFMA: probe_latency<4><<<1, 32, 0, s>>>(iters, sink); break;
         default: return DSE_EINVAL;
     }
     cudaError_t e = cudaGetLastError();

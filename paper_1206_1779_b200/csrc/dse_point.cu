@@ -446,9 +446,9 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     // tables of its first window of rows (H1), its first geometry record, the angular table -- one memory round trip
     // instead of three in a row (an L2 flush, or a first build, makes each of them a DRAM miss)
     const RowTab tab0 = pipe_row_tables(P, n_rows, g0, gmod, lane, 0);
-    double ctouch = 0.0;
     if (CONSTC && lane * 8 < 2 * Npad) {     // the coefficient bank was rewritten just before this launch: cold in the constant
-        asm volatile("ld.const.f64 %0, [%1];" : "=d"(ctouch) : "l"(c_coef + lane * 8));   // cache -- one lane per 64 B line asks now
+        double ctouch;                       // cache -- one lane per 64 B line asks now (volatile: the unused load stays)
+        asm volatile("ld.const.f64 %0, [%1];" : "=d"(ctouch) : "l"(c_coef + lane * 8));
     }
     int bi = (int)(r0 / Nr);
     int q = (int)(r0 - (long long)bi * Nr);
@@ -618,7 +618,6 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     if (GEOM) asm volatile("cp.async.wait_group 1;\n" ::: "memory");       // all but the geometry record
     else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     __syncthreads();
-    if (CONSTC && ctouch == 1.2345e-300) s_ang[0] = ctouch;  // (keeps the touch alive)
     int rem = (int)(t1 - t0);                              // batches left for this warp
     int cur = 0;                                           // stash half written by the current batch
     while (rem > 0) {

@@ -45,10 +45,12 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
     double *s_ang = smem;
-    double *sT = smem + (size_t)P.Ntpad * 6 + (size_t)warp * BT_WARP_DOUBLES;       // [8][BT_TS]
+    double *s_exp = smem + (size_t)P.Ntpad * 6;                                     // 2^(k/64): table of fast_exp_tab
+    double *sT = s_exp + EXPTAB_DOUBLES + (size_t)warp * BT_WARP_DOUBLES;           // [8][BT_TS]
     double4 *s_gbuf = reinterpret_cast<double4 *>(sT + 8 * BT_TS);                  // [2][32] geometry records
     double *sC = sT + 8 * BT_TS + GBUF_DOUBLES;                                     // [BT_KS][2][32] coefficient fragments
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
+    if (threadIdx.x < EXPTAB_DOUBLES) s_exp[threadIdx.x] = d_exp2_64[threadIdx.x];
     pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q)
     __syncthreads();
 
@@ -184,8 +186,8 @@ __global__ void __launch_bounds__(BT<NPADB>::THREADS, 1) point_kernel_batched(co
                     {
                         const double lnZz = lz0 + EZ, lnGz = lg0 + EG, lnPz = fma(P.e1, lnGz, P.e2 * lnZz);
                         const double lnZy = lz1 + EZ, lnGy = lg1 + EG, lnPy = fma(P.e1, lnGy, P.e2 * lnZy);
-                        double Zz = fast_exp(lnZz), Gz = fast_exp(lnGz), Pz = fast_exp(lnPz);
-                        double Zy = fast_exp(lnZy), Gw = fast_exp(lnGy), Pw = fast_exp(lnPy);
+                        double Zz = fast_exp_tab(lnZz, s_exp), Gz = fast_exp_tab(lnGz, s_exp), Pz = fast_exp_tab(lnPz, s_exp);
+                        double Zy = fast_exp_tab(lnZy, s_exp), Gw = fast_exp_tab(lnGy, s_exp), Pw = fast_exp_tab(lnPy, s_exp);
                         const int h0 = max(max(__double2hiint(lnZz) & 0x7fffffff, __double2hiint(lnGz) & 0x7fffffff),
                                            __double2hiint(lnPz) & 0x7fffffff);
                         const int h1 = max(max(__double2hiint(lnZy) & 0x7fffffff, __double2hiint(lnGy) & 0x7fffffff),
@@ -292,7 +294,7 @@ struct BatchedVariant { BatchedFn fn; int threads, smem; };
 BatchedVariant batched_variant(const KParams &k, bool jac)
 {
     const bool g = k.geom != nullptr;
-    const int base = (int)sizeof(double) * k.Ntpad * 6;
+    const int base = (int)sizeof(double) * (k.Ntpad * 6 + EXPTAB_DOUBLES);
 #define DSE_BT_CASE(NPADB) \
     return BatchedVariant{pick_batched<NPADB>(g, jac), BT<NPADB>::THREADS, \
                           base + (int)sizeof(double) * (BT<NPADB>::THREADS / 32) * BT<NPADB>::WARP_DOUBLES}

@@ -500,18 +500,26 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     auto phase2 = [&](int buf) {
         const double4 *pts = reinterpret_cast<const double4 *>(s_stash + buf * STASH);
         const double2 *trd = reinterpret_cast<const double2 *>(s_stash + buf * STASH + 132) + c_lane * (TCH_STRIDE / 2);
+        // the stash entries of round rd + 1 are requested before the 30 FMAs of round rd (their shared-memory latency was
+        // the one exposed stall of this block: ncu source view)
+        int pt = EXACT ? sub : min(sub, 32);                                     // slot 32: zero weights, finite T
+        double4 pw = pts[pt];
+        double2 tt = trd[pt];
 #pragma unroll
         for (int rd = 0; rd < ROUNDS; ++rd) {
-            const int pt = EXACT ? rd * SUB + sub : min(rd * SUB + sub, 32);     // slot 32: zero weights, finite T
-            const double4 pw = pts[pt];
-            const double2 tt = trd[pt];
+            const double4 cw = pw;
             double T0 = tt.x, T1 = tt.y;
-            accA[0] = fma(pw.y, T0, accA[0]); accB[0] = fma(pw.z, T0, accB[0]); accV[0] = fma(pw.w, T0, accV[0]);
-            accA[1] = fma(pw.y, T1, accA[1]); accB[1] = fma(pw.z, T1, accB[1]); accV[1] = fma(pw.w, T1, accV[1]);
+            if (rd + 1 < ROUNDS) {
+                pt = EXACT ? (rd + 1) * SUB + sub : min((rd + 1) * SUB + sub, 32);
+                pw = pts[pt];
+                tt = trd[pt];
+            }
+            accA[0] = fma(cw.y, T0, accA[0]); accB[0] = fma(cw.z, T0, accB[0]); accV[0] = fma(cw.w, T0, accV[0]);
+            accA[1] = fma(cw.y, T1, accA[1]); accB[1] = fma(cw.z, T1, accB[1]); accV[1] = fma(cw.w, T1, accV[1]);
 #pragma unroll
             for (int m = 2; m < CJ; ++m) {
-                const double T2 = fma(pw.x, T1, -T0);
-                accA[m] = fma(pw.y, T2, accA[m]); accB[m] = fma(pw.z, T2, accB[m]); accV[m] = fma(pw.w, T2, accV[m]);
+                const double T2 = fma(cw.x, T1, -T0);
+                accA[m] = fma(cw.y, T2, accA[m]); accB[m] = fma(cw.z, T2, accB[m]); accV[m] = fma(cw.w, T2, accV[m]);
                 T0 = T1; T1 = T2;
             }
         }

@@ -473,6 +473,64 @@ def run_probes():
         print(json.dumps({"probe": kind, "cycles_per_dependent_iteration": round(float(np.median(res)), 1)}), flush=True)
 
 
+def run_phase_timeline():
+    """--phase-timeline: the tables of DESIGN.md section 6 from the phase stamps of a library built with
+    -DDSE_PHASE_TIMING (include/dse_diag.h: dse_diag_phase_stamps).  Config 1 and config 3 builds with the L2 flushed;
+    the one-CTA LU at n = 32, 64, 128."""
+    import torch
+    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE, DSE_FLAG_CONST_COEF
+    from paper_1206_1779_b200.binding import phase_stamps
+    torch.cuda.set_device(0)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for cfg in (1, 3):
+        w, c, bc = config_inputs(cfg)
+        d = Dse(params_from_workload(w, flags=DSE_FLAG_GEOMETRY_CACHE | DSE_FLAG_CONST_COEF))
+        info = d.kernel_info()
+        ct, bt = torch.from_numpy(c).cuda(), torch.from_numpy(bc).cuda()
+        for _ in range(3):
+            d.jacobian(ct, bt)
+        flush.zero_()
+        torch.cuda.synchronize()
+        d.jacobian(ct, bt)
+        torch.cuda.synchronize()
+        a = phase_stamps(0).reshape(148, 16, 16).astype(np.float64)[:info["grid"], :info["block"] // 32, :]
+        t0 = a[:, :, 0].min()
+        print(f"## {w.name}: grid {info['grid']} x {info['block']} threads, us after the first CTA starts (min / mean / max over warps or owners)")
+
+        def row(name, x):
+            print("| %s | %.2f | %.2f | %.2f |" % (name, x.min() / 1e3, x.mean() / 1e3, x.max() / 1e3))
+        print("| phase | min | mean | max |\n|---|---|---|---|")
+        row("table requests issued", a[:, :, 1] - t0)
+        row("H1 done, first barrier passed", a[:, :, 2] - t0)
+        row("batches + segment ends (duration)", a[:, :, 3] - a[:, :, 2])
+        row("... of which flush + H7 (duration)", a[:, :, 9])
+        row("point phase ends", a[:, :, 3] - t0)
+        row("arrival counters done", a[:, :, 5] - t0)
+        for slot, name in ((6, "slot sums + derivative rows written (owners)"), (11, "subtraction rows seen (owners)"),
+                           (13, "rows of J, F written (owners)"), (8, "counters cleared (finishing CTA)")):
+            m = a[:, :, slot] > 0
+            if m.any():
+                row(name, (a[:, :, slot] - t0)[m])
+        row("kernel exit", a[:, :, 7] - t0)
+        d.close()
+    d = Dse(params_from_workload(CONFIGS[0]))
+    rng = np.random.default_rng(5)
+    print("## lu_panel_kernel, clock64 cycles of system 0 (warm, back-to-back solves)")
+    print("| n | load + equilibrate | elimination | back substitution | per panel: read record | apply to own columns | factorise + publish | hand-over to the next owner |\n|---|---|---|---|---|---|---|---|")
+    for n in (32, 64, 128):
+        A = torch.from_numpy(rng.normal(size=(1, n, n))).cuda()
+        b = torch.from_numpy(rng.normal(size=(1, n))).cuda()
+        for _ in range(5):
+            d.lu_solve(A, b)
+        torch.cuda.synchronize()
+        s = phase_stamps(1)
+        B = lambda P, k: s[256 + P * 8 + k]
+        r = np.array([(B(P, 1) - B(P, 0), B(P, 2) - B(P, 1), B(P, 3) - B(P, 2), B(P + 1, 0) - B(P, 3)) for P in range(1, n // 4 - 2)])
+        m = r.mean(axis=0)
+        print("| %d | %d | %d | %d | %.0f | %.0f | %.0f | %.0f |" % (n, s[1] - s[0], s[2] - s[1], s[4] - s[3], *m))
+    d.close()
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -535,9 +593,14 @@ def main():
                          "config 3 without the geometry cache")
     ap.add_argument("--per-config-steps", type=int, default=300)
     ap.add_argument("--probes", action="store_true", help="print the fp64 throughput probes (include/dse_diag.h) and exit")
+    ap.add_argument("--phase-timeline", action="store_true",
+                    help="print the phase timelines of the one-kernel build and of the LU (needs a library built with -DDSE_PHASE_TIMING) and exit")
     args = ap.parse_args()
     if args.probes:
         run_probes()
+        return
+    if args.phase_timeline:
+        run_phase_timeline()
         return
     if args.impl == "reference":
         w, c, bc = config_inputs(args.config)

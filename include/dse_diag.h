@@ -46,6 +46,14 @@ DSE_API double dse_probe_flops(int32_t kind, int32_t blocks, int32_t iters);
  * Applies to the builds launched after the call. */
 DSE_API int dse_diag_set_tail_polls(dse_handle *h, int32_t polls);
 
+/* Phase stamps of the last single-system Jacobian build (which = 0: %globaltimer ns, [148 CTAs][16 warps][16 slots], slot
+ * meanings in csrc/dse_tail.cuh) or of the last one-CTA LU (which = 1: clock64 of system 0, layout in csrc/dse_lu.cu), copied
+ * to a HOST array.  The stamps exist only in a library built with -DDSE_PHASE_TIMING
+ * (DSE_NVCC_EXTRA=-DDSE_PHASE_TIMING python -m paper_1206_1779_b200.build --force); otherwise DSE_EINVAL.  Returns the number
+ * of words copied.  Synchronises the device.  `python bench.py --phase-timeline` prints the tables of DESIGN.md section 6
+ * from them (profiles/r02c_phase_timeline.md). */
+DSE_API int dse_diag_phase_stamps(int32_t which, int64_t *out_host, int32_t max_words);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,7 @@ EXPORTS = [
     "dse_kernel_info", "dse_set_timing", "dse_get_timing", "dse_gauss_legendre", "dse_gauss_legendre_noalloc", "dse_schwinger",
     "dse_dressing",
     "dse_jacobian_fd", "dse_strerror", "dse_last_error",
-    "dse_probe", "dse_probe_flops", "dse_diag_set_tail_polls",
+    "dse_probe", "dse_probe_flops", "dse_diag_set_tail_polls", "dse_diag_phase_stamps",
 ]
 
 DSE_FLAG_GEOMETRY_CACHE = 1
@@ -89,6 +89,7 @@ def load_library():
     L.dse_dressing.argtypes = [vp, dp, dp, C.c_int32, dp, dp, dp, vp]
     L.dse_probe.argtypes = [C.c_int32, C.c_int32, C.c_int32, dp, vp]
     L.dse_diag_set_tail_polls.argtypes = [vp, C.c_int32]
+    L.dse_diag_phase_stamps.argtypes = [C.c_int32, vp, C.c_int32]
     L.dse_probe_flops.argtypes = [C.c_int32, C.c_int32, C.c_int32]
     L.dse_probe_flops.restype = C.c_double
     L.dse_strerror.argtypes = [C.c_int]
@@ -283,6 +284,18 @@ def probe(kind, blocks, iters, sink, stream=None):
     L = load_library()
     _check(L.dse_probe(k, blocks, iters, _dev_ptr(sink, blocks * 256), _stream_ptr(stream)))
     return L.dse_probe_flops(k, blocks, iters)
+
+
+def phase_stamps(which):
+    """include/dse_diag.h: the phase stamps of the last single-system build (which = 0) or one-CTA LU (which = 1) as an int64
+    numpy array; needs a library built with -DDSE_PHASE_TIMING."""
+    import numpy as np
+    n = 148 * 16 * 16 if which == 0 else 8192
+    out = np.zeros(n, dtype=np.int64)
+    rc = load_library().dse_diag_phase_stamps(int(which), C.c_void_p(out.ctypes.data), n)
+    if rc < 0:
+        _check(rc)
+    return out[:rc]
 
 
 def gauss_legendre(n, device="cuda", stream=None):

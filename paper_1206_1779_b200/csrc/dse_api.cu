@@ -527,6 +527,16 @@ int dse_get_tables(const dse_handle *h, double *x_ext_host, double *y_host, doub
 
 int64_t dse_launch_count(const dse_handle *h) { return h ? h->launches : 0; }
 
+int dse_diag_phase_stamps(int32_t which, int64_t *out_host, int32_t max_words)
+{
+    if (!out_host || max_words < 1 || (which != 0 && which != 1)) return DSE_EINVAL;
+    static_assert(sizeof(long long) == sizeof(int64_t), "stamp words");
+    const int n = which == 0 ? dse::phase_stamps_point(reinterpret_cast<long long *>(out_host), max_words)
+                             : dse::phase_stamps_lu(reinterpret_cast<long long *>(out_host), max_words);
+    if (n == 0) { dse::set_error_text("dse_diag_phase_stamps: the library was built without -DDSE_PHASE_TIMING"); return DSE_EINVAL; }
+    return n;
+}
+
 int dse_diag_set_tail_polls(dse_handle *h, int32_t polls)
 {
     if (!h || polls < 0) return DSE_EINVAL;

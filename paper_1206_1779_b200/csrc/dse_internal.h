@@ -96,6 +96,8 @@ int launch_fd_column(int n2, int B, const double *c, const double *Fp, const dou
                      void *stream);
 int launch_geometry(const KParams &k, double *geom, void *stream);
 // H9 (dse_lu.cu): n <= 128 one CTA, matrix in registers; 128 < n <= 256 a cluster of 4 CTAs (needs `scratch`)
+int phase_stamps_point(long long *out_host, int max_words);   // -DDSE_PHASE_TIMING builds: words copied (else 0) or < 0
+int phase_stamps_lu(long long *out_host, int max_words);
 int lu_configure(int n);          // opt-in attributes of the kernel that serves n, on the current device
 int launch_lu(int n, int n_sys, const double *A, const double *b, double *x, double *c_inout, double rho,
               double *stats, double *scratch, void *stream);

@@ -424,6 +424,10 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     constexpr int SLOT = 6 * Npad + 2;                                      // = slot_doubles(Npad)
     extern __shared__ __align__(16) double smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, WPB = blockDim.x >> 5;
+#ifdef DSE_PHASE_TIMING
+    if (lane == 0) for (int z = 0; z < PHASE_SLOTS; ++z) phase_rec()[z] = 0;
+#endif
+    PHASE_STAMP(0);
     const int STASH = stash_doubles(NCH);
     const int WD = pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
     double *s_ang = smem;
@@ -488,6 +492,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     }
     if (threadIdx.x < EXPTAB_DOUBLES) s_exp[threadIdx.x] = d_exp2_64[threadIdx.x];
     pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
+    PHASE_STAMP(1);
 
     if (t0 < t1) {
     const bool lane_on = EXACT || lane < NCH * SUB;
@@ -626,6 +631,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     if (GEOM) asm volatile("cp.async.wait_group 1;\n" ::: "memory");       // all but the geometry record
     else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
     __syncthreads();
+    PHASE_STAMP(2);
     int rem = (int)(t1 - t0);                              // batches left for this warp
     int cur = 0;                                           // stash half written by the current batch
     while (rem > 0) {
@@ -741,9 +747,11 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
             }
         }
         // epilogue: phase 2 of the segment's last batch, then the partial of this (warp, external point)
+        const long long t_seg = PHASE_NOW();
         phase2_last(cur ^ 1);
         flush(bi, cur);
         contract(bi, e, q_seg, last_partial ? q : q - 1, last_partial);
+        PHASE_ADD(9, PHASE_NOW() - t_seg); PHASE_ADD(10, 1);
         if (q >= Nr) {
             q = 0; ++bi; ++e;
             if (e == P.Next) {
@@ -757,6 +765,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
         asm volatile("cp.async.wait_group 0;\n" ::: "memory");
         __syncthreads();
     }
+    PHASE_STAMP(3);
     build_tail(P, smem);                                   // H8 by the last-arriving CTAs (dse_tail.cuh)
 }
 using KernelFn = void (*)(const KParams);
@@ -783,6 +792,19 @@ KernelFn pick(const KParams &k, bool jac)
 int fail(cudaError_t e, const char *what) { return cuda_fail((int)e, what); }
 
 }  // namespace
+
+// include/dse_diag.h: the phase stamps of the last single-system build (0 words unless built with -DDSE_PHASE_TIMING)
+int phase_stamps_point(long long *out_host, int max_words)
+{
+#ifdef DSE_PHASE_TIMING
+    const int n = PHASE_CTAS * PHASE_WARPS * PHASE_SLOTS < max_words ? PHASE_CTAS * PHASE_WARPS * PHASE_SLOTS : max_words;
+    const cudaError_t e = cudaMemcpyFromSymbol(out_host, g_phase, sizeof(long long) * n);
+    return e == cudaSuccess ? n : cuda_fail((int)e, "cudaMemcpyFromSymbol(phase stamps)");
+#else
+    (void)out_host; (void)max_words;
+    return 0;
+#endif
+}
 
 // DSE_FLAG_CONST_COEF: the __constant__ coefficient arrays are one slot per loaded library; a handle holds it from
 // dse_create to dse_destroy, and only if its caller asked for it.

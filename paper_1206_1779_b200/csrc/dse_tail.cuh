@@ -26,6 +26,27 @@
 
 namespace dse {
 
+// Phase stamps of the single-system build (profiles/r02c_phase_timeline.md): compiled in only with
+// -DDSE_PHASE_TIMING (DSE_NVCC_EXTRA=-DDSE_PHASE_TIMING python -m paper_1206_1779_b200.build --force), read back through
+// dse_diag_phase_stamps (include/dse_diag.h), printed by `bench.py --phase-timeline`.  One record of PHASE_SLOTS
+// %globaltimer values (ns) per warp: 0 kernel entry, 1 table requests issued, 2 H1 done and first barrier passed, 3 point
+// phase done, 4 tail entered (CTA barrier), 5 arrival counters done, 6 slot sums + derivative rows written (owners),
+// 7 kernel exit, 8 counters cleared (finishing CTA), 9 time inside flush + H7 (sum), 10 segments, 11 subtraction rows
+// seen (owners), 13 rows of J, F written (owners).
+constexpr int PHASE_SLOTS = 16, PHASE_WARPS = 16, PHASE_CTAS = 148;
+#ifdef DSE_PHASE_TIMING
+__device__ long long g_phase[PHASE_CTAS * PHASE_WARPS * PHASE_SLOTS];
+__device__ __forceinline__ long long phase_now() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+__device__ __forceinline__ long long *phase_rec() { return g_phase + ((size_t)(blockIdx.x % PHASE_CTAS) * PHASE_WARPS + ((threadIdx.x >> 5) % PHASE_WARPS)) * PHASE_SLOTS; }
+#define PHASE_STAMP(slot) do { if ((threadIdx.x & 31) == 0) phase_rec()[(slot)] = phase_now(); } while (0)
+#define PHASE_ADD(slot, v) do { if ((threadIdx.x & 31) == 0) phase_rec()[(slot)] += (v); } while (0)
+#define PHASE_NOW() phase_now()
+#else
+#define PHASE_STAMP(slot) do { } while (0)
+#define PHASE_ADD(slot, v) do { } while (0)
+#define PHASE_NOW() 0ll
+#endif
+
 
 // slot of one (warp, external point): [0, 3 Npad) Sa, Sb, Sv accumulated with T_0 = 1; [3 Npad, 6 Npad) Ra, Rb, Rv with the
 // table phi (phi_0 = 1/2); then Pi_G, Pi_Z
@@ -230,6 +251,7 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
     const int tid = threadIdx.x, lane = tid & 31, WPB = blockDim.x >> 5, T = blockDim.x;
     const int bi_lo = P.tail_cta[2 * blockIdx.x], bi_hi = P.tail_cta[2 * blockIdx.x + 1];
     __syncthreads();                               // the slots of every warp of this CTA are written (CTA scope) ...
+    PHASE_STAMP(4);
     for (int seg0 = bi_lo; seg0 <= bi_hi; seg0 += 32) {
         if (tid < 32) {
             const int bi = seg0 + lane;
@@ -245,6 +267,7 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             if (lane == 0) s_mask = m;
         }
         __syncthreads();
+        PHASE_STAMP(5);
         unsigned mask = s_mask;                    // external points this CTA arrived last at (usually none or one)
         while (mask) {
             __syncthreads();                       // (s_own, s_mask and the shared memory of the pass before are free)
@@ -258,6 +281,7 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             __syncthreads();
             tail_points(P, sm, s_own, nown);
             __syncthreads();                       // D rows, Pi, 1/G, 1/Z of the owned points are written
+            PHASE_STAMP(6);
             if (tid < 32) {
                 // owners of x_Z, x_G publish; owners of collocation points look for both -- at most P.tail_polls times
                 bool ok = false;
@@ -278,6 +302,7 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
                 if (lane == 0) s_mask = m;
             }
             __syncthreads();
+            PHASE_STAMP(11);
             {
                 const unsigned okm = s_mask;       // owned collocation points whose rows this CTA writes now
                 const int G = T / P.Npad > 0 ? T / P.Npad : 1, g = tid / P.Npad, j = tid - g * P.Npad;
@@ -285,6 +310,7 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
                     if (g < G && ((okm >> k) & 1u)) tail_point_rows(P, s_own[3 * k], j, P.Npad);
             }
             __syncthreads();                       // (release by the counting threads below covers the rows)
+            PHASE_STAMP(13);
             if (tid < 32) {                        // one count per finished point on its system's counter
                 bool fin = false;
                 if (lane < nown) {
@@ -304,10 +330,12 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
                 const int l = __ffs(fmask) - 1;
                 fmask &= fmask - 1;
                 tail_finish(P, s_own[3 * l] / P.Next, s_pend[l]);
+                PHASE_STAMP(8);
             }
         }
         __syncthreads();
     }
+    PHASE_STAMP(7);
 }
 
 }  // namespace dse

@@ -516,7 +516,7 @@ def run_phase_timeline():
     d = Dse(params_from_workload(CONFIGS[0]))
     rng = np.random.default_rng(5)
     print("## lu_panel_kernel, clock64 cycles of system 0 (warm, back-to-back solves)")
-    print("| n | load + equilibrate | elimination | back substitution | per panel: read record | apply to own columns | factorise + publish | hand-over to the next owner |\n|---|---|---|---|---|---|---|---|")
+    print("| n | columns per panel | load + equilibrate | elimination | back substitution | per panel: read record | apply to own columns | factorise + publish | hand-over to the next owner |\n|---|---|---|---|---|---|---|---|---|")
     for n in (32, 64, 128):
         A = torch.from_numpy(rng.normal(size=(1, n, n))).cuda()
         b = torch.from_numpy(rng.normal(size=(1, n))).cuda()
@@ -525,9 +525,10 @@ def run_phase_timeline():
         torch.cuda.synchronize()
         s = phase_stamps(1)
         B = lambda P, k: s[256 + P * 8 + k]
-        r = np.array([(B(P, 1) - B(P, 0), B(P, 2) - B(P, 1), B(P, 3) - B(P, 2), B(P + 1, 0) - B(P, 3)) for P in range(1, n // 4 - 2)])
+        pb = 2 if n > 96 else 4                             # panel widths of csrc/dse_lu.cu
+        r = np.array([(B(P, 1) - B(P, 0), B(P, 2) - B(P, 1), B(P, 3) - B(P, 2), B(P + 1, 0) - B(P, 3)) for P in range(1, n // pb - 2)])
         m = r.mean(axis=0)
-        print("| %d | %d | %d | %d | %.0f | %.0f | %.0f | %.0f |" % (n, s[1] - s[0], s[2] - s[1], s[4] - s[3], *m))
+        print("| %d | %d | %d | %d | %d | %.0f | %.0f | %.0f | %.0f |" % (n, pb, s[1] - s[0], s[2] - s[1], s[4] - s[3], *m))
     d.close()
 
 

@@ -432,7 +432,8 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
     const int WD = pipe_warp_doubles(Npad, NCH, CONSTC, GEOM);
     double *s_ang = smem;
     double *s_exp = smem + (size_t)P.Ntpad * 6;                              // 2^(k/64): table of fast_exp_tab
-    double *wbase = s_exp + EXPTAB_DOUBLES + (size_t)warp * WD;
+    double *s_log = s_exp + EXPTAB_DOUBLES;                                  // tables of fast_log_tab (geometry in registers only)
+    double *wbase = s_log + (GEOM ? 0 : LOGTAB_DOUBLES) + (size_t)warp * WD;
     double2 *s_coef = reinterpret_cast<double2 *>(wbase);
     double *s_stash = wbase + (CONSTC ? 0 : 2 * Npad);                       // [2][STASH]: pt (33 x 4) then T
     double2 *s_gp = reinterpret_cast<double2 *>(s_stash + 2 * STASH);       // [32] (G(y), P(y)) of a window of rows
@@ -491,6 +492,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
             asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char *>(P.phi_x) + l * 128));
     }
     if (threadIdx.x < EXPTAB_DOUBLES) s_exp[threadIdx.x] = d_exp2_64[threadIdx.x];
+    if (!GEOM && threadIdx.x < LOGTAB_DOUBLES) s_log[threadIdx.x] = d_logtab[threadIdx.x];
     pdl_wait();                                             // the coefficients may come from the kernel before (Newton update)
     PHASE_STAMP(1);
 
@@ -670,7 +672,7 @@ __global__ void __launch_bounds__(THR, 1) point_kernel_pipe(const __grid_constan
                     sraw = g0.x; gv = g0.y; gq = g1.x; gm = g1.y;
                     gphase ^= 1;
                 } else {
-                    point_geometry(rc, s_ang + (kb * 32 + lane) * 6, P.inv_eps2, P.two_over_Lg, sraw, gv, gq, gm);
+                    point_geometry_fast(rc, s_ang + (kb * 32 + lane) * 6, P.inv_eps2, P.two_over_Lg, s_log, sraw, gv, gq, gm);
                 }
                 double s = sraw, EG = 0.0, EZ = 0.0;
                 if (sraw < -1.0) {                       // z < eps2: eq.(16),(17)
@@ -922,7 +924,7 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
     KernelFn pf = k.g == 32 ? pick_pipe(k) : nullptr;
     if (pf) {
         auto psmem_of = [&](int thr) {
-            int d = k.Ntpad * 6 + EXPTAB_DOUBLES + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr);
+            int d = k.Ntpad * 6 + EXPTAB_DOUBLES + (k.geom ? 0 : LOGTAB_DOUBLES) + (thr / 32) * pipe_warp_doubles(k.Npad, k.NCH, k.use_constc != 0, k.geom != nullptr);
             const int need = tail_smem_doubles(k.Npad, thr);                // the fused tail reuses the dynamic shared memory
             if (d < need) d = need;
             return (int)sizeof(double) * d;

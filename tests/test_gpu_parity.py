@@ -450,3 +450,42 @@ def test_fused_tail_fallback_path(orc):
         Fo, Jo = orc.residual_jacobian(p, c[0], bc[0, 0], bc[0, 1])
         assert np.linalg.norm(J0.cpu().numpy()[0] - Jo) <= 1e-10 * np.linalg.norm(Jo)
         d.close()
+
+
+@pytest.mark.parametrize("kw,B", [(dict(n_cheb=12, n_r=40, n_theta=32, x_G=0.0, x_Z=5e4, n_ir=6, eps2=1e-6, L2=5e4), 1),
+                                   (dict(n_cheb=20, n_r=64, n_theta=64, x_G=3.0, x_Z=70.0, eps2=1e-8, L2=1e8), 3),
+                                   (dict(n_cheb=8, n_r=48, n_theta=16, eps2=1e-10, L2=1e10), 2)])
+def test_fused_tail_stress(orc, kw, B):
+    """The hand-shakes of the fused tail (arrival counters, published subtraction points, per-system counter, pending mask)
+    over 1500 back-to-back builds per shape: two subtraction points (x_G != x_Z, also x_G = 0), several systems per
+    handle on the per-system kernels, the generic kernel (n_theta = 16), alternating coefficient sets and poll budgets.
+    Every build must reproduce, bit for bit, the first build of its coefficient set; one of them is checked against the
+    oracle."""
+    torch = _torch()
+    from paper_1206_1779_b200 import Dse, params_from_workload, DSE_FLAG_GEOMETRY_CACHE
+    from workloads import Workload, draw_coefficients
+    w = Workload("tail-stress", **kw)
+    d = Dse(params_from_workload(w, n_batch=B, flags=DSE_FLAG_GEOMETRY_CACHE))
+    assert d.kernel_info()["variant"] != "batched-dmma"
+    cs = [torch.from_numpy(np.stack([draw_coefficients(900 + 10 * v + b, w.n_cheb) for b in range(B)])).cuda() for v in range(2)]
+    bt = torch.from_numpy(np.stack([[0.05 * b, 1.0 + 0.1 * b] for b in range(B)])).cuda()
+    n2 = 2 * w.n_cheb
+    ref = []
+    for v in range(2):
+        J, F = d.jacobian(cs[v], bt)
+        ref.append((J.clone(), F.clone()))
+    J = torch.empty((B, n2, n2), dtype=torch.float64, device="cuda"); F = torch.empty((B, n2), dtype=torch.float64, device="cuda")
+    bad = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for i in range(1500):
+        if i % 250 == 0:
+            d.set_tail_polls(0 if (i // 250) % 3 == 1 else (3 if (i // 250) % 3 == 2 else 4096))
+        v = (i * 7 + i // 5) % 2
+        d.jacobian(cs[v], bt, J, F)
+        bad += ((J != ref[v][0]).any() | (F != ref[v][1]).any()).to(torch.int64)      # checked on the device: the builds stay back to back
+    assert int(bad.item()) == 0
+    p = oracle_params(w)
+    c0 = cs[0].cpu().numpy(); b0 = bt.cpu().numpy()
+    for b in range(B):
+        Fo, Jo = orc.residual_jacobian(p, c0[b], b0[b, 0], b0[b, 1])
+        check(ref[0][0].cpu().numpy()[b], ref[0][1].cpu().numpy()[b], Jo, Fo)
+    d.close()

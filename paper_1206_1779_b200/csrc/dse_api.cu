@@ -241,6 +241,8 @@ static int create_impl(const dse_params *params, const dse_tables *user, dse_han
         if (rc < 0) { dse_destroy(h); return rc; }
     }
     k.W = h->cfg.grid * (h->cfg.block / 32);
+    // small builds on the generic kernel (n_theta < 32, ...): the kernel computes H1 itself, a build is one launch
+    k.self_h1 = (!h->cfg.pipelined && !h->cfg.batched && (long long)k.B * k.Gext * k.Nr <= dse::SELF_H1_MAX_ROWS) ? 1 : 0;
     k.upr = (h->cfg.pipelined || h->cfg.batched) ? (k.Ntpad / 32) : 1;      // these kernels partition 32-point batches
     k.bgroup = h->cfg.batched ? 8 : 1;
     // the batched kernel works on groups of 8 systems: the batch is padded with idle systems (zero coefficients, zero
@@ -550,7 +552,7 @@ int dse_kernel_info(const dse_handle *h, int32_t out[8])
     out[0] = h->cfg.grid; out[1] = h->cfg.block; out[2] = h->cfg.smem; out[3] = h->cfg.regs;
     out[4] = h->cfg.ctas_per_sm; out[5] = h->cfg.sms;
     out[6] = h->cfg.batched ? 2 : (h->cfg.pipelined ? 1 : 0);
-    out[7] = h->cfg.batched ? 4 : (h->cfg.pipelined ? 1 : 2);
+    out[7] = h->cfg.batched ? 4 : ((h->cfg.pipelined || h->k.self_h1) ? 1 : 2);
     return DSE_OK;
 }
 

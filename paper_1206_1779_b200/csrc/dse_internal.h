@@ -30,6 +30,7 @@ struct HostTables {
 void build_tables(const dse_params &p, const dse_tables *user, HostTables &t);
 
 // Everything the kernels need, passed by value.
+constexpr int SELF_H1_MAX_ROWS = 2048;   // generic kernel: largest B*Gext*Nr for which every CTA computes G(y_q), P(y_q) of all rows itself
 constexpr int TAIL_POLLS = 4096;       // fused tail: polls (64 ns apart + a memory round trip) for the subtraction points' rows before giving up
 
 struct KParams {
@@ -45,6 +46,7 @@ struct KParams {
     int want_jac;                      // 0: residual only (skip phase 2)
     int use_constc;                    // coefficients are constant-bank operands (DSE_FLAG_CONST_COEF, pipelined kernel)
     int tail;                          // the point kernel finishes the build itself (reduction, contraction, assembly)
+    int self_h1;                       // generic point kernel computes H1 itself (small builds: all B*Gext*Nr radial rows per CTA, in shared memory)
     int tail_polls;                    // polls an owner spends looking for the subtraction points' rows (dse_tail.cuh; default TAIL_POLLS)
     double eps2, L2, inv_eps2, two_over_Lg, Lg, pG, pZ, omega, delta, gamma, e1, e2, C;
     const double *x_ext, *sx_ext, *c3x_ext, *y, *sy, *Wy, *ang, *phi_y, *phi_x, *EGy, *EZy;

@@ -378,7 +378,7 @@ int launch_build(const KParams &k, const PointKernelConfig &cfg, const double *c
     kk.tail = kk.want_jac && !cfg.batched;               // single-system kernels finish the build themselves
     int launches = 0;
     cudaError_t e;
-    const bool one_kernel = kk.tail && cfg.pipelined;    // the pipelined kernel also does H1
+    const bool one_kernel = kk.tail && (cfg.pipelined || kk.self_h1);    // these kernels also do H1
     if (!one_kernel) {
         prep_kernel<<<dim3((kk.Gext * kk.Nr + kk.N + 7) / 8, kk.B), 256, 0, s>>>(kk, c_dev);
         if ((e = cudaGetLastError()) != cudaSuccess) return cuda_fail(e, "prep_kernel launch");

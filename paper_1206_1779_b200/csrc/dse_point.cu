@@ -45,7 +45,10 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
     const int ROUNDS = CT ? NCH_T : P.rounds;
     const int Npad = NCH * CJ;
     double *s_ang = smem;
-    double *wbase = smem + (size_t)P.Ntpad * 6 + (size_t)warp * warp_doubles(Npad, NCH);
+    // small Jacobian builds (P.self_h1): G(y_q), P(y_q) of ALL radial rows of all systems, computed by this CTA itself (H1)
+    const int NGB = (JAC && P.self_h1) ? P.B * P.Gext * P.Nr : 0;
+    double *s_Gy = smem + (size_t)P.Ntpad * 6, *s_Py = s_Gy + NGB;
+    double *wbase = s_Py + NGB + (size_t)warp * warp_doubles(Npad, NCH);
     double2 *s_coef = reinterpret_cast<double2 *>(wbase);
     double4 *s_pt = reinterpret_cast<double4 *>(wbase + 2 * Npad);       // 33 entries, entry 32 = 0
     double *s_T = wbase + 2 * Npad + 132;
@@ -54,7 +57,27 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
 
     for (int t = threadIdx.x; t < P.Ntpad * 6; t += blockDim.x) s_ang[t] = P.ang[t];
     if (lane == 0) s_pt[32] = make_double4(0.0, 0.0, 0.0, 0.0);
-    pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q)
+    pdl_wait();                                             // prep_kernel: coefficient pairs, G(y_q), P(y_q) (or the kernel before)
+    if (NGB) {
+        // H1 by the CTA itself: thread = radial row, both series ln G(y), ln Z(y) of eq.(23),(24) at s(y_q) with T_j from
+        // the three-term recurrence, plus the power-law terms of the infrared piece; G = exp(ln G), P = G^{e1} Z^{e2}
+        const int NG = P.Gext * P.Nr, N = P.N;
+        for (int it = threadIdx.x; it < NGB; it += blockDim.x) {
+            const int b = it / NG, row = it - b * NG;
+            const double *ca = P.c + (size_t)b * 2 * N, *cb = ca + N;
+            const double sy = __ldg(P.t_r + row), ts = 2.0 * sy;
+            double T0 = 1.0, T1 = sy;
+            double lnZ = 0.5 * __ldg(ca), lnG = 0.5 * __ldg(cb);                 // phi_0 = 1/2
+            for (int j = 1; j < N; ++j) {
+                lnZ = fma(__ldg(ca + j), T1, lnZ); lnG = fma(__ldg(cb + j), T1, lnG);
+                const double T2 = fma(ts, T1, -T0);
+                T0 = T1; T1 = T2;
+            }
+            lnG += __ldg(P.EGy + row); lnZ += __ldg(P.EZy + row);
+            s_Gy[it] = exp(lnG);
+            s_Py[it] = exp(P.e1 * lnG + P.e2 * lnZ);
+        }
+    }
     __syncthreads();
 
     const int Nr = P.Nr, g = P.g;
@@ -120,11 +143,19 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
     int e = (int)(bi - (long long)cur_b * P.Next);
     bool fresh = true;                                   // accumulators belong to a new external point
     bool first_row = true;                               // no row of this external point has reached the slot yet
-    if (r0 < r1) {
-        for (int j = lane; j < Npad; j += 32)
-            s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
+    auto load_coef = [&](int b) {                          // (a_j, b_j) pairs of system b, j = 0 pre-halved, zero padded
+        for (int j = lane; j < Npad; j += 32) {
+            if (NGB) {
+                const double *ca = P.c + (size_t)b * 2 * P.N;
+                const double h = j == 0 ? 0.5 : 1.0;
+                s_coef[j] = j < P.N ? make_double2(h * __ldg(ca + j), h * __ldg(ca + P.N + j)) : make_double2(0.0, 0.0);
+            } else {
+                s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)b * Npad + j];
+            }
+        }
         __syncwarp();
-    }
+    };
+    if (r0 < r1) load_coef(cur_b);
     while (r < r1) {
         if (fresh) {
 #pragma unroll
@@ -142,7 +173,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
         // row constants (identical in all lanes of a row)
         const double rowmask = rowact ? 1.0 : 0.0;
         const size_t gq = ((size_t)cur_b * P.Gext + (P.rstride ? e : 0)) * Nr + q;
-        const double Gy = P.Gy[gq] * rowmask, Py = P.Py[gq] * rowmask;
+        const double Gy = (NGB ? s_Gy[gq] : P.Gy[gq]) * rowmask, Py = (NGB ? s_Py[gq] : P.Py[gq]) * rowmask;
         RowConst rc;
         if (!GEOM) {
             const double x = P.x_ext[e], sx = P.sx_ext[e], c3x = P.c3x_ext[e];
@@ -276,9 +307,7 @@ __global__ void __launch_bounds__(POINT_THREADS, 1) point_kernel(const __grid_co
             if (e == P.Next && r < r1) {                 // next system: stage its coefficient pairs
                 e = 0; ++cur_b;
                 __syncwarp();
-                for (int j = lane; j < Npad; j += 32)
-                    s_coef[j] = reinterpret_cast<const double2 *>(P.coefP)[(size_t)cur_b * Npad + j];
-                __syncwarp();
+                load_coef(cur_b);
             }
         }
     }
@@ -894,8 +923,10 @@ int query_point_kernel(const KParams &k, PointKernelConfig &cfg)
 
     // residual-only build (and the Jacobian build of generic shapes): warp-independent kernel, 512 threads
     // (large N with full-warp angular batches: fewer warps per CTA until the per-warp stashes fit in shared memory)
+    const long long ngb = (long long)k.B * k.Gext * k.Nr;
+    const int h1_rows = ngb <= SELF_H1_MAX_ROWS ? (int)ngb : 0;      // (used by the Jacobian build of non-pipelined handles only)
     auto gsmem = [&](int thr) {
-        int d = k.Ntpad * 6 + (thr / 32) * warp_doubles(k.Npad, k.NCH);
+        int d = k.Ntpad * 6 + 2 * h1_rows + (thr / 32) * warp_doubles(k.Npad, k.NCH);
         const int need = tail_smem_doubles(k.Npad, thr);                    // the fused tail reuses the dynamic shared memory
         if (d < need) d = need;
         return (int)sizeof(double) * d;

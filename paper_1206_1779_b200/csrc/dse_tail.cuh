@@ -16,8 +16,9 @@
 //     scheduled -- and then writes the rows i and N + i of J and the entries i, N + i of F itself (MOM subtraction rows
 //     eq.(14),(15), local terms, the paper's layout eq.(29),(30),(35)): the assembly is spread over as many CTAs as
 //     there are external points.  An owner whose polls run out marks its point as pending instead;
-//   * every owner then bumps the system's counter of finished external points; the CTA that completes it writes the
-//     pending rows (normally none) and clears the counters for the next build.
+//   * every owner bumps the system's counter of finished external points as soon as its polls are over (before it writes
+//     its rows: the round trip overlaps them); the CTA that completes it writes the pending rows (normally none) and
+//     clears the counters for the next build.
 // The counters only decide WHO does a sum, never the order IN a sum: every reduction runs over row / slot indices in a
 // fixed order, so J and F are bitwise reproducible.  Data written by other CTAs of the same launch is read with
 // ld.global.cg after the counter handshake (L1 is not coherent).
@@ -245,7 +246,7 @@ __device__ __noinline__ void tail_finish(const KParams &P, int b, unsigned n_pen
 // tables are built by dse_create from the same partition formula the kernels use).  sm = the CTA's dynamic shared memory.
 __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
 {
-    __shared__ unsigned s_mask;
+    __shared__ unsigned s_mask, s_fin;
     __shared__ int s_own[3 * TAIL_OWN], s_w[64];
     __shared__ unsigned s_pend[TAIL_OWN];
     const int tid = threadIdx.x, lane = tid & 31, WPB = blockDim.x >> 5, T = blockDim.x;
@@ -303,29 +304,30 @@ __device__ __forceinline__ void build_tail(const KParams &P, double *sm)
             }
             __syncthreads();
             PHASE_STAMP(11);
-            {
-                const unsigned okm = s_mask;       // owned collocation points whose rows this CTA writes now
-                const int G = T / P.Npad > 0 ? T / P.Npad : 1, g = tid / P.Npad, j = tid - g * P.Npad;
-                for (int k = g; k < nown; k += G)
-                    if (g < G && ((okm >> k) & 1u)) tail_point_rows(P, s_own[3 * k], j, P.Npad);
-            }
-            __syncthreads();                       // (release by the counting threads below covers the rows)
-            PHASE_STAMP(13);
-            if (tid < 32) {                        // one count per finished point on its system's counter
+            const unsigned okm = s_mask;           // owned collocation points whose rows this CTA writes now
+            if (tid >= T - 32) {
+                // the LAST warp: one count per owned point on its system's counter -- now, not after the rows: the counter
+                // only has to follow the polls (it triggers the clearing of the counters the polls read) and the derivative
+                // rows that a pending point leaves to the finishing CTA; its round trip overlaps the other warps' rows
                 bool fin = false;
                 if (lane < nown) {
                     const int b = s_own[3 * lane] / P.Next, e = s_own[3 * lane] - b * P.Next;
-                    const bool pending = e < P.N && !((s_mask >> lane) & 1u);
+                    const bool pending = e < P.N && !((okm >> lane) & 1u);
                     const unsigned total = arrive_acq_rel(P.done + b, pending ? 1u + TAIL_PENDING : 1u) + 1u + (pending ? TAIL_PENDING : 0u);
                     fin = (total & (TAIL_PENDING - 1u)) == (unsigned)P.Next;
                     s_pend[lane] = total / TAIL_PENDING;
                 }
-                __syncwarp();
-                const unsigned m = __ballot_sync(FULL, fin);
-                if (lane == 0) s_mask = m;
+                const unsigned mf = __ballot_sync(FULL, fin);
+                if (lane == 0) s_fin = mf;
             }
+            {
+                const int G = T / P.Npad > 0 ? T / P.Npad : 1, g = tid / P.Npad, j = tid - g * P.Npad;
+                for (int k = g; k < nown; k += G)
+                    if (g < G && ((okm >> k) & 1u)) tail_point_rows(P, s_own[3 * k], j, P.Npad);
+            }
+            PHASE_STAMP(13);
             __syncthreads();
-            unsigned fmask = s_mask;
+            unsigned fmask = s_fin;
             while (fmask) {                        // systems whose last external point this CTA finished
                 const int l = __ffs(fmask) - 1;
                 fmask &= fmask - 1;

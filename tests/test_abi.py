@@ -79,3 +79,14 @@ def test_no_environment_switches_in_the_library():
     for f in os.listdir(src):
         if f.endswith((".cu", ".cuh", ".cpp", ".h")):
             assert "getenv" not in open(os.path.join(src, f)).read(), f
+
+
+def test_phase_stamps_need_an_instrumented_build(lib):
+    """include/dse_diag.h: the phase stamps exist only in a library built with -DDSE_PHASE_TIMING; the library the repository
+    builds by default (and ships to the GPU box) is the plain one, and says so."""
+    import numpy as np
+    out = np.zeros(16, dtype=np.int64)
+    lib.dse_diag_phase_stamps.argtypes = [ctypes.c_int32, ctypes.c_void_p, ctypes.c_int32]
+    assert lib.dse_diag_phase_stamps(0, ctypes.c_void_p(out.ctypes.data), 16) == -1
+    assert b"DSE_PHASE_TIMING" in lib.dse_last_error()
+    assert lib.dse_diag_phase_stamps(2, ctypes.c_void_p(out.ctypes.data), 16) == -1          # unknown selector
